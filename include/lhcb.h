@@ -1,0 +1,197 @@
+/*
+ * lhcb.h -- C ABI of the B200-native LHCb HLT1 Seeding + Matching hot path.
+ *
+ * The three calls follow the paper's statement of the problem (PAPER.md = arxiv/paper_2606_14480):
+ *   lhcb_geom_init  : detector description + tunables                      (Eq. 1-23, Tables 1-2)
+ *   lhcb_seeding    : per event, SciFi hits -> T-track seeds               (section 3)
+ *   lhcb_matching   : seeds x VELO tracks (+ UT hits) -> Long tracks       (section 4)
+ *
+ * Conventions
+ *   - Units: mm, MeV/c, q/p in 1/MeV, slopes dimensionless.  All floating point is IEEE float32.
+ *   - Every pointer inside lhcb_events_t / lhcb_seeds_t / lhcb_velo_t / lhcb_ut_t / lhcb_long_t is a
+ *     DEVICE pointer owned by the caller (e.g. a torch tensor's data_ptr()).  The *_t descriptor
+ *     structs themselves, lhcb_geom_t and lhcb_derived_t live in HOST memory.
+ *   - lhcb_seeding / lhcb_matching only enqueue work on `cuda_stream` (a cudaStream_t passed as
+ *     void*; NULL = legacy default stream).  They do not synchronise and do not allocate.
+ *   - Outputs are fully overwritten by each call (counts and status are reset by the call).
+ *   - Return value: LHCB_OK (0) or a negative lhcb_status code; lhcb_error_string() names it.
+ *     Per-event capacity overflow is NOT a return-code error: it is reported in the `status` output
+ *     words (LHCB_ST_* bits), and the affected event-half keeps the entries that fitted.
+ *   - One GPU per context.  A context may be used from one host thread at a time.
+ */
+#ifndef LHCB_H_
+#define LHCB_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LHCB_N_SCIFI_LAYERS 12
+#define LHCB_N_UT_LAYERS 4
+#define LHCB_NO_HIT 0xFFFFFFFFu
+
+typedef enum {
+  LHCB_OK = 0,
+  LHCB_ERR_BAD_ARGUMENT = -1,   /* NULL pointer, negative size, inconsistent capacities */
+  LHCB_ERR_BAD_GEOMETRY = -2,   /* not 6 x-layers + 6 stereo layers, seed triple not on x-layers, ... */
+  LHCB_ERR_CUDA = -3,           /* a CUDA runtime call failed (see lhcb_last_cuda_error) */
+  LHCB_ERR_NOT_INITIALISED = -4,
+  LHCB_ERR_CAPACITY = -5        /* requested capacities do not fit shared memory of the device */
+} lhcb_status;
+
+/* bits of the per-half / per-event `status` output words */
+#define LHCB_ST_TRIPLET_OVERFLOW 1u   /* more three-hit combinations than max_triplets_per_half */
+#define LHCB_ST_CAND_OVERFLOW 2u      /* more fitted x-z candidates than max_xz_cand_per_half */
+#define LHCB_ST_SEED_OVERFLOW 4u      /* more seeds than max_seeds_per_half */
+#define LHCB_ST_HITS_OVERFLOW 8u      /* event-half has more hits than max_hits_per_half: half skipped */
+#define LHCB_ST_MATCH_OVERFLOW 16u    /* more chi2-accepted pairs than max_match_cand_per_event */
+#define LHCB_ST_LONG_OVERFLOW 32u     /* more long tracks than max_long_per_event */
+#define LHCB_ST_VELO_OVERFLOW 64u     /* more VELO tracks than max_velo_per_event: event skipped */
+
+/* Detector description and tunables.  Host POD, copied by lhcb_geom_init.
+ * Citations: PAPER.md line / equation; "A<n>" = reading listed in DESIGN.md. */
+typedef struct {
+  float scifi_z[LHCB_N_SCIFI_LAYERS];          /* layer z, ascending                               L33 */
+  float scifi_tan_alpha[LHCB_N_SCIFI_LAYERS];  /* tan(stereo angle); exactly 0 for the six x-layers L33 */
+  float z_ref, d_ratio;                        /* Eq. 1 (L69-72) */
+  float p_min, inv_p_a, inv_p_b;               /* Eq. 5-8 (L114-131); a, b per MeV (A1) */
+  float alpha0, alpha1;                        /* Eq. 9-10 (L137-143) */
+  int32_t iter_layers[2][3];                   /* T1,T2,T3 x-layer of each iteration (L78, A5) */
+  float kappa_cx;                              /* c_x = polarity*q*kappa/p  (A3) */
+  float cx_band[4];                            /* third-hit band f_lo, f_hi, d_lo, d_hi (Fig. 6, A4) */
+  float tol_x_ext, tol_uv;                     /* 1 mm (L90), 2 mm (L215) */
+  int32_t min_x_hits, min_uv_hits;             /* 5 (L90; must be 5 or 6), 4 (A9) */
+  int32_t uv_first_layer[2];                   /* first stereo layer of the two UV passes (L215, A9) */
+  float sigma_hit, chi2x_max, chi2y_max;       /* chi2/ndf cuts (L90, A6) */
+  float y_min, y_max, y_half_tol;              /* detector halves: y>0 / y<0 (L372) */
+  float z_velo, z_scifi_state, z_match_y;      /* state planes; y matching plane at 10 m (L231) */
+  float mag[5];                                /* A_x..E_x of Eq. 18, Table 1 (L255-261) */
+  float gamma_ab[2];                           /* A_gamma, B_gamma of Eq. 20, Table 1 (L262-263) */
+  float kick_pt;                               /* K_B: q/p = polarity*dtx/K_B (A10) */
+  int32_t polarity;                            /* +1 / -1; used when no per-event polarity is given */
+  float presel[4];                             /* |dx|,|dy|,|dtx|,|dty| of Eq. 21 (L281) */
+  float match_tol[8];                          /* Eq. 23: 4/5, 10.12, 101.0, 1/5, 1.59, 212.1, tol_tx, 1/tol_ty */
+  float chi2_match_max;                        /* 2 (L301) */
+  float ut_z[LHCB_N_UT_LAYERS], ut_tan_alpha[LHCB_N_UT_LAYERS];   /* UTaX, UTaU, UTbV, UTbX (L315) */
+  float ut_loose[LHCB_N_UT_LAYERS][4];         /* A, B [mm GeV], min, max per layer: Table 2 (L323-340) */
+  float ut_tight[LHCB_N_UT_LAYERS][4];
+  float ut_y_tol;                              /* strip y-coverage tolerance (O13) */
+  int32_t min_ut_hits, ut_enabled;             /* 3 (L311); 0 disables the UT search (L307) */
+  /* capacities; 0 selects the default in brackets */
+  int32_t max_seeds_per_half;                  /* [256]  output slots per event-half */
+  int32_t max_xz_cand_per_half;                /* [1024] fitted x-z candidates per event-half */
+  int32_t max_long_per_event;                  /* [256]  output slots per event */
+  int32_t max_hits_per_half;                   /* [6144] SciFi hits staged per event-half (<= 32768) */
+  int32_t max_triplets_per_half;               /* [4096] three-hit combinations per half and iteration */
+  int32_t max_match_cand_per_event;            /* [1024] chi2-accepted seed-VELO pairs per event */
+  int32_t max_velo_per_event;                  /* [1024] */
+} lhcb_geom_t;
+
+/* Geometry-only constants the kernels use (O1).  Computed in double from the float
+ * geometry and rounded once to float.  Exposed so that host logic can be tested without a GPU. */
+typedef struct {
+  int32_t xl[6], ul[6], slot_of_layer[LHCB_N_SCIFI_LAYERS];
+  float zb[12], gz[12], tan_a[12], inv_tan[12], inv_z[12], zt[12];
+  float ywin_a[2][12], ywin_b[2][12];
+  int32_t l1[2], l2[2], l3[2];
+  float dx3max[2], alpha_corr[2], r13[2], inv_dz13[2], z1[2], dz12[2], K[2], inv_K[2], G13[2];
+  float a, b, kappa, inv_kappa, f_lo, f_hi, d_lo, d_hi, tol_x, tol_uv, chi2x_max, chi2y_max;
+  float wx[7], wy[7];
+  float zbS, gS, gpS;
+  float zS, zV, dzyS, dzyV, mag[5], presel[4], cx0, cx1, cy0, cy1, inv_tol_tx, inv_tol_ty, chi2m_max;
+  float inv_KB, Ag, Bg, inv_Bg, ut_dz[4], ut_dz2[4], ut_dz4[4], ut_tan[4], ut_y_tol;
+  float ut_loose[4][4], ut_tight[4][4];
+  float P[7][3][6];      /* x-z least-squares map per hit pattern (0: six hits, 1+k: x-slot k missing) */
+  float Q[64][2][6];     /* y-z least-squares map per stereo-slot bitmask */
+} lhcb_derived_t;
+
+typedef struct lhcb_ctx lhcb_ctx;
+
+/* SciFi hits of a batch of events (section 3; L372: tiled by detector half, sorted per layer). */
+typedef struct {
+  int32_t n_events;
+  uint32_t n_hits;           /* length of hit_x */
+  const uint32_t* zone_off;  /* [n_events*24+1]; zone = (event*2+half)*12+layer, half 0: y>0 */
+  const float* hit_x;        /* [n_hits] ascending inside each zone; stereo layers: x at y=0 */
+  const int8_t* polarity;    /* [n_events] +1/-1, or NULL -> geom.polarity */
+} lhcb_events_t;
+
+/* Seeds ("T tracks", L219).  Event-half h owns slots [h*max_seeds_per_half, +count[h]); the order
+ * inside a slot range is unspecified.  cap_total = n_events*2*max_seeds_per_half. */
+typedef struct {
+  int32_t n_events;
+  uint32_t* count;     /* [n_events*2] */
+  float* state;        /* SoA [5][cap_total]: x, y, tx, ty, q/p at z_scifi_state */
+  float* par;          /* SoA [7][cap_total]: ax, bx, cx, ay, by, chi2x, chi2y   (may be NULL for matching) */
+  uint32_t* hits;      /* SoA [12][cap_total]: global hit index per layer or LHCB_NO_HIT (may be NULL for matching) */
+  uint8_t* nx;         /* [cap_total] (may be NULL for matching) */
+  uint8_t* nuv;        /* [cap_total] (may be NULL for matching) */
+  uint32_t* status;    /* [n_events*2] LHCB_ST_* bits */
+} lhcb_seeds_t;
+
+/* VELO track states at z_velo (L239-244). */
+typedef struct {
+  int32_t n_events;
+  const uint32_t* off;       /* [n_events+1] */
+  const float *x, *y, *tx, *ty;
+  const int8_t* polarity;    /* [n_events] or NULL -> geom.polarity */
+} lhcb_velo_t;
+
+/* UT hits (L305-342): per (event, layer) sorted by x0 = x at y=0; strip covers [y_lo, y_hi]. */
+typedef struct {
+  const uint32_t* off;       /* [n_events*4+1] */
+  const float *x0, *y_lo, *y_hi;
+} lhcb_ut_t;
+
+/* Long tracks.  Event e owns slots [e*max_long_per_event, +count[e]); order unspecified.
+ * cap_total = n_events*max_long_per_event. */
+typedef struct {
+  uint32_t* count;     /* [n_events] */
+  uint32_t* seed_idx;  /* [cap_total] slot index into lhcb_seeds_t arrays */
+  uint32_t* velo_idx;  /* [cap_total] index into lhcb_velo_t arrays */
+  uint32_t* ut_idx;    /* SoA [4][cap_total] index into lhcb_ut_t arrays or LHCB_NO_HIT */
+  uint8_t* n_ut;       /* [cap_total] */
+  float* qop;          /* [cap_total] q/p: UT-refined (Eq. 20) if UT hits were added, else the kick estimate */
+  float* chi2;         /* [cap_total] chi2_match of Eq. 22 */
+  uint32_t* status;    /* [n_events] LHCB_ST_* bits */
+} lhcb_long_t;
+
+/* Host only.  Fills `out` from `g` (no CUDA call).  Returns LHCB_OK or LHCB_ERR_BAD_GEOMETRY /
+ * LHCB_ERR_BAD_ARGUMENT.  lhcb_geom_init uses exactly this function. */
+int lhcb_geom_derive(const lhcb_geom_t* g, lhcb_derived_t* out);
+
+/* Creates a context on CUDA device `device`: derives the constants, uploads the tables, checks the
+ * shared-memory budget of the capacities.  *out is owned by the caller until lhcb_destroy. */
+int lhcb_geom_init(const lhcb_geom_t* g, int device, lhcb_ctx** out);
+void lhcb_destroy(lhcb_ctx* ctx);
+
+/* The geometry the context holds, with capacity defaults resolved. */
+int lhcb_get_geom(const lhcb_ctx* ctx, lhcb_geom_t* out);
+
+/* Bytes of device scratch the two calls need for a batch (may be 0; pass NULL workspace then). */
+size_t lhcb_workspace_bytes(const lhcb_ctx* ctx, int n_events, size_t n_scifi_hits);
+
+/* Seeding: x-z two-/three-hit search, extension, fit, clone kill, u/v addition, y fit (section 3).
+ * One CTA per event-half.  `out` arrays must have cap_total = n_events*2*max_seeds_per_half slots. */
+int lhcb_seeding(lhcb_ctx* ctx, const lhcb_events_t* events, lhcb_seeds_t* out, void* workspace,
+                 void* cuda_stream);
+
+/* Matching: kink extrapolation, preselection, chi2_match, UT hit search, one-to-one selection
+ * (section 4).  `ut` may be NULL (no UT in the data taking, L307).  Only seeds->count and
+ * seeds->state are read. */
+int lhcb_matching(lhcb_ctx* ctx, const lhcb_seeds_t* seeds, const lhcb_velo_t* velo, const lhcb_ut_t* ut,
+                  lhcb_long_t* out, void* workspace, void* cuda_stream);
+
+const char* lhcb_error_string(int status);
+/* cudaError_t of the last failing CUDA call made through this context (0 if none). */
+int lhcb_last_cuda_error(const lhcb_ctx* ctx);
+/* Number of kernels the last lhcb_seeding / lhcb_matching call launched. */
+int lhcb_last_launch_count(const lhcb_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LHCB_H_ */

@@ -1,0 +1,8 @@
+"""B200-native (sm_100a) LHCb HLT1 Seeding + Matching hot path (arxiv/paper_2606_14480).
+
+The product is the C-ABI CUDA library declared in include/lhcb.h (sources in csrc/); this package is
+its thin Python binding.  There is no CPU fallback.
+"""
+from .binding import Context, DeviceEvents, lhcb_geom_derive, load_library, NO_HIT, EXPORTS
+
+__all__ = ["Context", "DeviceEvents", "lhcb_geom_derive", "load_library", "NO_HIT", "EXPORTS"]

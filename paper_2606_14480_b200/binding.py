@@ -1,0 +1,333 @@
+"""Thin ctypes binding of include/lhcb.h.  Argument marshalling only: every step of the path runs
+in the CUDA library.  PyTorch provides device memory and streams.
+
+There is no CPU fallback: importing works without a GPU (so the ABI can be checked), but creating a
+Context raises if the library or a CUDA device is missing.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+
+from . import build as _build
+
+F, I = C.c_float, C.c_int32
+NO_HIT = 0xFFFFFFFF
+
+ST_BITS = {1: "triplet_overflow", 2: "cand_overflow", 4: "seed_overflow", 8: "hits_overflow",
+           16: "match_overflow", 32: "long_overflow", 64: "velo_overflow"}
+
+EXPORTS = ["lhcb_geom_derive", "lhcb_geom_init", "lhcb_destroy", "lhcb_get_geom", "lhcb_workspace_bytes",
+           "lhcb_seeding", "lhcb_matching", "lhcb_error_string", "lhcb_last_cuda_error",
+           "lhcb_last_launch_count"]
+
+
+class LhcbGeom(C.Structure):
+    _fields_ = [
+        ("scifi_z", F * 12), ("scifi_tan_alpha", F * 12), ("z_ref", F), ("d_ratio", F),
+        ("p_min", F), ("inv_p_a", F), ("inv_p_b", F), ("alpha0", F), ("alpha1", F),
+        ("iter_layers", (I * 3) * 2), ("kappa_cx", F), ("cx_band", F * 4),
+        ("tol_x_ext", F), ("tol_uv", F), ("min_x_hits", I), ("min_uv_hits", I), ("uv_first_layer", I * 2),
+        ("sigma_hit", F), ("chi2x_max", F), ("chi2y_max", F), ("y_min", F), ("y_max", F), ("y_half_tol", F),
+        ("z_velo", F), ("z_scifi_state", F), ("z_match_y", F), ("mag", F * 5), ("gamma_ab", F * 2),
+        ("kick_pt", F), ("polarity", I), ("presel", F * 4), ("match_tol", F * 8), ("chi2_match_max", F),
+        ("ut_z", F * 4), ("ut_tan_alpha", F * 4), ("ut_loose", (F * 4) * 4), ("ut_tight", (F * 4) * 4),
+        ("ut_y_tol", F), ("min_ut_hits", I), ("ut_enabled", I),
+        ("max_seeds_per_half", I), ("max_xz_cand_per_half", I), ("max_long_per_event", I),
+        ("max_hits_per_half", I), ("max_triplets_per_half", I), ("max_match_cand_per_event", I),
+        ("max_velo_per_event", I),
+    ]
+
+
+class LhcbDerived(C.Structure):
+    _fields_ = [
+        ("xl", I * 6), ("ul", I * 6), ("slot_of_layer", I * 12),
+        ("zb", F * 12), ("gz", F * 12), ("tan_a", F * 12), ("inv_tan", F * 12), ("inv_z", F * 12), ("zt", F * 12),
+        ("ywin_a", (F * 12) * 2), ("ywin_b", (F * 12) * 2), ("l1", I * 2), ("l2", I * 2), ("l3", I * 2),
+        ("dx3max", F * 2), ("alpha_corr", F * 2), ("r13", F * 2), ("inv_dz13", F * 2), ("z1", F * 2),
+        ("dz12", F * 2), ("K", F * 2), ("inv_K", F * 2), ("G13", F * 2),
+        ("a", F), ("b", F), ("kappa", F), ("inv_kappa", F), ("f_lo", F), ("f_hi", F), ("d_lo", F), ("d_hi", F),
+        ("tol_x", F), ("tol_uv", F), ("chi2x_max", F), ("chi2y_max", F), ("wx", F * 7), ("wy", F * 7),
+        ("zbS", F), ("gS", F), ("gpS", F),
+        ("zS", F), ("zV", F), ("dzyS", F), ("dzyV", F), ("mag", F * 5), ("presel", F * 4),
+        ("cx0", F), ("cx1", F), ("cy0", F), ("cy1", F), ("inv_tol_tx", F), ("inv_tol_ty", F), ("chi2m_max", F),
+        ("inv_KB", F), ("Ag", F), ("Bg", F), ("inv_Bg", F), ("ut_dz", F * 4), ("ut_dz2", F * 4), ("ut_dz4", F * 4),
+        ("ut_tan", F * 4), ("ut_y_tol", F), ("ut_loose", (F * 4) * 4), ("ut_tight", (F * 4) * 4),
+        ("P", ((F * 6) * 3) * 7), ("Q", ((F * 6) * 2) * 64),
+    ]
+
+
+VP = C.c_void_p
+
+
+class LhcbEvents(C.Structure):
+    _fields_ = [("n_events", I), ("n_hits", C.c_uint32), ("zone_off", VP), ("hit_x", VP), ("polarity", VP)]
+
+
+class LhcbSeeds(C.Structure):
+    _fields_ = [("n_events", I), ("count", VP), ("state", VP), ("par", VP), ("hits", VP), ("nx", VP),
+                ("nuv", VP), ("status", VP)]
+
+
+class LhcbVelo(C.Structure):
+    _fields_ = [("n_events", I), ("off", VP), ("x", VP), ("y", VP), ("tx", VP), ("ty", VP), ("polarity", VP)]
+
+
+class LhcbUt(C.Structure):
+    _fields_ = [("off", VP), ("x0", VP), ("y_lo", VP), ("y_hi", VP)]
+
+
+class LhcbLong(C.Structure):
+    _fields_ = [("count", VP), ("seed_idx", VP), ("velo_idx", VP), ("ut_idx", VP), ("n_ut", VP), ("qop", VP),
+                ("chi2", VP), ("status", VP)]
+
+
+def fill_geom(geom: dict) -> LhcbGeom:
+    g = LhcbGeom()
+    for name, _ in LhcbGeom._fields_:
+        v = geom.get(name, 0)
+        if isinstance(v, (list, tuple)):
+            arr = getattr(g, name)
+            for i, vi in enumerate(v):
+                if isinstance(vi, (list, tuple)):
+                    for j, vj in enumerate(vi):
+                        arr[i][j] = vj
+                else:
+                    arr[i] = vi
+        else:
+            setattr(g, name, v)
+    return g
+
+
+_LIB = None
+
+
+def load_library(build: bool = True) -> C.CDLL:
+    """dlopen the in-tree library (building it first if the sources are newer)."""
+    global _LIB
+    if _LIB is None:
+        path = _build.build() if build else _build.LIB
+        if not os.path.exists(path):
+            raise RuntimeError(f"CUDA library {path} is missing: run python -m paper_2606_14480_b200.build")
+        lib = C.CDLL(path)
+        lib.lhcb_geom_derive.argtypes = [C.POINTER(LhcbGeom), C.POINTER(LhcbDerived)]
+        lib.lhcb_geom_init.argtypes = [C.POINTER(LhcbGeom), C.c_int, C.POINTER(VP)]
+        lib.lhcb_destroy.argtypes = [VP]
+        lib.lhcb_destroy.restype = None
+        lib.lhcb_get_geom.argtypes = [VP, C.POINTER(LhcbGeom)]
+        lib.lhcb_workspace_bytes.argtypes = [VP, C.c_int, C.c_size_t]
+        lib.lhcb_workspace_bytes.restype = C.c_size_t
+        lib.lhcb_seeding.argtypes = [VP, C.POINTER(LhcbEvents), C.POINTER(LhcbSeeds), VP, VP]
+        lib.lhcb_matching.argtypes = [VP, C.POINTER(LhcbSeeds), C.POINTER(LhcbVelo), C.POINTER(LhcbUt),
+                                      C.POINTER(LhcbLong), VP, VP]
+        lib.lhcb_error_string.argtypes = [C.c_int]
+        lib.lhcb_error_string.restype = C.c_char_p
+        lib.lhcb_last_cuda_error.argtypes = [VP]
+        lib.lhcb_last_launch_count.argtypes = [VP]
+        _LIB = lib
+    return _LIB
+
+
+def lhcb_geom_derive(geom: dict) -> LhcbDerived:
+    """Host-only: derived constants of a geometry (no GPU needed)."""
+    lib = load_library()
+    d = LhcbDerived()
+    rc = lib.lhcb_geom_derive(C.byref(fill_geom(geom)), C.byref(d))
+    if rc != 0:
+        raise ValueError(f"lhcb_geom_derive: {lib.lhcb_error_string(rc).decode()}")
+    return d
+
+
+def _check(lib, ctx, rc, what):
+    if rc != 0:
+        extra = f" (cudaError {lib.lhcb_last_cuda_error(ctx)})" if rc == -3 and ctx else ""
+        raise RuntimeError(f"{what}: {lib.lhcb_error_string(rc).decode()}{extra}")
+
+
+def _ptr(t):
+    return VP(t.data_ptr()) if t is not None else VP(0)
+
+
+@dataclass
+class DeviceEvents:
+    """A batch resident in device memory (torch tensors)."""
+    n_events: int
+    n_hits: int
+    zone_off: "torch.Tensor"
+    hit_x: "torch.Tensor"
+    polarity: Optional["torch.Tensor"]
+    velo_off: "torch.Tensor"
+    velo_x: "torch.Tensor"
+    velo_y: "torch.Tensor"
+    velo_tx: "torch.Tensor"
+    velo_ty: "torch.Tensor"
+    ut_off: Optional["torch.Tensor"] = None
+    ut_x0: Optional["torch.Tensor"] = None
+    ut_ylo: Optional["torch.Tensor"] = None
+    ut_yhi: Optional["torch.Tensor"] = None
+
+    @staticmethod
+    def from_host(ev, device="cuda:0"):
+        import torch
+
+        def up(a, dt):
+            return torch.from_numpy(np.ascontiguousarray(a, dt).view(
+                np.int32 if dt == np.uint32 else dt)).to(device)
+        has_ut = len(ev.ut_x0) > 0
+        return DeviceEvents(
+            n_events=ev.n_events, n_hits=ev.n_hits, zone_off=up(ev.zone_off, np.uint32),
+            hit_x=up(ev.hit_x, np.float32), polarity=up(ev.polarity, np.int8),
+            velo_off=up(ev.velo_off, np.uint32), velo_x=up(ev.velo_x, np.float32),
+            velo_y=up(ev.velo_y, np.float32), velo_tx=up(ev.velo_tx, np.float32),
+            velo_ty=up(ev.velo_ty, np.float32),
+            ut_off=up(ev.ut_off, np.uint32) if has_ut else None,
+            ut_x0=up(ev.ut_x0, np.float32) if has_ut else None,
+            ut_ylo=up(ev.ut_ylo, np.float32) if has_ut else None,
+            ut_yhi=up(ev.ut_yhi, np.float32) if has_ut else None)
+
+    def input_bytes(self):
+        n = 0
+        for t in (self.zone_off, self.hit_x, self.polarity, self.velo_off, self.velo_x, self.velo_y, self.velo_tx,
+                  self.velo_ty, self.ut_off, self.ut_x0, self.ut_ylo, self.ut_yhi):
+            if t is not None:
+                n += t.numel() * t.element_size()
+        return n
+
+
+class Context:
+    """lhcb_geom_init / lhcb_seeding / lhcb_matching on one CUDA device."""
+
+    def __init__(self, geom: dict, device: int = 0):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2606_14480_b200 needs a CUDA device: there is no CPU fallback")
+        self.torch = torch
+        self.lib = load_library()
+        self.device = device
+        self.dev = torch.device("cuda", device)
+        torch.cuda.init()
+        torch.zeros(1, device=self.dev)                 # make sure the primary context exists
+        self._ctx = VP(0)
+        rc = self.lib.lhcb_geom_init(C.byref(fill_geom(geom)), device, C.byref(self._ctx))
+        _check(self.lib, None, rc, "lhcb_geom_init")
+        g = LhcbGeom()
+        self.lib.lhcb_get_geom(self._ctx, C.byref(g))
+        self.max_seeds = g.max_seeds_per_half
+        self.max_long = g.max_long_per_event
+        self.geom = geom
+
+    def close(self):
+        if getattr(self, "_ctx", None) and self._ctx.value:
+            self.lib.lhcb_destroy(self._ctx)
+            self._ctx = VP(0)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _stream(self):
+        return VP(self.torch.cuda.current_stream(self.dev).cuda_stream)
+
+    # ------------------------------------------------------------------ outputs
+    def alloc_seeds(self, n_events):
+        t = self.torch
+        cap = n_events * 2 * self.max_seeds
+        kw = dict(device=self.dev)
+        return dict(n_events=n_events, cap_total=cap,
+                    count=t.empty(n_events * 2, dtype=t.int32, **kw), state=t.empty((5, cap), dtype=t.float32, **kw),
+                    par=t.empty((7, cap), dtype=t.float32, **kw), hits=t.empty((12, cap), dtype=t.int32, **kw),
+                    nx=t.empty(cap, dtype=t.uint8, **kw), nuv=t.empty(cap, dtype=t.uint8, **kw),
+                    status=t.empty(n_events * 2, dtype=t.int32, **kw))
+
+    def alloc_long(self, n_events):
+        t = self.torch
+        cap = n_events * self.max_long
+        kw = dict(device=self.dev)
+        return dict(n_events=n_events, cap_total=cap, count=t.empty(n_events, dtype=t.int32, **kw),
+                    seed_idx=t.empty(cap, dtype=t.int32, **kw), velo_idx=t.empty(cap, dtype=t.int32, **kw),
+                    ut_idx=t.empty((4, cap), dtype=t.int32, **kw), n_ut=t.empty(cap, dtype=t.uint8, **kw),
+                    qop=t.empty(cap, dtype=t.float32, **kw), chi2=t.empty(cap, dtype=t.float32, **kw),
+                    status=t.empty(n_events, dtype=t.int32, **kw))
+
+    @staticmethod
+    def _seeds_struct(s):
+        return LhcbSeeds(s["n_events"], _ptr(s["count"]), _ptr(s["state"]), _ptr(s.get("par")), _ptr(s.get("hits")),
+                         _ptr(s.get("nx")), _ptr(s.get("nuv")), _ptr(s.get("status")))
+
+    # ------------------------------------------------------------------ the two calls
+    def lhcb_seeding(self, dev: DeviceEvents, out: Optional[dict] = None) -> dict:
+        out = out if out is not None else self.alloc_seeds(dev.n_events)
+        e = LhcbEvents(dev.n_events, dev.n_hits, _ptr(dev.zone_off), _ptr(dev.hit_x), _ptr(dev.polarity))
+        s = self._seeds_struct(out)
+        rc = self.lib.lhcb_seeding(self._ctx, C.byref(e), C.byref(s), VP(0), self._stream())
+        _check(self.lib, self._ctx, rc, "lhcb_seeding")
+        return out
+
+    def lhcb_matching(self, seeds: dict, dev: DeviceEvents, out: Optional[dict] = None, use_ut: bool = True) -> dict:
+        out = out if out is not None else self.alloc_long(dev.n_events)
+        s = self._seeds_struct(seeds)
+        v = LhcbVelo(dev.n_events, _ptr(dev.velo_off), _ptr(dev.velo_x), _ptr(dev.velo_y), _ptr(dev.velo_tx),
+                     _ptr(dev.velo_ty), _ptr(dev.polarity))
+        u = None
+        if use_ut and dev.ut_off is not None:
+            u = C.byref(LhcbUt(_ptr(dev.ut_off), _ptr(dev.ut_x0), _ptr(dev.ut_ylo), _ptr(dev.ut_yhi)))
+        l = LhcbLong(_ptr(out["count"]), _ptr(out["seed_idx"]), _ptr(out["velo_idx"]), _ptr(out["ut_idx"]),
+                     _ptr(out["n_ut"]), _ptr(out["qop"]), _ptr(out["chi2"]), _ptr(out["status"]))
+        rc = self.lib.lhcb_matching(self._ctx, C.byref(s), C.byref(v), u, C.byref(l), VP(0), self._stream())
+        _check(self.lib, self._ctx, rc, "lhcb_matching")
+        return out
+
+    def last_launch_count(self):
+        return int(self.lib.lhcb_last_launch_count(self._ctx))
+
+    # ------------------------------------------------------------------ helpers (host views of outputs)
+    def seeds_from_states(self, n_events, seed_off, state):
+        """Direct seeds (BASELINE.json configs[4]): states [5][n] with per-event offsets -> slot layout.
+        Event e's seeds go to half 2e first, then half 2e+1, in input order."""
+        t = self.torch
+        out = self.alloc_seeds(n_events)
+        cap, ms = out["cap_total"], self.max_seeds
+        cnt = np.diff(seed_off.astype(np.int64))
+        if (cnt > 2 * ms).any():
+            raise ValueError("more direct seeds per event than 2*max_seeds_per_half")
+        ev = np.repeat(np.arange(n_events), cnt)
+        k = np.arange(len(ev)) - np.repeat(seed_off[:-1].astype(np.int64), cnt)
+        slot = np.where(k < ms, (2 * ev) * ms + k, (2 * ev + 1) * ms + (k - ms))
+        st = np.zeros((5, cap), np.float32)
+        st[:, slot] = state
+        count = np.zeros(2 * n_events, np.int32)
+        count[0::2] = np.minimum(cnt, ms); count[1::2] = np.maximum(cnt - ms, 0)
+        out["state"].copy_(t.from_numpy(st)); out["count"].copy_(t.from_numpy(count))
+        out["status"].zero_()
+        return out, slot
+
+    def seeds_to_host(self, s):
+        """Compact host view: per seed event, half, slot, state[5], par[7], hits[12], nx, nuv."""
+        cnt = s["count"].cpu().numpy().astype(np.int64)
+        ms = self.max_seeds
+        half = np.repeat(np.arange(len(cnt)), cnt)
+        k = np.arange(len(half)) - np.repeat(np.cumsum(cnt) - cnt, cnt)
+        slot = half * ms + k
+        st = s["state"].cpu().numpy()[:, slot].T
+        par = s["par"].cpu().numpy()[:, slot].T
+        hits = s["hits"].cpu().numpy().view(np.uint32)[:, slot].T
+        return dict(n=len(slot), event=half // 2, half=half % 2, slot=slot, state=st, par=par, hits=hits,
+                    nx=s["nx"].cpu().numpy()[slot], nuv=s["nuv"].cpu().numpy()[slot],
+                    status=s["status"].cpu().numpy().view(np.uint32))
+
+    def long_to_host(self, l):
+        cnt = l["count"].cpu().numpy().astype(np.int64)
+        ml = self.max_long
+        ev = np.repeat(np.arange(len(cnt)), cnt)
+        k = np.arange(len(ev)) - np.repeat(np.cumsum(cnt) - cnt, cnt)
+        slot = ev * ml + k
+        g = lambda name: l[name].cpu().numpy()
+        return dict(n=len(slot), event=ev, seed=g("seed_idx").view(np.uint32)[slot], velo=g("velo_idx").view(np.uint32)[slot],
+                    ut=g("ut_idx").view(np.uint32)[:, slot].T, n_ut=g("n_ut")[slot], qop=g("qop")[slot],
+                    chi2=g("chi2")[slot], status=g("status").view(np.uint32))

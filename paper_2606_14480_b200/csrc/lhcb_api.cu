@@ -1,0 +1,218 @@
+// C-ABI entry points (include/lhcb.h): argument checks, constant derivation, kernel launches.
+// No torch types: plain pointers and sizes.  Built with
+//   nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo -fmad=false -shared -Xcompiler -fPIC
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "../../include/lhcb.h"
+#include "derive.h"
+#include "matching.cuh"
+#include "seeding.cuh"
+
+struct lhcb_ctx {
+  lhcb_geom_t geom;
+  lhcb_derived_t der;
+  int device;
+  float* d_P;
+  float* d_Q;
+  size_t seed_smem, match_smem;
+  int last_cuda_error;
+  int last_launches;
+};
+
+namespace {
+
+int cuda_fail(lhcb_ctx* ctx, cudaError_t e) {
+  if (ctx) ctx->last_cuda_error = (int)e;
+  return LHCB_ERR_CUDA;
+}
+
+#define LHCB_CUDA(ctx, call)                                   \
+  do {                                                         \
+    cudaError_t err__ = (call);                                \
+    if (err__ != cudaSuccess) return cuda_fail((ctx), err__);  \
+  } while (0)
+
+template <class T, size_t N>
+void copy_arr(T (&dst)[N], const T (&src)[N]) { std::memcpy(dst, src, sizeof(T) * N); }
+
+void fill_seed_params(const lhcb_ctx* c, lhcb::SeedParams& p) {
+  const lhcb_derived_t& D = c->der;
+  const lhcb_geom_t& g = c->geom;
+  std::memset(&p, 0, sizeof(p));
+  copy_arr(p.zb, D.zb); copy_arr(p.gz, D.gz); copy_arr(p.tan_a, D.tan_a); copy_arr(p.inv_tan, D.inv_tan);
+  copy_arr(p.inv_z, D.inv_z); copy_arr(p.zt, D.zt);
+  std::memcpy(p.ywin_a, D.ywin_a, sizeof(p.ywin_a)); std::memcpy(p.ywin_b, D.ywin_b, sizeof(p.ywin_b));
+  for (int i = 0; i < 6; ++i) { p.xl[i] = D.xl[i]; p.ul[i] = D.ul[i]; }
+  for (int i = 0; i < 12; ++i) p.slot_of_layer[i] = D.slot_of_layer[i];
+  for (int i = 0; i < 2; ++i) {
+    p.l1[i] = D.l1[i]; p.l2[i] = D.l2[i]; p.l3[i] = D.l3[i];
+    p.dx3max[i] = D.dx3max[i]; p.r13[i] = D.r13[i]; p.inv_dz13[i] = D.inv_dz13[i]; p.z1[i] = D.z1[i];
+    p.dz12[i] = D.dz12[i]; p.K[i] = D.K[i]; p.inv_K[i] = D.inv_K[i]; p.G13[i] = D.G13[i];
+    p.uv_first[i] = g.uv_first_layer[i];
+  }
+  p.a = D.a; p.b = D.b; p.kappa = D.kappa; p.inv_kappa = D.inv_kappa;
+  p.f_lo = D.f_lo; p.f_hi = D.f_hi; p.d_lo = D.d_lo; p.d_hi = D.d_hi;
+  p.tol_x = D.tol_x; p.tol_uv = D.tol_uv; p.chi2x_max = D.chi2x_max; p.chi2y_max = D.chi2y_max;
+  copy_arr(p.wx, D.wx); copy_arr(p.wy, D.wy);
+  p.zbS = D.zbS; p.gS = D.gS; p.gpS = D.gpS;
+  p.min_x_hits = g.min_x_hits; p.min_uv_hits = g.min_uv_hits; p.polarity = g.polarity;
+  p.max_seeds = g.max_seeds_per_half; p.max_cand = g.max_xz_cand_per_half; p.max_hits = g.max_hits_per_half;
+  p.max_trip = g.max_triplets_per_half;
+  p.P = c->d_P; p.Q = c->d_Q;
+}
+
+void fill_match_params(const lhcb_ctx* c, lhcb::MatchParams& p) {
+  const lhcb_derived_t& D = c->der;
+  const lhcb_geom_t& g = c->geom;
+  std::memset(&p, 0, sizeof(p));
+  p.zS = D.zS; p.zV = D.zV; p.dzyS = D.dzyS; p.dzyV = D.dzyV;
+  copy_arr(p.mag, D.mag); copy_arr(p.presel, D.presel);
+  p.cx0 = D.cx0; p.cx1 = D.cx1; p.cy0 = D.cy0; p.cy1 = D.cy1;
+  p.inv_tol_tx = D.inv_tol_tx; p.inv_tol_ty = D.inv_tol_ty; p.chi2m_max = D.chi2m_max;
+  p.inv_KB = D.inv_KB; p.Ag = D.Ag; p.Bg = D.Bg; p.inv_Bg = D.inv_Bg;
+  copy_arr(p.ut_dz, D.ut_dz); copy_arr(p.ut_dz2, D.ut_dz2); copy_arr(p.ut_dz4, D.ut_dz4);
+  copy_arr(p.ut_tan, D.ut_tan); p.ut_y_tol = D.ut_y_tol;
+  std::memcpy(p.ut_loose, D.ut_loose, sizeof(p.ut_loose)); std::memcpy(p.ut_tight, D.ut_tight, sizeof(p.ut_tight));
+  p.min_ut_hits = g.min_ut_hits; p.polarity = g.polarity;
+  p.max_seeds = g.max_seeds_per_half; p.max_long = g.max_long_per_event;
+  p.max_mc = g.max_match_cand_per_event; p.max_velo = g.max_velo_per_event;
+}
+
+}  // namespace
+
+extern "C" {
+
+int lhcb_geom_derive(const lhcb_geom_t* g, lhcb_derived_t* out) {
+  if (!g || !out) return LHCB_ERR_BAD_ARGUMENT;
+  return lhcb::derive(*g, *out);
+}
+
+int lhcb_geom_init(const lhcb_geom_t* g, int device, lhcb_ctx** out) {
+  if (!g || !out || device < 0) return LHCB_ERR_BAD_ARGUMENT;
+  *out = nullptr;
+  lhcb_ctx* c = new (std::nothrow) lhcb_ctx();
+  if (!c) return LHCB_ERR_BAD_ARGUMENT;
+  std::memset(c, 0, sizeof(*c));
+  c->geom = *g;
+  lhcb::resolve_defaults(c->geom);
+  c->device = device;
+  const lhcb_geom_t& G = c->geom;
+  int rc = lhcb::derive(G, c->der);
+  if (rc != LHCB_OK) { delete c; return rc; }
+  if (G.max_hits_per_half > 32768 || G.max_xz_cand_per_half > 65535 || G.max_seeds_per_half > 32767 ||
+      G.max_velo_per_event > 65535 || G.max_triplets_per_half < 16) { delete c; return LHCB_ERR_BAD_ARGUMENT; }
+  c->seed_smem = lhcb::seed_smem_bytes(G.max_hits_per_half, G.max_xz_cand_per_half, G.max_triplets_per_half);
+  c->match_smem = lhcb::match_smem_bytes(G.max_seeds_per_half, G.max_match_cand_per_event, G.max_velo_per_event);
+  cudaError_t e = cudaSetDevice(device);
+  int max_optin = 0;
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
+  if (e != cudaSuccess) { c->last_cuda_error = (int)e; delete c; return LHCB_ERR_CUDA; }
+  if (c->seed_smem > (size_t)max_optin || c->match_smem > (size_t)max_optin) { delete c; return LHCB_ERR_CAPACITY; }
+  e = cudaFuncSetAttribute(lhcb::seeding_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->seed_smem);
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(lhcb::matching_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->match_smem);
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_P, sizeof(c->der.P));
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_Q, sizeof(c->der.Q));
+  if (e == cudaSuccess) e = cudaMemcpy(c->d_P, c->der.P, sizeof(c->der.P), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(c->d_Q, c->der.Q, sizeof(c->der.Q), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) {
+    cudaFree(c->d_P); cudaFree(c->d_Q);
+    delete c;
+    return LHCB_ERR_CUDA;
+  }
+  *out = c;
+  return LHCB_OK;
+}
+
+void lhcb_destroy(lhcb_ctx* c) {
+  if (!c) return;
+  cudaSetDevice(c->device);
+  cudaFree(c->d_P);
+  cudaFree(c->d_Q);
+  delete c;
+}
+
+int lhcb_get_geom(const lhcb_ctx* c, lhcb_geom_t* out) {
+  if (!c || !out) return LHCB_ERR_BAD_ARGUMENT;
+  *out = c->geom;
+  return LHCB_OK;
+}
+
+size_t lhcb_workspace_bytes(const lhcb_ctx* c, int n_events, size_t n_scifi_hits) {
+  (void)c; (void)n_events; (void)n_scifi_hits;
+  return 0;   // every intermediate lives in shared memory
+}
+
+int lhcb_seeding(lhcb_ctx* c, const lhcb_events_t* ev, lhcb_seeds_t* out, void* workspace, void* stream) {
+  (void)workspace;
+  if (!c) return LHCB_ERR_NOT_INITIALISED;
+  if (!ev || !out || ev->n_events < 0) return LHCB_ERR_BAD_ARGUMENT;
+  c->last_launches = 0;
+  if (ev->n_events == 0) return LHCB_OK;
+  if (!ev->zone_off || (!ev->hit_x && ev->n_hits) || !out->count || !out->state || !out->par || !out->hits ||
+      !out->nx || !out->nuv || !out->status)
+    return LHCB_ERR_BAD_ARGUMENT;
+  LHCB_CUDA(c, cudaSetDevice(c->device));
+  lhcb::SeedParams p;
+  fill_seed_params(c, p);
+  p.n_events = ev->n_events; p.n_hits = ev->n_hits; p.zone_off = ev->zone_off; p.hit_x = ev->hit_x;
+  p.pol = ev->polarity;
+  p.count = out->count; p.state = out->state; p.par = out->par; p.hits = out->hits; p.nx = out->nx;
+  p.nuv = out->nuv; p.status = out->status;
+  p.cap_total = (size_t)ev->n_events * 2 * (size_t)c->geom.max_seeds_per_half;
+  lhcb::seeding_kernel<<<ev->n_events * 2, lhcb::kSeedThreads, c->seed_smem, (cudaStream_t)stream>>>(p);
+  LHCB_CUDA(c, cudaGetLastError());
+  c->last_launches = 1;
+  return LHCB_OK;
+}
+
+int lhcb_matching(lhcb_ctx* c, const lhcb_seeds_t* seeds, const lhcb_velo_t* velo, const lhcb_ut_t* ut,
+                  lhcb_long_t* out, void* workspace, void* stream) {
+  (void)workspace;
+  if (!c) return LHCB_ERR_NOT_INITIALISED;
+  if (!seeds || !velo || !out || velo->n_events < 0 || seeds->n_events != velo->n_events)
+    return LHCB_ERR_BAD_ARGUMENT;
+  c->last_launches = 0;
+  if (velo->n_events == 0) return LHCB_OK;
+  if (!seeds->count || !seeds->state || !velo->off || !out->count || !out->seed_idx || !out->velo_idx ||
+      !out->ut_idx || !out->n_ut || !out->qop || !out->chi2 || !out->status)
+    return LHCB_ERR_BAD_ARGUMENT;
+  if (ut && (!ut->off || !ut->x0 || !ut->y_lo || !ut->y_hi)) return LHCB_ERR_BAD_ARGUMENT;
+  LHCB_CUDA(c, cudaSetDevice(c->device));
+  lhcb::MatchParams p;
+  fill_match_params(c, p);
+  p.use_ut = (c->geom.ut_enabled && ut) ? 1 : 0;
+  p.n_events = velo->n_events;
+  p.seed_count = seeds->count; p.state = seeds->state;
+  p.seed_cap_total = (size_t)velo->n_events * 2 * (size_t)c->geom.max_seeds_per_half;
+  p.velo_off = velo->off; p.vx = velo->x; p.vy = velo->y; p.vtx = velo->tx; p.vty = velo->ty; p.pol = velo->polarity;
+  if (ut) { p.ut_off = ut->off; p.ux = ut->x0; p.uylo = ut->y_lo; p.uyhi = ut->y_hi; }
+  p.count = out->count; p.seed_idx = out->seed_idx; p.velo_idx = out->velo_idx; p.ut_idx = out->ut_idx;
+  p.n_ut = out->n_ut; p.qop = out->qop; p.chi2 = out->chi2; p.status = out->status;
+  p.long_cap_total = (size_t)velo->n_events * (size_t)c->geom.max_long_per_event;
+  lhcb::matching_kernel<<<velo->n_events, lhcb::kMatchThreads, c->match_smem, (cudaStream_t)stream>>>(p);
+  LHCB_CUDA(c, cudaGetLastError());
+  c->last_launches = 1;
+  return LHCB_OK;
+}
+
+const char* lhcb_error_string(int s) {
+  switch (s) {
+    case LHCB_OK: return "ok";
+    case LHCB_ERR_BAD_ARGUMENT: return "bad argument";
+    case LHCB_ERR_BAD_GEOMETRY: return "bad geometry";
+    case LHCB_ERR_CUDA: return "CUDA runtime error";
+    case LHCB_ERR_NOT_INITIALISED: return "context not initialised";
+    case LHCB_ERR_CAPACITY: return "capacities exceed the shared memory of the device";
+    default: return "unknown status";
+  }
+}
+
+int lhcb_last_cuda_error(const lhcb_ctx* c) { return c ? c->last_cuda_error : 0; }
+int lhcb_last_launch_count(const lhcb_ctx* c) { return c ? c->last_launches : 0; }
+
+}  // extern "C"

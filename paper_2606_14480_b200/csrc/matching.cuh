@@ -1,0 +1,266 @@
+// VELO-SciFi Matching kernel (section 4) for sm_100a.
+//
+// One CTA per event.  The event's VELO states are staged in shared memory.
+//   M1/M2  warp per seed, lanes over VELO tracks: kink extrapolation (Eq. 17-18), preselection
+//          (Eq. 21), chi2_match (Eq. 22-23) < 2; accepted pairs are queued in shared memory
+//   M3     thread per queued pair: UT hit search (Eq. 19-20, Table 2)
+//   M4     one-to-one selection with two rounds of 64-bit atomicMin (reading A14), output
+//
+// Arithmetic follows DESIGN.md "Arithmetic specification"; compiled with -fmad=false.
+#pragma once
+#include <cstdint>
+
+#include "../../include/lhcb.h"
+#include "seeding.cuh"   // lower_bound, kNoKey
+
+namespace lhcb {
+
+constexpr int kMatchThreads = 256;
+
+struct MatchParams {
+  float zS, zV, dzyS, dzyV, mag[5], presel[4], cx0, cx1, cy0, cy1, inv_tol_tx, inv_tol_ty, chi2m_max;
+  float inv_KB, Ag, Bg, inv_Bg, ut_dz[4], ut_dz2[4], ut_dz4[4], ut_tan[4], ut_y_tol;
+  float ut_loose[4][4], ut_tight[4][4];
+  int min_ut_hits, use_ut, polarity;
+  int max_seeds, max_long, max_mc, max_velo;
+  // batch
+  int n_events;
+  const uint32_t* seed_count;
+  const float* state;
+  size_t seed_cap_total;
+  const uint32_t* velo_off;
+  const float *vx, *vy, *vtx, *vty;
+  const int8_t* pol;
+  const uint32_t* ut_off;
+  const float *ux, *uylo, *uyhi;
+  uint32_t* count;
+  uint32_t* seed_idx;
+  uint32_t* velo_idx;
+  uint32_t* ut_idx;
+  uint8_t* n_ut;
+  float* qop;
+  float* chi2;
+  uint32_t* status;
+  size_t long_cap_total;
+};
+
+struct __align__(16) MatchCand {
+  uint16_t seed, velo;      // event-local indices
+  float chi2, q0, gamma;
+  uint32_t ut[4];           // global UT hit indices
+  uint8_t n_ut, valid, pad[2];
+};
+
+__host__ __device__ inline size_t match_smem_bytes(int max_seeds, int max_mc, int max_velo) {
+  size_t b = 64;
+  b += (size_t)max_velo * 16;                // VELO states
+  b += (size_t)max_mc * sizeof(MatchCand);
+  b = (b + 7) & ~(size_t)7;
+  b += (size_t)2 * max_seeds * 8;            // best key per seed
+  b += (size_t)max_velo * 8;                 // best key per VELO track
+  return b;
+}
+
+struct UtHyp { int n; uint32_t idx[4]; float gamma, ssq; };
+
+__device__ __forceinline__ float ut_window(const float* w, float invpG) {
+  const float v = w[0] + w[1] * invpG;                      // L315
+  const float lo = v > w[2] ? v : w[2];
+  return lo < w[3] ? lo : w[3];
+}
+
+// O13: loose window until the first layer with hits; every loose hit starts a hypothesis (A13),
+// remaining layers use tight windows and the closest hit; gamma_x is refitted after each hit.
+__device__ inline bool ut_search(const MatchParams& p, float xV, float yV, float txV, float tyV, float q0,
+                                 const uint32_t* __restrict__ uo, UtHyp& best) {
+  const float invpG = fabsf(q0) * 1000.f;
+  const float gamma0 = p.Ag + p.Bg * q0;                    // Eq. 20
+  bool have = false;
+  for (int i0 = 0; i0 < 4; ++i0) {
+    if (4 - i0 < p.min_ut_hits) break;
+    const float yi = yV + tyV * p.ut_dz[i0];
+    const float xi = (xV + txV * p.ut_dz[i0]) + gamma0 * p.ut_dz2[i0];        // Eq. 19
+    const float x0e = xi - yi * p.ut_tan[i0];
+    const float w = ut_window(p.ut_loose[i0], invpG);
+    const float lo = x0e - w, hi = x0e + w;
+    const int b = (int)uo[i0], e = (int)uo[i0 + 1];
+    bool found = false;
+    for (int j = lower_bound(p.ux, b, e, lo); j < e && p.ux[j] <= hi; ++j) {
+      if (!(p.uylo[j] - p.ut_y_tol <= yi && yi <= p.uyhi[j] + p.ut_y_tol)) continue;
+      found = true;
+      UtHyp hy;
+      float dj[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) { hy.idx[k] = LHCB_NO_HIT; dj[k] = 0.f; }
+      hy.n = 1; hy.idx[i0] = (uint32_t)j;
+      dj[i0] = ((p.ux[j] + yi * p.ut_tan[i0]) - xV) - txV * p.ut_dz[i0];
+      float num = dj[i0] * p.ut_dz2[i0], den = p.ut_dz4[i0];
+      float gam = num / den;
+      for (int i = i0 + 1; i < 4; ++i) {
+        const float yt = yV + tyV * p.ut_dz[i];
+        const float xt = (xV + txV * p.ut_dz[i]) + gam * p.ut_dz2[i];
+        const float xe = xt - yt * p.ut_tan[i];
+        const float wt = ut_window(p.ut_tight[i], invpG);
+        const float tlo = xe - wt, thi = xe + wt;
+        const int bb = (int)uo[i], ee = (int)uo[i + 1];
+        int bj = -1;
+        float bd = 0.f;
+        for (int jj = lower_bound(p.ux, bb, ee, tlo); jj < ee && p.ux[jj] <= thi; ++jj) {
+          if (!(p.uylo[jj] - p.ut_y_tol <= yt && yt <= p.uyhi[jj] + p.ut_y_tol)) continue;
+          const float dd = fabsf(p.ux[jj] - xe);
+          if (bj < 0 || dd < bd) { bj = jj; bd = dd; }
+        }
+        if (bj >= 0) {
+          hy.idx[i] = (uint32_t)bj; ++hy.n;
+          dj[i] = ((p.ux[bj] + yt * p.ut_tan[i]) - xV) - txV * p.ut_dz[i];
+          num = num + dj[i] * p.ut_dz2[i]; den = den + p.ut_dz4[i];
+          gam = num / den;
+        }
+      }
+      hy.gamma = gam; hy.ssq = 0.f;
+      bool first = true;
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+        if (hy.idx[i] != LHCB_NO_HIT) {
+          const float res = dj[i] - gam * p.ut_dz2[i];
+          hy.ssq = first ? res * res : hy.ssq + res * res;
+          first = false;
+        }
+      if (!have || hy.n > best.n || (hy.n == best.n && hy.ssq < best.ssq)) { best = hy; have = true; }
+    }
+    if (found) break;
+  }
+  return have && best.n >= p.min_ut_hits;
+}
+
+__global__ void __launch_bounds__(kMatchThreads)
+matching_kernel(const __grid_constant__ MatchParams p) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  int* hdr = reinterpret_cast<int*>(smem);                  // [0] n_mc, [1] n_long, [2] status
+  float* svx = reinterpret_cast<float*>(smem + 64);
+  float* svy = svx + p.max_velo;
+  float* svtx = svy + p.max_velo;
+  float* svty = svtx + p.max_velo;
+  size_t off = 64 + (size_t)p.max_velo * 16;
+  MatchCand* mc = reinterpret_cast<MatchCand*>(smem + off);
+  off += (size_t)p.max_mc * sizeof(MatchCand);
+  off = (off + 7) & ~(size_t)7;
+  unsigned long long* seed_best = reinterpret_cast<unsigned long long*>(smem + off);
+  unsigned long long* velo_best = seed_best + 2 * p.max_seeds;
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = kMatchThreads / 32;
+  const int e = blockIdx.x;
+  const uint32_t v0 = p.velo_off[e];
+  const int nv = (int)(p.velo_off[e + 1] - v0);
+  int c0 = (int)p.seed_count[2 * e], c1 = (int)p.seed_count[2 * e + 1];
+  if (c0 > p.max_seeds) c0 = p.max_seeds;
+  if (c1 > p.max_seeds) c1 = p.max_seeds;
+  const int ns = c0 + c1;
+  if (nv > p.max_velo) {
+    if (tid == 0) { p.count[e] = 0; p.status[e] = LHCB_ST_VELO_OVERFLOW; }
+    return;
+  }
+  if (tid < 3) hdr[tid] = 0;
+  for (int v = tid; v < nv; v += kMatchThreads) {
+    svx[v] = p.vx[v0 + v]; svy[v] = p.vy[v0 + v]; svtx[v] = p.vtx[v0 + v]; svty[v] = p.vty[v0 + v];
+    velo_best[v] = kNoKey;
+  }
+  for (int s = tid; s < ns; s += kMatchThreads) seed_best[s] = kNoKey;
+  __syncthreads();
+
+  // ---- M1/M2: all seed x VELO pairs (L279) ---------------------------------------------------
+  const size_t sct = p.seed_cap_total;
+  for (int s = warp; s < ns; s += nwarps) {
+    const size_t slot = s < c0 ? (size_t)(2 * e) * p.max_seeds + s : (size_t)(2 * e + 1) * p.max_seeds + (s - c0);
+    const float xS = p.state[slot], yS = p.state[sct + slot], txS = p.state[2 * sct + slot],
+                tyS = p.state[3 * sct + slot];
+    const float axS = fabsf(xS);
+    const float ys = yS + p.dzyS * tyS;                                          // L231
+    for (int v = lane; v < nv; v += 32) {
+      const float xV = svx[v], yV = svy[v], txV = svtx[v], tyV = svty[v];
+      const float dtx = txS - txV, dty = tyS - tyV, adtx = fabsf(dtx);
+      const float zm = (((p.mag[0] + p.mag[1] * adtx) + p.mag[2] * (dtx * dtx)) + p.mag[3] * axS) +
+                       p.mag[4] * (txV * txV);                                   // Eq. 18
+      const float xs = xS + (zm - p.zS) * txS, xv = xV + (zm - p.zV) * txV;      // Eq. 17
+      const float yv = yV + p.dzyV * tyV;
+      const float dx = xs - xv, dy = ys - yv;
+      if (!(fabsf(dx) < p.presel[0] && fabsf(dy) < p.presel[1] && adtx < p.presel[2] &&
+            fabsf(dty) < p.presel[3]))                                           // Eq. 21
+        continue;
+      const float tolx = p.cx0 + p.cx1 * (dtx * dtx);                            // Eq. 23
+      const float toly = p.cy0 + p.cy1 * (txV * txV + tyV * tyV);
+      const float chi2 = (((dx * dx) / tolx + (dy * dy) / toly) + (dtx * dtx) * p.inv_tol_tx) +
+                         (dty * dty) * p.inv_tol_ty;                             // Eq. 22
+      if (!(chi2 < p.chi2m_max)) continue;                                       // L301
+      const int k = atomicAdd(&hdr[0], 1);
+      if (k < p.max_mc) {
+        MatchCand m;
+        m.seed = (uint16_t)s; m.velo = (uint16_t)v; m.chi2 = chi2; m.q0 = dtx * p.inv_KB; m.gamma = 0.f;
+        m.ut[0] = m.ut[1] = m.ut[2] = m.ut[3] = LHCB_NO_HIT;
+        m.n_ut = 0; m.valid = 1; m.pad[0] = m.pad[1] = 0;
+        mc[k] = m;
+      }
+    }
+  }
+  __syncthreads();
+  int nm = hdr[0];
+  if (nm > p.max_mc) { nm = p.max_mc; if (tid == 0) hdr[2] |= LHCB_ST_MATCH_OVERFLOW; }
+
+  // ---- M3: UT hits (O13) -----------------------------------------------------------------------
+  for (int k = tid; k < nm; k += kMatchThreads) {
+    MatchCand& m = mc[k];
+    if (p.use_ut) {
+      UtHyp hy;
+      hy.n = 0; hy.gamma = 0.f; hy.ssq = 0.f;
+      hy.idx[0] = hy.idx[1] = hy.idx[2] = hy.idx[3] = LHCB_NO_HIT;
+      const int v = m.velo;
+      const bool ok = ut_search(p, svx[v], svy[v], svtx[v], svty[v], m.q0, p.ut_off + (size_t)e * 4, hy);
+      m.valid = ok;
+      if (ok) {
+        m.n_ut = (uint8_t)hy.n; m.gamma = hy.gamma;
+        m.ut[0] = hy.idx[0]; m.ut[1] = hy.idx[1]; m.ut[2] = hy.idx[2]; m.ut[3] = hy.idx[3];
+      }
+    }
+    if (m.valid)
+      atomicMin(&seed_best[m.seed], ((unsigned long long)__float_as_uint(m.chi2) << 32) | m.velo);
+  }
+  __syncthreads();
+  // ---- M4: one-to-one selection (O14) -------------------------------------------------------------
+  for (int k = tid; k < nm; k += kMatchThreads) {
+    const MatchCand& m = mc[k];
+    if (!m.valid) continue;
+    const unsigned long long cb = (unsigned long long)__float_as_uint(m.chi2) << 32;
+    if (seed_best[m.seed] != (cb | m.velo)) continue;
+    atomicMin(&velo_best[m.velo], cb | m.seed);
+  }
+  __syncthreads();
+  const int pol = p.pol ? (int)p.pol[e] : p.polarity;
+  for (int k = tid; k < nm; k += kMatchThreads) {
+    const MatchCand& m = mc[k];
+    if (!m.valid) continue;
+    const unsigned long long cb = (unsigned long long)__float_as_uint(m.chi2) << 32;
+    if (seed_best[m.seed] != (cb | m.velo) || velo_best[m.velo] != (cb | m.seed)) continue;
+    const int slot = atomicAdd(&hdr[1], 1);
+    if (slot >= p.max_long) continue;
+    const size_t o = (size_t)e * p.max_long + slot, ct = p.long_cap_total;
+    const int s = m.seed;
+    p.seed_idx[o] = s < c0 ? (uint32_t)((2 * e) * p.max_seeds + s) : (uint32_t)((2 * e + 1) * p.max_seeds + (s - c0));
+    p.velo_idx[o] = v0 + m.velo;
+    p.ut_idx[0 * ct + o] = m.ut[0]; p.ut_idx[1 * ct + o] = m.ut[1];
+    p.ut_idx[2 * ct + o] = m.ut[2]; p.ut_idx[3 * ct + o] = m.ut[3];
+    p.n_ut[o] = m.n_ut;
+    const float q = p.use_ut ? (m.gamma - p.Ag) * p.inv_Bg : m.q0;               // Eq. 20 inverted / A10
+    p.qop[o] = pol > 0 ? q : -q;
+    p.chi2[o] = m.chi2;
+  }
+  __syncthreads();
+  if (tid == 0) {
+    int nl = hdr[1];
+    unsigned st = (unsigned)hdr[2];
+    if (nl > p.max_long) { nl = p.max_long; st |= LHCB_ST_LONG_OVERFLOW; }
+    p.count[e] = (uint32_t)nl;
+    p.status[e] = st;
+  }
+}
+
+}  // namespace lhcb
