@@ -419,26 +419,39 @@ def _cat_off(chunks, key, sub=None):
     return np.concatenate(out).astype(np.uint32)
 
 
-def generate(cfg: GenConfig, geom: Optional[dict] = None) -> Events:
+def _run_chunk(args):
+    cfg, geom, k, e0, n = args
+    rng = np.random.Generator(np.random.PCG64(np.random.SeedSequence([cfg.seed, k])))
+    fn = _gen_chunk_direct if cfg.direct_seeds else _gen_chunk
+    return fn(cfg, geom, rng, n, e0)
+
+
+def generate(cfg: GenConfig, geom: Optional[dict] = None, workers: int = 1, first_chunk: int = 0) -> Events:
     """Generate cfg.n_events events, in independent chunks of CHUNK events.
 
-    Chunk k draws from numpy's PCG64 seeded with SeedSequence([cfg.seed, k]), so the first
-    n events of a config do not depend on how many follow them (cfg3 batch slicing).
+    Chunk k draws from numpy's PCG64 seeded with SeedSequence([cfg.seed, k]), so a full chunk does
+    not depend on how many chunks follow it (cfg3 batch slicing).  `first_chunk` shifts the chunk
+    indices (rank r of a multi-GPU run takes its own chunk range).  `workers` > 1 generates chunks
+    in parallel processes; the result is identical.
     """
     geom = default_geom() if geom is None else geom
-    chunks, pid_base = [], 0
-    for k, e0 in enumerate(range(0, cfg.n_events, CHUNK)):
-        n = min(CHUNK, cfg.n_events - e0)
-        rng = np.random.Generator(np.random.PCG64(np.random.SeedSequence([cfg.seed, k])))
-        fn = _gen_chunk_direct if cfg.direct_seeds else _gen_chunk
-        c = fn(cfg, geom, rng, n, e0)
+    jobs = []
+    for j, e0 in enumerate(range(0, cfg.n_events, CHUNK)):
+        jobs.append((cfg, geom, first_chunk + j, first_chunk * CHUNK + e0, min(CHUNK, cfg.n_events - e0)))
+    if workers > 1 and len(jobs) > 1:
+        import multiprocessing as mp
+        with mp.get_context("fork").Pool(min(workers, len(jobs))) as pool:
+            chunks = pool.map(_run_chunk, jobs)
+    else:
+        chunks = [_run_chunk(j) for j in jobs]
+    pid_base = 0
+    for c in chunks:
         for key in ("hit_pid", "velo_pid", "seed_pid"):
             if key in c and c[key] is not None:
                 c[key] = np.where(c[key] >= 0, c[key] + pid_base, -1).astype(np.int32)
         u = list(c["ut"]); u[4] = np.where(u[4] >= 0, u[4] + pid_base, -1).astype(np.int32)
         c["ut"] = tuple(u)
         pid_base += c["n_particles"]
-        chunks.append(c)
 
     cat = lambda key: np.concatenate([c[key] for c in chunks])
     hit_x64 = cat("hit_x64")

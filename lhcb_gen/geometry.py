@@ -79,10 +79,14 @@ DEFAULT_GEOM = {
     "ut_y_tol": 1.0,            # DESIGN.md O13
     "min_ut_hits": 3,           # L311 ("more than two")
     "ut_enabled": 1,
-    # --- capacities (per event-half / per event) ------------------------------
-    "max_seeds_per_half": 256,
-    "max_xz_cand_per_half": 2048,
-    "max_long_per_event": 256,
+    # --- capacities (per event-half / per event); 0 = library default (include/lhcb.h) ---------
+    "max_seeds_per_half": 0,
+    "max_xz_cand_per_half": 0,
+    "max_long_per_event": 0,
+    "max_hits_per_half": 0,
+    "max_triplets_per_half": 0,
+    "max_match_cand_per_event": 0,
+    "max_velo_per_event": 0,
 }
 
 
