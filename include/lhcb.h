@@ -185,6 +185,23 @@ int lhcb_seeding(lhcb_ctx* ctx, const lhcb_events_t* events, lhcb_seeds_t* out, 
 int lhcb_matching(lhcb_ctx* ctx, const lhcb_seeds_t* seeds, const lhcb_velo_t* velo, const lhcb_ut_t* ut,
                   lhcb_long_t* out, void* workspace, void* cuda_stream);
 
+/* ---- host-buffer pipeline (end-to-end path: H2D copies + seeding + matching + D2H copies) ---------
+ * A pipeline owns device buffers sized at creation and two CUDA streams.  lhcb_reconstruct_host takes
+ * the SAME descriptor structs as above but with HOST pointers (pinned memory for full copy/compute
+ * overlap; pageable memory works, slower), splits the batch into event slices, and overlaps the
+ * copies of one slice with the kernels of another.  It blocks until every output has landed in the
+ * caller's host arrays.  Outputs: `out` (host arrays laid out for the whole batch, cap_total =
+ * n_events*max_long_per_event) and, if non-NULL, seed_count[n_events*2].  The seeds themselves stay on
+ * the device.  Returns LHCB_ERR_CAPACITY if the batch exceeds the sizes given at creation. */
+typedef struct lhcb_pipeline lhcb_pipeline;
+int lhcb_pipeline_create(lhcb_ctx* ctx, int max_events, size_t max_scifi_hits, size_t max_velo, size_t max_ut_hits,
+                         int slice_events, lhcb_pipeline** out);
+void lhcb_pipeline_destroy(lhcb_pipeline* p);
+int lhcb_reconstruct_host(lhcb_pipeline* p, const lhcb_events_t* host_events, const lhcb_velo_t* host_velo,
+                          const lhcb_ut_t* host_ut, lhcb_long_t* host_out, uint32_t* host_seed_count);
+/* bytes moved by the last lhcb_reconstruct_host call */
+int lhcb_pipeline_last_bytes(const lhcb_pipeline* p, uint64_t* h2d, uint64_t* d2h);
+
 const char* lhcb_error_string(int status);
 /* cudaError_t of the last failing CUDA call made through this context (0 if none). */
 int lhcb_last_cuda_error(const lhcb_ctx* ctx);

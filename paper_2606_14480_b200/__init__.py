@@ -3,6 +3,6 @@
 The product is the C-ABI CUDA library declared in include/lhcb.h (sources in csrc/); this package is
 its thin Python binding.  There is no CPU fallback.
 """
-from .binding import Context, DeviceEvents, lhcb_geom_derive, load_library, NO_HIT, EXPORTS
+from .binding import Context, DeviceEvents, HostPipeline, lhcb_geom_derive, load_library, NO_HIT, EXPORTS
 
-__all__ = ["Context", "DeviceEvents", "lhcb_geom_derive", "load_library", "NO_HIT", "EXPORTS"]
+__all__ = ["Context", "DeviceEvents", "HostPipeline", "lhcb_geom_derive", "load_library", "NO_HIT", "EXPORTS"]

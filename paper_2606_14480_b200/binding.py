@@ -23,7 +23,8 @@ ST_BITS = {1: "triplet_overflow", 2: "cand_overflow", 4: "seed_overflow", 8: "hi
 
 EXPORTS = ["lhcb_geom_derive", "lhcb_geom_init", "lhcb_destroy", "lhcb_get_geom", "lhcb_workspace_bytes",
            "lhcb_seeding", "lhcb_matching", "lhcb_error_string", "lhcb_last_cuda_error",
-           "lhcb_last_launch_count"]
+           "lhcb_last_launch_count", "lhcb_pipeline_create", "lhcb_pipeline_destroy", "lhcb_reconstruct_host",
+           "lhcb_pipeline_last_bytes"]
 
 
 class LhcbGeom(C.Structure):
@@ -128,6 +129,12 @@ def load_library(build: bool = True) -> C.CDLL:
         lib.lhcb_error_string.restype = C.c_char_p
         lib.lhcb_last_cuda_error.argtypes = [VP]
         lib.lhcb_last_launch_count.argtypes = [VP]
+        lib.lhcb_pipeline_create.argtypes = [VP, C.c_int, C.c_size_t, C.c_size_t, C.c_size_t, C.c_int, C.POINTER(VP)]
+        lib.lhcb_pipeline_destroy.argtypes = [VP]
+        lib.lhcb_pipeline_destroy.restype = None
+        lib.lhcb_reconstruct_host.argtypes = [VP, C.POINTER(LhcbEvents), C.POINTER(LhcbVelo), C.POINTER(LhcbUt),
+                                              C.POINTER(LhcbLong), VP]
+        lib.lhcb_pipeline_last_bytes.argtypes = [VP, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
         _LIB = lib
     return _LIB
 
@@ -331,3 +338,71 @@ class Context:
         return dict(n=len(slot), event=ev, seed=g("seed_idx").view(np.uint32)[slot], velo=g("velo_idx").view(np.uint32)[slot],
                     ut=g("ut_idx").view(np.uint32)[:, slot].T, n_ut=g("n_ut")[slot], qop=g("qop")[slot],
                     chi2=g("chi2")[slot], status=g("status").view(np.uint32))
+
+
+class HostPipeline:
+    """lhcb_pipeline_create / lhcb_reconstruct_host: host buffers in, host buffers out (the end-to-end
+    path: H2D copies, seeding, matching and D2H copies all inside one C-ABI call)."""
+
+    def __init__(self, ctx: Context, ev, slice_events: int = 2048, use_ut: bool = True):
+        """ev: a host batch (lhcb_gen.Events-like).  Its arrays are copied once into pinned host memory;
+        the pipeline's device buffers are sized for this batch."""
+        import torch
+        self.ctx, self.torch = ctx, torch
+        self.n_events = ev.n_events
+
+        def pin(a, dt):
+            a = np.ascontiguousarray(a, dt)
+            t = torch.from_numpy(a.view(np.int32) if dt == np.uint32 else a)
+            return t.pin_memory() if len(a) else t
+        self.h = dict(zone_off=pin(ev.zone_off, np.uint32), hit_x=pin(ev.hit_x, np.float32),
+                      polarity=pin(ev.polarity, np.int8), velo_off=pin(ev.velo_off, np.uint32),
+                      velo_x=pin(ev.velo_x, np.float32), velo_y=pin(ev.velo_y, np.float32),
+                      velo_tx=pin(ev.velo_tx, np.float32), velo_ty=pin(ev.velo_ty, np.float32))
+        self.has_ut = use_ut and len(ev.ut_x0) > 0
+        if self.has_ut:
+            self.h.update(ut_off=pin(ev.ut_off, np.uint32), ut_x0=pin(ev.ut_x0, np.float32),
+                          ut_ylo=pin(ev.ut_ylo, np.float32), ut_yhi=pin(ev.ut_yhi, np.float32))
+        n, cap = ev.n_events, ev.n_events * ctx.max_long
+        z = lambda shape, dt: torch.zeros(shape, dtype=dt).pin_memory()
+        self.out = dict(n_events=n, cap_total=cap, count=z(n, torch.int32), seed_idx=z(cap, torch.int32),
+                        velo_idx=z(cap, torch.int32), ut_idx=z((4, cap), torch.int32), n_ut=z(cap, torch.uint8),
+                        qop=z(cap, torch.float32), chi2=z(cap, torch.float32), status=z(n, torch.int32))
+        self.seed_count = z(2 * n, torch.int32)
+        self._p = VP(0)
+        rc = ctx.lib.lhcb_pipeline_create(ctx._ctx, n, ev.n_hits, len(ev.velo_x),
+                                          len(ev.ut_x0) if self.has_ut else 0, slice_events, C.byref(self._p))
+        _check(ctx.lib, ctx._ctx, rc, "lhcb_pipeline_create")
+        h = self.h
+        self._ev = LhcbEvents(n, ev.n_hits, _ptr(h["zone_off"]), _ptr(h["hit_x"]), _ptr(h["polarity"]))
+        self._velo = LhcbVelo(n, _ptr(h["velo_off"]), _ptr(h["velo_x"]), _ptr(h["velo_y"]), _ptr(h["velo_tx"]),
+                              _ptr(h["velo_ty"]), _ptr(h["polarity"]))
+        self._ut = LhcbUt(_ptr(h["ut_off"]), _ptr(h["ut_x0"]), _ptr(h["ut_ylo"]), _ptr(h["ut_yhi"])) if self.has_ut else None
+        o = self.out
+        self._long = LhcbLong(_ptr(o["count"]), _ptr(o["seed_idx"]), _ptr(o["velo_idx"]), _ptr(o["ut_idx"]),
+                              _ptr(o["n_ut"]), _ptr(o["qop"]), _ptr(o["chi2"]), _ptr(o["status"]))
+
+    def lhcb_reconstruct_host(self):
+        """One end-to-end pass; returns (h2d_bytes, d2h_bytes, kernel launches).  Results are in self.out."""
+        lib = self.ctx.lib
+        rc = lib.lhcb_reconstruct_host(self._p, C.byref(self._ev), C.byref(self._velo),
+                                       C.byref(self._ut) if self._ut is not None else None, C.byref(self._long),
+                                       _ptr(self.seed_count))
+        _check(lib, self.ctx._ctx, rc, "lhcb_reconstruct_host")
+        a, b = C.c_uint64(0), C.c_uint64(0)
+        launches = lib.lhcb_pipeline_last_bytes(self._p, C.byref(a), C.byref(b))
+        return a.value, b.value, launches
+
+    def long_to_host(self):
+        return self.ctx.long_to_host(self.out)
+
+    def close(self):
+        if self._p.value:
+            self.ctx.lib.lhcb_pipeline_destroy(self._p)
+            self._p = VP(0)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

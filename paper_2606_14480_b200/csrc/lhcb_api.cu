@@ -216,3 +216,169 @@ int lhcb_last_cuda_error(const lhcb_ctx* c) { return c ? c->last_cuda_error : 0;
 int lhcb_last_launch_count(const lhcb_ctx* c) { return c ? c->last_launches : 0; }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// Host-buffer pipeline: slices of events, two streams, copies of one slice overlap kernels of another.
+struct lhcb_pipeline {
+  lhcb_ctx* ctx;
+  int max_events, slice;
+  size_t max_hits, max_velo, max_ut;
+  cudaStream_t st[2];
+  // inputs (whole batch, same offsets as on the host)
+  uint32_t *zone_off, *velo_off, *ut_off;
+  float *hit_x, *vx, *vy, *vtx, *vty, *ux, *uylo, *uyhi;
+  int8_t* pol;
+  // per-stream seeds and long-track buffers (one slice each)
+  struct Slot {
+    uint32_t *s_count, *s_hits, *s_status; float *s_state, *s_par; uint8_t *s_nx, *s_nuv;
+    uint32_t *l_count, *l_seed, *l_velo, *l_ut, *l_status; uint8_t* l_nut; float *l_qop, *l_chi2;
+  } slot[2];
+  uint64_t h2d, d2h;
+  int launches;
+};
+
+namespace {
+template <class T>
+cudaError_t dalloc(T** p, size_t n) { return cudaMalloc((void**)p, (n ? n : 1) * sizeof(T)); }
+}  // namespace
+
+extern "C" {
+
+void lhcb_pipeline_destroy(lhcb_pipeline* p) {
+  if (!p) return;
+  cudaSetDevice(p->ctx->device);
+  for (int i = 0; i < 2; ++i) {
+    if (p->st[i]) { cudaStreamSynchronize(p->st[i]); cudaStreamDestroy(p->st[i]); }
+    lhcb_pipeline::Slot& s = p->slot[i];
+    cudaFree(s.s_count); cudaFree(s.s_hits); cudaFree(s.s_status); cudaFree(s.s_state); cudaFree(s.s_par);
+    cudaFree(s.s_nx); cudaFree(s.s_nuv); cudaFree(s.l_count); cudaFree(s.l_seed); cudaFree(s.l_velo);
+    cudaFree(s.l_ut); cudaFree(s.l_status); cudaFree(s.l_nut); cudaFree(s.l_qop); cudaFree(s.l_chi2);
+  }
+  cudaFree(p->zone_off); cudaFree(p->velo_off); cudaFree(p->ut_off); cudaFree(p->hit_x); cudaFree(p->vx);
+  cudaFree(p->vy); cudaFree(p->vtx); cudaFree(p->vty); cudaFree(p->ux); cudaFree(p->uylo); cudaFree(p->uyhi);
+  cudaFree(p->pol);
+  delete p;
+}
+
+int lhcb_pipeline_create(lhcb_ctx* c, int max_events, size_t max_hits, size_t max_velo, size_t max_ut,
+                         int slice_events, lhcb_pipeline** out) {
+  if (!c) return LHCB_ERR_NOT_INITIALISED;
+  if (!out || max_events <= 0 || slice_events <= 0) return LHCB_ERR_BAD_ARGUMENT;
+  *out = nullptr;
+  LHCB_CUDA(c, cudaSetDevice(c->device));
+  lhcb_pipeline* p = new (std::nothrow) lhcb_pipeline();
+  if (!p) return LHCB_ERR_BAD_ARGUMENT;
+  std::memset(p, 0, sizeof(*p));
+  p->ctx = c; p->max_events = max_events; p->slice = slice_events < max_events ? slice_events : max_events;
+  p->max_hits = max_hits; p->max_velo = max_velo; p->max_ut = max_ut;
+  const size_t ms = c->geom.max_seeds_per_half, ml = c->geom.max_long_per_event, sl = p->slice;
+  cudaError_t e = cudaSuccess;
+  auto ok = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+  for (int i = 0; i < 2; ++i) ok(cudaStreamCreateWithFlags(&p->st[i], cudaStreamNonBlocking));
+  ok(dalloc(&p->zone_off, (size_t)max_events * 24 + 1)); ok(dalloc(&p->velo_off, (size_t)max_events + 1));
+  ok(dalloc(&p->ut_off, (size_t)max_events * 4 + 1)); ok(dalloc(&p->hit_x, max_hits + 4));
+  ok(dalloc(&p->vx, max_velo)); ok(dalloc(&p->vy, max_velo)); ok(dalloc(&p->vtx, max_velo)); ok(dalloc(&p->vty, max_velo));
+  ok(dalloc(&p->ux, max_ut)); ok(dalloc(&p->uylo, max_ut)); ok(dalloc(&p->uyhi, max_ut));
+  ok(dalloc(&p->pol, (size_t)max_events));
+  for (int i = 0; i < 2; ++i) {
+    lhcb_pipeline::Slot& s = p->slot[i];
+    const size_t cs = sl * 2 * ms, cl = sl * ml;
+    ok(dalloc(&s.s_count, sl * 2)); ok(dalloc(&s.s_status, sl * 2)); ok(dalloc(&s.s_state, 5 * cs));
+    ok(dalloc(&s.s_par, 7 * cs)); ok(dalloc(&s.s_hits, 12 * cs)); ok(dalloc(&s.s_nx, cs)); ok(dalloc(&s.s_nuv, cs));
+    ok(dalloc(&s.l_count, sl)); ok(dalloc(&s.l_status, sl)); ok(dalloc(&s.l_seed, cl)); ok(dalloc(&s.l_velo, cl));
+    ok(dalloc(&s.l_ut, 4 * cl)); ok(dalloc(&s.l_nut, cl)); ok(dalloc(&s.l_qop, cl)); ok(dalloc(&s.l_chi2, cl));
+  }
+  if (e != cudaSuccess) { c->last_cuda_error = (int)e; lhcb_pipeline_destroy(p); return LHCB_ERR_CUDA; }
+  *out = p;
+  return LHCB_OK;
+}
+
+int lhcb_reconstruct_host(lhcb_pipeline* p, const lhcb_events_t* ev, const lhcb_velo_t* velo, const lhcb_ut_t* ut,
+                          lhcb_long_t* out, uint32_t* host_seed_count) {
+  if (!p) return LHCB_ERR_NOT_INITIALISED;
+  lhcb_ctx* c = p->ctx;
+  if (!ev || !velo || !out || ev->n_events < 0 || velo->n_events != ev->n_events || !ev->zone_off || !velo->off ||
+      !out->count || !out->seed_idx || !out->velo_idx || !out->ut_idx || !out->n_ut || !out->qop || !out->chi2 ||
+      !out->status)
+    return LHCB_ERR_BAD_ARGUMENT;
+  const int n = ev->n_events;
+  p->h2d = p->d2h = 0; p->launches = 0;
+  if (n == 0) return LHCB_OK;
+  if (n > p->max_events || ev->n_hits > p->max_hits) return LHCB_ERR_CAPACITY;
+  const size_t n_velo = velo->off[n];
+  const size_t n_ut = ut ? ut->off[(size_t)n * 4] : 0;
+  if (n_velo > p->max_velo || n_ut > p->max_ut) return LHCB_ERR_CAPACITY;
+  LHCB_CUDA(c, cudaSetDevice(c->device));
+  const size_t ms = c->geom.max_seeds_per_half, ml = c->geom.max_long_per_event;
+  const size_t ct_all = (size_t)n * ml;
+  auto H2D = [&](void* d, const void* h, size_t bytes, cudaStream_t s) {
+    p->h2d += bytes;
+    return bytes ? cudaMemcpyAsync(d, h, bytes, cudaMemcpyHostToDevice, s) : cudaSuccess;
+  };
+  auto D2H = [&](void* h, const void* d, size_t bytes, cudaStream_t s) {
+    p->d2h += bytes;
+    return bytes ? cudaMemcpyAsync(h, d, bytes, cudaMemcpyDeviceToHost, s) : cudaSuccess;
+  };
+  int k = 0;
+  for (int e0 = 0; e0 < n; e0 += p->slice, ++k) {
+    const int ne = (n - e0) < p->slice ? (n - e0) : p->slice;
+    cudaStream_t s = p->st[k & 1];
+    lhcb_pipeline::Slot& S = p->slot[k & 1];
+    // ---- inputs of this slice, at the same offsets as on the host
+    const size_t z0 = (size_t)e0 * 24, z1 = (size_t)(e0 + ne) * 24;
+    const size_t h0 = ev->zone_off[z0], h1 = ev->zone_off[z1];
+    const size_t v0 = velo->off[e0], v1 = velo->off[e0 + ne];
+    LHCB_CUDA(c, H2D(p->zone_off + z0, ev->zone_off + z0, (z1 - z0 + 1) * 4, s));
+    LHCB_CUDA(c, H2D(p->hit_x + h0, ev->hit_x + h0, (h1 - h0) * 4, s));
+    if (ev->polarity) LHCB_CUDA(c, H2D(p->pol + e0, ev->polarity + e0, (size_t)ne, s));
+    LHCB_CUDA(c, H2D(p->velo_off + e0, velo->off + e0, ((size_t)ne + 1) * 4, s));
+    LHCB_CUDA(c, H2D(p->vx + v0, velo->x + v0, (v1 - v0) * 4, s));
+    LHCB_CUDA(c, H2D(p->vy + v0, velo->y + v0, (v1 - v0) * 4, s));
+    LHCB_CUDA(c, H2D(p->vtx + v0, velo->tx + v0, (v1 - v0) * 4, s));
+    LHCB_CUDA(c, H2D(p->vty + v0, velo->ty + v0, (v1 - v0) * 4, s));
+    if (ut) {
+      const size_t u0 = ut->off[(size_t)e0 * 4], u1 = ut->off[(size_t)(e0 + ne) * 4];
+      LHCB_CUDA(c, H2D(p->ut_off + (size_t)e0 * 4, ut->off + (size_t)e0 * 4, ((size_t)ne * 4 + 1) * 4, s));
+      LHCB_CUDA(c, H2D(p->ux + u0, ut->x0 + u0, (u1 - u0) * 4, s));
+      LHCB_CUDA(c, H2D(p->uylo + u0, ut->y_lo + u0, (u1 - u0) * 4, s));
+      LHCB_CUDA(c, H2D(p->uyhi + u0, ut->y_hi + u0, (u1 - u0) * 4, s));
+    }
+    // ---- kernels
+    lhcb_events_t dev_ev = {ne, (uint32_t)p->max_hits, p->zone_off + z0, p->hit_x, ev->polarity ? p->pol + e0 : nullptr};
+    dev_ev.n_hits = ev->n_hits;
+    lhcb_seeds_t dev_s = {ne, S.s_count, S.s_state, S.s_par, S.s_hits, S.s_nx, S.s_nuv, S.s_status};
+    int rc = lhcb_seeding(c, &dev_ev, &dev_s, nullptr, s);
+    if (rc != LHCB_OK) return rc;
+    p->launches += c->last_launches;
+    lhcb_velo_t dev_v = {ne, p->velo_off + e0, p->vx, p->vy, p->vtx, p->vty, ev->polarity ? p->pol + e0 : nullptr};
+    lhcb_ut_t dev_u = {p->ut_off + (size_t)e0 * 4, p->ux, p->uylo, p->uyhi};
+    lhcb_long_t dev_l = {S.l_count, S.l_seed, S.l_velo, S.l_ut, S.l_nut, S.l_qop, S.l_chi2, S.l_status};
+    rc = lhcb_matching(c, &dev_s, &dev_v, ut ? &dev_u : nullptr, &dev_l, nullptr, s);
+    if (rc != LHCB_OK) return rc;
+    p->launches += c->last_launches;
+    // ---- outputs of this slice
+    const size_t o = (size_t)e0 * ml, cl = (size_t)ne * ml;
+    LHCB_CUDA(c, D2H(out->count + e0, S.l_count, (size_t)ne * 4, s));
+    LHCB_CUDA(c, D2H(out->status + e0, S.l_status, (size_t)ne * 4, s));
+    LHCB_CUDA(c, D2H(out->seed_idx + o, S.l_seed, cl * 4, s));
+    LHCB_CUDA(c, D2H(out->velo_idx + o, S.l_velo, cl * 4, s));
+    for (int l = 0; l < 4; ++l) LHCB_CUDA(c, D2H(out->ut_idx + (size_t)l * ct_all + o, S.l_ut + (size_t)l * cl, cl * 4, s));
+    LHCB_CUDA(c, D2H(out->n_ut + o, S.l_nut, cl, s));
+    LHCB_CUDA(c, D2H(out->qop + o, S.l_qop, cl * 4, s));
+    LHCB_CUDA(c, D2H(out->chi2 + o, S.l_chi2, cl * 4, s));
+    if (host_seed_count) LHCB_CUDA(c, D2H(host_seed_count + (size_t)e0 * 2, S.s_count, (size_t)ne * 8, s));
+  }
+  LHCB_CUDA(c, cudaStreamSynchronize(p->st[0]));
+  LHCB_CUDA(c, cudaStreamSynchronize(p->st[1]));
+  (void)ms;
+  return LHCB_OK;
+}
+
+int lhcb_pipeline_last_bytes(const lhcb_pipeline* p, uint64_t* h2d, uint64_t* d2h) {
+  if (!p) return LHCB_ERR_NOT_INITIALISED;
+  if (h2d) *h2d = p->h2d;
+  if (d2h) *d2h = p->d2h;
+  return p->launches;
+}
+
+}  // extern "C"
