@@ -3,14 +3,17 @@
 // One CTA per event-half (L372): the half's twelve sorted hit zones are staged into shared memory
 // with one bulk async copy (cp.async.bulk + mbarrier) and stay there for every step (L370).
 // Stages, separated by __syncthreads():
-//   S1  two-hit + three-hit search     warp per T1 hit, lanes over the T3 window (Eq. 8-11),
-//                                      per pair Eq. 3-5 and the T2 band (Eq. 12-13, A3/A4);
-//                                      triplets are queued in shared memory
+//   S0  staging + bin tables           per zone, a 256-bin table "first hit with bin >= k" turns every
+//                                      lower/upper bound into one lookup plus a short forward scan
+//   S1  two-hit + three-hit search     thread per T1 hit finds its T3 window (Eq. 8-11); a block scan
+//                                      flattens all pairs; each thread walks a contiguous chunk of
+//                                      pairs: Eq. 3-5 and the T2 band (Eq. 12-13, A3/A4); triplets are
+//                                      queued in shared memory
 //   S2  extension + fit                thread per queued triplet: exact parabola, +-1 mm closest hit in
 //                                      the other three x-layers, >=5 hits, fixed-matrix least squares (L90)
 //   S3  clone kill                     64-bit atomicMin table per x-hit, vote pass (L183-200, Eq. 15)
-//   S4  u/v addition                   8-lane group per (survivor, pass), lanes over first-layer hits
-//                                      (Eq. 16); best combination by packed-key min
+//   S4  u/v addition                   (survivor, pass, first-layer hit) items flattened the same way
+//                                      (Eq. 16); best combination by packed-key atomicMin
 //   S5  seed output                    thread per survivor: rebuild the winning combination, y fit, store
 //
 // Arithmetic: every formula follows DESIGN.md "Arithmetic specification" operation by operation;
@@ -23,7 +26,7 @@
 namespace lhcb {
 
 constexpr int kSeedThreads = 256;
-constexpr int kUvGroup = 8;
+constexpr int kLutBins = 256;                 // bins of the per-zone search table
 constexpr unsigned long long kNoKey = ~0ull;
 
 struct SeedParams {
@@ -58,27 +61,63 @@ struct SeedParams {
 struct __align__(8) Triplet { uint16_t i1, i2, i3, it; };                 // zone-local indices
 struct __align__(16) Cand { float ax, bx, cx, chi2; uint16_t hit[6]; uint8_t nx, it, keep, pad; };
 
+struct __align__(16) Zone { int b, e; float x0, invw; };   // one 16-byte shared-memory load
+
 struct SeedSmemHeader {
   unsigned long long mbar;
   int zl[13];          // zone offsets relative to the staged tile
   int xbase[7];        // prefix of x-zone sizes (clone-table index base per x-slot)
+  Zone zi[12];         // per zone: [b, e) in the tile and bin(v) = clamp((v - x0) * invw, 0, kLutBins-1)
   int n_trip, n_cand, n_kept, n_seed;
   unsigned int status;
+  int warp_sums[kSeedThreads / 32 + 1];
 };
 
+constexpr int kSeedHeaderBytes = 512;
+static_assert(sizeof(SeedSmemHeader) <= kSeedHeaderBytes, "shared-memory header overflows its slot");
+
+// work-list scratch of the flattened loops: exclusive offsets + first index of one tile of owners
+struct SeedScan { int offs[kSeedThreads + 1]; uint16_t first[kSeedThreads]; };
+
 __host__ __device__ inline size_t seed_smem_bytes(int max_hits, int max_cand, int max_trip) {
-  size_t b = 256;                                          // header
+  size_t b = kSeedHeaderBytes;                             // header
   b += ((size_t)max_hits + 8) * 4;                         // hits tile (16-byte aligned superset)
   b = (b + 15) & ~(size_t)15;
   b += (size_t)max_cand * sizeof(Cand);
   b += (size_t)max_cand * 2;                               // kept list
   b = (b + 15) & ~(size_t)15;
   b += (size_t)max_trip * 8;                               // triplet queue / clone table / best keys
+  b += 12 * (kLutBins + 1) * 2;                            // bin tables
+  b = (b + 15) & ~(size_t)15;
+  b += sizeof(SeedScan);
   return b;
 }
 
 // ------------------------------------------------------------------------------------ searches
+// Sorted zone + bin table.  lut[k] = first tile index whose bin is >= k (lut[kLutBins] = zone end).
+// bin() is monotone in v, so every hit before lut[bin(v)] is < v: the exact lower/upper bound is
+// lut[bin(v)] plus a forward scan inside one bin (about one hit per bin).  Pure comparisons: the
+// result is identical to a binary search, whatever the rounding of bin().
+__device__ __forceinline__ int zone_bin(const Zone& z, float v) {
+  float t = (v - z.x0) * z.invw;
+  t = fminf(fmaxf(t, 0.f), (float)(kLutBins - 1));
+  return (int)t;
+}
 // first index in [b, e) with x[i] >= v
+__device__ __forceinline__ int lower_bound(const float* __restrict__ x, const uint16_t* __restrict__ lut,
+                                           const Zone& z, float v) {
+  int i = lut[zone_bin(z, v)];
+  while (i < z.e && x[i] < v) ++i;
+  return i;
+}
+// first index in [b, e) with x[i] > v
+__device__ __forceinline__ int upper_bound(const float* __restrict__ x, const uint16_t* __restrict__ lut,
+                                           const Zone& z, float v) {
+  int i = lut[zone_bin(z, v)];
+  while (i < z.e && x[i] <= v) ++i;
+  return i;
+}
+// plain binary searches (global-memory arrays without a bin table)
 __device__ __forceinline__ int lower_bound(const float* __restrict__ x, int b, int e, float v) {
   int n = e - b;
   while (n > 0) {
@@ -89,34 +128,61 @@ __device__ __forceinline__ int lower_bound(const float* __restrict__ x, int b, i
   }
   return b;
 }
-// first index in [b, e) with x[i] > v
-__device__ __forceinline__ int upper_bound(const float* __restrict__ x, int b, int e, float v) {
-  int n = e - b;
-  while (n > 0) {
+// largest t in [0, n) with offs[t] <= p (offs ascending, offs[0] = 0 <= p)
+__device__ __forceinline__ int owner_of(const int* offs, int n, int p) {
+  int b = 0;
+  while (n > 1) {
     const int h = n >> 1;
-    const bool le = x[b + h] <= v;
-    b = le ? b + h + 1 : b;
-    n = le ? n - h - 1 : h;
+    const bool le = offs[b + h] <= p;
+    b = le ? b + h : b;
+    n = le ? n - h : h;
   }
   return b;
 }
 // index of the hit closest to xp with |x - xp| <= tol, ties to the lower index; -1 if none
-__device__ __forceinline__ int closest_hit(const float* __restrict__ x, int b, int e, float xp, float tol) {
-  const int j = lower_bound(x, b, e, xp);
+__device__ __forceinline__ int closest_hit(const float* __restrict__ x, const uint16_t* __restrict__ lut,
+                                           const Zone& z, float xp, float tol) {
+  const int j = lower_bound(x, lut, z, xp);
   int best = -1;
   float bd = 0.f;
-  if (j > b) {
+  if (j > z.b) {
     int l = j - 1;
     const float xl = x[l];
-    while (l > b && x[l - 1] == xl) --l;     // equal x: the lower index wins
+    while (l > z.b && x[l - 1] == xl) --l;     // equal x: the lower index wins
     const float d = fabsf(xl - xp);
     if (d <= tol) { best = l; bd = d; }
   }
-  if (j < e) {
+  if (j < z.e) {
     const float d = fabsf(x[j] - xp);
     if (d <= tol && (best < 0 || d < bd)) best = j;
   }
   return best;
+}
+
+// exclusive prefix sum of one int per thread over the CTA; total returned to every thread
+__device__ __forceinline__ int block_exscan(int v, int* warp_sums, int& total) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  int inc = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int t = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += t;
+  }
+  if (lane == 31) warp_sums[warp] = inc;
+  __syncthreads();
+  if (warp == 0) {
+    int w = lane < kSeedThreads / 32 ? warp_sums[lane] : 0;
+#pragma unroll
+    for (int o = 1; o < kSeedThreads / 32; o <<= 1) {
+      const int t = __shfl_up_sync(0xffffffffu, w, o);
+      if (lane >= o) w += t;
+    }
+    if (lane < kSeedThreads / 32) warp_sums[lane] = w;       // inclusive warp totals
+  }
+  __syncthreads();
+  total = warp_sums[kSeedThreads / 32 - 1];
+  const int base = warp ? warp_sums[warp - 1] : 0;
+  return base + inc - v;
 }
 
 __device__ __forceinline__ float xz_at(const SeedParams& p, float ax, float bx, float cx, int layer) {
@@ -135,8 +201,9 @@ struct UvComb { int n, mask; float m[6]; int hit[6]; };
 
 // O8 for one first-layer hit ih (tile index) of pass pp: closest hits within tol_uv in the other
 // five stereo layers, running-average t_y (A7).
-__device__ __forceinline__ void uv_walk(const SeedParams& p, const float* __restrict__ hx, const int* zl,
-                                        const float* xp, int sf, int ih, UvComb& c) {
+__device__ __forceinline__ void uv_walk(const SeedParams& p, const float* __restrict__ hx, const Zone* zi,
+                                        const uint16_t* __restrict__ lut, const float* xp, int sf, int ih,
+                                        UvComb& c) {
   const int lf = p.ul[sf];
   const float xh = hx[ih];
   const float y0 = (xp[sf] - xh) * p.inv_tan[lf];          // Eq. 16
@@ -149,7 +216,8 @@ __device__ __forceinline__ void uv_walk(const SeedParams& p, const float* __rest
     if (s == sf) continue;
     const int l = p.ul[s];
     const float xe = xp[s] - ty * p.zt[l];
-    const int h = closest_hit(hx, zl[l], zl[l + 1], xe, p.tol_uv);
+    const Zone z = zi[l];
+    const int h = closest_hit(hx, lut + l * (kLutBins + 1), z, xe, p.tol_uv);
     if (h >= 0) {
       const float xhh = hx[h];
       const float yl = (xp[s] - xhh) * p.inv_tan[l];
@@ -191,12 +259,26 @@ __device__ __forceinline__ float fit_y(const SeedParams& p, const UvComb& c, flo
 }
 
 // ------------------------------------------------------------------------------------ kernel
-__global__ void __launch_bounds__(kSeedThreads)
+// uv_walk with the first-layer slot as a compile-time constant (keeps xp[]/m[]/hit[] in registers)
+__device__ __forceinline__ void uv_walk_sf(const SeedParams& p, const float* __restrict__ hx, const Zone* zn,
+                                           const uint16_t* __restrict__ lut, const float* xp, int sf, int ih,
+                                           UvComb& c) {
+  switch (sf) {
+    case 0: uv_walk(p, hx, zn, lut, xp, 0, ih, c); break;
+    case 1: uv_walk(p, hx, zn, lut, xp, 1, ih, c); break;
+    case 2: uv_walk(p, hx, zn, lut, xp, 2, ih, c); break;
+    case 3: uv_walk(p, hx, zn, lut, xp, 3, ih, c); break;
+    case 4: uv_walk(p, hx, zn, lut, xp, 4, ih, c); break;
+    default: uv_walk(p, hx, zn, lut, xp, 5, ih, c); break;
+  }
+}
+
+__global__ void __launch_bounds__(kSeedThreads, 3)
 seeding_kernel(const __grid_constant__ SeedParams p) {
   extern __shared__ __align__(16) unsigned char smem[];
   SeedSmemHeader& H = *reinterpret_cast<SeedSmemHeader*>(smem);
-  float* hx = reinterpret_cast<float*>(smem + 256);
-  size_t off = 256 + ((size_t)p.max_hits + 8) * 4;
+  float* hx = reinterpret_cast<float*>(smem + kSeedHeaderBytes);
+  size_t off = kSeedHeaderBytes + ((size_t)p.max_hits + 8) * 4;
   off = (off + 15) & ~(size_t)15;
   Cand* cand = reinterpret_cast<Cand*>(smem + off);
   off += (size_t)p.max_cand * sizeof(Cand);
@@ -205,9 +287,14 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   off = (off + 15) & ~(size_t)15;
   Triplet* trip = reinterpret_cast<Triplet*>(smem + off);
   unsigned long long* tbl = reinterpret_cast<unsigned long long*>(smem + off);   // aliases trip
+  off += (size_t)p.max_trip * 8;
+  uint16_t* lut = reinterpret_cast<uint16_t*>(smem + off);
+  off += 12 * (kLutBins + 1) * 2;
+  off = (off + 15) & ~(size_t)15;
+  SeedScan& scan = *reinterpret_cast<SeedScan*>(smem + off);
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int nwarps = kSeedThreads / 32;
+  constexpr int T = kSeedThreads, nwarps = kSeedThreads / 32;
   const int half_id = blockIdx.x, event = half_id >> 1, h = half_id & 1;
   const uint32_t* zo = p.zone_off + (size_t)half_id * 12;
 
@@ -251,7 +338,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     }
   }
   // tail (and the whole tile when the source is not 16-byte aligned) with plain loads
-  for (uint32_t i = a1 + tid; i < g_end; i += kSeedThreads) hx[i - a0] = p.hit_x[i];
+  for (uint32_t i = a1 + tid; i < g_end; i += T) hx[i - a0] = p.hit_x[i];
   {
     uint32_t done = 0;
     while (!done) {
@@ -270,48 +357,105 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     if (tid == 0) { p.count[half_id] = 0; p.status[half_id] = LHCB_ST_HITS_OVERFLOW; }
     return;
   }
+  // bin tables: per zone, bins span [first hit, last hit]
+  if (tid < 12) {
+    const int b = zl[tid], e = zl[tid + 1];
+    float x0 = 0.f, invw = 0.f;
+    if (e > b) {
+      x0 = hx[b];
+      const float span = hx[e - 1] - x0;
+      invw = span > 0.f ? (float)kLutBins / span : 0.f;
+    }
+    Zone z; z.b = b; z.e = e; z.x0 = x0; z.invw = invw;
+    H.zi[tid] = z;
+  }
+  __syncthreads();
+  for (int z = warp; z < 12; z += nwarps) {
+    const Zone zz = H.zi[z];
+    uint16_t* L = lut + z * (kLutBins + 1);
+    if (zz.e == zz.b) {
+      for (int k = lane; k <= kLutBins; k += 32) L[k] = (uint16_t)zz.b;
+    } else {
+      for (int i = zz.b + lane; i < zz.e; i += 32) {
+        const int k1 = zone_bin(zz, hx[i]);
+        const int k0 = i == zz.b ? -1 : zone_bin(zz, hx[i - 1]);
+        for (int k = k0 + 1; k <= k1; ++k) L[k] = (uint16_t)i;
+        if (i == zz.e - 1)
+          for (int k = k1 + 1; k <= kLutBins; ++k) L[k] = (uint16_t)zz.e;
+      }
+    }
+  }
+  __syncthreads();
 
   // ---- S1 + S2 per iteration -----------------------------------------------------------
   for (int it = 0; it < 2; ++it) {
     const int l1 = p.l1[it], l2 = p.l2[it], l3 = p.l3[it];
-    const int b1 = zl[l1], e1 = zl[l1 + 1], b2 = zl[l2], e2 = zl[l2 + 1], b3 = zl[l3], e3 = zl[l3 + 1];
+    const Zone z1n = H.zi[l1], z2n = H.zi[l2], z3n = H.zi[l3];
+    const uint16_t* lut2 = lut + l2 * (kLutBins + 1);
+    const uint16_t* lut3 = lut + l3 * (kLutBins + 1);
+    const int b1 = z1n.b, n1 = z1n.e - z1n.b, b2 = z2n.b, e2 = z2n.e, b3 = z3n.b;
     const float r13 = p.r13[it], dx3 = p.dx3max[it], idz = p.inv_dz13[it], z1 = p.z1[it], dz12 = p.dz12[it];
     const float K = p.K[it];
 
-    for (int i1 = b1 + warp; i1 < e1; i1 += nwarps) {                          // O2
-      const float x1 = hx[i1];
-      const float c = x1 * r13;                                                // Eq. 11
-      const float lo = c - dx3, hi = c + dx3;
-      const int first = lower_bound(hx, b3, e3, lo), last = upper_bound(hx, b3, e3, hi);
-      for (int i3 = first + lane; i3 < last; i3 += 32) {
-        const float x3 = hx[i3];
-        const float t13 = (x3 - x1) * idz;                                     // O3, Eq. 4
-        const float x0 = x1 - z1 * t13;                                        // Eq. 3
-        const float invp = p.a * fabsf(x0) + p.b * (x0 * x0);                  // Eq. 5
-        const float x2c = x1 + dz12 * t13;                                     // O4, Eq. 12
-        const float kinv = p.kappa * invp;
-        const float cxp = x0 >= 0.f ? -kinv : kinv;                            // A3
-        const float ca = p.f_lo * cxp, cb = p.f_hi * cxp;                      // A4
-        const float cxlo = (ca < cb ? ca : cb) - p.d_lo, cxhi = (ca > cb ? ca : cb) + p.d_hi;
-        const float ea = x2c + K * cxlo, eb = x2c + K * cxhi;
-        const float lo2 = ea < eb ? ea : eb, hi2 = ea > eb ? ea : eb;
-        int j = lower_bound(hx, b2, e2, lo2);
-        while (j < e2 && hx[j] <= hi2) {
-          const int k = atomicAdd(&H.n_trip, 1);
-          if (k < p.max_trip) {
-            Triplet t;
-            t.i1 = (uint16_t)(i1 - b1); t.i2 = (uint16_t)(j - b2); t.i3 = (uint16_t)(i3 - b3); t.it = (uint16_t)it;
-            trip[k] = t;
+    for (int tile0 = 0; tile0 < n1; tile0 += T) {
+      // O2: T3 window of this thread's T1 hit
+      const int nt1 = n1 - tile0 < T ? n1 - tile0 : T;
+      int cnt = 0, fst = 0;
+      if (tid < nt1) {
+        const float x1 = hx[b1 + tile0 + tid];
+        const float c = x1 * r13;                                                // Eq. 11
+        const float lo = c - dx3, hi = c + dx3;
+        fst = lower_bound(hx, lut3, z3n, lo);
+        cnt = upper_bound(hx, lut3, z3n, hi) - fst;
+      }
+      int total;
+      const int ex = block_exscan(cnt, H.warp_sums, total);
+      scan.offs[tid] = ex; scan.first[tid] = (uint16_t)fst;
+      if (tid == T - 1) scan.offs[T] = total;
+      __syncthreads();
+      // flattened pairs: thread owns pairs [p0, p1)
+      const int chunk = (total + T - 1) / T;
+      const int p0 = tid * chunk, p1 = p0 + chunk < total ? p0 + chunk : total;
+      if (p0 < p1) {
+        int t = owner_of(scan.offs, nt1, p0);
+        int nxt = scan.offs[t + 1];
+        int i1 = b1 + tile0 + t;
+        float x1 = hx[i1];
+        int f = (int)scan.first[t] - scan.offs[t];
+        for (int pp = p0; pp < p1; ++pp) {
+          while (pp >= nxt) {
+            ++t; nxt = scan.offs[t + 1]; i1 = b1 + tile0 + t; x1 = hx[i1]; f = (int)scan.first[t] - scan.offs[t];
           }
-          ++j;
+          const int i3 = f + pp;
+          const float x3 = hx[i3];
+          const float t13 = (x3 - x1) * idz;                                     // O3, Eq. 4
+          const float x0 = x1 - z1 * t13;                                        // Eq. 3
+          const float invp = p.a * fabsf(x0) + p.b * (x0 * x0);                  // Eq. 5
+          const float x2c = x1 + dz12 * t13;                                     // O4, Eq. 12
+          const float kinv = p.kappa * invp;
+          const float cxp = x0 >= 0.f ? -kinv : kinv;                            // A3
+          const float ca = p.f_lo * cxp, cb = p.f_hi * cxp;                      // A4
+          const float cxlo = (ca < cb ? ca : cb) - p.d_lo, cxhi = (ca > cb ? ca : cb) + p.d_hi;
+          const float ea = x2c + K * cxlo, eb = x2c + K * cxhi;
+          const float lo2 = ea < eb ? ea : eb, hi2 = ea > eb ? ea : eb;
+          int j = lower_bound(hx, lut2, z2n, lo2);
+          while (j < e2 && hx[j] <= hi2) {
+            const int k = atomicAdd(&H.n_trip, 1);
+            if (k < p.max_trip) {
+              Triplet tr;
+              tr.i1 = (uint16_t)(i1 - b1); tr.i2 = (uint16_t)(j - b2); tr.i3 = (uint16_t)(i3 - b3); tr.it = (uint16_t)it;
+              trip[k] = tr;
+            }
+            ++j;
+          }
         }
       }
+      __syncthreads();
     }
-    __syncthreads();
     int nt = H.n_trip;
     if (nt > p.max_trip) { nt = p.max_trip; if (tid == 0) H.status |= LHCB_ST_TRIPLET_OVERFLOW; }
 
-    for (int t = tid; t < nt; t += kSeedThreads) {                             // O5 + O6
+    for (int t = tid; t < nt; t += T) {                                          // O5 + O6
       const Triplet tr = trip[t];
       const int i1 = b1 + tr.i1, i2 = b2 + tr.i2, i3 = b3 + tr.i3;
       const float x1 = hx[i1], x2 = hx[i2], x3 = hx[i3];
@@ -331,7 +475,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
         if (l == l1) hh = i1;
         else if (l == l2) hh = i2;
         else if (l == l3) hh = i3;
-        else hh = closest_hit(hx, zl[l], zl[l + 1], xp, p.tol_x);
+        else { const Zone z = H.zi[l]; hh = closest_hit(hx, lut + l * (kLutBins + 1), z, xp, p.tol_x); }
         if (hh < 0) { hit[s] = -1; pattern = 1 + s; r[s] = 0.f; }
         else { hit[s] = hh - zl[l]; r[s] = hx[hh] - xp; ++nx; }
       }
@@ -384,9 +528,9 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   int nc = H.n_cand;
   if (nc > p.max_cand) { nc = p.max_cand; if (tid == 0) H.status |= LHCB_ST_CAND_OVERFLOW; }
   const int n_xhits = H.xbase[6];
-  for (int i = tid; i < n_xhits; i += kSeedThreads) tbl[i] = kNoKey;
+  for (int i = tid; i < n_xhits; i += T) tbl[i] = kNoKey;
   __syncthreads();
-  for (int c = tid; c < nc; c += kSeedThreads) {
+  for (int c = tid; c < nc; c += T) {
     const Cand& cd = cand[c];
     const unsigned long long key = clone_key(cd.chi2, cd.cx, cd.nx, cd.it);
 #pragma unroll
@@ -394,7 +538,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
       if (cd.hit[s] != 0xFFFF) atomicMin(&tbl[H.xbase[s] + cd.hit[s]], key);
   }
   __syncthreads();
-  for (int c = tid; c < nc; c += kSeedThreads) {
+  for (int c = tid; c < nc; c += T) {
     Cand& cd = cand[c];
     const unsigned long long key = clone_key(cd.chi2, cd.cx, cd.nx, cd.it);
     int own = 0;
@@ -408,39 +552,56 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   __syncthreads();
   const int nk = H.n_kept;
   unsigned long long* best = tbl;                            // table is dead: reuse for the best u/v keys
-  for (int i = tid; i < nk; i += kSeedThreads) best[i] = kNoKey;
+  for (int i = tid; i < nk; i += T) best[i] = kNoKey;        // nk <= nc <= max_cand <= max_trip (checked at init)
   __syncthreads();
 
   // ---- S4: u/v addition (O8, O9) --------------------------------------------------------------
-  {
-    const int gl = tid % kUvGroup, gid = tid / kUvGroup, ngroups = kSeedThreads / kUvGroup;
-    const unsigned gmask = ((1u << kUvGroup) - 1u) << ((lane / kUvGroup) * kUvGroup);
-    for (int w = gid; w < 2 * nk; w += ngroups) {
-      const int k = w >> 1, pp = w & 1;
-      const Cand& cd = cand[kept[k]];
-      float xp[6];
-#pragma unroll
-      for (int s = 0; s < 6; ++s) xp[s] = xz_at(p, cd.ax, cd.bx, cd.cx, p.ul[s]);
-      const int lf = p.uv_first[pp], sf = p.slot_of_layer[lf];
-      float xpf = xp[0];
-#pragma unroll
-      for (int s = 1; s < 6; ++s) xpf = (s == sf) ? xp[s] : xpf;
+  // owners w = 2*k + pass (k-th survivor); items = first-layer hits in the window of Eq. 16
+  for (int tile0 = 0; tile0 < 2 * nk; tile0 += T) {
+    const int nown = 2 * nk - tile0 < T ? 2 * nk - tile0 : T;
+    int cnt = 0, fst = 0;
+    if (tid < nown) {
+      const int w = tile0 + tid, pp = w & 1;
+      const Cand& cd = cand[kept[w >> 1]];
+      const int lf = p.uv_first[pp];
+      const float xpf = xz_at(p, cd.ax, cd.bx, cd.cx, lf);
       const float wa = xpf - p.ywin_a[h][lf], wb = xpf - p.ywin_b[h][lf];
       const float wlo = wa < wb ? wa : wb, whi = wa > wb ? wa : wb;
-      const int bf = zl[lf], ef = zl[lf + 1];
-      const int first = lower_bound(hx, bf, ef, wlo), last = upper_bound(hx, bf, ef, whi);
+      const Zone zf = H.zi[lf];
+      const uint16_t* lutf = lut + lf * (kLutBins + 1);
+      fst = lower_bound(hx, lutf, zf, wlo);
+      cnt = upper_bound(hx, lutf, zf, whi) - fst;
+    }
+    int total;
+    const int ex = block_exscan(cnt, H.warp_sums, total);
+    scan.offs[tid] = ex; scan.first[tid] = (uint16_t)fst;
+    if (tid == T - 1) scan.offs[T] = total;
+    __syncthreads();
+    const int chunk = (total + T - 1) / T;
+    const int p0 = tid * chunk, p1 = p0 + chunk < total ? p0 + chunk : total;
+    if (p0 < p1) {
+      int t = owner_of(scan.offs, nown, p0) - 1;             // forces a reload on the first item
+      int nxt = -1;
+      int f = 0, pp = 0, sf = 0, bf = 0, kk = 0;
+      float xp[6];
       unsigned long long bk = kNoKey;
-      for (int ih = first + gl; ih < last; ih += kUvGroup) {
-        UvComb c;
-        // sf is one of two values per launch; dispatch so that the walk is fully unrolled
-        switch (sf) {
-          case 0: uv_walk(p, hx, zl, xp, 0, ih, c); break;
-          case 1: uv_walk(p, hx, zl, xp, 1, ih, c); break;
-          case 2: uv_walk(p, hx, zl, xp, 2, ih, c); break;
-          case 3: uv_walk(p, hx, zl, xp, 3, ih, c); break;
-          case 4: uv_walk(p, hx, zl, xp, 4, ih, c); break;
-          default: uv_walk(p, hx, zl, xp, 5, ih, c); break;
+      for (int q = p0; q < p1; ++q) {
+        if (q >= nxt) {
+          if (bk != kNoKey) atomicMin(&best[kk], bk);
+          bk = kNoKey;
+          do { ++t; nxt = scan.offs[t + 1]; } while (q >= nxt);
+          const int w = tile0 + t;
+          kk = w >> 1; pp = w & 1;
+          const Cand& cd = cand[kept[kk]];
+#pragma unroll
+          for (int s = 0; s < 6; ++s) xp[s] = xz_at(p, cd.ax, cd.bx, cd.cx, p.ul[s]);
+          const int lf = p.uv_first[pp];
+          sf = p.slot_of_layer[lf]; bf = zl[lf];
+          f = (int)scan.first[t] - scan.offs[t];
         }
+        const int ih = f + q;
+        UvComb c;
+        uv_walk_sf(p, hx, H.zi, lut, xp, sf, ih, c);
         if (c.n < p.min_uv_hits) continue;
         float ay, by;
         const float chi2y = fit_y(p, c, ay, by);
@@ -450,19 +611,14 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
                                        ((unsigned long long)pp << 16) | (unsigned long long)(ih - bf);
         bk = key < bk ? key : bk;
       }
-#pragma unroll
-      for (int o = kUvGroup / 2; o > 0; o >>= 1) {
-        const unsigned long long other = __shfl_xor_sync(gmask, bk, o);
-        bk = other < bk ? other : bk;
-      }
-      if (gl == 0 && bk != kNoKey) atomicMin(&best[k], bk);
+      if (bk != kNoKey) atomicMin(&best[kk], bk);
     }
+    __syncthreads();
   }
-  __syncthreads();
 
   // ---- S5: seeds (O10) ------------------------------------------------------------------------
   const int pol = p.pol ? (int)p.pol[event] : p.polarity;
-  for (int k = tid; k < nk; k += kSeedThreads) {
+  for (int k = tid; k < nk; k += T) {
     const unsigned long long key = best[k];
     if (key == kNoKey) continue;                             // fake x-z projection (L219)
     const Cand& cd = cand[kept[k]];
@@ -473,14 +629,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
 #pragma unroll
     for (int s = 0; s < 6; ++s) xp[s] = xz_at(p, cd.ax, cd.bx, cd.cx, p.ul[s]);
     UvComb c;
-    switch (sf) {
-      case 0: uv_walk(p, hx, zl, xp, 0, ih, c); break;
-      case 1: uv_walk(p, hx, zl, xp, 1, ih, c); break;
-      case 2: uv_walk(p, hx, zl, xp, 2, ih, c); break;
-      case 3: uv_walk(p, hx, zl, xp, 3, ih, c); break;
-      case 4: uv_walk(p, hx, zl, xp, 4, ih, c); break;
-      default: uv_walk(p, hx, zl, xp, 5, ih, c); break;
-    }
+    uv_walk_sf(p, hx, H.zi, lut, xp, sf, ih, c);
     float ay, by;
     const float chi2y = fit_y(p, c, ay, by);
     const int slot = atomicAdd(&H.n_seed, 1);
