@@ -50,6 +50,7 @@ typedef enum {
 #define LHCB_ST_MATCH_OVERFLOW 16u    /* more chi2-accepted pairs than max_match_cand_per_event */
 #define LHCB_ST_LONG_OVERFLOW 32u     /* more long tracks than max_long_per_event */
 #define LHCB_ST_VELO_OVERFLOW 64u     /* more VELO tracks than max_velo_per_event: event skipped */
+#define LHCB_ST_UT_OVERFLOW 128u      /* more than 65534 UT hits in one event: event skipped */
 
 /* Detector description and tunables.  Host POD, copied by lhcb_geom_init.
  * Citations: PAPER.md line / equation; "A<n>" = reading listed in DESIGN.md. */
@@ -86,8 +87,10 @@ typedef struct {
   int32_t max_long_per_event;                  /* [256]  output slots per event */
   int32_t max_hits_per_half;                   /* [6144] SciFi hits staged per event-half (<= 32768) */
   int32_t max_triplets_per_half;               /* [4096] three-hit combinations per half and iteration */
-  int32_t max_match_cand_per_event;            /* [1024] chi2-accepted seed-VELO pairs per event */
-  int32_t max_velo_per_event;                  /* [1024] */
+  int32_t max_match_cand_per_event;            /* [768]  chi2-accepted seed-VELO pairs per event */
+  int32_t max_velo_per_event;                  /* [512] */
+  int32_t max_ut_per_event;                    /* [6144] UT hits staged in shared memory per event; events with
+                                                  more are searched in global memory (slower, same result) */
 } lhcb_geom_t;
 
 /* Geometry-only constants the kernels use (O1).  Computed in double from the float
@@ -142,6 +145,7 @@ typedef struct {
 
 /* UT hits (L305-342): per (event, layer) sorted by x0 = x at y=0; strip covers [y_lo, y_hi]. */
 typedef struct {
+  uint32_t n_hits;           /* length of x0, y_lo, y_hi */
   const uint32_t* off;       /* [n_events*4+1] */
   const float *x0, *y_lo, *y_hi;
 } lhcb_ut_t;

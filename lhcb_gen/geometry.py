@@ -87,6 +87,7 @@ DEFAULT_GEOM = {
     "max_triplets_per_half": 0,
     "max_match_cand_per_event": 0,
     "max_velo_per_event": 0,
+    "max_ut_per_event": 0,
 }
 
 

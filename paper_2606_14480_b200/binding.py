@@ -19,7 +19,7 @@ F, I = C.c_float, C.c_int32
 NO_HIT = 0xFFFFFFFF
 
 ST_BITS = {1: "triplet_overflow", 2: "cand_overflow", 4: "seed_overflow", 8: "hits_overflow",
-           16: "match_overflow", 32: "long_overflow", 64: "velo_overflow"}
+           16: "match_overflow", 32: "long_overflow", 64: "velo_overflow", 128: "ut_overflow"}
 
 EXPORTS = ["lhcb_geom_derive", "lhcb_geom_init", "lhcb_destroy", "lhcb_get_geom", "lhcb_workspace_bytes",
            "lhcb_seeding", "lhcb_matching", "lhcb_error_string", "lhcb_last_cuda_error",
@@ -40,7 +40,7 @@ class LhcbGeom(C.Structure):
         ("ut_y_tol", F), ("min_ut_hits", I), ("ut_enabled", I),
         ("max_seeds_per_half", I), ("max_xz_cand_per_half", I), ("max_long_per_event", I),
         ("max_hits_per_half", I), ("max_triplets_per_half", I), ("max_match_cand_per_event", I),
-        ("max_velo_per_event", I),
+        ("max_velo_per_event", I), ("max_ut_per_event", I),
     ]
 
 
@@ -79,7 +79,7 @@ class LhcbVelo(C.Structure):
 
 
 class LhcbUt(C.Structure):
-    _fields_ = [("off", VP), ("x0", VP), ("y_lo", VP), ("y_hi", VP)]
+    _fields_ = [("n_hits", C.c_uint32), ("off", VP), ("x0", VP), ("y_lo", VP), ("y_hi", VP)]
 
 
 class LhcbLong(C.Structure):
@@ -283,7 +283,7 @@ class Context:
                      _ptr(dev.velo_ty), _ptr(dev.polarity))
         u = None
         if use_ut and dev.ut_off is not None:
-            u = C.byref(LhcbUt(_ptr(dev.ut_off), _ptr(dev.ut_x0), _ptr(dev.ut_ylo), _ptr(dev.ut_yhi)))
+            u = C.byref(LhcbUt(dev.ut_x0.numel(), _ptr(dev.ut_off), _ptr(dev.ut_x0), _ptr(dev.ut_ylo), _ptr(dev.ut_yhi)))
         l = LhcbLong(_ptr(out["count"]), _ptr(out["seed_idx"]), _ptr(out["velo_idx"]), _ptr(out["ut_idx"]),
                      _ptr(out["n_ut"]), _ptr(out["qop"]), _ptr(out["chi2"]), _ptr(out["status"]))
         rc = self.lib.lhcb_matching(self._ctx, C.byref(s), C.byref(v), u, C.byref(l), VP(0), self._stream())
@@ -377,7 +377,7 @@ class HostPipeline:
         self._ev = LhcbEvents(n, ev.n_hits, _ptr(h["zone_off"]), _ptr(h["hit_x"]), _ptr(h["polarity"]))
         self._velo = LhcbVelo(n, _ptr(h["velo_off"]), _ptr(h["velo_x"]), _ptr(h["velo_y"]), _ptr(h["velo_tx"]),
                               _ptr(h["velo_ty"]), _ptr(h["polarity"]))
-        self._ut = LhcbUt(_ptr(h["ut_off"]), _ptr(h["ut_x0"]), _ptr(h["ut_ylo"]), _ptr(h["ut_yhi"])) if self.has_ut else None
+        self._ut = LhcbUt(len(ev.ut_x0), _ptr(h["ut_off"]), _ptr(h["ut_x0"]), _ptr(h["ut_ylo"]), _ptr(h["ut_yhi"])) if self.has_ut else None
         o = self.out
         self._long = LhcbLong(_ptr(o["count"]), _ptr(o["seed_idx"]), _ptr(o["velo_idx"]), _ptr(o["ut_idx"]),
                               _ptr(o["n_ut"]), _ptr(o["qop"]), _ptr(o["chi2"]), _ptr(o["status"]))

@@ -79,7 +79,7 @@ void fill_match_params(const lhcb_ctx* c, lhcb::MatchParams& p) {
   std::memcpy(p.ut_loose, D.ut_loose, sizeof(p.ut_loose)); std::memcpy(p.ut_tight, D.ut_tight, sizeof(p.ut_tight));
   p.min_ut_hits = g.min_ut_hits; p.polarity = g.polarity;
   p.max_seeds = g.max_seeds_per_half; p.max_long = g.max_long_per_event;
-  p.max_mc = g.max_match_cand_per_event; p.max_velo = g.max_velo_per_event;
+  p.max_mc = g.max_match_cand_per_event; p.max_velo = g.max_velo_per_event; p.max_ut = g.max_ut_per_event;
 }
 
 }  // namespace
@@ -104,9 +104,10 @@ int lhcb_geom_init(const lhcb_geom_t* g, int device, lhcb_ctx** out) {
   int rc = lhcb::derive(G, c->der);
   if (rc != LHCB_OK) { delete c; return rc; }
   if (G.max_hits_per_half > 32768 || G.max_xz_cand_per_half > 65535 || G.max_seeds_per_half > 32767 ||
-      G.max_velo_per_event > 65535 || G.max_triplets_per_half < G.max_xz_cand_per_half) { delete c; return LHCB_ERR_BAD_ARGUMENT; }
+      G.max_velo_per_event > 65535 || G.max_ut_per_event > 65534 || G.max_triplets_per_half < G.max_xz_cand_per_half) { delete c; return LHCB_ERR_BAD_ARGUMENT; }
   c->seed_smem = lhcb::seed_smem_bytes(G.max_hits_per_half, G.max_xz_cand_per_half, G.max_triplets_per_half);
-  c->match_smem = lhcb::match_smem_bytes(G.max_seeds_per_half, G.max_match_cand_per_event, G.max_velo_per_event);
+  c->match_smem = lhcb::match_smem_bytes(G.max_seeds_per_half, G.max_match_cand_per_event, G.max_velo_per_event,
+                                         G.max_ut_per_event);
   cudaError_t e = cudaSetDevice(device);
   int max_optin = 0;
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
@@ -190,7 +191,7 @@ int lhcb_matching(lhcb_ctx* c, const lhcb_seeds_t* seeds, const lhcb_velo_t* vel
   p.seed_count = seeds->count; p.state = seeds->state;
   p.seed_cap_total = (size_t)velo->n_events * 2 * (size_t)c->geom.max_seeds_per_half;
   p.velo_off = velo->off; p.vx = velo->x; p.vy = velo->y; p.vtx = velo->tx; p.vty = velo->ty; p.pol = velo->polarity;
-  if (ut) { p.ut_off = ut->off; p.ux = ut->x0; p.uylo = ut->y_lo; p.uyhi = ut->y_hi; }
+  if (ut) { p.ut_off = ut->off; p.ux = ut->x0; p.uylo = ut->y_lo; p.uyhi = ut->y_hi; p.n_ut_total = ut->n_hits; }
   p.count = out->count; p.seed_idx = out->seed_idx; p.velo_idx = out->velo_idx; p.ut_idx = out->ut_idx;
   p.n_ut = out->n_ut; p.qop = out->qop; p.chi2 = out->chi2; p.status = out->status;
   p.long_cap_total = (size_t)velo->n_events * (size_t)c->geom.max_long_per_event;
@@ -351,7 +352,7 @@ int lhcb_reconstruct_host(lhcb_pipeline* p, const lhcb_events_t* ev, const lhcb_
     if (rc != LHCB_OK) return rc;
     p->launches += c->last_launches;
     lhcb_velo_t dev_v = {ne, p->velo_off + e0, p->vx, p->vy, p->vtx, p->vty, ev->polarity ? p->pol + e0 : nullptr};
-    lhcb_ut_t dev_u = {p->ut_off + (size_t)e0 * 4, p->ux, p->uylo, p->uyhi};
+    lhcb_ut_t dev_u = {(uint32_t)n_ut, p->ut_off + (size_t)e0 * 4, p->ux, p->uylo, p->uyhi};
     lhcb_long_t dev_l = {S.l_count, S.l_seed, S.l_velo, S.l_ut, S.l_nut, S.l_qop, S.l_chi2, S.l_status};
     rc = lhcb_matching(c, &dev_s, &dev_v, ut ? &dev_u : nullptr, &dev_l, nullptr, s);
     if (rc != LHCB_OK) return rc;

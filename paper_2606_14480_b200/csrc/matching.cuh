@@ -1,6 +1,8 @@
 // VELO-SciFi Matching kernel (section 4) for sm_100a.
 //
-// One CTA per event.  The event's VELO states are staged in shared memory.
+// One CTA per event.  The event's VELO states are staged in shared memory; the x0 of the event's UT
+// hits (four sorted layers, contiguous in memory) is fetched with one bulk async copy that lands while
+// the all-pairs loop runs, so the UT searches are shared-memory binary searches.
 //   M1/M2  warp per seed, lanes over VELO tracks: kink extrapolation (Eq. 17-18), preselection
 //          (Eq. 21), chi2_match (Eq. 22-23) < 2; accepted pairs are queued in shared memory
 //   M3     thread per queued pair: UT hit search (Eq. 19-20, Table 2)
@@ -15,14 +17,18 @@
 
 namespace lhcb {
 
-constexpr int kMatchThreads = 256;
+#ifndef LHCB_MATCH_THREADS
+#define LHCB_MATCH_THREADS 256
+#endif
+constexpr int kMatchThreads = LHCB_MATCH_THREADS;
 
 struct MatchParams {
   float zS, zV, dzyS, dzyV, mag[5], presel[4], cx0, cx1, cy0, cy1, inv_tol_tx, inv_tol_ty, chi2m_max;
   float inv_KB, Ag, Bg, inv_Bg, ut_dz[4], ut_dz2[4], ut_dz4[4], ut_tan[4], ut_y_tol;
   float ut_loose[4][4], ut_tight[4][4];
   int min_ut_hits, use_ut, polarity;
-  int max_seeds, max_long, max_mc, max_velo;
+  int max_seeds, max_long, max_mc, max_velo, max_ut;
+  uint32_t n_ut_total;
   // batch
   int n_events;
   const uint32_t* seed_count;
@@ -47,21 +53,23 @@ struct MatchParams {
 struct __align__(16) MatchCand {
   uint16_t seed, velo;      // event-local indices
   float chi2, q0, gamma;
-  uint32_t ut[4];           // global UT hit indices
-  uint8_t n_ut, valid, pad[2];
+  uint16_t ut[4];           // UT hit index relative to the event's first UT hit, 0xFFFF = none
+  uint8_t n_ut, valid, pad[6];
 };
+static_assert(sizeof(MatchCand) == 32, "MatchCand is 32 bytes");
 
-__host__ __device__ inline size_t match_smem_bytes(int max_seeds, int max_mc, int max_velo) {
+__host__ __device__ inline size_t match_smem_bytes(int max_seeds, int max_mc, int max_velo, int max_ut) {
   size_t b = 64;
+  b += ((size_t)max_ut + 8) * 4;             // UT x0 tile (16-byte aligned superset)
   b += (size_t)max_velo * 16;                // VELO states
+  b = (b + 15) & ~(size_t)15;
   b += (size_t)max_mc * sizeof(MatchCand);
-  b = (b + 7) & ~(size_t)7;
   b += (size_t)2 * max_seeds * 8;            // best key per seed
   b += (size_t)max_velo * 8;                 // best key per VELO track
   return b;
 }
 
-struct UtHyp { int n; uint32_t idx[4]; float gamma, ssq; };
+struct UtHyp { int n; int idx[4]; float gamma, ssq; };      // idx: position in the searched x0 array, -1 = none
 
 __device__ __forceinline__ float ut_window(const float* w, float invpG) {
   const float v = w[0] + w[1] * invpG;                      // L315
@@ -71,8 +79,12 @@ __device__ __forceinline__ float ut_window(const float* w, float invpG) {
 
 // O13: loose window until the first layer with hits; every loose hit starts a hypothesis (A13),
 // remaining layers use tight windows and the closest hit; gamma_x is refitted after each hit.
+// ux[i] is the x0 of the UT hit whose y-range is (uylo[i + ybase], uyhi[i + ybase]); uo[] are the layer
+// offsets in the indexing of ux (shared-memory tile or the global array).
 __device__ inline bool ut_search(const MatchParams& p, float xV, float yV, float txV, float tyV, float q0,
-                                 const uint32_t* __restrict__ uo, UtHyp& best) {
+                                 const float* __restrict__ ux, const int* uo, int ybase, UtHyp& best) {
+  const float* __restrict__ uylo = p.uylo + ybase;
+  const float* __restrict__ uyhi = p.uyhi + ybase;
   const float invpG = fabsf(q0) * 1000.f;
   const float gamma0 = p.Ag + p.Bg * q0;                    // Eq. 20
   bool have = false;
@@ -83,17 +95,17 @@ __device__ inline bool ut_search(const MatchParams& p, float xV, float yV, float
     const float x0e = xi - yi * p.ut_tan[i0];
     const float w = ut_window(p.ut_loose[i0], invpG);
     const float lo = x0e - w, hi = x0e + w;
-    const int b = (int)uo[i0], e = (int)uo[i0 + 1];
+    const int b = uo[i0], e = uo[i0 + 1];
     bool found = false;
-    for (int j = lower_bound(p.ux, b, e, lo); j < e && p.ux[j] <= hi; ++j) {
-      if (!(p.uylo[j] - p.ut_y_tol <= yi && yi <= p.uyhi[j] + p.ut_y_tol)) continue;
+    for (int j = lower_bound(ux, b, e, lo); j < e && ux[j] <= hi; ++j) {
+      if (!(uylo[j] - p.ut_y_tol <= yi && yi <= uyhi[j] + p.ut_y_tol)) continue;
       found = true;
       UtHyp hy;
       float dj[4];
 #pragma unroll
-      for (int k = 0; k < 4; ++k) { hy.idx[k] = LHCB_NO_HIT; dj[k] = 0.f; }
-      hy.n = 1; hy.idx[i0] = (uint32_t)j;
-      dj[i0] = ((p.ux[j] + yi * p.ut_tan[i0]) - xV) - txV * p.ut_dz[i0];
+      for (int k = 0; k < 4; ++k) { hy.idx[k] = -1; dj[k] = 0.f; }
+      hy.n = 1; hy.idx[i0] = j;
+      dj[i0] = ((ux[j] + yi * p.ut_tan[i0]) - xV) - txV * p.ut_dz[i0];
       float num = dj[i0] * p.ut_dz2[i0], den = p.ut_dz4[i0];
       float gam = num / den;
       for (int i = i0 + 1; i < 4; ++i) {
@@ -102,17 +114,17 @@ __device__ inline bool ut_search(const MatchParams& p, float xV, float yV, float
         const float xe = xt - yt * p.ut_tan[i];
         const float wt = ut_window(p.ut_tight[i], invpG);
         const float tlo = xe - wt, thi = xe + wt;
-        const int bb = (int)uo[i], ee = (int)uo[i + 1];
+        const int bb = uo[i], ee = uo[i + 1];
         int bj = -1;
         float bd = 0.f;
-        for (int jj = lower_bound(p.ux, bb, ee, tlo); jj < ee && p.ux[jj] <= thi; ++jj) {
-          if (!(p.uylo[jj] - p.ut_y_tol <= yt && yt <= p.uyhi[jj] + p.ut_y_tol)) continue;
-          const float dd = fabsf(p.ux[jj] - xe);
+        for (int jj = lower_bound(ux, bb, ee, tlo); jj < ee && ux[jj] <= thi; ++jj) {
+          if (!(uylo[jj] - p.ut_y_tol <= yt && yt <= uyhi[jj] + p.ut_y_tol)) continue;
+          const float dd = fabsf(ux[jj] - xe);
           if (bj < 0 || dd < bd) { bj = jj; bd = dd; }
         }
         if (bj >= 0) {
-          hy.idx[i] = (uint32_t)bj; ++hy.n;
-          dj[i] = ((p.ux[bj] + yt * p.ut_tan[i]) - xV) - txV * p.ut_dz[i];
+          hy.idx[i] = bj; ++hy.n;
+          dj[i] = ((ux[bj] + yt * p.ut_tan[i]) - xV) - txV * p.ut_dz[i];
           num = num + dj[i] * p.ut_dz2[i]; den = den + p.ut_dz4[i];
           gam = num / den;
         }
@@ -121,7 +133,7 @@ __device__ inline bool ut_search(const MatchParams& p, float xV, float yV, float
       bool first = true;
 #pragma unroll
       for (int i = 0; i < 4; ++i)
-        if (hy.idx[i] != LHCB_NO_HIT) {
+        if (hy.idx[i] >= 0) {
           const float res = dj[i] - gam * p.ut_dz2[i];
           hy.ssq = first ? res * res : hy.ssq + res * res;
           first = false;
@@ -136,15 +148,17 @@ __device__ inline bool ut_search(const MatchParams& p, float xV, float yV, float
 __global__ void __launch_bounds__(kMatchThreads)
 matching_kernel(const __grid_constant__ MatchParams p) {
   extern __shared__ __align__(16) unsigned char smem[];
-  int* hdr = reinterpret_cast<int*>(smem);                  // [0] n_mc, [1] n_long, [2] status
-  float* svx = reinterpret_cast<float*>(smem + 64);
+  int* hdr = reinterpret_cast<int*>(smem);                  // [0] n_mc, [1] n_long, [2] status, [4..8] UT offsets
+  unsigned long long* mbar = reinterpret_cast<unsigned long long*>(smem + 48);
+  float* sux = reinterpret_cast<float*>(smem + 64);
+  float* svx = sux + p.max_ut + 8;
   float* svy = svx + p.max_velo;
   float* svtx = svy + p.max_velo;
   float* svty = svtx + p.max_velo;
-  size_t off = 64 + (size_t)p.max_velo * 16;
+  size_t off = 64 + ((size_t)p.max_ut + 8) * 4 + (size_t)p.max_velo * 16;
+  off = (off + 15) & ~(size_t)15;
   MatchCand* mc = reinterpret_cast<MatchCand*>(smem + off);
   off += (size_t)p.max_mc * sizeof(MatchCand);
-  off = (off + 7) & ~(size_t)7;
   unsigned long long* seed_best = reinterpret_cast<unsigned long long*>(smem + off);
   unsigned long long* velo_best = seed_best + 2 * p.max_seeds;
 
@@ -161,6 +175,44 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     return;
   }
   if (tid < 3) hdr[tid] = 0;
+  // ---- UT x0 of this event: one bulk copy, overlapped with the all-pairs loop -----------------
+  uint32_t u_begin = 0, u_end = 0, ua0 = 0, ua1 = 0;
+  bool ut_in_smem = false;
+  const uint32_t mbar_addr = (uint32_t)__cvta_generic_to_shared(mbar);
+  if (p.use_ut) {
+    u_begin = p.ut_off[(size_t)e * 4]; u_end = p.ut_off[(size_t)e * 4 + 4];
+    if (u_end - u_begin > 65534u) {                          // 16-bit event-local UT indices
+      if (tid == 0) { p.count[e] = 0; p.status[e] = LHCB_ST_UT_OVERFLOW; }
+      return;
+    }
+    ua0 = u_begin & ~3u;
+    ut_in_smem = (int)(u_end - u_begin) <= p.max_ut;
+    if (ut_in_smem) {
+      const bool aligned = (reinterpret_cast<uintptr_t>(p.ux) & 15) == 0;
+      ua1 = (u_end + 3u) & ~3u;
+      if (ua1 > (p.n_ut_total & ~3u)) ua1 = p.n_ut_total & ~3u;
+      if (!aligned || ua1 < ua0) ua1 = ua0;
+      if (tid == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar_addr));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        const uint32_t bytes = (ua1 - ua0) * 4u;
+        if (bytes > 0) {
+          asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar_addr), "r"(bytes) : "memory");
+          asm volatile(
+              "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                  (uint32_t)__cvta_generic_to_shared(sux)),
+              "l"(p.ux + ua0), "r"(bytes), "r"(mbar_addr)
+              : "memory");
+        } else {
+          asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(mbar_addr) : "memory");
+        }
+      }
+      for (uint32_t i = ua1 + tid; i < u_end; i += kMatchThreads) sux[i - ua0] = p.ux[i];
+      if (tid < 5) hdr[4 + tid] = (int)(p.ut_off[(size_t)e * 4 + tid] - ua0);
+    } else if (tid < 5) {
+      hdr[4 + tid] = (int)p.ut_off[(size_t)e * 4 + tid];
+    }
+  }
   for (int v = tid; v < nv; v += kMatchThreads) {
     svx[v] = p.vx[v0 + v]; svy[v] = p.vy[v0 + v]; svtx[v] = p.vtx[v0 + v]; svty[v] = p.vty[v0 + v];
     velo_best[v] = kNoKey;
@@ -196,8 +248,8 @@ matching_kernel(const __grid_constant__ MatchParams p) {
       if (k < p.max_mc) {
         MatchCand m;
         m.seed = (uint16_t)s; m.velo = (uint16_t)v; m.chi2 = chi2; m.q0 = dtx * p.inv_KB; m.gamma = 0.f;
-        m.ut[0] = m.ut[1] = m.ut[2] = m.ut[3] = LHCB_NO_HIT;
-        m.n_ut = 0; m.valid = 1; m.pad[0] = m.pad[1] = 0;
+        m.ut[0] = m.ut[1] = m.ut[2] = m.ut[3] = 0xFFFF;
+        m.n_ut = 0; m.valid = 1;
         mc[k] = m;
       }
     }
@@ -207,18 +259,35 @@ matching_kernel(const __grid_constant__ MatchParams p) {
   if (nm > p.max_mc) { nm = p.max_mc; if (tid == 0) hdr[2] |= LHCB_ST_MATCH_OVERFLOW; }
 
   // ---- M3: UT hits (O13) -----------------------------------------------------------------------
+  if (ut_in_smem) {
+    uint32_t done = 0;
+    while (!done) {
+      asm volatile(
+          "{\n\t.reg .pred q;\n\t"
+          "mbarrier.try_wait.parity.shared::cta.b64 q, [%1], 0;\n\t"
+          "selp.u32 %0, 1, 0, q;\n\t}"
+          : "=r"(done)
+          : "r"(mbar_addr)
+          : "memory");
+    }
+  }
+  // index of hit i of the searched array relative to the event's first UT hit
+  const int rel0 = ut_in_smem ? (int)(ua0 - u_begin) : -(int)u_begin;
   for (int k = tid; k < nm; k += kMatchThreads) {
     MatchCand& m = mc[k];
     if (p.use_ut) {
       UtHyp hy;
       hy.n = 0; hy.gamma = 0.f; hy.ssq = 0.f;
-      hy.idx[0] = hy.idx[1] = hy.idx[2] = hy.idx[3] = LHCB_NO_HIT;
+      hy.idx[0] = hy.idx[1] = hy.idx[2] = hy.idx[3] = -1;
       const int v = m.velo;
-      const bool ok = ut_search(p, svx[v], svy[v], svtx[v], svty[v], m.q0, p.ut_off + (size_t)e * 4, hy);
+      const bool ok = ut_in_smem
+          ? ut_search(p, svx[v], svy[v], svtx[v], svty[v], m.q0, sux, hdr + 4, (int)ua0, hy)
+          : ut_search(p, svx[v], svy[v], svtx[v], svty[v], m.q0, p.ux, hdr + 4, 0, hy);
       m.valid = ok;
       if (ok) {
         m.n_ut = (uint8_t)hy.n; m.gamma = hy.gamma;
-        m.ut[0] = hy.idx[0]; m.ut[1] = hy.idx[1]; m.ut[2] = hy.idx[2]; m.ut[3] = hy.idx[3];
+#pragma unroll
+        for (int l = 0; l < 4; ++l) m.ut[l] = hy.idx[l] < 0 ? (uint16_t)0xFFFF : (uint16_t)(hy.idx[l] + rel0);
       }
     }
     if (m.valid)
@@ -246,8 +315,8 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     const int s = m.seed;
     p.seed_idx[o] = s < c0 ? (uint32_t)((2 * e) * p.max_seeds + s) : (uint32_t)((2 * e + 1) * p.max_seeds + (s - c0));
     p.velo_idx[o] = v0 + m.velo;
-    p.ut_idx[0 * ct + o] = m.ut[0]; p.ut_idx[1 * ct + o] = m.ut[1];
-    p.ut_idx[2 * ct + o] = m.ut[2]; p.ut_idx[3 * ct + o] = m.ut[3];
+#pragma unroll
+    for (int l = 0; l < 4; ++l) p.ut_idx[(size_t)l * ct + o] = m.ut[l] == 0xFFFF ? LHCB_NO_HIT : u_begin + m.ut[l];
     p.n_ut[o] = m.n_ut;
     const float q = p.use_ut ? (m.gamma - p.Ag) * p.inv_Bg : m.q0;               // Eq. 20 inverted / A10
     p.qop[o] = pol > 0 ? q : -q;

@@ -25,8 +25,17 @@
 
 namespace lhcb {
 
-constexpr int kSeedThreads = 256;
-constexpr int kLutBins = 256;                 // bins of the per-zone search table
+#ifndef LHCB_SEED_THREADS
+#define LHCB_SEED_THREADS 512
+#endif
+#ifndef LHCB_SEED_MIN_CTAS
+#define LHCB_SEED_MIN_CTAS 2
+#endif
+#ifndef LHCB_LUT_BINS
+#define LHCB_LUT_BINS 256
+#endif
+constexpr int kSeedThreads = LHCB_SEED_THREADS;
+constexpr int kLutBins = LHCB_LUT_BINS;       // bins of the per-zone search table
 constexpr unsigned long long kNoKey = ~0ull;
 
 struct SeedParams {
@@ -107,14 +116,25 @@ __device__ __forceinline__ int zone_bin(const Zone& z, float v) {
 __device__ __forceinline__ int lower_bound(const float* __restrict__ x, const uint16_t* __restrict__ lut,
                                            const Zone& z, float v) {
   int i = lut[zone_bin(z, v)];
-  while (i < z.e && x[i] < v) ++i;
+  // about one hit per bin: two predicated steps cover almost every call, the loop is the rare tail
+  bool m = i < z.e && x[i] < v;
+  i += m;
+  m = m && i < z.e && x[i] < v;
+  i += m;
+  if (m)
+    while (i < z.e && x[i] < v) ++i;
   return i;
 }
 // first index in [b, e) with x[i] > v
 __device__ __forceinline__ int upper_bound(const float* __restrict__ x, const uint16_t* __restrict__ lut,
                                            const Zone& z, float v) {
   int i = lut[zone_bin(z, v)];
-  while (i < z.e && x[i] <= v) ++i;
+  bool m = i < z.e && x[i] <= v;
+  i += m;
+  m = m && i < z.e && x[i] <= v;
+  i += m;
+  if (m)
+    while (i < z.e && x[i] <= v) ++i;
   return i;
 }
 // plain binary searches (global-memory arrays without a bin table)
@@ -203,7 +223,7 @@ struct UvComb { int n, mask; float m[6]; int hit[6]; };
 // five stereo layers, running-average t_y (A7).
 __device__ __forceinline__ void uv_walk(const SeedParams& p, const float* __restrict__ hx, const Zone* zi,
                                         const uint16_t* __restrict__ lut, const float* xp, int sf, int ih,
-                                        UvComb& c) {
+                                        int min_n, UvComb& c) {
   const int lf = p.ul[sf];
   const float xh = hx[ih];
   const float y0 = (xp[sf] - xh) * p.inv_tan[lf];          // Eq. 16
@@ -211,9 +231,12 @@ __device__ __forceinline__ void uv_walk(const SeedParams& p, const float* __rest
 #pragma unroll
   for (int s = 0; s < 6; ++s) { c.hit[s] = -1; c.m[s] = 0.f; }
   c.hit[sf] = ih; c.m[sf] = xh - xp[sf]; c.mask = 1 << sf; c.n = 1;
+  int left = 5;                                   // stereo layers still to visit
 #pragma unroll
   for (int s = 0; s < 6; ++s) {
     if (s == sf) continue;
+    if (c.n + left < min_n) break;                // cannot reach min_uv_hits: the combination is dropped anyway
+    --left;
     const int l = p.ul[s];
     const float xe = xp[s] - ty * p.zt[l];
     const Zone z = zi[l];
@@ -262,18 +285,18 @@ __device__ __forceinline__ float fit_y(const SeedParams& p, const UvComb& c, flo
 // uv_walk with the first-layer slot as a compile-time constant (keeps xp[]/m[]/hit[] in registers)
 __device__ __forceinline__ void uv_walk_sf(const SeedParams& p, const float* __restrict__ hx, const Zone* zn,
                                            const uint16_t* __restrict__ lut, const float* xp, int sf, int ih,
-                                           UvComb& c) {
+                                           int min_n, UvComb& c) {
   switch (sf) {
-    case 0: uv_walk(p, hx, zn, lut, xp, 0, ih, c); break;
-    case 1: uv_walk(p, hx, zn, lut, xp, 1, ih, c); break;
-    case 2: uv_walk(p, hx, zn, lut, xp, 2, ih, c); break;
-    case 3: uv_walk(p, hx, zn, lut, xp, 3, ih, c); break;
-    case 4: uv_walk(p, hx, zn, lut, xp, 4, ih, c); break;
-    default: uv_walk(p, hx, zn, lut, xp, 5, ih, c); break;
+    case 0: uv_walk(p, hx, zn, lut, xp, 0, ih, min_n, c); break;
+    case 1: uv_walk(p, hx, zn, lut, xp, 1, ih, min_n, c); break;
+    case 2: uv_walk(p, hx, zn, lut, xp, 2, ih, min_n, c); break;
+    case 3: uv_walk(p, hx, zn, lut, xp, 3, ih, min_n, c); break;
+    case 4: uv_walk(p, hx, zn, lut, xp, 4, ih, min_n, c); break;
+    default: uv_walk(p, hx, zn, lut, xp, 5, ih, min_n, c); break;
   }
 }
 
-__global__ void __launch_bounds__(kSeedThreads, 3)
+__global__ void __launch_bounds__(kSeedThreads, LHCB_SEED_MIN_CTAS)
 seeding_kernel(const __grid_constant__ SeedParams p) {
   extern __shared__ __align__(16) unsigned char smem[];
   SeedSmemHeader& H = *reinterpret_cast<SeedSmemHeader*>(smem);
@@ -601,7 +624,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
         }
         const int ih = f + q;
         UvComb c;
-        uv_walk_sf(p, hx, H.zi, lut, xp, sf, ih, c);
+        uv_walk_sf(p, hx, H.zi, lut, xp, sf, ih, p.min_uv_hits, c);
         if (c.n < p.min_uv_hits) continue;
         float ay, by;
         const float chi2y = fit_y(p, c, ay, by);
@@ -629,7 +652,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
 #pragma unroll
     for (int s = 0; s < 6; ++s) xp[s] = xz_at(p, cd.ax, cd.bx, cd.cx, p.ul[s]);
     UvComb c;
-    uv_walk_sf(p, hx, H.zi, lut, xp, sf, ih, c);
+    uv_walk_sf(p, hx, H.zi, lut, xp, sf, ih, 0, c);
     float ay, by;
     const float chi2y = fit_y(p, c, ay, by);
     const int slot = atomicAdd(&H.n_seed, 1);
