@@ -168,9 +168,11 @@ __device__ __forceinline__ int closest_hit(const float* __restrict__ x, const ui
   if (j > z.b) {
     int l = j - 1;
     const float xl = x[l];
-    while (l > z.b && x[l - 1] == xl) --l;     // equal x: the lower index wins
     const float d = fabsf(xl - xp);
-    if (d <= tol) { best = l; bd = d; }
+    if (d <= tol) {
+      while (l > z.b && x[l - 1] == xl) --l;   // equal x: the lower index wins
+      best = l; bd = d;
+    }
   }
   if (j < z.e) {
     const float d = fabsf(x[j] - xp);
@@ -218,6 +220,7 @@ __device__ __forceinline__ unsigned long long clone_key(float chi2, float cx, in
 
 // ------------------------------------------------------------------------------------ u/v walk
 struct UvComb { int n, mask; float m[6]; int hit[6]; };
+struct __align__(16) UvSuccess { uint16_t k; uint8_t pp, n; uint16_t hit[6]; };   // hit: tile index or 0xFFFF
 
 // O8 for one first-layer hit ih (tile index) of pass pp: closest hits within tol_uv in the other
 // five stereo layers, running-average t_y (A7).
@@ -573,9 +576,23 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     if (keep) kept[atomicAdd(&H.n_kept, 1)] = (uint16_t)c;
   }
   __syncthreads();
-  const int nk = H.n_kept;
-  unsigned long long* best = tbl;                            // table is dead: reuse for the best u/v keys
-  for (int i = tid; i < nk; i += T) best[i] = kNoKey;        // nk <= nc <= max_cand <= max_trip (checked at init)
+  int nk = H.n_kept;
+  {                                                            // survivors must leave room for the success queue
+    const int nk_max = ((int)p.max_trip * 8 - 4096) / 40;
+    if (nk > nk_max) { nk = nk_max > 0 ? nk_max : 0; if (tid == 0) H.status |= LHCB_ST_CAND_OVERFLOW; }
+  }
+  // table is dead: reuse the region for [best key per survivor | predictions per survivor | success queue]
+  unsigned long long* best = tbl;
+  float* xps = reinterpret_cast<float*>(best + ((nk + 1) & ~1));          // [nk][8], 16-byte aligned: x_pred per stereo layer
+  UvSuccess* succ = reinterpret_cast<UvSuccess*>(xps + (size_t)nk * 8);
+  const int succ_cap = (int)(((size_t)p.max_trip * 8 - (size_t)nk * 40 - 8) / sizeof(UvSuccess));   // nk <= max_cand <= max_trip/5
+  for (int k = tid; k < nk; k += T) {
+    best[k] = kNoKey;
+    const Cand& cd = cand[kept[k]];
+#pragma unroll
+    for (int s = 0; s < 6; ++s) xps[k * 8 + s] = xz_at(p, cd.ax, cd.bx, cd.cx, p.ul[s]);
+  }
+  if (tid == 0) H.n_trip = 0;                                            // reused as the success counter
   __syncthreads();
 
   // ---- S4: u/v addition (O8, O9) --------------------------------------------------------------
@@ -585,9 +602,8 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     int cnt = 0, fst = 0;
     if (tid < nown) {
       const int w = tile0 + tid, pp = w & 1;
-      const Cand& cd = cand[kept[w >> 1]];
       const int lf = p.uv_first[pp];
-      const float xpf = xz_at(p, cd.ax, cd.bx, cd.cx, lf);
+      const float xpf = xps[(w >> 1) * 8 + p.slot_of_layer[lf]];
       const float wa = xpf - p.ywin_a[h][lf], wb = xpf - p.ywin_b[h][lf];
       const float wlo = wa < wb ? wa : wb, whi = wa > wb ? wa : wb;
       const Zone zf = H.zi[lf];
@@ -605,56 +621,73 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     if (p0 < p1) {
       int t = owner_of(scan.offs, nown, p0) - 1;             // forces a reload on the first item
       int nxt = -1;
-      int f = 0, pp = 0, sf = 0, bf = 0, kk = 0;
+      int f = 0, pp = 0, sf = 0, kk = 0;
       float xp[6];
-      unsigned long long bk = kNoKey;
       for (int q = p0; q < p1; ++q) {
         if (q >= nxt) {
-          if (bk != kNoKey) atomicMin(&best[kk], bk);
-          bk = kNoKey;
           do { ++t; nxt = scan.offs[t + 1]; } while (q >= nxt);
           const int w = tile0 + t;
           kk = w >> 1; pp = w & 1;
-          const Cand& cd = cand[kept[kk]];
-#pragma unroll
-          for (int s = 0; s < 6; ++s) xp[s] = xz_at(p, cd.ax, cd.bx, cd.cx, p.ul[s]);
-          const int lf = p.uv_first[pp];
-          sf = p.slot_of_layer[lf]; bf = zl[lf];
+          const float4 lo4 = *reinterpret_cast<const float4*>(xps + kk * 8);
+          const float2 hi2 = *reinterpret_cast<const float2*>(xps + kk * 8 + 4);
+          xp[0] = lo4.x; xp[1] = lo4.y; xp[2] = lo4.z; xp[3] = lo4.w; xp[4] = hi2.x; xp[5] = hi2.y;
+          sf = p.slot_of_layer[p.uv_first[pp]];
           f = (int)scan.first[t] - scan.offs[t];
         }
         const int ih = f + q;
         UvComb c;
         uv_walk_sf(p, hx, H.zi, lut, xp, sf, ih, p.min_uv_hits, c);
         if (c.n < p.min_uv_hits) continue;
-        float ay, by;
-        const float chi2y = fit_y(p, c, ay, by);
-        if (chi2y > p.chi2y_max) continue;
-        const unsigned long long key = ((unsigned long long)(6 - c.n) << 49) |
-                                       ((unsigned long long)__float_as_uint(chi2y) << 17) |
-                                       ((unsigned long long)pp << 16) | (unsigned long long)(ih - bf);
-        bk = key < bk ? key : bk;
+        const int slot = atomicAdd(&H.n_trip, 1);            // enough hits: queue for the dense fit pass
+        if (slot < succ_cap) {
+          UvSuccess u;
+          u.k = (uint16_t)kk; u.pp = (uint8_t)pp; u.n = (uint8_t)c.n;
+#pragma unroll
+          for (int s = 0; s < 6; ++s) u.hit[s] = c.hit[s] < 0 ? (uint16_t)0xFFFF : (uint16_t)c.hit[s];
+          succ[slot] = u;
+        }
       }
-      if (bk != kNoKey) atomicMin(&best[kk], bk);
     }
     __syncthreads();
   }
+  int nsucc = H.n_trip;
+  if (nsucc > succ_cap) { nsucc = succ_cap; if (tid == 0) H.status |= LHCB_ST_CAND_OVERFLOW; }
 
-  // ---- S5: seeds (O10) ------------------------------------------------------------------------
+  // ---- S5: y fit of every queued combination, best per survivor, seeds (O9, O10) ------------------
   const int pol = p.pol ? (int)p.pol[event] : p.polarity;
-  for (int k = tid; k < nk; k += T) {
-    const unsigned long long key = best[k];
-    if (key == kNoKey) continue;                             // fake x-z projection (L219)
-    const Cand& cd = cand[kept[k]];
-    const int pp = (int)(key >> 16) & 1;
-    const int lf = p.uv_first[pp], sf = p.slot_of_layer[lf];
-    const int ih = zl[lf] + (int)(key & 0xFFFF);
-    float xp[6];
-#pragma unroll
-    for (int s = 0; s < 6; ++s) xp[s] = xz_at(p, cd.ax, cd.bx, cd.cx, p.ul[s]);
+  const bool single = nsucc <= T;                              // the usual case: one combination per thread
+  UvSuccess u;
+  float ay = 0.f, by = 0.f, chi2y = 0.f;
+  unsigned long long key = kNoKey;
+  auto fit_success = [&](int i) {
+    u = succ[i];
     UvComb c;
-    uv_walk_sf(p, hx, H.zi, lut, xp, sf, ih, 0, c);
-    float ay, by;
-    const float chi2y = fit_y(p, c, ay, by);
+    c.n = u.n; c.mask = 0;
+#pragma unroll
+    for (int s = 0; s < 6; ++s) {
+      c.m[s] = 0.f; c.hit[s] = -1;
+      if (u.hit[s] != 0xFFFF) { c.m[s] = hx[u.hit[s]] - xps[u.k * 8 + s]; c.mask |= 1 << s; }
+    }
+    chi2y = fit_y(p, c, ay, by);
+    key = kNoKey;
+    if (!(chi2y > p.chi2y_max)) {
+      const int sf = p.slot_of_layer[p.uv_first[u.pp]];
+      int first_local = 0;
+#pragma unroll
+      for (int s = 0; s < 6; ++s) first_local = (s == sf) ? (int)u.hit[s] - zl[p.ul[s]] : first_local;
+      key = ((unsigned long long)(6 - u.n) << 49) | ((unsigned long long)__float_as_uint(chi2y) << 17) |
+            ((unsigned long long)u.pp << 16) | (unsigned long long)first_local;
+    }
+  };
+  for (int i = tid; i < nsucc; i += T) {
+    fit_success(i);
+    if (key != kNoKey) atomicMin(&best[u.k], key);
+  }
+  __syncthreads();
+  for (int i = tid; i < nsucc; i += T) {
+    if (!single) fit_success(i);                               // more than one round: redo the (cheap) fit
+    if (key == kNoKey || best[u.k] != key) continue;           // not the best combination of its survivor
+    const Cand& cd = cand[kept[u.k]];
     const int slot = atomicAdd(&H.n_seed, 1);
     if (slot >= p.max_seeds) continue;
     const size_t o = (size_t)slot0 + slot, ct = p.cap_total;
@@ -670,10 +703,10 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     for (int s = 0; s < 6; ++s) {
       const int lx = p.xl[s], lu = p.ul[s];
       p.hits[(size_t)lx * ct + o] = cd.hit[s] == 0xFFFF ? LHCB_NO_HIT : a0 + (uint32_t)(zl[lx] + cd.hit[s]);
-      p.hits[(size_t)lu * ct + o] = c.hit[s] < 0 ? LHCB_NO_HIT : a0 + (uint32_t)c.hit[s];
+      p.hits[(size_t)lu * ct + o] = u.hit[s] == 0xFFFF ? LHCB_NO_HIT : a0 + (uint32_t)u.hit[s];
     }
     p.nx[o] = cd.nx;
-    p.nuv[o] = (uint8_t)c.n;
+    p.nuv[o] = u.n;
   }
   __syncthreads();
   if (tid == 0) {
