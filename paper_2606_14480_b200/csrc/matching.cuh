@@ -3,8 +3,13 @@
 // One CTA per event.  The event's VELO states are staged in shared memory; the x0 of the event's UT
 // hits (four sorted layers, contiguous in memory) is fetched with one bulk async copy that lands while
 // the all-pairs loop runs, so the UT searches are shared-memory binary searches.
-//   M1/M2  warp per seed, lanes over VELO tracks: kink extrapolation (Eq. 17-18), preselection
-//          (Eq. 21), chi2_match (Eq. 22-23) < 2; accepted pairs are queued in shared memory
+//   M0     VELO states are rank-sorted by t_y into shared memory
+//   M1/M2  "all seed x VELO pairs" (L279) without touching most of them: the |dty| cut of Eq. 21 selects
+//          a contiguous range of the t_y-sorted VELO states (found by binary search with a safety
+//          margin; the literal cut is still applied to every pair in the range, so the accepted set
+//          is exactly that of the exhaustive loop).  Pairs in range are flattened over the CTA:
+//          kink extrapolation (Eq. 17-18), preselection (Eq. 21), chi2_match (Eq. 22-23) < 2; accepted
+//          pairs are queued in shared memory
 //   M3     thread per queued pair: UT hit search (Eq. 19-20, Table 2)
 //   M4     one-to-one selection with two rounds of 64-bit atomicMin (reading A14), output
 //
@@ -51,7 +56,7 @@ struct MatchParams {
 };
 
 struct __align__(16) MatchCand {
-  uint16_t seed, velo;      // event-local indices
+  uint16_t seed, velo;      // event-local seed index; rank of the VELO state in t_y order
   float chi2, q0, gamma;
   uint16_t ut[4];           // UT hit index relative to the event's first UT hit, 0xFFFF = none
   uint8_t n_ut, valid, pad[6];
@@ -61,7 +66,11 @@ static_assert(sizeof(MatchCand) == 32, "MatchCand is 32 bytes");
 __host__ __device__ inline size_t match_smem_bytes(int max_seeds, int max_mc, int max_velo, int max_ut) {
   size_t b = 64;
   b += ((size_t)max_ut + 8) * 4;             // UT x0 tile (16-byte aligned superset)
-  b += (size_t)max_velo * 16;                // VELO states
+  b += (size_t)max_velo * 16;                // VELO states, sorted by ty
+  b += (size_t)max_velo * 4;                 // unsorted ty (rank sort input)
+  b += (size_t)max_velo * 2;                 // original index of each sorted state
+  b = (b + 15) & ~(size_t)15;
+  b += (kMatchThreads + 1) * 4 + kMatchThreads * 2 + 64;   // work-list scan scratch
   b = (b + 15) & ~(size_t)15;
   b += (size_t)max_mc * sizeof(MatchCand);
   b += (size_t)2 * max_seeds * 8;            // best key per seed
@@ -155,14 +164,21 @@ matching_kernel(const __grid_constant__ MatchParams p) {
   float* svy = svx + p.max_velo;
   float* svtx = svy + p.max_velo;
   float* svty = svtx + p.max_velo;
-  size_t off = 64 + ((size_t)p.max_ut + 8) * 4 + (size_t)p.max_velo * 16;
+  float* tmp_ty = svty + p.max_velo;
+  uint16_t* sorig = reinterpret_cast<uint16_t*>(tmp_ty + p.max_velo);
+  size_t off = 64 + ((size_t)p.max_ut + 8) * 4 + (size_t)p.max_velo * 22;
+  off = (off + 15) & ~(size_t)15;
+  int* offs = reinterpret_cast<int*>(smem + off);                         // [kMatchThreads + 1]
+  uint16_t* firsts = reinterpret_cast<uint16_t*>(offs + kMatchThreads + 1);
+  int* warp_sums = reinterpret_cast<int*>(smem + off + (kMatchThreads + 1) * 4 + kMatchThreads * 2);
+  off += (kMatchThreads + 1) * 4 + kMatchThreads * 2 + 64;
   off = (off + 15) & ~(size_t)15;
   MatchCand* mc = reinterpret_cast<MatchCand*>(smem + off);
   off += (size_t)p.max_mc * sizeof(MatchCand);
   unsigned long long* seed_best = reinterpret_cast<unsigned long long*>(smem + off);
   unsigned long long* velo_best = seed_best + 2 * p.max_seeds;
 
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = kMatchThreads / 32;
+  const int tid = threadIdx.x;
   const int e = blockIdx.x;
   const uint32_t v0 = p.velo_off[e];
   const int nv = (int)(p.velo_off[e + 1] - v0);
@@ -213,46 +229,89 @@ matching_kernel(const __grid_constant__ MatchParams p) {
       hdr[4 + tid] = (int)p.ut_off[(size_t)e * 4 + tid];
     }
   }
-  for (int v = tid; v < nv; v += kMatchThreads) {
-    svx[v] = p.vx[v0 + v]; svy[v] = p.vy[v0 + v]; svtx[v] = p.vtx[v0 + v]; svty[v] = p.vty[v0 + v];
-    velo_best[v] = kNoKey;
-  }
+  for (int v = tid; v < nv; v += kMatchThreads) { tmp_ty[v] = p.vty[v0 + v]; velo_best[v] = kNoKey; }
   for (int s = tid; s < ns; s += kMatchThreads) seed_best[s] = kNoKey;
   __syncthreads();
+  // ---- M0: rank sort of the VELO states by ty (ties by index) ---------------------------------
+  for (int v = tid; v < nv; v += kMatchThreads) {
+    const float t = tmp_ty[v];
+    int r = 0;
+    for (int u = 0; u < nv; ++u) {
+      const float tu = tmp_ty[u];
+      r += (tu < t || (tu == t && u < v)) ? 1 : 0;
+    }
+    svx[r] = p.vx[v0 + v]; svy[r] = p.vy[v0 + v]; svtx[r] = p.vtx[v0 + v]; svty[r] = t;
+    sorig[r] = (uint16_t)v;
+  }
+  __syncthreads();
 
-  // ---- M1/M2: all seed x VELO pairs (L279) ---------------------------------------------------
+  // ---- M1/M2: all seed x VELO pairs (L279), restricted to the |dty| range of each seed ----------
   const size_t sct = p.seed_cap_total;
-  for (int s = warp; s < ns; s += nwarps) {
-    const size_t slot = s < c0 ? (size_t)(2 * e) * p.max_seeds + s : (size_t)(2 * e + 1) * p.max_seeds + (s - c0);
-    const float xS = p.state[slot], yS = p.state[sct + slot], txS = p.state[2 * sct + slot],
-                tyS = p.state[3 * sct + slot];
-    const float axS = fabsf(xS);
-    const float ys = yS + p.dzyS * tyS;                                          // L231
-    for (int v = lane; v < nv; v += 32) {
-      const float xV = svx[v], yV = svy[v], txV = svtx[v], tyV = svty[v];
-      const float dtx = txS - txV, dty = tyS - tyV, adtx = fabsf(dtx);
-      const float zm = (((p.mag[0] + p.mag[1] * adtx) + p.mag[2] * (dtx * dtx)) + p.mag[3] * axS) +
-                       p.mag[4] * (txV * txV);                                   // Eq. 18
-      const float xs = xS + (zm - p.zS) * txS, xv = xV + (zm - p.zV) * txV;      // Eq. 17
-      const float yv = yV + p.dzyV * tyV;
-      const float dx = xs - xv, dy = ys - yv;
-      if (!(fabsf(dx) < p.presel[0] && fabsf(dy) < p.presel[1] && adtx < p.presel[2] &&
-            fabsf(dty) < p.presel[3]))                                           // Eq. 21
-        continue;
-      const float tolx = p.cx0 + p.cx1 * (dtx * dtx);                            // Eq. 23
-      const float toly = p.cy0 + p.cy1 * (txV * txV + tyV * tyV);
-      const float chi2 = (((dx * dx) / tolx + (dy * dy) / toly) + (dtx * dtx) * p.inv_tol_tx) +
-                         (dty * dty) * p.inv_tol_ty;                             // Eq. 22
-      if (!(chi2 < p.chi2m_max)) continue;                                       // L301
-      const int k = atomicAdd(&hdr[0], 1);
-      if (k < p.max_mc) {
-        MatchCand m;
-        m.seed = (uint16_t)s; m.velo = (uint16_t)v; m.chi2 = chi2; m.q0 = dtx * p.inv_KB; m.gamma = 0.f;
-        m.ut[0] = m.ut[1] = m.ut[2] = m.ut[3] = 0xFFFF;
-        m.n_ut = 0; m.valid = 1;
-        mc[k] = m;
+  constexpr int T = kMatchThreads;
+  for (int tile0 = 0; tile0 < ns; tile0 += T) {
+    const int nown = ns - tile0 < T ? ns - tile0 : T;
+    int cnt = 0, fst = 0;
+    if (tid < nown) {
+      const int s = tile0 + tid;
+      const size_t slot = s < c0 ? (size_t)(2 * e) * p.max_seeds + s : (size_t)(2 * e + 1) * p.max_seeds + (s - c0);
+      const float tyS = p.state[3 * sct + slot];
+      // superset of {v : |tyS - tyV| < presel[3]} whatever the rounding of the subtraction
+      const float w = p.presel[3] + 1e-6f * (fabsf(tyS) + p.presel[3]) + 1e-30f;
+      fst = lower_bound(svty, 0, nv, tyS - w);
+      int lst = fst;
+      { int n = nv - fst; const float hi = tyS + w;
+        while (n > 0) { const int hh = n >> 1; const bool le = svty[lst + hh] <= hi; lst = le ? lst + hh + 1 : lst; n = le ? n - hh - 1 : hh; } }
+      cnt = lst - fst;
+    }
+    int total;
+    const int ex = block_exscan<T>(cnt, warp_sums, total);
+    offs[tid] = ex; firsts[tid] = (uint16_t)fst;
+    if (tid == T - 1) offs[T] = total;
+    __syncthreads();
+    const int chunk = (total + T - 1) / T;
+    const int p0 = tid * chunk, p1 = p0 + chunk < total ? p0 + chunk : total;
+    if (p0 < p1) {
+      int t = owner_of(offs, nown, p0) - 1;
+      int nxt = -1, f = 0, s = 0;
+      float xS = 0.f, txS = 0.f, tyS = 0.f, axS = 0.f, ys = 0.f;
+      for (int q = p0; q < p1; ++q) {
+        if (q >= nxt) {
+          do { ++t; nxt = offs[t + 1]; } while (q >= nxt);
+          s = tile0 + t;
+          const size_t slot = s < c0 ? (size_t)(2 * e) * p.max_seeds + s : (size_t)(2 * e + 1) * p.max_seeds + (s - c0);
+          xS = p.state[slot]; const float yS = p.state[sct + slot]; txS = p.state[2 * sct + slot];
+          tyS = p.state[3 * sct + slot];
+          axS = fabsf(xS);
+          ys = yS + p.dzyS * tyS;                                                  // L231
+          f = (int)firsts[t] - offs[t];
+        }
+        const int v = f + q;                                                       // rank in ty order
+        const float xV = svx[v], yV = svy[v], txV = svtx[v], tyV = svty[v];
+        const float dtx = txS - txV, dty = tyS - tyV, adtx = fabsf(dtx);
+        const float zm = (((p.mag[0] + p.mag[1] * adtx) + p.mag[2] * (dtx * dtx)) + p.mag[3] * axS) +
+                         p.mag[4] * (txV * txV);                                   // Eq. 18
+        const float xs = xS + (zm - p.zS) * txS, xv = xV + (zm - p.zV) * txV;      // Eq. 17
+        const float yv = yV + p.dzyV * tyV;
+        const float dx = xs - xv, dy = ys - yv;
+        if (!(fabsf(dx) < p.presel[0] && fabsf(dy) < p.presel[1] && adtx < p.presel[2] &&
+              fabsf(dty) < p.presel[3]))                                           // Eq. 21
+          continue;
+        const float tolx = p.cx0 + p.cx1 * (dtx * dtx);                            // Eq. 23
+        const float toly = p.cy0 + p.cy1 * (txV * txV + tyV * tyV);
+        const float chi2 = (((dx * dx) / tolx + (dy * dy) / toly) + (dtx * dtx) * p.inv_tol_tx) +
+                           (dty * dty) * p.inv_tol_ty;                             // Eq. 22
+        if (!(chi2 < p.chi2m_max)) continue;                                       // L301
+        const int k = atomicAdd(&hdr[0], 1);
+        if (k < p.max_mc) {
+          MatchCand m;
+          m.seed = (uint16_t)s; m.velo = (uint16_t)v; m.chi2 = chi2; m.q0 = dtx * p.inv_KB; m.gamma = 0.f;
+          m.ut[0] = m.ut[1] = m.ut[2] = m.ut[3] = 0xFFFF;
+          m.n_ut = 0; m.valid = 1;
+          mc[k] = m;
+        }
       }
     }
+    __syncthreads();
   }
   __syncthreads();
   int nm = hdr[0];
@@ -291,7 +350,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
       }
     }
     if (m.valid)
-      atomicMin(&seed_best[m.seed], ((unsigned long long)__float_as_uint(m.chi2) << 32) | m.velo);
+      atomicMin(&seed_best[m.seed], ((unsigned long long)__float_as_uint(m.chi2) << 32) | sorig[m.velo]);
   }
   __syncthreads();
   // ---- M4: one-to-one selection (O14) -------------------------------------------------------------
@@ -299,8 +358,8 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     const MatchCand& m = mc[k];
     if (!m.valid) continue;
     const unsigned long long cb = (unsigned long long)__float_as_uint(m.chi2) << 32;
-    if (seed_best[m.seed] != (cb | m.velo)) continue;
-    atomicMin(&velo_best[m.velo], cb | m.seed);
+    if (seed_best[m.seed] != (cb | sorig[m.velo])) continue;
+    atomicMin(&velo_best[sorig[m.velo]], cb | m.seed);
   }
   __syncthreads();
   const int pol = p.pol ? (int)p.pol[e] : p.polarity;
@@ -308,13 +367,14 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     const MatchCand& m = mc[k];
     if (!m.valid) continue;
     const unsigned long long cb = (unsigned long long)__float_as_uint(m.chi2) << 32;
-    if (seed_best[m.seed] != (cb | m.velo) || velo_best[m.velo] != (cb | m.seed)) continue;
+    const int vo = sorig[m.velo];
+    if (seed_best[m.seed] != (cb | vo) || velo_best[vo] != (cb | m.seed)) continue;
     const int slot = atomicAdd(&hdr[1], 1);
     if (slot >= p.max_long) continue;
     const size_t o = (size_t)e * p.max_long + slot, ct = p.long_cap_total;
     const int s = m.seed;
     p.seed_idx[o] = s < c0 ? (uint32_t)((2 * e) * p.max_seeds + s) : (uint32_t)((2 * e + 1) * p.max_seeds + (s - c0));
-    p.velo_idx[o] = v0 + m.velo;
+    p.velo_idx[o] = v0 + vo;
 #pragma unroll
     for (int l = 0; l < 4; ++l) p.ut_idx[(size_t)l * ct + o] = m.ut[l] == 0xFFFF ? LHCB_NO_HIT : u_begin + m.ut[l];
     p.n_ut[o] = m.n_ut;

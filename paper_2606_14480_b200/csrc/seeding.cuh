@@ -182,6 +182,7 @@ __device__ __forceinline__ int closest_hit(const float* __restrict__ x, const ui
 }
 
 // exclusive prefix sum of one int per thread over the CTA; total returned to every thread
+template <int NT>
 __device__ __forceinline__ int block_exscan(int v, int* warp_sums, int& total) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   int inc = v;
@@ -193,16 +194,16 @@ __device__ __forceinline__ int block_exscan(int v, int* warp_sums, int& total) {
   if (lane == 31) warp_sums[warp] = inc;
   __syncthreads();
   if (warp == 0) {
-    int w = lane < kSeedThreads / 32 ? warp_sums[lane] : 0;
+    int w = lane < NT / 32 ? warp_sums[lane] : 0;
 #pragma unroll
-    for (int o = 1; o < kSeedThreads / 32; o <<= 1) {
+    for (int o = 1; o < NT / 32; o <<= 1) {
       const int t = __shfl_up_sync(0xffffffffu, w, o);
       if (lane >= o) w += t;
     }
-    if (lane < kSeedThreads / 32) warp_sums[lane] = w;       // inclusive warp totals
+    if (lane < NT / 32) warp_sums[lane] = w;                 // inclusive warp totals
   }
   __syncthreads();
-  total = warp_sums[kSeedThreads / 32 - 1];
+  total = warp_sums[NT / 32 - 1];
   const int base = warp ? warp_sums[warp - 1] : 0;
   return base + inc - v;
 }
@@ -435,7 +436,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
         cnt = upper_bound(hx, lut3, z3n, hi) - fst;
       }
       int total;
-      const int ex = block_exscan(cnt, H.warp_sums, total);
+      const int ex = block_exscan<kSeedThreads>(cnt, H.warp_sums, total);
       scan.offs[tid] = ex; scan.first[tid] = (uint16_t)fst;
       if (tid == T - 1) scan.offs[T] = total;
       __syncthreads();
@@ -612,7 +613,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
       cnt = upper_bound(hx, lutf, zf, whi) - fst;
     }
     int total;
-    const int ex = block_exscan(cnt, H.warp_sums, total);
+    const int ex = block_exscan<kSeedThreads>(cnt, H.warp_sums, total);
     scan.offs[tid] = ex; scan.first[tid] = (uint16_t)fst;
     if (tid == T - 1) scan.offs[T] = total;
     __syncthreads();
