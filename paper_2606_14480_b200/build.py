@@ -30,6 +30,9 @@ def _deps():
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
+    override = os.environ.get("LHCB_B200_LIB")       # a prebuilt variant (e.g. a -DLHCB_STAGE_CLOCKS diagnostic build)
+    if override:
+        return override
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in _deps()):
         return LIB
     cmd = [NVCC, *FLAGS, *sources(), "-o", LIB]

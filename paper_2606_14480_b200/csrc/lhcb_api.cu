@@ -213,6 +213,18 @@ const char* lhcb_error_string(int s) {
   }
 }
 
+#ifdef LHCB_STAGE_CLOCKS
+// diagnostic builds only: cycles summed over CTAs per seeding stage; reset != 0 zeroes the counters
+int lhcb_debug_stage_clocks(unsigned long long* out, int reset) {
+  if (out && cudaMemcpyFromSymbol(out, lhcb::g_stage_clk, sizeof(lhcb::g_stage_clk)) != cudaSuccess) return LHCB_ERR_CUDA;
+  if (reset) {
+    unsigned long long z[16] = {0};
+    if (cudaMemcpyToSymbol(lhcb::g_stage_clk, z, sizeof(z)) != cudaSuccess) return LHCB_ERR_CUDA;
+  }
+  return LHCB_OK;
+}
+#endif
+
 int lhcb_last_cuda_error(const lhcb_ctx* c) { return c ? c->last_cuda_error : 0; }
 int lhcb_last_launch_count(const lhcb_ctx* c) { return c ? c->last_launches : 0; }
 

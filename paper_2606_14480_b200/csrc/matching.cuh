@@ -180,6 +180,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
 
   const int tid = threadIdx.x;
   const int e = blockIdx.x;
+  LHCB_CLK_INIT
   const uint32_t v0 = p.velo_off[e];
   const int nv = (int)(p.velo_off[e + 1] - v0);
   int c0 = (int)p.seed_count[2 * e], c1 = (int)p.seed_count[2 * e + 1];
@@ -244,6 +245,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     sorig[r] = (uint16_t)v;
   }
   __syncthreads();
+  LHCB_CLK(9)
 
   // ---- M1/M2: all seed x VELO pairs (L279), restricted to the |dty| range of each seed ----------
   const size_t sct = p.seed_cap_total;
@@ -268,6 +270,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     offs[tid] = ex; firsts[tid] = (uint16_t)fst;
     if (tid == T - 1) offs[T] = total;
     __syncthreads();
+    LHCB_CLK(10)
     const int chunk = (total + T - 1) / T;
     const int p0 = tid * chunk, p1 = p0 + chunk < total ? p0 + chunk : total;
     if (p0 < p1) {
@@ -312,6 +315,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
       }
     }
     __syncthreads();
+    LHCB_CLK(11)
   }
   __syncthreads();
   int nm = hdr[0];
@@ -353,6 +357,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
       atomicMin(&seed_best[m.seed], ((unsigned long long)__float_as_uint(m.chi2) << 32) | sorig[m.velo]);
   }
   __syncthreads();
+  LHCB_CLK(12)
   // ---- M4: one-to-one selection (O14) -------------------------------------------------------------
   for (int k = tid; k < nm; k += kMatchThreads) {
     const MatchCand& m = mc[k];
@@ -383,6 +388,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     p.chi2[o] = m.chi2;
   }
   __syncthreads();
+  LHCB_CLK(13)
   if (tid == 0) {
     int nl = hdr[1];
     unsigned st = (unsigned)hdr[2];

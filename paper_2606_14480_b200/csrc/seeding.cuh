@@ -38,6 +38,22 @@ constexpr int kSeedThreads = LHCB_SEED_THREADS;
 constexpr int kLutBins = LHCB_LUT_BINS;       // bins of the per-zone search table
 constexpr unsigned long long kNoKey = ~0ull;
 
+// Optional per-stage cycle counters (diagnostic builds only: -DLHCB_STAGE_CLOCKS).  Thread 0 of every
+// CTA adds the cycles since its previous mark to g_stage_clk[i]; lhcb_debug_stage_clocks() reads them.
+#ifdef LHCB_STAGE_CLOCKS
+__device__ unsigned long long g_stage_clk[16];
+#define LHCB_CLK_INIT long long clk_prev__ = clock64();
+#define LHCB_CLK(i)                                                                         \
+  if (threadIdx.x == 0) {                                                                   \
+    const long long t__ = clock64();                                                        \
+    atomicAdd(&g_stage_clk[i], (unsigned long long)(t__ - clk_prev__));                     \
+    clk_prev__ = t__;                                                                       \
+  }
+#else
+#define LHCB_CLK_INIT
+#define LHCB_CLK(i)
+#endif
+
 struct SeedParams {
   float zb[12], gz[12], tan_a[12], inv_tan[12], inv_z[12], zt[12];
   float ywin_a[2][12], ywin_b[2][12];
@@ -322,6 +338,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   constexpr int T = kSeedThreads, nwarps = kSeedThreads / 32;
+  LHCB_CLK_INIT
   const int half_id = blockIdx.x, event = half_id >> 1, h = half_id & 1;
   const uint32_t* zo = p.zone_off + (size_t)half_id * 12;
 
@@ -379,6 +396,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     }
   }
   __syncthreads();
+  LHCB_CLK(0)
   const int* zl = H.zl;
   if (H.xbase[6] > p.max_trip) {                            // clone table would not fit
     if (tid == 0) { p.count[half_id] = 0; p.status[half_id] = LHCB_ST_HITS_OVERFLOW; }
@@ -413,6 +431,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     }
   }
   __syncthreads();
+  LHCB_CLK(1)
 
   // ---- S1 + S2 per iteration -----------------------------------------------------------
   for (int it = 0; it < 2; ++it) {
@@ -440,6 +459,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
       scan.offs[tid] = ex; scan.first[tid] = (uint16_t)fst;
       if (tid == T - 1) scan.offs[T] = total;
       __syncthreads();
+      LHCB_CLK(2)
       // flattened pairs: thread owns pairs [p0, p1)
       const int chunk = (total + T - 1) / T;
       const int p0 = tid * chunk, p1 = p0 + chunk < total ? p0 + chunk : total;
@@ -478,6 +498,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
         }
       }
       __syncthreads();
+      LHCB_CLK(3)
     }
     int nt = H.n_trip;
     if (nt > p.max_trip) { nt = p.max_trip; if (tid == 0) H.status |= LHCB_ST_TRIPLET_OVERFLOW; }
@@ -547,6 +568,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
       }
     }
     __syncthreads();
+    LHCB_CLK(4)
     if (tid == 0) H.n_trip = 0;
     __syncthreads();
   }
@@ -595,6 +617,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   }
   if (tid == 0) H.n_trip = 0;                                            // reused as the success counter
   __syncthreads();
+  LHCB_CLK(5)
 
   // ---- S4: u/v addition (O8, O9) --------------------------------------------------------------
   // owners w = 2*k + pass (k-th survivor); items = first-layer hits in the window of Eq. 16
@@ -617,6 +640,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     scan.offs[tid] = ex; scan.first[tid] = (uint16_t)fst;
     if (tid == T - 1) scan.offs[T] = total;
     __syncthreads();
+    LHCB_CLK(6)
     const int chunk = (total + T - 1) / T;
     const int p0 = tid * chunk, p1 = p0 + chunk < total ? p0 + chunk : total;
     if (p0 < p1) {
@@ -650,6 +674,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
       }
     }
     __syncthreads();
+    LHCB_CLK(7)
   }
   int nsucc = H.n_trip;
   if (nsucc > succ_cap) { nsucc = succ_cap; if (tid == 0) H.status |= LHCB_ST_CAND_OVERFLOW; }
@@ -710,6 +735,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     p.nuv[o] = u.n;
   }
   __syncthreads();
+  LHCB_CLK(8)
   if (tid == 0) {
     int ns = H.n_seed;
     unsigned st = H.status;
