@@ -10,8 +10,12 @@
 //          is exactly that of the exhaustive loop).  Pairs in range are flattened over the CTA:
 //          kink extrapolation (Eq. 17-18), preselection (Eq. 21), chi2_match (Eq. 22-23) < 2; accepted
 //          pairs are queued in shared memory
-//   M3     thread per queued pair: UT hit search (Eq. 19-20, Table 2)
-//   M4     one-to-one selection with two rounds of 64-bit atomicMin (reading A14), output
+//   M3a    thread per queued pair: loose UT window, layer by layer until one has hits; every such hit
+//          becomes a queued hypothesis (Eq. 19-20, Table 2, reading A13)
+//   M3b    thread per hypothesis: tight windows in the remaining layers, gamma_x refits; the best
+//          hypothesis of each pair wins a packed-key atomicMin (max hits, min residuals, first hit)
+//   M4     one-to-one selection with two rounds of 64-bit atomicMin (reading A14); the winning
+//          hypothesis of each selected pair is walked once more to write its hits
 //
 // Arithmetic follows DESIGN.md "Arithmetic specification"; compiled with -fmad=false.
 #pragma once
@@ -55,13 +59,13 @@ struct MatchParams {
   size_t long_cap_total;
 };
 
-struct __align__(16) MatchCand {
+struct __align__(8) MatchCand {
   uint16_t seed, velo;      // event-local seed index; rank of the VELO state in t_y order
-  float chi2, q0, gamma;
-  uint16_t ut[4];           // UT hit index relative to the event's first UT hit, 0xFFFF = none
-  uint8_t n_ut, valid, pad[6];
+  float chi2, q0;
+  uint32_t valid;
+  unsigned long long key;   // best UT hypothesis: (4 - n_ut) << 50 | f32 bits of sum res^2 << 18 | layer << 16 | first hit
 };
-static_assert(sizeof(MatchCand) == 32, "MatchCand is 32 bytes");
+static_assert(sizeof(MatchCand) == 24, "MatchCand is 24 bytes");
 
 __host__ __device__ inline size_t match_smem_bytes(int max_seeds, int max_mc, int max_velo, int max_ut) {
   size_t b = 64;
@@ -73,6 +77,8 @@ __host__ __device__ inline size_t match_smem_bytes(int max_seeds, int max_mc, in
   b += (kMatchThreads + 1) * 4 + kMatchThreads * 2 + 64;   // work-list scan scratch
   b = (b + 15) & ~(size_t)15;
   b += (size_t)max_mc * sizeof(MatchCand);
+  b += (size_t)max_mc * 4;                   // UT hypothesis queue
+  b = (b + 15) & ~(size_t)15;
   b += (size_t)2 * max_seeds * 8;            // best key per seed
   b += (size_t)max_velo * 8;                 // best key per VELO track
   return b;
@@ -86,78 +92,61 @@ __device__ __forceinline__ float ut_window(const float* w, float invpG) {
   return lo < w[3] ? lo : w[3];
 }
 
-// O13: loose window until the first layer with hits; every loose hit starts a hypothesis (A13),
-// remaining layers use tight windows and the closest hit; gamma_x is refitted after each hit.
-// ux[i] is the x0 of the UT hit whose y-range is (uylo[i + ybase], uyhi[i + ybase]); uo[] are the layer
-// offsets in the indexing of ux (shared-memory tile or the global array).
-__device__ inline bool ut_search(const MatchParams& p, float xV, float yV, float txV, float tyV, float q0,
-                                 const float* __restrict__ ux, const int* uo, int ybase, UtHyp& best) {
-  const float* __restrict__ uylo = p.uylo + ybase;
-  const float* __restrict__ uyhi = p.uyhi + ybase;
-  const float invpG = fabsf(q0) * 1000.f;
-  const float gamma0 = p.Ag + p.Bg * q0;                    // Eq. 20
-  bool have = false;
-  for (int i0 = 0; i0 < 4; ++i0) {
-    if (4 - i0 < p.min_ut_hits) break;
-    const float yi = yV + tyV * p.ut_dz[i0];
-    const float xi = (xV + txV * p.ut_dz[i0]) + gamma0 * p.ut_dz2[i0];        // Eq. 19
-    const float x0e = xi - yi * p.ut_tan[i0];
-    const float w = ut_window(p.ut_loose[i0], invpG);
-    const float lo = x0e - w, hi = x0e + w;
-    const int b = uo[i0], e = uo[i0 + 1];
-    bool found = false;
-    for (int j = lower_bound(ux, b, e, lo); j < e && ux[j] <= hi; ++j) {
-      if (!(uylo[j] - p.ut_y_tol <= yi && yi <= uyhi[j] + p.ut_y_tol)) continue;
-      found = true;
-      UtHyp hy;
-      float dj[4];
+// O13, second half: hypothesis (layer i0, hit j) of one accepted pair.  The remaining layers use tight
+// windows and the closest hit; gamma_x is refitted after each hit (L309).  ux is the searched x0 array
+// (shared-memory tile or the global array), uo[] its layer offsets; the y-range of hit i of ux is
+// (uylo[i], uyhi[i]) (global memory, already offset to the indexing of ux).
+__device__ __forceinline__ void ut_tight_walk(const MatchParams& p, float xV, float yV, float txV, float tyV,
+                                              float invpG, int i0, int j, const float* __restrict__ ux,
+                                              const float* __restrict__ uylo, const float* __restrict__ uyhi,
+                                              const int* uo, UtHyp& hy) {
+  float dj[4];
+  float num = 0.f, den = 0.f, gam = 0.f;
+  hy.n = 0;
 #pragma unroll
-      for (int k = 0; k < 4; ++k) { hy.idx[k] = -1; dj[k] = 0.f; }
-      hy.n = 1; hy.idx[i0] = j;
-      dj[i0] = ((ux[j] + yi * p.ut_tan[i0]) - xV) - txV * p.ut_dz[i0];
-      float num = dj[i0] * p.ut_dz2[i0], den = p.ut_dz4[i0];
-      float gam = num / den;
-      for (int i = i0 + 1; i < 4; ++i) {
-        const float yt = yV + tyV * p.ut_dz[i];
-        const float xt = (xV + txV * p.ut_dz[i]) + gam * p.ut_dz2[i];
-        const float xe = xt - yt * p.ut_tan[i];
-        const float wt = ut_window(p.ut_tight[i], invpG);
-        const float tlo = xe - wt, thi = xe + wt;
-        const int bb = uo[i], ee = uo[i + 1];
-        int bj = -1;
-        float bd = 0.f;
-        for (int jj = lower_bound(ux, bb, ee, tlo); jj < ee && ux[jj] <= thi; ++jj) {
-          if (!(uylo[jj] - p.ut_y_tol <= yt && yt <= uyhi[jj] + p.ut_y_tol)) continue;
-          const float dd = fabsf(ux[jj] - xe);
-          if (bj < 0 || dd < bd) { bj = jj; bd = dd; }
-        }
-        if (bj >= 0) {
-          hy.idx[i] = bj; ++hy.n;
-          dj[i] = ((ux[bj] + yt * p.ut_tan[i]) - xV) - txV * p.ut_dz[i];
-          num = num + dj[i] * p.ut_dz2[i]; den = den + p.ut_dz4[i];
-          gam = num / den;
-        }
+  for (int i = 0; i < 4; ++i) {
+    hy.idx[i] = -1; dj[i] = 0.f;
+    if (i < i0) continue;
+    const float yt = yV + tyV * p.ut_dz[i];
+    int bj = -1;
+    if (i == i0) {
+      bj = j;
+    } else {
+      const float xt = (xV + txV * p.ut_dz[i]) + gam * p.ut_dz2[i];            // Eq. 19
+      const float xe = xt - yt * p.ut_tan[i];
+      const float wt = ut_window(p.ut_tight[i], invpG);
+      const float tlo = xe - wt, thi = xe + wt;
+      const int bb = uo[i], ee = uo[i + 1];
+      float bd = 0.f;
+      for (int jj = lower_bound(ux, bb, ee, tlo); jj < ee && ux[jj] <= thi; ++jj) {
+        if (!(uylo[jj] - p.ut_y_tol <= yt && yt <= uyhi[jj] + p.ut_y_tol)) continue;
+        const float dd = fabsf(ux[jj] - xe);
+        if (bj < 0 || dd < bd) { bj = jj; bd = dd; }
       }
-      hy.gamma = gam; hy.ssq = 0.f;
-      bool first = true;
-#pragma unroll
-      for (int i = 0; i < 4; ++i)
-        if (hy.idx[i] >= 0) {
-          const float res = dj[i] - gam * p.ut_dz2[i];
-          hy.ssq = first ? res * res : hy.ssq + res * res;
-          first = false;
-        }
-      if (!have || hy.n > best.n || (hy.n == best.n && hy.ssq < best.ssq)) { best = hy; have = true; }
     }
-    if (found) break;
+    if (bj >= 0) {
+      hy.idx[i] = bj; ++hy.n;
+      dj[i] = ((ux[bj] + yt * p.ut_tan[i]) - xV) - txV * p.ut_dz[i];
+      if (i == i0) { num = dj[i] * p.ut_dz2[i]; den = p.ut_dz4[i]; }
+      else { num = num + dj[i] * p.ut_dz2[i]; den = den + p.ut_dz4[i]; }
+      gam = num / den;
+    }
   }
-  return have && best.n >= p.min_ut_hits;
+  hy.gamma = gam; hy.ssq = 0.f;
+  bool first = true;
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+    if (hy.idx[i] >= 0) {
+      const float res = dj[i] - gam * p.ut_dz2[i];
+      hy.ssq = first ? res * res : hy.ssq + res * res;
+      first = false;
+    }
 }
 
 __global__ void __launch_bounds__(kMatchThreads)
 matching_kernel(const __grid_constant__ MatchParams p) {
   extern __shared__ __align__(16) unsigned char smem[];
-  int* hdr = reinterpret_cast<int*>(smem);                  // [0] n_mc, [1] n_long, [2] status, [4..8] UT offsets
+  int* hdr = reinterpret_cast<int*>(smem);                  // [0] n_mc, [1] n_long, [2] status, [3] n_hyp, [4..8] UT offsets
   unsigned long long* mbar = reinterpret_cast<unsigned long long*>(smem + 48);
   float* sux = reinterpret_cast<float*>(smem + 64);
   float* svx = sux + p.max_ut + 8;
@@ -175,6 +164,9 @@ matching_kernel(const __grid_constant__ MatchParams p) {
   off = (off + 15) & ~(size_t)15;
   MatchCand* mc = reinterpret_cast<MatchCand*>(smem + off);
   off += (size_t)p.max_mc * sizeof(MatchCand);
+  uint32_t* hyq = reinterpret_cast<uint32_t*>(smem + off);                 // (pair << 18) | (layer << 16) | first hit
+  off += (size_t)p.max_mc * 4;
+  off = (off + 15) & ~(size_t)15;
   unsigned long long* seed_best = reinterpret_cast<unsigned long long*>(smem + off);
   unsigned long long* velo_best = seed_best + 2 * p.max_seeds;
 
@@ -191,7 +183,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     if (tid == 0) { p.count[e] = 0; p.status[e] = LHCB_ST_VELO_OVERFLOW; }
     return;
   }
-  if (tid < 3) hdr[tid] = 0;
+  if (tid < 4) hdr[tid] = 0;
   // ---- UT x0 of this event: one bulk copy, overlapped with the all-pairs loop -----------------
   uint32_t u_begin = 0, u_end = 0, ua0 = 0, ua1 = 0;
   bool ut_in_smem = false;
@@ -307,9 +299,8 @@ matching_kernel(const __grid_constant__ MatchParams p) {
         const int k = atomicAdd(&hdr[0], 1);
         if (k < p.max_mc) {
           MatchCand m;
-          m.seed = (uint16_t)s; m.velo = (uint16_t)v; m.chi2 = chi2; m.q0 = dtx * p.inv_KB; m.gamma = 0.f;
-          m.ut[0] = m.ut[1] = m.ut[2] = m.ut[3] = 0xFFFF;
-          m.n_ut = 0; m.valid = 1;
+          m.seed = (uint16_t)s; m.velo = (uint16_t)v; m.chi2 = chi2; m.q0 = dtx * p.inv_KB;   // A10
+          m.valid = 1; m.key = kNoKey;
           mc[k] = m;
         }
       }
@@ -334,25 +325,60 @@ matching_kernel(const __grid_constant__ MatchParams p) {
           : "memory");
     }
   }
-  // index of hit i of the searched array relative to the event's first UT hit
+  LHCB_CLK(14)
+  // searched x0 array (shared tile or global), its y ranges, and the index of its element 0 relative to
+  // the event's first UT hit
+  const float* __restrict__ ux = ut_in_smem ? sux : p.ux;
+  const float* __restrict__ uylo = p.uylo + (ut_in_smem ? ua0 : 0u);
+  const float* __restrict__ uyhi = p.uyhi + (ut_in_smem ? ua0 : 0u);
   const int rel0 = ut_in_smem ? (int)(ua0 - u_begin) : -(int)u_begin;
+  const int* uo = hdr + 4;
+  if (p.use_ut) {
+    // M3a: loose windows, layer by layer until one has hits; each hit is a hypothesis (A13)
+    for (int k = tid; k < nm; k += kMatchThreads) {
+      MatchCand& m = mc[k];
+      const int v = m.velo;
+      const float xV = svx[v], yV = svy[v], txV = svtx[v], tyV = svty[v], q0 = m.q0;
+      const float invpG = fabsf(q0) * 1000.f;
+      const float gamma0 = p.Ag + p.Bg * q0;                                      // Eq. 20
+      bool found = false;
+      for (int i0 = 0; i0 < 4 && !found; ++i0) {
+        if (4 - i0 < p.min_ut_hits) break;
+        const float yi = yV + tyV * p.ut_dz[i0];
+        const float xi = (xV + txV * p.ut_dz[i0]) + gamma0 * p.ut_dz2[i0];        // Eq. 19
+        const float x0e = xi - yi * p.ut_tan[i0];
+        const float w = ut_window(p.ut_loose[i0], invpG);
+        const float lo = x0e - w, hi = x0e + w;
+        const int b = uo[i0], ee = uo[i0 + 1];
+        for (int j = lower_bound(ux, b, ee, lo); j < ee && ux[j] <= hi; ++j) {
+          if (!(uylo[j] - p.ut_y_tol <= yi && yi <= uyhi[j] + p.ut_y_tol)) continue;
+          found = true;
+          const int slot = atomicAdd(&hdr[3], 1);
+          if (slot < p.max_mc) hyq[slot] = ((uint32_t)k << 18) | ((uint32_t)i0 << 16) | (uint32_t)(j + rel0);
+        }
+      }
+      m.valid = found;
+    }
+    __syncthreads();
+    int nh = hdr[3];
+    if (nh > p.max_mc) { nh = p.max_mc; if (tid == 0) hdr[2] |= LHCB_ST_MATCH_OVERFLOW; }
+    // M3b: tight walk of every hypothesis; the best one of each pair wins the atomicMin
+    for (int i = tid; i < nh; i += kMatchThreads) {
+      const uint32_t hq = hyq[i];
+      const int k = (int)(hq >> 18), i0 = (int)((hq >> 16) & 3u), jrel = (int)(hq & 0xFFFFu);
+      const MatchCand& m = mc[k];
+      const int v = m.velo;
+      UtHyp hy;
+      ut_tight_walk(p, svx[v], svy[v], svtx[v], svty[v], fabsf(m.q0) * 1000.f, i0, jrel - rel0, ux, uylo, uyhi, uo, hy);
+      const unsigned long long key = ((unsigned long long)(4 - hy.n) << 50) |
+                                     ((unsigned long long)__float_as_uint(hy.ssq) << 18) | (hq & 0x3FFFFu);
+      atomicMin(&mc[k].key, key);
+    }
+    __syncthreads();
+  }
   for (int k = tid; k < nm; k += kMatchThreads) {
     MatchCand& m = mc[k];
-    if (p.use_ut) {
-      UtHyp hy;
-      hy.n = 0; hy.gamma = 0.f; hy.ssq = 0.f;
-      hy.idx[0] = hy.idx[1] = hy.idx[2] = hy.idx[3] = -1;
-      const int v = m.velo;
-      const bool ok = ut_in_smem
-          ? ut_search(p, svx[v], svy[v], svtx[v], svty[v], m.q0, sux, hdr + 4, (int)ua0, hy)
-          : ut_search(p, svx[v], svy[v], svtx[v], svty[v], m.q0, p.ux, hdr + 4, 0, hy);
-      m.valid = ok;
-      if (ok) {
-        m.n_ut = (uint8_t)hy.n; m.gamma = hy.gamma;
-#pragma unroll
-        for (int l = 0; l < 4; ++l) m.ut[l] = hy.idx[l] < 0 ? (uint16_t)0xFFFF : (uint16_t)(hy.idx[l] + rel0);
-      }
-    }
+    if (p.use_ut && m.valid) m.valid = (4 - (int)(m.key >> 50)) >= p.min_ut_hits;   // L311
     if (m.valid)
       atomicMin(&seed_best[m.seed], ((unsigned long long)__float_as_uint(m.chi2) << 32) | sorig[m.velo]);
   }
@@ -380,10 +406,22 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     const int s = m.seed;
     p.seed_idx[o] = s < c0 ? (uint32_t)((2 * e) * p.max_seeds + s) : (uint32_t)((2 * e + 1) * p.max_seeds + (s - c0));
     p.velo_idx[o] = v0 + vo;
+    float q = m.q0;                                                              // A10
+    if (p.use_ut) {                                          // walk the winning hypothesis once more for its hits
+      const int v = m.velo;
+      const int i0 = (int)((m.key >> 16) & 3u), jrel = (int)(m.key & 0xFFFFu);
+      UtHyp hy;
+      ut_tight_walk(p, svx[v], svy[v], svtx[v], svty[v], fabsf(m.q0) * 1000.f, i0, jrel - rel0, ux, uylo, uyhi, uo, hy);
 #pragma unroll
-    for (int l = 0; l < 4; ++l) p.ut_idx[(size_t)l * ct + o] = m.ut[l] == 0xFFFF ? LHCB_NO_HIT : u_begin + m.ut[l];
-    p.n_ut[o] = m.n_ut;
-    const float q = p.use_ut ? (m.gamma - p.Ag) * p.inv_Bg : m.q0;               // Eq. 20 inverted / A10
+      for (int l = 0; l < 4; ++l)
+        p.ut_idx[(size_t)l * ct + o] = hy.idx[l] < 0 ? LHCB_NO_HIT : u_begin + (uint32_t)(hy.idx[l] + rel0);
+      p.n_ut[o] = (uint8_t)hy.n;
+      q = (hy.gamma - p.Ag) * p.inv_Bg;                                          // Eq. 20 inverted
+    } else {
+#pragma unroll
+      for (int l = 0; l < 4; ++l) p.ut_idx[(size_t)l * ct + o] = LHCB_NO_HIT;
+      p.n_ut[o] = 0;
+    }
     p.qop[o] = pol > 0 ? q : -q;
     p.chi2[o] = m.chi2;
   }
