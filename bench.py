@@ -112,7 +112,7 @@ def main():
     import torch
     import torch.distributed as dist
     from lhcb_gen import config, generate
-    from paper_2606_14480_b200 import Context, DeviceEvents, HostPipeline, workmodel
+    from paper_2606_14480_b200 import Context, DeviceEvents, HostPipeline, shard, workmodel
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
@@ -122,9 +122,9 @@ def main():
 
     # ---- workload: cfg3, this rank's own batch --------------------------------------------------
     n = args.events
-    chunks_per_rank = (n + 1023) // 1024
+    first_chunk, _ = shard.weak_chunks(rank, n)              # rank r generates its own chunk range (weak scaling)
     workers = max(1, min(8, (os.cpu_count() or 8) // max(world, 1)))
-    ev = generate(config(3, n), workers=workers, first_chunk=rank * chunks_per_rank)
+    ev = generate(config(3, n), workers=workers, first_chunk=first_chunk)
     ctx = Context(ev.geom, device=local_rank)
     dev = DeviceEvents.from_host(ev, f"cuda:{local_rank}")
     seeds, longs = ctx.alloc_seeds(n), ctx.alloc_long(n)
@@ -168,11 +168,8 @@ def main():
     torch.cuda.synchronize()
     stop.set(); th.join()
     total_ms = t0.elapsed_time(t1)
-    if world > 1:
-        t = torch.tensor([total_ms], device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); total_ms = float(t.item())
-        c = torch.tensor([n_long], device="cuda", dtype=torch.int64); dist.all_reduce(c); n_long_all = int(c.item())
-    else:
-        n_long_all = n_long
+    total_ms, summed = shard.reduce_report(total_ms, {"long": n_long}, device="cuda")   # max time, summed counters
+    n_long_all = summed["long"]
     seed_ms = np.array([e[0].elapsed_time(e[1]) for e in evts]); match_ms = np.array([e[1].elapsed_time(e[2]) for e in evts])
     ms_per_step = total_ms / K
     value = world * n / (ms_per_step * 1e-3)
@@ -238,7 +235,9 @@ def main():
         pass
     hbm_peak = peaks.get("hbm_gbs", 6650.0)
     roofline = {"bound": "alu", "kernel": "seeding_kernel", "achieved": achieved / 1e12, "peak": peak / 1e12,
-                "unit": "Tlane-op/s", "frac": achieved / peak, "traffic": None,
+                "unit": "Tlane-op/s", "frac": achieved / peak,
+                "traffic": workmodel.NCU_DRAM_BYTES_PER_LAUNCH["seeding_kernel"] if n == 16384 else None,
+                "traffic_source": workmodel.NCU_DRAM_SOURCE,
                 "algorithmic_lane_ops_per_event": {"seeding": ops_seed, "matching": ops_match},
                 "kernel_ms": {"seeding": float(np.mean(seed_ms)), "matching": float(np.mean(match_ms))},
                 "kernel_share_of_step": {"seeding": float(seed_ms.sum() / (seed_ms.sum() + match_ms.sum())),
