@@ -175,24 +175,24 @@ __device__ __forceinline__ int owner_of(const int* offs, int n, int p) {
   }
   return b;
 }
-// index of the hit closest to xp with |x - xp| <= tol, ties to the lower index; -1 if none
+// index of the hit closest to xp with |x - xp| <= tol, ties to the lower index; -1 if none.
+// One forward scan: it starts at the bin of (xp - tol - guard), so every hit that can pass the literal
+// predicate fabsf(x - xp) <= tol is visited (the guard of 1/64 mm is far above one rounding of x - xp at
+// |x| < 2^15 mm), and ends at the first hit above xp + tol + guard.  Strict "<" keeps the lowest index
+// among equal distances, like the oracle's linear scan.
 __device__ __forceinline__ int closest_hit(const float* __restrict__ x, const uint16_t* __restrict__ lut,
-                                           const Zone& z, float xp, float tol) {
-  const int j = lower_bound(x, lut, z, xp);
+                                           const Zone& z, float xp, float tol, float& xbest) {
+  const float guard = tol + 0.015625f;
+  const float hi = xp + guard;
+  int i = lut[zone_bin(z, xp - guard)];
   int best = -1;
   float bd = 0.f;
-  if (j > z.b) {
-    int l = j - 1;
-    const float xl = x[l];
-    const float d = fabsf(xl - xp);
-    if (d <= tol) {
-      while (l > z.b && x[l - 1] == xl) --l;   // equal x: the lower index wins
-      best = l; bd = d;
-    }
-  }
-  if (j < z.e) {
-    const float d = fabsf(x[j] - xp);
-    if (d <= tol && (best < 0 || d < bd)) best = j;
+  while (i < z.e) {
+    const float xi = x[i];
+    if (xi > hi) break;
+    const float d = fabsf(xi - xp);
+    if (d <= tol && (best < 0 || d < bd)) { best = i; bd = d; xbest = xi; }
+    ++i;
   }
   return best;
 }
@@ -260,9 +260,9 @@ __device__ __forceinline__ void uv_walk(const SeedParams& p, const float* __rest
     const int l = p.ul[s];
     const float xe = xp[s] - ty * p.zt[l];
     const Zone z = zi[l];
-    const int h = closest_hit(hx, lut + l * (kLutBins + 1), z, xe, p.tol_uv);
+    float xhh = 0.f;
+    const int h = closest_hit(hx, lut + l * (kLutBins + 1), z, xe, p.tol_uv, xhh);
     if (h >= 0) {
-      const float xhh = hx[h];
       const float yl = (xp[s] - xhh) * p.inv_tan[l];
       ty = 0.5f * (ty + yl * p.inv_z[l]);
       c.hit[s] = h; c.m[s] = xhh - xp[s]; c.mask |= 1 << s; ++c.n;
@@ -520,12 +520,14 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
         const int l = p.xl[s];
         const float xp = xz_at(p, ax, bx, cx, l);
         int hh;
-        if (l == l1) hh = i1;
-        else if (l == l2) hh = i2;
-        else if (l == l3) hh = i3;
-        else { const Zone z = H.zi[l]; hh = closest_hit(hx, lut + l * (kLutBins + 1), z, xp, p.tol_x); }
+        float xh = 0.f;
+        if (l == l1) { hh = i1; xh = x1; }
+        else if (l == l2) { hh = i2; xh = x2; }
+        else if (l == l3) { hh = i3; xh = x3; }
+        else { const Zone z = H.zi[l]; hh = closest_hit(hx, lut + l * (kLutBins + 1), z, xp, p.tol_x, xh); }
         if (hh < 0) { hit[s] = -1; pattern = 1 + s; r[s] = 0.f; }
-        else { hit[s] = hh - zl[l]; r[s] = hx[hh] - xp; ++nx; }
+        else { hit[s] = hh - zl[l]; r[s] = xh - xp; ++nx; }
+        if (s + 1 - nx > 6 - p.min_x_hits) break;               // too many layers missed already
       }
       if (nx < p.min_x_hits) continue;
       // fixed-matrix least squares on the residuals w.r.t. the three-point parabola
