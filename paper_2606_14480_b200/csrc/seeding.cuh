@@ -93,12 +93,13 @@ struct SeedSmemHeader {
   int zl[13];          // zone offsets relative to the staged tile
   int xbase[7];        // prefix of x-zone sizes (clone-table index base per x-slot)
   Zone zi[12];         // per zone: [b, e) in the tile and bin(v) = clamp((v - x0) * invw, 0, kLutBins-1)
-  int n_trip, n_cand, n_kept, n_seed;
+  float4 uvc[6];       // per stereo slot: {z tan(alpha), 1/tan(alpha), 1/z, layer index (int bits)}
+  int n_trip, n_cand, n_kept, n_seed, n_live;
   unsigned int status;
   int warp_sums[kSeedThreads / 32 + 1];
 };
 
-constexpr int kSeedHeaderBytes = 512;
+constexpr int kSeedHeaderBytes = 640;
 static_assert(sizeof(SeedSmemHeader) <= kSeedHeaderBytes, "shared-memory header overflows its slot");
 
 // work-list scratch of the flattened loops: exclusive offsets + first index of one tile of owners
@@ -239,37 +240,6 @@ __device__ __forceinline__ unsigned long long clone_key(float chi2, float cx, in
 struct UvComb { int n, mask; float m[6]; int hit[6]; };
 struct __align__(16) UvSuccess { uint16_t k; uint8_t pp, n; uint16_t hit[6]; };   // hit: tile index or 0xFFFF
 
-// O8 for one first-layer hit ih (tile index) of pass pp: closest hits within tol_uv in the other
-// five stereo layers, running-average t_y (A7).
-__device__ __forceinline__ void uv_walk(const SeedParams& p, const float* __restrict__ hx, const Zone* zi,
-                                        const uint16_t* __restrict__ lut, const float* xp, int sf, int ih,
-                                        int min_n, UvComb& c) {
-  const int lf = p.ul[sf];
-  const float xh = hx[ih];
-  const float y0 = (xp[sf] - xh) * p.inv_tan[lf];          // Eq. 16
-  float ty = y0 * p.inv_z[lf];
-#pragma unroll
-  for (int s = 0; s < 6; ++s) { c.hit[s] = -1; c.m[s] = 0.f; }
-  c.hit[sf] = ih; c.m[sf] = xh - xp[sf]; c.mask = 1 << sf; c.n = 1;
-  int left = 5;                                   // stereo layers still to visit
-#pragma unroll
-  for (int s = 0; s < 6; ++s) {
-    if (s == sf) continue;
-    if (c.n + left < min_n) break;                // cannot reach min_uv_hits: the combination is dropped anyway
-    --left;
-    const int l = p.ul[s];
-    const float xe = xp[s] - ty * p.zt[l];
-    const Zone z = zi[l];
-    float xhh = 0.f;
-    const int h = closest_hit(hx, lut + l * (kLutBins + 1), z, xe, p.tol_uv, xhh);
-    if (h >= 0) {
-      const float yl = (xp[s] - xhh) * p.inv_tan[l];
-      ty = 0.5f * (ty + yl * p.inv_z[l]);
-      c.hit[s] = h; c.m[s] = xhh - xp[s]; c.mask |= 1 << s; ++c.n;
-    }
-  }
-}
-
 // O9: theta = -Q[mask] m ; r = m + tan(alpha) (ay + by zb) ; chi2 = sum r^2 * wy[n]
 __device__ __forceinline__ float fit_y(const SeedParams& p, const UvComb& c, float& ay, float& by) {
   const float* __restrict__ Q = p.Q + c.mask * 12;
@@ -302,18 +272,28 @@ __device__ __forceinline__ float fit_y(const SeedParams& p, const UvComb& c, flo
 }
 
 // ------------------------------------------------------------------------------------ kernel
-// uv_walk with the first-layer slot as a compile-time constant (keeps xp[]/m[]/hit[] in registers)
-__device__ __forceinline__ void uv_walk_sf(const SeedParams& p, const float* __restrict__ hx, const Zone* zn,
-                                           const uint16_t* __restrict__ lut, const float* xp, int sf, int ih,
-                                           int min_n, UvComb& c) {
-  switch (sf) {
-    case 0: uv_walk(p, hx, zn, lut, xp, 0, ih, min_n, c); break;
-    case 1: uv_walk(p, hx, zn, lut, xp, 1, ih, min_n, c); break;
-    case 2: uv_walk(p, hx, zn, lut, xp, 2, ih, min_n, c); break;
-    case 3: uv_walk(p, hx, zn, lut, xp, 3, ih, min_n, c); break;
-    case 4: uv_walk(p, hx, zn, lut, xp, 4, ih, min_n, c); break;
-    default: uv_walk(p, hx, zn, lut, xp, 5, ih, min_n, c); break;
+// one u/v walk that can still reach min_uv_hits after phase A: (owner << 16 | first hit), running t_y, the
+// hits of the first three other stereo layers (tile index or 0xFFFF) and the hit count so far
+struct __align__(16) UvLive { uint32_t item; float ty; uint16_t h[3]; uint16_t n; };
+
+// O8, one layer of the walk: stereo slot s of the survivor whose predictions are xpk[0..5]; closest hit
+// within tol of the prediction at the running t_y; a found hit updates t_y (A7) and the count.
+__device__ __forceinline__ int uv_step(const SeedSmemHeader& H, const float* __restrict__ hx,
+                                       const uint16_t* __restrict__ lut, const float* xpk, int s, float tol,
+                                       float& ty, int& n) {
+  const float4 cf = H.uvc[s];                                // {z tan(alpha), 1/tan(alpha), 1/z, layer}
+  const int l = __float_as_int(cf.w);
+  const float xs = xpk[s];
+  const float xe = xs - ty * cf.x;
+  const Zone z = H.zi[l];
+  float xhh = 0.f;
+  const int h = closest_hit(hx, lut + l * (kLutBins + 1), z, xe, tol, xhh);
+  if (h >= 0) {
+    const float yl = (xs - xhh) * cf.y;
+    ty = 0.5f * (ty + yl * cf.z);
+    ++n;
   }
+  return h;
 }
 
 __global__ void __launch_bounds__(kSeedThreads, LHCB_SEED_MIN_CTAS)
@@ -364,6 +344,10 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (tid < 13) H.zl[tid] = (int)(zo[tid] - a0);
+  if (tid >= 32 && tid < 38) {
+    const int l = p.ul[tid - 32];
+    H.uvc[tid - 32] = make_float4(p.zt[l], p.inv_tan[l], p.inv_z[l], __int_as_float(l));
+  }
   __syncthreads();
   if (tid == 0) {
     int acc = 0;
@@ -602,15 +586,22 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   }
   __syncthreads();
   int nk = H.n_kept;
-  {                                                            // survivors must leave room for the success queue
-    const int nk_max = ((int)p.max_trip * 8 - 4096) / 40;
+  const int wbytes = p.max_trip * 8;
+  {                                                            // survivors must leave room for the queues
+    const int nk_max = (wbytes - 4096) / 40;
     if (nk > nk_max) { nk = nk_max > 0 ? nk_max : 0; if (tid == 0) H.status |= LHCB_ST_CAND_OVERFLOW; }
   }
-  // table is dead: reuse the region for [best key per survivor | predictions per survivor | success queue]
+  // table is dead: reuse the region for
+  //   [best key per survivor | predictions per survivor | item chunk | live walks | success queue]
   unsigned long long* best = tbl;
   float* xps = reinterpret_cast<float*>(best + ((nk + 1) & ~1));          // [nk][8], 16-byte aligned: x_pred per stereo layer
-  UvSuccess* succ = reinterpret_cast<UvSuccess*>(xps + (size_t)nk * 8);
-  const int succ_cap = (int)(((size_t)p.max_trip * 8 - (size_t)nk * 40 - 8) / sizeof(UvSuccess));   // nk <= max_cand <= max_trip/5
+  const int rest = wbytes - ((nk + 1) & ~1) * 8 - nk * 32;                // >= 4096 - 8
+  int C = ((rest / 2) / 20) & ~31;                                        // items per chunk: 4 B item + 16 B live walk
+  if (C < 32) C = 32;
+  uint32_t* items = reinterpret_cast<uint32_t*>(xps + (size_t)nk * 8);
+  UvLive* live = reinterpret_cast<UvLive*>(items + C);
+  UvSuccess* succ = reinterpret_cast<UvSuccess*>(live + C);
+  const int succ_cap = (rest - C * 20) / (int)sizeof(UvSuccess);
   for (int k = tid; k < nk; k += T) {
     best[k] = kNoKey;
     const Cand& cd = cand[kept[k]];
@@ -622,14 +613,17 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   LHCB_CLK(5)
 
   // ---- S4: u/v addition (O8, O9) --------------------------------------------------------------
-  // owners w = 2*k + pass (k-th survivor); items = first-layer hits in the window of Eq. 16
+  // owners w = 2*k + pass (k-th survivor); items = first-layer hits in the window of Eq. 16.  Every item
+  // is queued as (owner, hit); phase A walks the first three other stereo layers of every item (dense),
+  // the walks that can still reach min_uv_hits are queued with their state; phase B finishes them.
+  const int sf0 = p.slot_of_layer[p.uv_first[0]], sf1 = p.slot_of_layer[p.uv_first[1]];
   for (int tile0 = 0; tile0 < 2 * nk; tile0 += T) {
     const int nown = 2 * nk - tile0 < T ? 2 * nk - tile0 : T;
     int cnt = 0, fst = 0;
     if (tid < nown) {
       const int w = tile0 + tid, pp = w & 1;
       const int lf = p.uv_first[pp];
-      const float xpf = xps[(w >> 1) * 8 + p.slot_of_layer[lf]];
+      const float xpf = xps[(w >> 1) * 8 + (pp ? sf1 : sf0)];
       const float wa = xpf - p.ywin_a[h][lf], wb = xpf - p.ywin_b[h][lf];
       const float wlo = wa < wb ? wa : wb, whi = wa > wb ? wa : wb;
       const Zone zf = H.zi[lf];
@@ -639,43 +633,57 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     }
     int total;
     const int ex = block_exscan<kSeedThreads>(cnt, H.warp_sums, total);
-    scan.offs[tid] = ex; scan.first[tid] = (uint16_t)fst;
-    if (tid == T - 1) scan.offs[T] = total;
-    __syncthreads();
     LHCB_CLK(6)
-    const int chunk = (total + T - 1) / T;
-    const int p0 = tid * chunk, p1 = p0 + chunk < total ? p0 + chunk : total;
-    if (p0 < p1) {
-      int t = owner_of(scan.offs, nown, p0) - 1;             // forces a reload on the first item
-      int nxt = -1;
-      int f = 0, pp = 0, sf = 0, kk = 0;
-      float xp[6];
-      for (int q = p0; q < p1; ++q) {
-        if (q >= nxt) {
-          do { ++t; nxt = scan.offs[t + 1]; } while (q >= nxt);
-          const int w = tile0 + t;
-          kk = w >> 1; pp = w & 1;
-          const float4 lo4 = *reinterpret_cast<const float4*>(xps + kk * 8);
-          const float2 hi2 = *reinterpret_cast<const float2*>(xps + kk * 8 + 4);
-          xp[0] = lo4.x; xp[1] = lo4.y; xp[2] = lo4.z; xp[3] = lo4.w; xp[4] = hi2.x; xp[5] = hi2.y;
-          sf = p.slot_of_layer[p.uv_first[pp]];
-          f = (int)scan.first[t] - scan.offs[t];
-        }
-        const int ih = f + q;
-        UvComb c;
-        uv_walk_sf(p, hx, H.zi, lut, xp, sf, ih, p.min_uv_hits, c);
-        if (c.n < p.min_uv_hits) continue;
+    for (int q0 = 0; q0 < total; q0 += C) {                  // uniform: chunks of C items
+      if (tid == 0) H.n_live = 0;
+      {
+        int i = q0 - ex; if (i < 0) i = 0;
+        int iend = q0 + C - ex; if (iend > cnt) iend = cnt;
+        for (; i < iend; ++i) items[ex + i - q0] = ((uint32_t)tid << 16) | (uint32_t)(fst + i);
+      }
+      __syncthreads();
+      const int nitems = total - q0 < C ? total - q0 : C;
+      for (int i = tid; i < nitems; i += T) {                // phase A
+        const uint32_t item = items[i];
+        const int w = tile0 + (int)(item >> 16), ih = (int)(item & 0xFFFFu);
+        const int sf = (w & 1) ? sf1 : sf0;
+        const float* xpk = xps + (w >> 1) * 8;
+        const float4 cf = H.uvc[sf];
+        const float y0 = (xpk[sf] - hx[ih]) * cf.y;          // Eq. 16
+        float ty = y0 * cf.z;
+        int n = 1;
+        const int h0 = uv_step(H, hx, lut, xpk, 0 + (0 >= sf), p.tol_uv, ty, n);
+        const int h1 = uv_step(H, hx, lut, xpk, 1 + (1 >= sf), p.tol_uv, ty, n);
+        const int h2 = uv_step(H, hx, lut, xpk, 2 + (2 >= sf), p.tol_uv, ty, n);
+        if (n + 2 < p.min_uv_hits) continue;                 // cannot reach min_uv_hits any more
+        UvLive lv;
+        lv.item = ((uint32_t)w << 16) | (uint32_t)ih; lv.ty = ty;
+        lv.h[0] = (uint16_t)h0; lv.h[1] = (uint16_t)h1; lv.h[2] = (uint16_t)h2; lv.n = (uint16_t)n;
+        live[atomicAdd(&H.n_live, 1)] = lv;
+      }
+      __syncthreads();
+      const int nl = H.n_live;
+      for (int i = tid; i < nl; i += T) {                    // phase B
+        const UvLive lv = live[i];
+        const int w = (int)(lv.item >> 16), ih = (int)(lv.item & 0xFFFFu);
+        const int sf = (w & 1) ? sf1 : sf0;
+        const float* xpk = xps + (w >> 1) * 8;
+        float ty = lv.ty;
+        int n = lv.n;
+        const int h3 = uv_step(H, hx, lut, xpk, 3 + (3 >= sf), p.tol_uv, ty, n);
+        const int h4 = (n + 1 < p.min_uv_hits) ? -1 : uv_step(H, hx, lut, xpk, 4 + (4 >= sf), p.tol_uv, ty, n);
+        if (n < p.min_uv_hits) continue;
         const int slot = atomicAdd(&H.n_trip, 1);            // enough hits: queue for the dense fit pass
         if (slot < succ_cap) {
-          UvSuccess u;
-          u.k = (uint16_t)kk; u.pp = (uint8_t)pp; u.n = (uint8_t)c.n;
-#pragma unroll
-          for (int s = 0; s < 6; ++s) u.hit[s] = c.hit[s] < 0 ? (uint16_t)0xFFFF : (uint16_t)c.hit[s];
-          succ[slot] = u;
+          UvSuccess& u = succ[slot];
+          u.k = (uint16_t)(w >> 1); u.pp = (uint8_t)(w & 1); u.n = (uint8_t)n;
+          u.hit[sf] = (uint16_t)ih;
+          u.hit[0 + (0 >= sf)] = lv.h[0]; u.hit[1 + (1 >= sf)] = lv.h[1]; u.hit[2 + (2 >= sf)] = lv.h[2];
+          u.hit[3 + (3 >= sf)] = (uint16_t)h3; u.hit[4 + (4 >= sf)] = (uint16_t)h4;
         }
       }
+      __syncthreads();
     }
-    __syncthreads();
     LHCB_CLK(7)
   }
   int nsucc = H.n_trip;
