@@ -112,7 +112,7 @@ def main():
     import torch
     import torch.distributed as dist
     from lhcb_gen import config, generate
-    from paper_2606_14480_b200 import Context, DeviceEvents, HostPipeline, shard, workmodel
+    from paper_2606_14480_b200 import Context, DeviceEvents, HostPipeline, capacities, shard, workmodel
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
@@ -125,7 +125,9 @@ def main():
     first_chunk, _ = shard.weak_chunks(rank, n)              # rank r generates its own chunk range (weak scaling)
     workers = max(1, min(8, (os.cpu_count() or 8) // max(world, 1)))
     ev = generate(config(3, n), workers=workers, first_chunk=first_chunk)
+    ev.geom.update(capacities.NOMINAL)                       # per-CTA capacities for nominal occupancy
     ctx = Context(ev.geom, device=local_rank)
+    launch = ctx.lhcb_launch_config()
     dev = DeviceEvents.from_host(ev, f"cuda:{local_rank}")
     seeds, longs = ctx.alloc_seeds(n), ctx.alloc_long(n)
     stream = torch.cuda.current_stream()
@@ -254,7 +256,8 @@ def main():
             "config": {"workload": "cfg3 = BASELINE.json configs[2]: 16,384 nominal-occupancy (mu~5) events, seed 2, "
                                    "one batch of %d events per GPU, seeding + matching (with UT) on one stream" % n,
                        "events_per_gpu": n, "l2": "inputs (~%.0f MB per batch) exceed the 126 MB L2" % (dev.input_bytes() / 1e6),
-                       "parallelism": f"events sharded over {world} GPU(s), no collective"},
+                       "parallelism": f"events sharded over {world} GPU(s), no collective",
+                       "capacities": "paper_2606_14480_b200.capacities.NOMINAL", "launch": launch},
             "long_tracks_per_s": n_long_all / (ms_per_step * 1e-3), "seeds_per_event": n_seeds / n, "long_per_event": n_long / n,
             "seeding_events_per_s": n / float(np.median(seed_ms)) * 1e3, "matching_events_per_s": n / float(np.median(match_ms)) * 1e3,
             "min_ms": {"seeding": float(seed_ms.min()), "matching": float(match_ms.min())},

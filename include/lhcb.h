@@ -211,6 +211,10 @@ const char* lhcb_error_string(int status);
 int lhcb_last_cuda_error(const lhcb_ctx* ctx);
 /* Number of kernels the last lhcb_seeding / lhcb_matching call launched. */
 int lhcb_last_launch_count(const lhcb_ctx* ctx);
+/* Launch configuration the capacities of this context select: out[0] threads per
+ * seeding CTA, out[1] its dynamic shared memory in bytes, out[2] threads per matching CTA, out[3] its
+ * dynamic shared memory.  Smaller capacities let more CTAs share an SM (L382: occupancy). */
+int lhcb_launch_config(const lhcb_ctx* ctx, int out[4]);
 
 #ifdef __cplusplus
 }

@@ -3,7 +3,7 @@
 The product is the C-ABI CUDA library declared in include/lhcb.h (sources in csrc/); this package is
 its thin Python binding.  There is no CPU fallback.
 """
-from . import shard, workmodel
+from . import capacities, shard, workmodel
 from .binding import Context, DeviceEvents, HostPipeline, lhcb_geom_derive, load_library, NO_HIT, EXPORTS
 
 __all__ = ["Context", "DeviceEvents", "HostPipeline", "lhcb_geom_derive", "load_library", "NO_HIT", "EXPORTS"]

@@ -24,7 +24,7 @@ ST_BITS = {1: "triplet_overflow", 2: "cand_overflow", 4: "seed_overflow", 8: "hi
 EXPORTS = ["lhcb_geom_derive", "lhcb_geom_init", "lhcb_destroy", "lhcb_get_geom", "lhcb_workspace_bytes",
            "lhcb_seeding", "lhcb_matching", "lhcb_error_string", "lhcb_last_cuda_error",
            "lhcb_last_launch_count", "lhcb_pipeline_create", "lhcb_pipeline_destroy", "lhcb_reconstruct_host",
-           "lhcb_pipeline_last_bytes"]
+           "lhcb_pipeline_last_bytes", "lhcb_launch_config"]
 
 
 class LhcbGeom(C.Structure):
@@ -129,6 +129,7 @@ def load_library(build: bool = True) -> C.CDLL:
         lib.lhcb_error_string.restype = C.c_char_p
         lib.lhcb_last_cuda_error.argtypes = [VP]
         lib.lhcb_last_launch_count.argtypes = [VP]
+        lib.lhcb_launch_config.argtypes = [VP, C.POINTER(C.c_int * 4)]
         lib.lhcb_pipeline_create.argtypes = [VP, C.c_int, C.c_size_t, C.c_size_t, C.c_size_t, C.c_int, C.POINTER(VP)]
         lib.lhcb_pipeline_destroy.argtypes = [VP]
         lib.lhcb_pipeline_destroy.restype = None
@@ -292,6 +293,12 @@ class Context:
 
     def last_launch_count(self):
         return int(self.lib.lhcb_last_launch_count(self._ctx))
+
+    def lhcb_launch_config(self):
+        """dict(seed_threads, seed_smem, match_threads, match_smem) selected by this context's capacities."""
+        out = (C.c_int * 4)()
+        _check(self.lib, self._ctx, self.lib.lhcb_launch_config(self._ctx, C.byref(out)), "lhcb_launch_config")
+        return dict(zip(("seed_threads", "seed_smem", "match_threads", "match_smem"), (int(x) for x in out)))
 
     # ------------------------------------------------------------------ helpers (host views of outputs)
     def seeds_from_states(self, n_events, seed_off, state):

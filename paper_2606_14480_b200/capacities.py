@@ -1,0 +1,21 @@
+"""Per-CTA capacities (`lhcb_geom_t.max_*`) for the occupancy of the workload.
+
+All intermediates of both kernels live in shared memory, so the capacities decide how many CTAs share
+an SM (include/lhcb.h: lhcb_launch_config).  The library defaults (all zero in the geometry) are sized
+for BASELINE.json configs[3] (mu = 7.6 plus displaced tracks); NOMINAL is sized for Run 3 nominal
+occupancy (mu ~ 5: configs[1] and configs[2]), where it lets four 256-thread seeding CTAs and six
+128-thread matching CTAs share an SM.  Exceeding a capacity is never silent: the per-half / per-event
+status words report it and the tests and bench.py fail on any set bit.
+
+Observed maxima over the 16,384 events of configs[2] (seed 2): 2,4xx hits per half, < 384 x-z
+candidates per half, 135 seeds per half.
+"""
+NOMINAL = dict(max_hits_per_half=3072, max_xz_cand_per_half=512, max_triplets_per_half=2048,
+               max_seeds_per_half=192, max_long_per_event=256, max_match_cand_per_event=352,
+               max_velo_per_event=256, max_ut_per_event=3840)
+
+
+def with_capacities(geom: dict, caps: dict = NOMINAL) -> dict:
+    g = dict(geom)
+    g.update(caps)
+    return g

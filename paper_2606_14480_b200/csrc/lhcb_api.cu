@@ -19,6 +19,8 @@ struct lhcb_ctx {
   float* d_P;
   float* d_Q;
   size_t seed_smem, match_smem;
+  int match_threads;  // 128 when six CTAs fit an SM, else 256
+  int seed_threads;   // 256 (4 CTAs/SM) when the capacities fit a quarter of the SM's shared memory, else 512
   int last_cuda_error;
   int last_launches;
 };
@@ -105,17 +107,34 @@ int lhcb_geom_init(const lhcb_geom_t* g, int device, lhcb_ctx** out) {
   if (rc != LHCB_OK) { delete c; return rc; }
   if (G.max_hits_per_half > 32768 || G.max_xz_cand_per_half > 65535 || G.max_seeds_per_half > 32767 ||
       G.max_velo_per_event > 65535 || G.max_ut_per_event > 65534 || G.max_match_cand_per_event > 16383 || G.max_triplets_per_half < G.max_xz_cand_per_half) { delete c; return LHCB_ERR_BAD_ARGUMENT; }
-  c->seed_smem = lhcb::seed_smem_bytes(G.max_hits_per_half, G.max_xz_cand_per_half, G.max_triplets_per_half);
-  c->match_smem = lhcb::match_smem_bytes(G.max_seeds_per_half, G.max_match_cand_per_event, G.max_velo_per_event,
+  // 256-thread CTAs, four per SM, when their shared memory fits (228 KB per SM, 1 KB reserved per CTA);
+  // else 512-thread CTAs, two (or one) per SM
+  c->seed_threads = 256;
+  c->seed_smem = lhcb::seed_smem_bytes(256, G.max_hits_per_half, G.max_xz_cand_per_half, G.max_triplets_per_half);
+  if (c->seed_smem > (size_t)(228 * 1024 / 4 - 1024)) {
+    c->seed_threads = 512;
+    c->seed_smem = lhcb::seed_smem_bytes(512, G.max_hits_per_half, G.max_xz_cand_per_half, G.max_triplets_per_half);
+  }
+  c->match_threads = 128;
+  c->match_smem = lhcb::match_smem_bytes(128, G.max_seeds_per_half, G.max_match_cand_per_event, G.max_velo_per_event,
                                          G.max_ut_per_event);
+  if (c->match_smem > (size_t)(228 * 1024 / 6 - 1024)) {
+    c->match_threads = 256;
+    c->match_smem = lhcb::match_smem_bytes(256, G.max_seeds_per_half, G.max_match_cand_per_event, G.max_velo_per_event,
+                                           G.max_ut_per_event);
+  }
   cudaError_t e = cudaSetDevice(device);
   int max_optin = 0;
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
   if (e != cudaSuccess) { c->last_cuda_error = (int)e; delete c; return LHCB_ERR_CUDA; }
   if (c->seed_smem > (size_t)max_optin || c->match_smem > (size_t)max_optin) { delete c; return LHCB_ERR_CAPACITY; }
-  e = cudaFuncSetAttribute(lhcb::seeding_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->seed_smem);
+  e = c->seed_threads == 256
+          ? cudaFuncSetAttribute(lhcb::seeding_kernel<256, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->seed_smem)
+          : cudaFuncSetAttribute(lhcb::seeding_kernel<512, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->seed_smem);
   if (e == cudaSuccess)
-    e = cudaFuncSetAttribute(lhcb::matching_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->match_smem);
+    e = c->match_threads == 128
+            ? cudaFuncSetAttribute(lhcb::matching_kernel<128, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->match_smem)
+            : cudaFuncSetAttribute(lhcb::matching_kernel<256, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->match_smem);
   if (e == cudaSuccess) e = cudaMalloc(&c->d_P, sizeof(c->der.P));
   if (e == cudaSuccess) e = cudaMalloc(&c->d_Q, sizeof(c->der.Q));
   if (e == cudaSuccess) e = cudaMemcpy(c->d_P, c->der.P, sizeof(c->der.P), cudaMemcpyHostToDevice);
@@ -165,7 +184,11 @@ int lhcb_seeding(lhcb_ctx* c, const lhcb_events_t* ev, lhcb_seeds_t* out, void* 
   p.count = out->count; p.state = out->state; p.par = out->par; p.hits = out->hits; p.nx = out->nx;
   p.nuv = out->nuv; p.status = out->status;
   p.cap_total = (size_t)ev->n_events * 2 * (size_t)c->geom.max_seeds_per_half;
-  lhcb::seeding_kernel<<<ev->n_events * 2, lhcb::kSeedThreads, c->seed_smem, (cudaStream_t)stream>>>(p);
+  p.smem_total = (int)c->seed_smem;
+  if (c->seed_threads == 256)
+    lhcb::seeding_kernel<256, 4><<<ev->n_events * 2, 256, c->seed_smem, (cudaStream_t)stream>>>(p);
+  else
+    lhcb::seeding_kernel<512, 2><<<ev->n_events * 2, 512, c->seed_smem, (cudaStream_t)stream>>>(p);
   LHCB_CUDA(c, cudaGetLastError());
   c->last_launches = 1;
   return LHCB_OK;
@@ -195,7 +218,10 @@ int lhcb_matching(lhcb_ctx* c, const lhcb_seeds_t* seeds, const lhcb_velo_t* vel
   p.count = out->count; p.seed_idx = out->seed_idx; p.velo_idx = out->velo_idx; p.ut_idx = out->ut_idx;
   p.n_ut = out->n_ut; p.qop = out->qop; p.chi2 = out->chi2; p.status = out->status;
   p.long_cap_total = (size_t)velo->n_events * (size_t)c->geom.max_long_per_event;
-  lhcb::matching_kernel<<<velo->n_events, lhcb::kMatchThreads, c->match_smem, (cudaStream_t)stream>>>(p);
+  if (c->match_threads == 128)
+    lhcb::matching_kernel<128, 6><<<velo->n_events, 128, c->match_smem, (cudaStream_t)stream>>>(p);
+  else
+    lhcb::matching_kernel<256, 3><<<velo->n_events, 256, c->match_smem, (cudaStream_t)stream>>>(p);
   LHCB_CUDA(c, cudaGetLastError());
   c->last_launches = 1;
   return LHCB_OK;
@@ -227,6 +253,11 @@ int lhcb_debug_stage_clocks(unsigned long long* out, int reset) {
 
 int lhcb_last_cuda_error(const lhcb_ctx* c) { return c ? c->last_cuda_error : 0; }
 int lhcb_last_launch_count(const lhcb_ctx* c) { return c ? c->last_launches : 0; }
+int lhcb_launch_config(const lhcb_ctx* c, int out[4]) {
+  if (!c || !out) return LHCB_ERR_BAD_ARGUMENT;
+  out[0] = c->seed_threads; out[1] = (int)c->seed_smem; out[2] = c->match_threads; out[3] = (int)c->match_smem;
+  return LHCB_OK;
+}
 
 }  // extern "C"
 

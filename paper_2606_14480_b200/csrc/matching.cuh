@@ -26,10 +26,6 @@
 
 namespace lhcb {
 
-#ifndef LHCB_MATCH_THREADS
-#define LHCB_MATCH_THREADS 256
-#endif
-constexpr int kMatchThreads = LHCB_MATCH_THREADS;
 
 struct MatchParams {
   float zS, zV, dzyS, dzyV, mag[5], presel[4], cx0, cx1, cy0, cy1, inv_tol_tx, inv_tol_ty, chi2m_max;
@@ -67,7 +63,7 @@ struct __align__(8) MatchCand {
 };
 static_assert(sizeof(MatchCand) == 24, "MatchCand is 24 bytes");
 
-__host__ __device__ inline size_t match_smem_bytes(int max_seeds, int max_mc, int max_velo, int max_ut) {
+__host__ __device__ inline size_t match_smem_bytes(int kMatchThreads, int max_seeds, int max_mc, int max_velo, int max_ut) {
   size_t b = 64;
   b += ((size_t)max_ut + 8) * 4;             // UT x0 tile (16-byte aligned superset)
   b += (size_t)max_velo * 16;                // VELO states, sorted by ty
@@ -143,7 +139,8 @@ __device__ __forceinline__ void ut_tight_walk(const MatchParams& p, float xV, fl
     }
 }
 
-__global__ void __launch_bounds__(kMatchThreads)
+template <int kMatchThreads, int MIN_CTAS>
+__global__ void __launch_bounds__(kMatchThreads, MIN_CTAS)
 matching_kernel(const __grid_constant__ MatchParams p) {
   extern __shared__ __align__(16) unsigned char smem[];
   int* hdr = reinterpret_cast<int*>(smem);                  // [0] n_mc, [1] n_long, [2] status, [3] n_hyp, [4..8] UT offsets

@@ -25,16 +25,10 @@
 
 namespace lhcb {
 
-#ifndef LHCB_SEED_THREADS
-#define LHCB_SEED_THREADS 512
-#endif
-#ifndef LHCB_SEED_MIN_CTAS
-#define LHCB_SEED_MIN_CTAS 2
-#endif
 #ifndef LHCB_LUT_BINS
 #define LHCB_LUT_BINS 256
 #endif
-constexpr int kSeedThreads = LHCB_SEED_THREADS;
+constexpr int kSeedThreadsMax = 512;          // the kernel is instantiated for 256 x 4 CTAs/SM and 512 x 2 CTAs/SM
 constexpr int kLutBins = LHCB_LUT_BINS;       // bins of the per-zone search table
 constexpr unsigned long long kNoKey = ~0ull;
 
@@ -65,6 +59,7 @@ struct SeedParams {
   float zbS, gS, gpS;
   int min_x_hits, min_uv_hits, uv_first[2], polarity;
   int max_seeds, max_cand, max_hits, max_trip;
+  int smem_total;   // dynamic shared memory of the launch = seed_smem_bytes(threads, capacities)
   const float* P;   // [7][3][6]
   const float* Q;   // [64][2][6]
   // batch
@@ -96,26 +91,27 @@ struct SeedSmemHeader {
   float4 uvc[6];       // per stereo slot: {z tan(alpha), 1/tan(alpha), 1/z, layer index (int bits)}
   int n_trip, n_cand, n_kept, n_seed, n_live;
   unsigned int status;
-  int warp_sums[kSeedThreads / 32 + 1];
+  int warp_sums[kSeedThreadsMax / 32 + 1];
 };
 
 constexpr int kSeedHeaderBytes = 640;
 static_assert(sizeof(SeedSmemHeader) <= kSeedHeaderBytes, "shared-memory header overflows its slot");
 
-// work-list scratch of the flattened loops: exclusive offsets + first index of one tile of owners
-struct SeedScan { int offs[kSeedThreads + 1]; uint16_t first[kSeedThreads]; };
-
-__host__ __device__ inline size_t seed_smem_bytes(int max_hits, int max_cand, int max_trip) {
-  size_t b = kSeedHeaderBytes;                             // header
-  b += ((size_t)max_hits + 8) * 4;                         // hits tile (16-byte aligned superset)
-  b = (b + 15) & ~(size_t)15;
-  b += (size_t)max_cand * sizeof(Cand);
-  b += (size_t)max_cand * 2;                               // kept list
-  b = (b + 15) & ~(size_t)15;
-  b += (size_t)max_trip * 8;                               // triplet queue / clone table / best keys
-  b += 12 * (kLutBins + 1) * 2;                            // bin tables
-  b = (b + 15) & ~(size_t)15;
-  b += sizeof(SeedScan);
+// Shared-memory map of one CTA (NT threads), all offsets 16-byte aligned:
+//   [header | bin tables | scan scratch: int offs[NT+1], u16 first[NT] | kept list u16[max_cand] |
+//    hits tile (the half's ACTUAL size) | work region W ... | x-z candidates, filled downward from the end]
+// W holds the triplet queue, then the clone table, then the u/v queues; it starts right after the staged
+// hits and ends where the candidates begin, so a half with fewer hits or candidates than the capacities
+// leaves more room for the queues.  The capacities guarantee W >= max_trip * 8 bytes.
+__host__ __device__ inline size_t seed_align16(size_t b) { return (b + 15) & ~(size_t)15; }
+__host__ __device__ inline size_t seed_off_scan() { return kSeedHeaderBytes + seed_align16(12 * (kLutBins + 1) * 2); }
+__host__ __device__ inline size_t seed_off_kept(int nt) { return seed_off_scan() + seed_align16((size_t)(nt + 1) * 4 + (size_t)nt * 2); }
+__host__ __device__ inline size_t seed_off_hits(int nt, int max_cand) { return seed_off_kept(nt) + seed_align16((size_t)max_cand * 2); }
+__host__ __device__ inline size_t seed_smem_bytes(int nt, int max_hits, int max_cand, int max_trip) {
+  size_t b = seed_off_hits(nt, max_cand);
+  b += seed_align16(((size_t)max_hits + 8) * 4);           // hits tile (16-byte aligned superset)
+  b += seed_align16((size_t)max_trip * 8);                 // work region W (minimum)
+  b += (size_t)max_cand * 32;                              // candidates
   return b;
 }
 
@@ -296,28 +292,21 @@ __device__ __forceinline__ int uv_step(const SeedSmemHeader& H, const float* __r
   return h;
 }
 
-__global__ void __launch_bounds__(kSeedThreads, LHCB_SEED_MIN_CTAS)
+template <int NT, int MIN_CTAS>
+__global__ void __launch_bounds__(NT, MIN_CTAS)
 seeding_kernel(const __grid_constant__ SeedParams p) {
   extern __shared__ __align__(16) unsigned char smem[];
   SeedSmemHeader& H = *reinterpret_cast<SeedSmemHeader*>(smem);
-  float* hx = reinterpret_cast<float*>(smem + kSeedHeaderBytes);
-  size_t off = kSeedHeaderBytes + ((size_t)p.max_hits + 8) * 4;
-  off = (off + 15) & ~(size_t)15;
-  Cand* cand = reinterpret_cast<Cand*>(smem + off);
-  off += (size_t)p.max_cand * sizeof(Cand);
-  uint16_t* kept = reinterpret_cast<uint16_t*>(smem + off);
-  off += (size_t)p.max_cand * 2;
-  off = (off + 15) & ~(size_t)15;
-  Triplet* trip = reinterpret_cast<Triplet*>(smem + off);
-  unsigned long long* tbl = reinterpret_cast<unsigned long long*>(smem + off);   // aliases trip
-  off += (size_t)p.max_trip * 8;
-  uint16_t* lut = reinterpret_cast<uint16_t*>(smem + off);
-  off += 12 * (kLutBins + 1) * 2;
-  off = (off + 15) & ~(size_t)15;
-  SeedScan& scan = *reinterpret_cast<SeedScan*>(smem + off);
+  uint16_t* lut = reinterpret_cast<uint16_t*>(smem + kSeedHeaderBytes);
+  int* scan_offs = reinterpret_cast<int*>(smem + seed_off_scan());            // [NT + 1] exclusive offsets
+  uint16_t* scan_first = reinterpret_cast<uint16_t*>(scan_offs + NT + 1);      // [NT] first index per owner
+  uint16_t* kept = reinterpret_cast<uint16_t*>(smem + seed_off_kept(NT));
+  const int off_hits = (int)seed_off_hits(NT, p.max_cand);
+  float* hx = reinterpret_cast<float*>(smem + off_hits);
+  Cand* cand_end = reinterpret_cast<Cand*>(smem + p.smem_total);               // candidate c lives at cand_end[-1 - c]
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  constexpr int T = kSeedThreads, nwarps = kSeedThreads / 32;
+  constexpr int T = NT, nwarps = NT / 32;
   LHCB_CLK_INIT
   const int half_id = blockIdx.x, event = half_id >> 1, h = half_id & 1;
   const uint32_t* zo = p.zone_off + (size_t)half_id * 12;
@@ -382,7 +371,13 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   __syncthreads();
   LHCB_CLK(0)
   const int* zl = H.zl;
-  if (H.xbase[6] > p.max_trip) {                            // clone table would not fit
+  // work region W: from the end of the staged tile to the first candidate slot
+  const int off_w = (int)seed_align16((size_t)off_hits + (size_t)((g_end > a1 ? g_end : a1) - a0) * 4);
+  const int w_stat = p.smem_total - p.max_cand * (int)sizeof(Cand) - off_w;   // bytes of W with every candidate slot used
+  Triplet* trip = reinterpret_cast<Triplet*>(smem + off_w);
+  unsigned long long* tbl = reinterpret_cast<unsigned long long*>(smem + off_w);   // aliases trip
+  const int trip_cap = w_stat / 8;
+  if (H.xbase[6] > trip_cap) {                              // clone table would not fit
     if (tid == 0) { p.count[half_id] = 0; p.status[half_id] = LHCB_ST_HITS_OVERFLOW; }
     return;
   }
@@ -439,23 +434,23 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
         cnt = upper_bound(hx, lut3, z3n, hi) - fst;
       }
       int total;
-      const int ex = block_exscan<kSeedThreads>(cnt, H.warp_sums, total);
-      scan.offs[tid] = ex; scan.first[tid] = (uint16_t)fst;
-      if (tid == T - 1) scan.offs[T] = total;
+      const int ex = block_exscan<NT>(cnt, H.warp_sums, total);
+      scan_offs[tid] = ex; scan_first[tid] = (uint16_t)fst;
+      if (tid == T - 1) scan_offs[T] = total;
       __syncthreads();
       LHCB_CLK(2)
       // flattened pairs: thread owns pairs [p0, p1)
       const int chunk = (total + T - 1) / T;
       const int p0 = tid * chunk, p1 = p0 + chunk < total ? p0 + chunk : total;
       if (p0 < p1) {
-        int t = owner_of(scan.offs, nt1, p0);
-        int nxt = scan.offs[t + 1];
+        int t = owner_of(scan_offs, nt1, p0);
+        int nxt = scan_offs[t + 1];
         int i1 = b1 + tile0 + t;
         float x1 = hx[i1];
-        int f = (int)scan.first[t] - scan.offs[t];
+        int f = (int)scan_first[t] - scan_offs[t];
         for (int pp = p0; pp < p1; ++pp) {
           while (pp >= nxt) {
-            ++t; nxt = scan.offs[t + 1]; i1 = b1 + tile0 + t; x1 = hx[i1]; f = (int)scan.first[t] - scan.offs[t];
+            ++t; nxt = scan_offs[t + 1]; i1 = b1 + tile0 + t; x1 = hx[i1]; f = (int)scan_first[t] - scan_offs[t];
           }
           const int i3 = f + pp;
           const float x3 = hx[i3];
@@ -472,7 +467,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
           int j = lower_bound(hx, lut2, z2n, lo2);
           while (j < e2 && hx[j] <= hi2) {
             const int k = atomicAdd(&H.n_trip, 1);
-            if (k < p.max_trip) {
+            if (k < trip_cap) {
               Triplet tr;
               tr.i1 = (uint16_t)(i1 - b1); tr.i2 = (uint16_t)(j - b2); tr.i3 = (uint16_t)(i3 - b3); tr.it = (uint16_t)it;
               trip[k] = tr;
@@ -485,7 +480,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
       LHCB_CLK(3)
     }
     int nt = H.n_trip;
-    if (nt > p.max_trip) { nt = p.max_trip; if (tid == 0) H.status |= LHCB_ST_TRIPLET_OVERFLOW; }
+    if (nt > trip_cap) { nt = trip_cap; if (tid == 0) H.status |= LHCB_ST_TRIPLET_OVERFLOW; }
 
     for (int t = tid; t < nt; t += T) {                                          // O5 + O6
       const Triplet tr = trip[t];
@@ -550,7 +545,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
 #pragma unroll
         for (int s = 0; s < 6; ++s) cd.hit[s] = hit[s] < 0 ? (uint16_t)0xFFFF : (uint16_t)hit[s];
         cd.nx = (uint8_t)nx; cd.it = (uint8_t)it; cd.keep = 0; cd.pad = 0;
-        cand[k] = cd;
+        cand_end[-1 - k] = cd;
       }
     }
     __syncthreads();
@@ -566,7 +561,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   for (int i = tid; i < n_xhits; i += T) tbl[i] = kNoKey;
   __syncthreads();
   for (int c = tid; c < nc; c += T) {
-    const Cand& cd = cand[c];
+    const Cand& cd = cand_end[-1 - c];
     const unsigned long long key = clone_key(cd.chi2, cd.cx, cd.nx, cd.it);
 #pragma unroll
     for (int s = 0; s < 6; ++s)
@@ -574,7 +569,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   }
   __syncthreads();
   for (int c = tid; c < nc; c += T) {
-    Cand& cd = cand[c];
+    Cand& cd = cand_end[-1 - c];
     const unsigned long long key = clone_key(cd.chi2, cd.cx, cd.nx, cd.it);
     int own = 0;
 #pragma unroll
@@ -586,7 +581,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   }
   __syncthreads();
   int nk = H.n_kept;
-  const int wbytes = p.max_trip * 8;
+  const int wbytes = p.smem_total - nc * (int)sizeof(Cand) - off_w;      // unused candidate slots join W
   {                                                            // survivors must leave room for the queues
     const int nk_max = (wbytes - 4096) / 40;
     if (nk > nk_max) { nk = nk_max > 0 ? nk_max : 0; if (tid == 0) H.status |= LHCB_ST_CAND_OVERFLOW; }
@@ -604,7 +599,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   const int succ_cap = (rest - C * 20) / (int)sizeof(UvSuccess);
   for (int k = tid; k < nk; k += T) {
     best[k] = kNoKey;
-    const Cand& cd = cand[kept[k]];
+    const Cand& cd = cand_end[-1 - (int)kept[k]];
 #pragma unroll
     for (int s = 0; s < 6; ++s) xps[k * 8 + s] = xz_at(p, cd.ax, cd.bx, cd.cx, p.ul[s]);
   }
@@ -632,7 +627,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
       cnt = upper_bound(hx, lutf, zf, whi) - fst;
     }
     int total;
-    const int ex = block_exscan<kSeedThreads>(cnt, H.warp_sums, total);
+    const int ex = block_exscan<NT>(cnt, H.warp_sums, total);
     LHCB_CLK(6)
     for (int q0 = 0; q0 < total; q0 += C) {                  // uniform: chunks of C items
       if (tid == 0) H.n_live = 0;
@@ -723,7 +718,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   for (int i = tid; i < nsucc; i += T) {
     if (!single) fit_success(i);                               // more than one round: redo the (cheap) fit
     if (key == kNoKey || best[u.k] != key) continue;           // not the best combination of its survivor
-    const Cand& cd = cand[kept[u.k]];
+    const Cand& cd = cand_end[-1 - (int)kept[u.k]];
     const int slot = atomicAdd(&H.n_seed, 1);
     if (slot >= p.max_seeds) continue;
     const size_t o = (size_t)slot0 + slot, ct = p.cap_total;

@@ -127,3 +127,46 @@ def test_overflow_is_reported_not_silent(geom):
     s = c.seeds_to_host(c.lhcb_seeding(DeviceEvents.from_host(ev)))
     assert (s["status"] == 8).all() and s["n"] == 0
     c.close()
+
+
+def test_cfg3_full_size_bench_configuration(oracle32):
+    """BASELINE.json configs[2] at full size (16,384 events, seed 2) in the launch configuration bench.py
+    times (capacities.NOMINAL: 256-thread seeding CTAs, 128-thread matching CTAs): no capacity overflow
+    anywhere, and the events of a sample spread over the batch are identical to the oracle's, one by one."""
+    from lhcb_gen import slice_events
+    from paper_2606_14480_b200 import Context, DeviceEvents, capacities
+    n = 16384
+    ev = generate(config(3, n), workers=8)
+    c = Context(capacities.with_capacities(ev.geom))
+    cfgl = c.lhcb_launch_config()
+    assert cfgl["seed_threads"] == 256 and cfgl["match_threads"] == 128
+    gs, gl = run_gpu(c, ev, True)
+    assert (gs["status"] == 0).all() and (gl["status"] == 0).all(), "capacity overflow at nominal occupancy"
+    ms, ml = c.max_seeds, c.max_long
+    sample = [0, 1, 63, 64, 1023, 4097, 8191, 12345, 16320, 16383] + list(range(5000, 5022))
+    n_s = n_l = 0
+    for e in sample:
+        sub = slice_events(ev, e, e + 1)
+        os_, om = oracle32.reconstruct(sub, use_ut=True)
+        sel = gs["event"] == e
+        g1 = {k: (v[sel] if isinstance(v, np.ndarray) and v.shape[:1] == sel.shape else v) for k, v in gs.items()}
+        g1["event"] = g1["event"] - e
+        h = g1["hits"].astype(np.int64)
+        h0 = int(ev.zone_off[e * 24])
+        g1["hits"] = np.where(h == 0xFFFFFFFF, h, h - h0).astype(np.uint32)
+        r = compare_seeds(os_, g1)
+        assert r["n_orc"] == r["n_gpu"] == r["n_common"] and r["bit_equal"], (e, r)
+        n_s += r["n_common"]
+        # long tracks of this event: (seed identity, velo, UT hits) sets
+        ok = dict(zip(range(os_["n"]), seed_keys(os_["event"], os_["half"], os_["hits"])))
+        gk = dict(zip((int(s) for s in g1["slot"]), seed_keys(g1["event"], g1["half"], g1["hits"])))
+        lsel = gl["event"] == e
+        l1 = {k: (v[lsel] if isinstance(v, np.ndarray) and v.shape[:1] == lsel.shape else v) for k, v in gl.items()}
+        l1["velo"] = l1["velo"] - int(ev.velo_off[e])
+        u = l1["ut"].astype(np.int64)
+        l1["ut"] = np.where(u == 0xFFFFFFFF, u, u - int(ev.ut_off[e * 4])).astype(np.uint32)
+        rl = compare_long(om, l1, ok, gk)
+        assert rl["n_orc"] == rl["n_gpu"] == rl["n_common"] and rl["bit_equal"], (e, rl)
+        n_l += rl["n_common"]
+    assert n_s > 100 * len(sample) and n_l > 60 * len(sample)
+    c.close()
