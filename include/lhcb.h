@@ -44,13 +44,14 @@ typedef enum {
 
 /* bits of the per-half / per-event `status` output words */
 #define LHCB_ST_TRIPLET_OVERFLOW 1u   /* more three-hit combinations than max_triplets_per_half */
-#define LHCB_ST_CAND_OVERFLOW 2u      /* more fitted x-z candidates than max_xz_cand_per_half */
+#define LHCB_ST_CAND_OVERFLOW 2u      /* more x-z candidates (>= min_x_hits) than max_xz_cand_per_half */
 #define LHCB_ST_SEED_OVERFLOW 4u      /* more seeds than max_seeds_per_half */
 #define LHCB_ST_HITS_OVERFLOW 8u      /* event-half has more hits than max_hits_per_half: half skipped */
 #define LHCB_ST_MATCH_OVERFLOW 16u    /* more chi2-accepted pairs than max_match_cand_per_event */
 #define LHCB_ST_LONG_OVERFLOW 32u     /* more long tracks than max_long_per_event */
 #define LHCB_ST_VELO_OVERFLOW 64u     /* more VELO tracks than max_velo_per_event: event skipped */
 #define LHCB_ST_UT_OVERFLOW 128u      /* more than 65534 UT hits in one event: event skipped */
+#define LHCB_ST_UV_QUEUE_OVERFLOW 256u /* stereo stage: survivors or queued u/v combinations exceed the shared work region */
 
 /* Detector description and tunables.  Host POD, copied by lhcb_geom_init.
  * Citations: PAPER.md line / equation; "A<n>" = reading listed in DESIGN.md. */

@@ -19,7 +19,7 @@ F, I = C.c_float, C.c_int32
 NO_HIT = 0xFFFFFFFF
 
 ST_BITS = {1: "triplet_overflow", 2: "cand_overflow", 4: "seed_overflow", 8: "hits_overflow",
-           16: "match_overflow", 32: "long_overflow", 64: "velo_overflow", 128: "ut_overflow"}
+           16: "match_overflow", 32: "long_overflow", 64: "velo_overflow", 128: "ut_overflow", 256: "uv_queue_overflow"}
 
 EXPORTS = ["lhcb_geom_derive", "lhcb_geom_init", "lhcb_destroy", "lhcb_get_geom", "lhcb_workspace_bytes",
            "lhcb_seeding", "lhcb_matching", "lhcb_error_string", "lhcb_last_cuda_error",

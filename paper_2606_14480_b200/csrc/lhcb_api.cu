@@ -20,7 +20,8 @@ struct lhcb_ctx {
   float* d_Q;
   size_t seed_smem, match_smem;
   int match_threads;  // 128 when six CTAs fit an SM, else 256
-  int seed_threads;   // 256 (4 CTAs/SM) when the capacities fit a quarter of the SM's shared memory, else 512
+  int seed_threads;   // 256 when four CTAs fit the SM's shared memory, else 512
+  int seed_ctas;      // CTAs per SM the seeding kernel is compiled for (register budget)
   int last_cuda_error;
   int last_launches;
 };
@@ -107,12 +108,13 @@ int lhcb_geom_init(const lhcb_geom_t* g, int device, lhcb_ctx** out) {
   if (rc != LHCB_OK) { delete c; return rc; }
   if (G.max_hits_per_half > 32768 || G.max_xz_cand_per_half > 65535 || G.max_seeds_per_half > 32767 ||
       G.max_velo_per_event > 65535 || G.max_ut_per_event > 65534 || G.max_match_cand_per_event > 16383 || G.max_triplets_per_half < G.max_xz_cand_per_half) { delete c; return LHCB_ERR_BAD_ARGUMENT; }
-  // 256-thread CTAs, four per SM, when their shared memory fits (228 KB per SM, 1 KB reserved per CTA);
-  // else 512-thread CTAs, two (or one) per SM
+  // 256-thread CTAs, four per SM, when their shared memory fits (228 KB per SM, 1 KB reserved per
+  // CTA); else 512-thread CTAs, two (or one) per SM
   c->seed_threads = 256;
   c->seed_smem = lhcb::seed_smem_bytes(256, G.max_hits_per_half, G.max_xz_cand_per_half, G.max_triplets_per_half);
+  c->seed_ctas = 4;   // (five 48-register CTAs per SM measured slower than four 64-register ones)
   if (c->seed_smem > (size_t)(228 * 1024 / 4 - 1024)) {
-    c->seed_threads = 512;
+    c->seed_threads = 512; c->seed_ctas = 2;
     c->seed_smem = lhcb::seed_smem_bytes(512, G.max_hits_per_half, G.max_xz_cand_per_half, G.max_triplets_per_half);
   }
   c->match_threads = 128;
@@ -128,9 +130,11 @@ int lhcb_geom_init(const lhcb_geom_t* g, int device, lhcb_ctx** out) {
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
   if (e != cudaSuccess) { c->last_cuda_error = (int)e; delete c; return LHCB_ERR_CUDA; }
   if (c->seed_smem > (size_t)max_optin || c->match_smem > (size_t)max_optin) { delete c; return LHCB_ERR_CAPACITY; }
-  e = c->seed_threads == 256
-          ? cudaFuncSetAttribute(lhcb::seeding_kernel<256, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->seed_smem)
-          : cudaFuncSetAttribute(lhcb::seeding_kernel<512, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->seed_smem);
+  {
+    const void* fn = c->seed_ctas == 4 ? (const void*)lhcb::seeding_kernel<256, 4>
+                                       : (const void*)lhcb::seeding_kernel<512, 2>;
+    e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->seed_smem);
+  }
   if (e == cudaSuccess)
     e = c->match_threads == 128
             ? cudaFuncSetAttribute(lhcb::matching_kernel<128, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->match_smem)
@@ -185,7 +189,7 @@ int lhcb_seeding(lhcb_ctx* c, const lhcb_events_t* ev, lhcb_seeds_t* out, void* 
   p.nuv = out->nuv; p.status = out->status;
   p.cap_total = (size_t)ev->n_events * 2 * (size_t)c->geom.max_seeds_per_half;
   p.smem_total = (int)c->seed_smem;
-  if (c->seed_threads == 256)
+  if (c->seed_ctas == 4)
     lhcb::seeding_kernel<256, 4><<<ev->n_events * 2, 256, c->seed_smem, (cudaStream_t)stream>>>(p);
   else
     lhcb::seeding_kernel<512, 2><<<ev->n_events * 2, 512, c->seed_smem, (cudaStream_t)stream>>>(p);
@@ -243,6 +247,12 @@ const char* lhcb_error_string(int s) {
 // diagnostic builds only: cycles summed over CTAs per seeding stage; reset != 0 zeroes the counters
 int lhcb_debug_stage_clocks(unsigned long long* out, int reset) {
   if (out && cudaMemcpyFromSymbol(out, lhcb::g_stage_clk, sizeof(lhcb::g_stage_clk)) != cudaSuccess) return LHCB_ERR_CUDA;
+  if (out) {                                                 // out[15] = four 16-bit maxima (lhcb::g_dbg_max)
+    unsigned int m[8];
+    if (cudaMemcpyFromSymbol(m, lhcb::g_dbg_max, sizeof(m)) != cudaSuccess) return LHCB_ERR_CUDA;
+    out[15] = (unsigned long long)(m[0] & 0xFFFF) | ((unsigned long long)(m[1] & 0xFFFF) << 16) |
+              ((unsigned long long)(m[2] & 0xFFFF) << 32) | ((unsigned long long)(m[3] & 0xFFFF) << 48);
+  }
   if (reset) {
     unsigned long long z[16] = {0};
     if (cudaMemcpyToSymbol(lhcb::g_stage_clk, z, sizeof(z)) != cudaSuccess) return LHCB_ERR_CUDA;

@@ -36,6 +36,8 @@ constexpr unsigned long long kNoKey = ~0ull;
 // CTA adds the cycles since its previous mark to g_stage_clk[i]; lhcb_debug_stage_clocks() reads them.
 #ifdef LHCB_STAGE_CLOCKS
 __device__ unsigned long long g_stage_clk[16];
+__device__ unsigned int g_dbg_max[8];     // maxima over CTAs: triplets per iteration, candidates, survivors, queued u/v combinations
+#define LHCB_DBG_MAX(i, v) if (threadIdx.x == 0) atomicMax(&g_dbg_max[i], (unsigned int)(v));
 #define LHCB_CLK_INIT long long clk_prev__ = clock64();
 #define LHCB_CLK(i)                                                                         \
   if (threadIdx.x == 0) {                                                                   \
@@ -46,6 +48,7 @@ __device__ unsigned long long g_stage_clk[16];
 #else
 #define LHCB_CLK_INIT
 #define LHCB_CLK(i)
+#define LHCB_DBG_MAX(i, v)
 #endif
 
 struct SeedParams {
@@ -79,7 +82,7 @@ struct SeedParams {
 };
 
 struct __align__(8) Triplet { uint16_t i1, i2, i3, it; };                 // zone-local indices
-struct __align__(16) Cand { float ax, bx, cx, chi2; uint16_t hit[6]; uint8_t nx, it, keep, pad; };
+struct __align__(16) Cand { float ax, bx, cx, chi2; uint16_t hit[6]; uint8_t nx, it, keep, pattern; };   // nx = 0: rejected by the fit
 
 struct __align__(16) Zone { int b, e; float x0, invw; };   // one 16-byte shared-memory load
 
@@ -98,15 +101,18 @@ constexpr int kSeedHeaderBytes = 640;
 static_assert(sizeof(SeedSmemHeader) <= kSeedHeaderBytes, "shared-memory header overflows its slot");
 
 // Shared-memory map of one CTA (NT threads), all offsets 16-byte aligned:
-//   [header | bin tables | scan scratch: int offs[NT+1], u16 first[NT] | kept list u16[max_cand] |
+//   [header | bin tables | scan scratch: int offs[NT+1], u16 first[NT], later the kept list u16[max_cand] |
 //    hits tile (the half's ACTUAL size) | work region W ... | x-z candidates, filled downward from the end]
 // W holds the triplet queue, then the clone table, then the u/v queues; it starts right after the staged
 // hits and ends where the candidates begin, so a half with fewer hits or candidates than the capacities
 // leaves more room for the queues.  The capacities guarantee W >= max_trip * 8 bytes.
 __host__ __device__ inline size_t seed_align16(size_t b) { return (b + 15) & ~(size_t)15; }
 __host__ __device__ inline size_t seed_off_scan() { return kSeedHeaderBytes + seed_align16(12 * (kLutBins + 1) * 2); }
-__host__ __device__ inline size_t seed_off_kept(int nt) { return seed_off_scan() + seed_align16((size_t)(nt + 1) * 4 + (size_t)nt * 2); }
-__host__ __device__ inline size_t seed_off_hits(int nt, int max_cand) { return seed_off_kept(nt) + seed_align16((size_t)max_cand * 2); }
+// the kept list (clone-kill survivors, used from S3 on) shares its slot with the scan scratch (used by S1 only)
+__host__ __device__ inline size_t seed_off_hits(int nt, int max_cand) {
+  const size_t scan = (size_t)(nt + 1) * 4 + (size_t)nt * 2, kept = (size_t)max_cand * 2;
+  return seed_off_scan() + seed_align16(scan > kept ? scan : kept);
+}
 __host__ __device__ inline size_t seed_smem_bytes(int nt, int max_hits, int max_cand, int max_trip) {
   size_t b = seed_off_hits(nt, max_cand);
   b += seed_align16(((size_t)max_hits + 8) * 4);           // hits tile (16-byte aligned superset)
@@ -173,23 +179,37 @@ __device__ __forceinline__ int owner_of(const int* offs, int n, int p) {
   return b;
 }
 // index of the hit closest to xp with |x - xp| <= tol, ties to the lower index; -1 if none.
-// One forward scan: it starts at the bin of (xp - tol - guard), so every hit that can pass the literal
-// predicate fabsf(x - xp) <= tol is visited (the guard of 1/64 mm is far above one rounding of x - xp at
+// The scan starts at the bin of (xp - tol - guard), so every hit that can pass the literal predicate
+// fabsf(x - xp) <= tol is visited (the guard of 1/64 mm is far above one rounding of x - xp at
 // |x| < 2^15 mm), and ends at the first hit above xp + tol + guard.  Strict "<" keeps the lowest index
-// among equal distances, like the oracle's linear scan.
+// among equal distances, like the oracle's linear scan.  With about 0.6 hits per bin the first three
+// hits from the bin start almost always reach past the window: they are probed without a branch (every
+// lane of the warp does the same work); the loop is the rare tail.
 __device__ __forceinline__ int closest_hit(const float* __restrict__ x, const uint16_t* __restrict__ lut,
                                            const Zone& z, float xp, float tol, float& xbest) {
   const float guard = tol + 0.015625f;
   const float hi = xp + guard;
-  int i = lut[zone_bin(z, xp - guard)];
+  const int i0 = lut[zone_bin(z, xp - guard)];
   int best = -1;
-  float bd = 0.f;
-  while (i < z.e) {
-    const float xi = x[i];
-    if (xi > hi) break;
+  float bd = 0.f, xlast = 0.f;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const float v = x[i0 + k];                               // at most 3 floats past the zone: still shared memory
+    const float xi = i0 + k < z.e ? v : __int_as_float(0x7f800000);
     const float d = fabsf(xi - xp);
-    if (d <= tol && (best < 0 || d < bd)) { best = i; bd = d; xbest = xi; }
-    ++i;
+    const bool ok = d <= tol && (best < 0 || d < bd);
+    best = ok ? i0 + k : best; bd = ok ? d : bd; xbest = ok ? xi : xbest;
+    xlast = xi;
+  }
+  if (xlast <= hi) {
+    int i = i0 + 3;
+    while (i < z.e) {
+      const float xi = x[i];
+      if (xi > hi) break;
+      const float d = fabsf(xi - xp);
+      if (d <= tol && (best < 0 || d < bd)) { best = i; bd = d; xbest = xi; }
+      ++i;
+    }
   }
   return best;
 }
@@ -300,7 +320,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   uint16_t* lut = reinterpret_cast<uint16_t*>(smem + kSeedHeaderBytes);
   int* scan_offs = reinterpret_cast<int*>(smem + seed_off_scan());            // [NT + 1] exclusive offsets
   uint16_t* scan_first = reinterpret_cast<uint16_t*>(scan_offs + NT + 1);      // [NT] first index per owner
-  uint16_t* kept = reinterpret_cast<uint16_t*>(smem + seed_off_kept(NT));
+  uint16_t* kept = reinterpret_cast<uint16_t*>(smem + seed_off_scan());         // aliases the scan scratch
   const int off_hits = (int)seed_off_hits(NT, p.max_cand);
   float* hx = reinterpret_cast<float*>(smem + off_hits);
   Cand* cand_end = reinterpret_cast<Cand*>(smem + p.smem_total);               // candidate c lives at cand_end[-1 - c]
@@ -461,9 +481,9 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
           const float kinv = p.kappa * invp;
           const float cxp = x0 >= 0.f ? -kinv : kinv;                            // A3
           const float ca = p.f_lo * cxp, cb = p.f_hi * cxp;                      // A4
-          const float cxlo = (ca < cb ? ca : cb) - p.d_lo, cxhi = (ca > cb ? ca : cb) + p.d_hi;
+          const float cxlo = fminf(ca, cb) - p.d_lo, cxhi = fmaxf(ca, cb) + p.d_hi;
           const float ea = x2c + K * cxlo, eb = x2c + K * cxhi;
-          const float lo2 = ea < eb ? ea : eb, hi2 = ea > eb ? ea : eb;
+          const float lo2 = fminf(ea, eb), hi2 = fmaxf(ea, eb);
           int j = lower_bound(hx, lut2, z2n, lo2);
           while (j < e2 && hx[j] <= hi2) {
             const int k = atomicAdd(&H.n_trip, 1);
@@ -480,6 +500,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
       LHCB_CLK(3)
     }
     int nt = H.n_trip;
+    LHCB_DBG_MAX(0, nt)
     if (nt > trip_cap) { nt = trip_cap; if (tid == 0) H.status |= LHCB_ST_TRIPLET_OVERFLOW; }
 
     for (int t = tid; t < nt; t += T) {                                          // O5 + O6
@@ -491,60 +512,34 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
       float cx = (x2 - x2c) * p.inv_K[it];
       float bx = t13 - cx * p.G13[it];
       float ax = (x1 - bx * p.zb[l1]) - cx * p.gz[l1];
-      float r[6];
       int hit[6];
       int nx = 0, pattern = 0;
 #pragma unroll
       for (int s = 0; s < 6; ++s) {
         const int l = p.xl[s];
-        const float xp = xz_at(p, ax, bx, cx, l);
         int hh;
-        float xh = 0.f;
-        if (l == l1) { hh = i1; xh = x1; }
-        else if (l == l2) { hh = i2; xh = x2; }
-        else if (l == l3) { hh = i3; xh = x3; }
-        else { const Zone z = H.zi[l]; hh = closest_hit(hx, lut + l * (kLutBins + 1), z, xp, p.tol_x, xh); }
-        if (hh < 0) { hit[s] = -1; pattern = 1 + s; r[s] = 0.f; }
-        else { hit[s] = hh - zl[l]; r[s] = xh - xp; ++nx; }
+        if (l == l1) hh = i1;
+        else if (l == l2) hh = i2;
+        else if (l == l3) hh = i3;
+        else {
+          const Zone z = H.zi[l];
+          float xh;
+          hh = closest_hit(hx, lut + l * (kLutBins + 1), z, xz_at(p, ax, bx, cx, l), p.tol_x, xh);
+        }
+        if (hh < 0) { hit[s] = -1; pattern = 1 + s; }
+        else { hit[s] = hh - zl[l]; ++nx; }
         if (s + 1 - nx > 6 - p.min_x_hits) break;               // too many layers missed already
       }
       if (nx < p.min_x_hits) continue;
-      // fixed-matrix least squares on the residuals w.r.t. the three-point parabola
-      const float* __restrict__ P = p.P + pattern * 18;
-      float d[3];
-#pragma unroll
-      for (int k = 0; k < 3; ++k) {
-        float acc = 0.f;
-        bool first = true;
-#pragma unroll
-        for (int s = 0; s < 6; ++s) {
-          if (pattern == 1 + s) continue;
-          const float tt = __ldg(P + k * 6 + s) * r[s];
-          acc = first ? tt : acc + tt;
-          first = false;
-        }
-        d[k] = acc;
-      }
-      float ssq = 0.f;
-      bool first = true;
-#pragma unroll
-      for (int s = 0; s < 6; ++s) {
-        if (pattern == 1 + s) continue;
-        const int l = p.xl[s];
-        const float rr = r[s] - ((d[0] + d[1] * p.zb[l]) + d[2] * p.gz[l]);
-        ssq = first ? rr * rr : ssq + rr * rr;
-        first = false;
-      }
-      ax = ax + d[0]; bx = bx + d[1]; cx = cx + d[2];
-      const float chi2 = ssq * p.wx[nx];
-      if (chi2 > p.chi2x_max) continue;
+      // enough x-hits: queue the three-point parabola and its hits; the least-squares fit runs as a dense
+      // pass over the queued candidates of both iterations (S2b)
       const int k = atomicAdd(&H.n_cand, 1);
       if (k < p.max_cand) {
         Cand cd;
-        cd.ax = ax; cd.bx = bx; cd.cx = cx; cd.chi2 = chi2;
+        cd.ax = ax; cd.bx = bx; cd.cx = cx; cd.chi2 = 0.f;
 #pragma unroll
         for (int s = 0; s < 6; ++s) cd.hit[s] = hit[s] < 0 ? (uint16_t)0xFFFF : (uint16_t)hit[s];
-        cd.nx = (uint8_t)nx; cd.it = (uint8_t)it; cd.keep = 0; cd.pad = 0;
+        cd.nx = (uint8_t)nx; cd.it = (uint8_t)it; cd.keep = 0; cd.pattern = (uint8_t)pattern;
         cand_end[-1 - k] = cd;
       }
     }
@@ -554,14 +549,59 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     __syncthreads();
   }
 
-  // ---- S3: clone kill (O7) ------------------------------------------------------------------
   int nc = H.n_cand;
+  LHCB_DBG_MAX(1, nc)
   if (nc > p.max_cand) { nc = p.max_cand; if (tid == 0) H.status |= LHCB_ST_CAND_OVERFLOW; }
+  // ---- S2b: least-squares fit of every queued candidate (O6): fixed pseudo-inverse map per missing-layer
+  // pattern applied to the residuals w.r.t. the three-point parabola
+  for (int c = tid; c < nc; c += T) {
+    Cand& cd = cand_end[-1 - c];
+    const int pattern = cd.pattern;
+    float ax = cd.ax, bx = cd.bx, cx = cd.cx;
+    float r[6];
+#pragma unroll
+    for (int s = 0; s < 6; ++s) {
+      const int l = p.xl[s];
+      r[s] = 0.f;
+      if (pattern != 1 + s) r[s] = hx[zl[l] + cd.hit[s]] - xz_at(p, ax, bx, cx, l);
+    }
+    const float* __restrict__ P = p.P + pattern * 18;
+    float d[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      float acc = 0.f;
+      bool first = true;
+#pragma unroll
+      for (int s = 0; s < 6; ++s) {
+        if (pattern == 1 + s) continue;
+        const float tt = __ldg(P + k * 6 + s) * r[s];
+        acc = first ? tt : acc + tt;
+        first = false;
+      }
+      d[k] = acc;
+    }
+    float ssq = 0.f;
+    bool first = true;
+#pragma unroll
+    for (int s = 0; s < 6; ++s) {
+      if (pattern == 1 + s) continue;
+      const int l = p.xl[s];
+      const float rr = r[s] - ((d[0] + d[1] * p.zb[l]) + d[2] * p.gz[l]);
+      ssq = first ? rr * rr : ssq + rr * rr;
+      first = false;
+    }
+    const float chi2 = ssq * p.wx[cd.nx];
+    cd.ax = ax + d[0]; cd.bx = bx + d[1]; cd.cx = cx + d[2]; cd.chi2 = chi2;
+    if (chi2 > p.chi2x_max) cd.nx = 0;
+  }
+  __syncthreads();
+  // ---- S3: clone kill (O7) ------------------------------------------------------------------
   const int n_xhits = H.xbase[6];
   for (int i = tid; i < n_xhits; i += T) tbl[i] = kNoKey;
   __syncthreads();
   for (int c = tid; c < nc; c += T) {
     const Cand& cd = cand_end[-1 - c];
+    if (cd.nx == 0) continue;
     const unsigned long long key = clone_key(cd.chi2, cd.cx, cd.nx, cd.it);
 #pragma unroll
     for (int s = 0; s < 6; ++s)
@@ -570,6 +610,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   __syncthreads();
   for (int c = tid; c < nc; c += T) {
     Cand& cd = cand_end[-1 - c];
+    if (cd.nx == 0) continue;
     const unsigned long long key = clone_key(cd.chi2, cd.cx, cd.nx, cd.it);
     int own = 0;
 #pragma unroll
@@ -581,25 +622,32 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   }
   __syncthreads();
   int nk = H.n_kept;
-  const int wbytes = p.smem_total - nc * (int)sizeof(Cand) - off_w;      // unused candidate slots join W
-  {                                                            // survivors must leave room for the queues
-    const int nk_max = (wbytes - 4096) / 40;
-    if (nk > nk_max) { nk = nk_max > 0 ? nk_max : 0; if (tid == 0) H.status |= LHCB_ST_CAND_OVERFLOW; }
+  LHCB_DBG_MAX(2, nk)
+  // The clone table is dead.  The survivors move to the bottom of W; after that every candidate slot is
+  // dead too and W extends to the end of shared memory:
+  //   [survivors | best key per survivor | predictions per survivor | item chunk | live walks | success queue]
+  const int wbytes = p.smem_total - off_w;
+  {                                                            // survivors must fit below the candidate slots (the
+    int nk_max = (wbytes - 4096) / 72;                         // copy is in place) and leave room for the queues
+    if (nk_max > w_stat / 32) nk_max = w_stat / 32;
+    if (nk > nk_max) { nk = nk_max > 0 ? nk_max : 0; if (tid == 0) H.status |= LHCB_ST_UV_QUEUE_OVERFLOW; }
   }
-  // table is dead: reuse the region for
-  //   [best key per survivor | predictions per survivor | item chunk | live walks | success queue]
-  unsigned long long* best = tbl;
+  Cand* surv = reinterpret_cast<Cand*>(smem + off_w);
+  for (int k = tid; k < nk; k += T) surv[k] = cand_end[-1 - (int)kept[k]];
+  unsigned long long* best = reinterpret_cast<unsigned long long*>(surv + nk);
   float* xps = reinterpret_cast<float*>(best + ((nk + 1) & ~1));          // [nk][8], 16-byte aligned: x_pred per stereo layer
-  const int rest = wbytes - ((nk + 1) & ~1) * 8 - nk * 32;                // >= 4096 - 8
-  int C = ((rest / 2) / 20) & ~31;                                        // items per chunk: 4 B item + 16 B live walk
+  const int rest = wbytes - nk * 32 - ((nk + 1) & ~1) * 8 - nk * 32;      // >= 4096 - 8
+  int C = (rest / 2) / 20;                                                // items per chunk: 4 B item + 16 B live walk
+  C = C >= T ? C / T * T : (C & ~31);                                     // whole rounds of the CTA when possible
   if (C < 32) C = 32;
   uint32_t* items = reinterpret_cast<uint32_t*>(xps + (size_t)nk * 8);
   UvLive* live = reinterpret_cast<UvLive*>(items + C);
   UvSuccess* succ = reinterpret_cast<UvSuccess*>(live + C);
   const int succ_cap = (rest - C * 20) / (int)sizeof(UvSuccess);
+  __syncthreads();
   for (int k = tid; k < nk; k += T) {
     best[k] = kNoKey;
-    const Cand& cd = cand_end[-1 - (int)kept[k]];
+    const Cand& cd = surv[k];
 #pragma unroll
     for (int s = 0; s < 6; ++s) xps[k * 8 + s] = xz_at(p, cd.ax, cd.bx, cd.cx, p.ul[s]);
   }
@@ -682,7 +730,8 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     LHCB_CLK(7)
   }
   int nsucc = H.n_trip;
-  if (nsucc > succ_cap) { nsucc = succ_cap; if (tid == 0) H.status |= LHCB_ST_CAND_OVERFLOW; }
+  LHCB_DBG_MAX(3, nsucc)
+  if (nsucc > succ_cap) { nsucc = succ_cap; if (tid == 0) H.status |= LHCB_ST_UV_QUEUE_OVERFLOW; }
 
   // ---- S5: y fit of every queued combination, best per survivor, seeds (O9, O10) ------------------
   const int pol = p.pol ? (int)p.pol[event] : p.polarity;
@@ -718,7 +767,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   for (int i = tid; i < nsucc; i += T) {
     if (!single) fit_success(i);                               // more than one round: redo the (cheap) fit
     if (key == kNoKey || best[u.k] != key) continue;           // not the best combination of its survivor
-    const Cand& cd = cand_end[-1 - (int)kept[u.k]];
+    const Cand& cd = surv[u.k];
     const int slot = atomicAdd(&H.n_seed, 1);
     if (slot >= p.max_seeds) continue;
     const size_t o = (size_t)slot0 + slot, ct = p.cap_total;
