@@ -244,18 +244,20 @@ const char* lhcb_error_string(int s) {
 }
 
 #ifdef LHCB_STAGE_CLOCKS
-// diagnostic builds only: cycles summed over CTAs per seeding stage; reset != 0 zeroes the counters
+// diagnostic builds only: out[0..15] cycles summed over CTAs per stage, out[16..23] maxima over CTAs of the
+// queue fills (lhcb::g_dbg_max); reset != 0 zeroes both
 int lhcb_debug_stage_clocks(unsigned long long* out, int reset) {
-  if (out && cudaMemcpyFromSymbol(out, lhcb::g_stage_clk, sizeof(lhcb::g_stage_clk)) != cudaSuccess) return LHCB_ERR_CUDA;
-  if (out) {                                                 // out[15] = four 16-bit maxima (lhcb::g_dbg_max)
+  if (out) {
+    if (cudaMemcpyFromSymbol(out, lhcb::g_stage_clk, sizeof(lhcb::g_stage_clk)) != cudaSuccess) return LHCB_ERR_CUDA;
     unsigned int m[8];
     if (cudaMemcpyFromSymbol(m, lhcb::g_dbg_max, sizeof(m)) != cudaSuccess) return LHCB_ERR_CUDA;
-    out[15] = (unsigned long long)(m[0] & 0xFFFF) | ((unsigned long long)(m[1] & 0xFFFF) << 16) |
-              ((unsigned long long)(m[2] & 0xFFFF) << 32) | ((unsigned long long)(m[3] & 0xFFFF) << 48);
+    for (int i = 0; i < 8; ++i) out[16 + i] = m[i];
   }
   if (reset) {
     unsigned long long z[16] = {0};
+    unsigned int zm[8] = {0};
     if (cudaMemcpyToSymbol(lhcb::g_stage_clk, z, sizeof(z)) != cudaSuccess) return LHCB_ERR_CUDA;
+    if (cudaMemcpyToSymbol(lhcb::g_dbg_max, zm, sizeof(zm)) != cudaSuccess) return LHCB_ERR_CUDA;
   }
   return LHCB_OK;
 }

@@ -57,11 +57,11 @@ struct MatchParams {
 
 struct __align__(8) MatchCand {
   uint16_t seed, velo;      // event-local seed index; rank of the VELO state in t_y order
-  float chi2, q0;
-  uint32_t valid;
+  float chi2, q0, gamma;    // chi2_match, kick q/p (A10), gamma_x of the best UT hypothesis
   unsigned long long key;   // best UT hypothesis: (4 - n_ut) << 50 | f32 bits of sum res^2 << 18 | layer << 16 | first hit
+  uint16_t ut[4];           // its hits, relative to the event's first UT hit (0xFFFF = none)
 };
-static_assert(sizeof(MatchCand) == 24, "MatchCand is 24 bytes");
+static_assert(sizeof(MatchCand) == 32, "MatchCand is 32 bytes");
 
 __host__ __device__ inline size_t match_smem_bytes(int kMatchThreads, int max_seeds, int max_mc, int max_velo, int max_ut) {
   size_t b = 64;
@@ -297,7 +297,9 @@ matching_kernel(const __grid_constant__ MatchParams p) {
         if (k < p.max_mc) {
           MatchCand m;
           m.seed = (uint16_t)s; m.velo = (uint16_t)v; m.chi2 = chi2; m.q0 = dtx * p.inv_KB;   // A10
-          m.valid = 1; m.key = kNoKey;
+          m.gamma = 0.f; m.key = kNoKey;
+#pragma unroll
+          for (int l = 0; l < 4; ++l) m.ut[l] = 0xFFFF;
           mc[k] = m;
         }
       }
@@ -307,6 +309,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
   }
   __syncthreads();
   int nm = hdr[0];
+  LHCB_DBG_MAX(4, nm)
   if (nm > p.max_mc) { nm = p.max_mc; if (tid == 0) hdr[2] |= LHCB_ST_MATCH_OVERFLOW; }
 
   // ---- M3: UT hits (O13) -----------------------------------------------------------------------
@@ -354,29 +357,45 @@ matching_kernel(const __grid_constant__ MatchParams p) {
           if (slot < p.max_mc) hyq[slot] = ((uint32_t)k << 18) | ((uint32_t)i0 << 16) | (uint32_t)(j + rel0);
         }
       }
-      m.valid = found;
     }
     __syncthreads();
     int nh = hdr[3];
+    LHCB_DBG_MAX(5, nh)
     if (nh > p.max_mc) { nh = p.max_mc; if (tid == 0) hdr[2] |= LHCB_ST_MATCH_OVERFLOW; }
-    // M3b: tight walk of every hypothesis; the best one of each pair wins the atomicMin
-    for (int i = tid; i < nh; i += kMatchThreads) {
-      const uint32_t hq = hyq[i];
-      const int k = (int)(hq >> 18), i0 = (int)((hq >> 16) & 3u), jrel = (int)(hq & 0xFFFFu);
-      const MatchCand& m = mc[k];
-      const int v = m.velo;
+    // M3b: tight walk of every hypothesis; the best one of each pair wins the atomicMin and, after the
+    // barrier, leaves its hits and gamma_x in the pair's record (a better hypothesis of a later round
+    // overwrites them)
+    for (int i0r = 0; i0r < nh; i0r += kMatchThreads) {
+      const int i = i0r + tid;
       UtHyp hy;
-      ut_tight_walk(p, svx[v], svy[v], svtx[v], svty[v], fabsf(m.q0) * 1000.f, i0, jrel - rel0, ux, uylo, uyhi, uo, hy);
-      const unsigned long long key = ((unsigned long long)(4 - hy.n) << 50) |
-                                     ((unsigned long long)__float_as_uint(hy.ssq) << 18) | (hq & 0x3FFFFu);
-      atomicMin(&mc[k].key, key);
+      unsigned long long key = kNoKey;
+      int k = 0;
+      if (i < nh) {
+        const uint32_t hq = hyq[i];
+        k = (int)(hq >> 18);
+        const int i0 = (int)((hq >> 16) & 3u), jrel = (int)(hq & 0xFFFFu);
+        const MatchCand& m = mc[k];
+        const int v = m.velo;
+        ut_tight_walk(p, svx[v], svy[v], svtx[v], svty[v], fabsf(m.q0) * 1000.f, i0, jrel - rel0, ux, uylo, uyhi, uo, hy);
+        key = ((unsigned long long)(4 - hy.n) << 50) | ((unsigned long long)__float_as_uint(hy.ssq) << 18) |
+              (hq & 0x3FFFFu);
+        atomicMin(&mc[k].key, key);
+      }
+      __syncthreads();
+      if (i < nh && mc[k].key == key) {
+        MatchCand& m = mc[k];
+        m.gamma = hy.gamma;
+#pragma unroll
+        for (int l = 0; l < 4; ++l) m.ut[l] = hy.idx[l] < 0 ? (uint16_t)0xFFFF : (uint16_t)(hy.idx[l] + rel0);
+      }
     }
     __syncthreads();
   }
+  // a pair is valid if its best hypothesis has enough UT hits (L311); without UT every pair is
+  const unsigned long long key_ok = p.use_ut ? (unsigned long long)(4 - p.min_ut_hits) : ~0ull >> 50;
   for (int k = tid; k < nm; k += kMatchThreads) {
-    MatchCand& m = mc[k];
-    if (p.use_ut && m.valid) m.valid = (4 - (int)(m.key >> 50)) >= p.min_ut_hits;   // L311
-    if (m.valid)
+    const MatchCand& m = mc[k];
+    if ((m.key >> 50) <= key_ok)
       atomicMin(&seed_best[m.seed], ((unsigned long long)__float_as_uint(m.chi2) << 32) | sorig[m.velo]);
   }
   __syncthreads();
@@ -384,7 +403,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
   // ---- M4: one-to-one selection (O14) -------------------------------------------------------------
   for (int k = tid; k < nm; k += kMatchThreads) {
     const MatchCand& m = mc[k];
-    if (!m.valid) continue;
+    if ((m.key >> 50) > key_ok) continue;
     const unsigned long long cb = (unsigned long long)__float_as_uint(m.chi2) << 32;
     if (seed_best[m.seed] != (cb | sorig[m.velo])) continue;
     atomicMin(&velo_best[sorig[m.velo]], cb | m.seed);
@@ -393,7 +412,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
   const int pol = p.pol ? (int)p.pol[e] : p.polarity;
   for (int k = tid; k < nm; k += kMatchThreads) {
     const MatchCand& m = mc[k];
-    if (!m.valid) continue;
+    if ((m.key >> 50) > key_ok) continue;
     const unsigned long long cb = (unsigned long long)__float_as_uint(m.chi2) << 32;
     const int vo = sorig[m.velo];
     if (seed_best[m.seed] != (cb | vo) || velo_best[vo] != (cb | m.seed)) continue;
@@ -404,16 +423,12 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     p.seed_idx[o] = s < c0 ? (uint32_t)((2 * e) * p.max_seeds + s) : (uint32_t)((2 * e + 1) * p.max_seeds + (s - c0));
     p.velo_idx[o] = v0 + vo;
     float q = m.q0;                                                              // A10
-    if (p.use_ut) {                                          // walk the winning hypothesis once more for its hits
-      const int v = m.velo;
-      const int i0 = (int)((m.key >> 16) & 3u), jrel = (int)(m.key & 0xFFFFu);
-      UtHyp hy;
-      ut_tight_walk(p, svx[v], svy[v], svtx[v], svty[v], fabsf(m.q0) * 1000.f, i0, jrel - rel0, ux, uylo, uyhi, uo, hy);
+    if (p.use_ut) {
 #pragma unroll
       for (int l = 0; l < 4; ++l)
-        p.ut_idx[(size_t)l * ct + o] = hy.idx[l] < 0 ? LHCB_NO_HIT : u_begin + (uint32_t)(hy.idx[l] + rel0);
-      p.n_ut[o] = (uint8_t)hy.n;
-      q = (hy.gamma - p.Ag) * p.inv_Bg;                                          // Eq. 20 inverted
+        p.ut_idx[(size_t)l * ct + o] = m.ut[l] == 0xFFFF ? LHCB_NO_HIT : u_begin + (uint32_t)m.ut[l];
+      p.n_ut[o] = (uint8_t)(4 - (int)(m.key >> 50));
+      q = (m.gamma - p.Ag) * p.inv_Bg;                                           // Eq. 20 inverted
     } else {
 #pragma unroll
       for (int l = 0; l < 4; ++l) p.ut_idx[(size_t)l * ct + o] = LHCB_NO_HIT;
