@@ -213,6 +213,12 @@ matching_kernel(const __grid_constant__ MatchParams p) {
           asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(mbar_addr) : "memory");
         }
       }
+      if (tid == 32 && aligned && ua1 > ua0 && ((reinterpret_cast<uintptr_t>(p.uylo) | reinterpret_cast<uintptr_t>(p.uyhi)) & 15) == 0) {
+        // the y ranges of the hits the UT search will touch: pull the event's slice into L2 while M0-M2 run
+        const uint32_t bytes = (ua1 - ua0) * 4u;
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p.uylo + ua0), "r"(bytes) : "memory");
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p.uyhi + ua0), "r"(bytes) : "memory");
+      }
       for (uint32_t i = ua1 + tid; i < u_end; i += kMatchThreads) sux[i - ua0] = p.ux[i];
       if (tid < 5) hdr[4 + tid] = (int)(p.ut_off[(size_t)e * 4 + tid] - ua0);
     } else if (tid < 5) {
