@@ -144,6 +144,22 @@ __device__ __forceinline__ int lower_bound(const float* __restrict__ x, const ui
     while (i < z.e && x[i] < v) ++i;
   return i;
 }
+// the same, also returning x[i] (+inf when i == e)
+__device__ __forceinline__ int lower_bound_v(const float* __restrict__ x, const uint16_t* __restrict__ lut,
+                                             const Zone& z, float v, float& xv) {
+  const float inf = __int_as_float(0x7f800000);
+  int i = lut[zone_bin(z, v)];
+  float xi = i < z.e ? x[i] : inf;
+  if (xi < v) {
+    ++i; xi = i < z.e ? x[i] : inf;
+    if (xi < v) {
+      ++i; xi = i < z.e ? x[i] : inf;
+      while (xi < v) { ++i; xi = i < z.e ? x[i] : inf; }
+    }
+  }
+  xv = xi;
+  return i;
+}
 // first index in [b, e) with x[i] > v
 __device__ __forceinline__ int upper_bound(const float* __restrict__ x, const uint16_t* __restrict__ lut,
                                            const Zone& z, float v) {
@@ -484,8 +500,9 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
           const float cxlo = fminf(ca, cb) - p.d_lo, cxhi = fmaxf(ca, cb) + p.d_hi;
           const float ea = x2c + K * cxlo, eb = x2c + K * cxhi;
           const float lo2 = fminf(ea, eb), hi2 = fmaxf(ea, eb);
-          int j = lower_bound(hx, lut2, z2n, lo2);
-          while (j < e2 && hx[j] <= hi2) {
+          float xj;
+          int j = lower_bound_v(hx, lut2, z2n, lo2, xj);
+          while (xj <= hi2) {
             const int k = atomicAdd(&H.n_trip, 1);
             if (k < trip_cap) {
               Triplet tr;
@@ -493,6 +510,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
               trip[k] = tr;
             }
             ++j;
+            xj = j < e2 ? hx[j] : __int_as_float(0x7f800000);
           }
         }
       }
