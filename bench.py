@@ -40,7 +40,7 @@ def sample_clocks(stop, out, gpu_index):
                 out.append(f)
         except Exception:
             pass
-        stop.wait(0.1)
+        stop.wait(0.05)
 
 
 def clocks_summary(samples):
@@ -96,7 +96,7 @@ def run_reference(args, rank, world):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--events", type=int, default=16384, help="events per GPU batch (cfg3: 16384)")
