@@ -6,6 +6,7 @@ reconstruction arithmetic.
 from .geometry import DEFAULT_GEOM, default_geom, X_LAYERS, UV_LAYERS, TAN5
 from .events import GenConfig, Events, config, generate, slice_events
 from . import truth
+from .raw import shuffle_raw
 
 __all__ = ["DEFAULT_GEOM", "default_geom", "X_LAYERS", "UV_LAYERS", "TAN5",
-           "GenConfig", "Events", "config", "generate", "slice_events", "truth"]
+           "GenConfig", "Events", "config", "generate", "slice_events", "truth", "shuffle_raw"]
