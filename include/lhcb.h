@@ -51,6 +51,7 @@ typedef enum {
 #define LHCB_ST_LONG_OVERFLOW 32u     /* more long tracks than max_long_per_event */
 #define LHCB_ST_VELO_OVERFLOW 64u     /* more VELO tracks than max_velo_per_event: event skipped */
 #define LHCB_ST_UT_OVERFLOW 128u      /* more than 65534 UT hits in one event: event skipped */
+#define LHCB_ST_BAD_RAW_HIT 512u       /* lhcb_prepare: a raw hit with zone >= 24 or a non-finite x: event passed through unsorted */
 #define LHCB_ST_UV_QUEUE_OVERFLOW 256u /* stereo stage: survivors or queued u/v combinations exceed the shared work region */
 
 /* Detector description and tunables.  Host POD, copied by lhcb_geom_init.
@@ -123,6 +124,15 @@ typedef struct {
   const int8_t* polarity;    /* [n_events] +1/-1, or NULL -> geom.polarity */
 } lhcb_events_t;
 
+/* Raw SciFi hits of a batch of events, in any order inside each event: the input of lhcb_prepare. */
+typedef struct {
+  int32_t n_events;
+  uint32_t n_hits;           /* length of x and zone */
+  const uint32_t* off;       /* [n_events+1] first raw hit of each event */
+  const float* x;            /* [n_hits] finite; stereo layers: x at y=0 */
+  const uint8_t* zone;       /* [n_hits] half*12 + layer, in [0, 24); half 0: y>0 */
+} lhcb_raw_t;
+
 /* Seeds ("T tracks", L219).  Event-half h owns slots [h*max_seeds_per_half, +count[h]); the order
  * inside a slot range is unspecified.  cap_total = n_events*2*max_seeds_per_half. */
 typedef struct {
@@ -178,6 +188,20 @@ int lhcb_get_geom(const lhcb_ctx* ctx, lhcb_geom_t* out);
 
 /* Bytes of device scratch the two calls need for a batch (may be 0; pass NULL workspace then). */
 size_t lhcb_workspace_bytes(const lhcb_ctx* ctx, int n_events, size_t n_scifi_hits);
+
+/* Event preparation, the step before the hot path (hits tiled by detector half and layer;
+ * the searches of section 3 need them sorted in x).  Inside each event the raw hits are
+ * ordered by (zone, x, raw index): a stable sort.  Outputs (device pointers, caller-owned, overwritten):
+ *   zone_off [n_events*24+1]  prefix offsets; event e keeps the range [raw.off[e], raw.off[e+1])
+ *   hit_x    [n_hits]         x in sorted order: with zone_off, the lhcb_events_t that lhcb_seeding reads
+ *   perm     [n_hits] or NULL perm[k] = raw index of sorted hit k
+ *   status   [n_events]       0, or LHCB_ST_HITS_OVERFLOW (more raw hits in the event than
+ *                             2*max_hits_per_half or than 65535) / LHCB_ST_BAD_RAW_HIT; such an event is
+ *                             passed through unsorted with all its hits in zone 0 (lhcb_seeding then finds
+ *                             nothing in it): reported, never silent.
+ * Enqueues one kernel on cuda_stream; does not synchronise or allocate. */
+int lhcb_prepare(lhcb_ctx* ctx, const lhcb_raw_t* raw, uint32_t* zone_off, float* hit_x, uint32_t* perm,
+                 uint32_t* status, void* cuda_stream);
 
 /* Seeding: x-z two-/three-hit search, extension, fit, clone kill, u/v addition, y fit (section 3).
  * One CTA per event-half.  `out` arrays must have cap_total = n_events*2*max_seeds_per_half slots. */

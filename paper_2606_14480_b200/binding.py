@@ -19,12 +19,12 @@ F, I = C.c_float, C.c_int32
 NO_HIT = 0xFFFFFFFF
 
 ST_BITS = {1: "triplet_overflow", 2: "cand_overflow", 4: "seed_overflow", 8: "hits_overflow",
-           16: "match_overflow", 32: "long_overflow", 64: "velo_overflow", 128: "ut_overflow", 256: "uv_queue_overflow"}
+           16: "match_overflow", 32: "long_overflow", 64: "velo_overflow", 128: "ut_overflow", 256: "uv_queue_overflow", 512: "bad_raw_hit"}
 
 EXPORTS = ["lhcb_geom_derive", "lhcb_geom_init", "lhcb_destroy", "lhcb_get_geom", "lhcb_workspace_bytes",
            "lhcb_seeding", "lhcb_matching", "lhcb_error_string", "lhcb_last_cuda_error",
            "lhcb_last_launch_count", "lhcb_pipeline_create", "lhcb_pipeline_destroy", "lhcb_reconstruct_host",
-           "lhcb_pipeline_last_bytes", "lhcb_launch_config"]
+           "lhcb_pipeline_last_bytes", "lhcb_launch_config", "lhcb_prepare"]
 
 
 class LhcbGeom(C.Structure):
@@ -67,6 +67,10 @@ VP = C.c_void_p
 
 class LhcbEvents(C.Structure):
     _fields_ = [("n_events", I), ("n_hits", C.c_uint32), ("zone_off", VP), ("hit_x", VP), ("polarity", VP)]
+
+
+class LhcbRaw(C.Structure):
+    _fields_ = [("n_events", I), ("n_hits", C.c_uint32), ("off", VP), ("x", VP), ("zone", VP)]
 
 
 class LhcbSeeds(C.Structure):
@@ -130,6 +134,7 @@ def load_library(build: bool = True) -> C.CDLL:
         lib.lhcb_last_cuda_error.argtypes = [VP]
         lib.lhcb_last_launch_count.argtypes = [VP]
         lib.lhcb_launch_config.argtypes = [VP, C.POINTER(C.c_int * 4)]
+        lib.lhcb_prepare.argtypes = [VP, C.POINTER(LhcbRaw), VP, VP, VP, VP, VP]
         lib.lhcb_pipeline_create.argtypes = [VP, C.c_int, C.c_size_t, C.c_size_t, C.c_size_t, C.c_int, C.POINTER(VP)]
         lib.lhcb_pipeline_destroy.argtypes = [VP]
         lib.lhcb_pipeline_destroy.restype = None
@@ -268,7 +273,23 @@ class Context:
         return LhcbSeeds(s["n_events"], _ptr(s["count"]), _ptr(s["state"]), _ptr(s.get("par")), _ptr(s.get("hits")),
                          _ptr(s.get("nx")), _ptr(s.get("nuv")), _ptr(s.get("status")))
 
-    # ------------------------------------------------------------------ the two calls
+    # ------------------------------------------------------------------ the calls
+    def lhcb_prepare(self, raw_off, raw_x, raw_zone, out: Optional[dict] = None, want_perm: bool = True) -> dict:
+        """Raw hits (device tensors: int32 view of u32 offsets [n_events+1], float32 x, uint8 zone) ->
+        dict(zone_off, hit_x, perm, status) of device tensors in the layout lhcb_seeding reads."""
+        t = self.torch
+        n_events, n_hits = raw_off.numel() - 1, raw_x.numel()
+        if out is None:
+            kw = dict(device=self.dev)
+            out = dict(zone_off=t.empty(n_events * 24 + 1, dtype=t.int32, **kw), hit_x=t.empty(n_hits, dtype=t.float32, **kw),
+                       perm=t.empty(n_hits, dtype=t.int32, **kw) if want_perm else None,
+                       status=t.empty(n_events, dtype=t.int32, **kw))
+        r = LhcbRaw(n_events, n_hits, _ptr(raw_off), _ptr(raw_x), _ptr(raw_zone))
+        rc = self.lib.lhcb_prepare(self._ctx, C.byref(r), _ptr(out["zone_off"]), _ptr(out["hit_x"]), _ptr(out.get("perm")),
+                                   _ptr(out["status"]), self._stream())
+        _check(self.lib, self._ctx, rc, "lhcb_prepare")
+        return out
+
     def lhcb_seeding(self, dev: DeviceEvents, out: Optional[dict] = None) -> dict:
         out = out if out is not None else self.alloc_seeds(dev.n_events)
         e = LhcbEvents(dev.n_events, dev.n_hits, _ptr(dev.zone_off), _ptr(dev.hit_x), _ptr(dev.polarity))

@@ -10,6 +10,7 @@
 #include "../../include/lhcb.h"
 #include "derive.h"
 #include "matching.cuh"
+#include "prepare.cuh"
 #include "seeding.cuh"
 
 struct lhcb_ctx {
@@ -18,7 +19,7 @@ struct lhcb_ctx {
   int device;
   float* d_P;
   float* d_Q;
-  size_t seed_smem, match_smem;
+  size_t seed_smem, match_smem, prep_smem;
   int match_threads;  // 128 when six CTAs fit an SM, else 256
   int seed_threads;   // 256 when four CTAs fit the SM's shared memory, else 512
   int seed_ctas;      // CTAs per SM the seeding kernel is compiled for (register budget)
@@ -125,11 +126,12 @@ int lhcb_geom_init(const lhcb_geom_t* g, int device, lhcb_ctx** out) {
     c->match_smem = lhcb::match_smem_bytes(256, G.max_seeds_per_half, G.max_match_cand_per_event, G.max_velo_per_event,
                                            G.max_ut_per_event);
   }
+  c->prep_smem = lhcb::prep_smem_bytes(2 * G.max_hits_per_half);
   cudaError_t e = cudaSetDevice(device);
   int max_optin = 0;
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
   if (e != cudaSuccess) { c->last_cuda_error = (int)e; delete c; return LHCB_ERR_CUDA; }
-  if (c->seed_smem > (size_t)max_optin || c->match_smem > (size_t)max_optin) { delete c; return LHCB_ERR_CAPACITY; }
+  if (c->seed_smem > (size_t)max_optin || c->match_smem > (size_t)max_optin || c->prep_smem > (size_t)max_optin) { delete c; return LHCB_ERR_CAPACITY; }
   {
     const void* fn = c->seed_ctas == 4 ? (const void*)lhcb::seeding_kernel<256, 4>
                                        : (const void*)lhcb::seeding_kernel<512, 2>;
@@ -139,6 +141,8 @@ int lhcb_geom_init(const lhcb_geom_t* g, int device, lhcb_ctx** out) {
     e = c->match_threads == 128
             ? cudaFuncSetAttribute(lhcb::matching_kernel<128, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->match_smem)
             : cudaFuncSetAttribute(lhcb::matching_kernel<256, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->match_smem);
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(lhcb::prepare_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->prep_smem);
   if (e == cudaSuccess) e = cudaMalloc(&c->d_P, sizeof(c->der.P));
   if (e == cudaSuccess) e = cudaMalloc(&c->d_Q, sizeof(c->der.Q));
   if (e == cudaSuccess) e = cudaMemcpy(c->d_P, c->der.P, sizeof(c->der.P), cudaMemcpyHostToDevice);
@@ -169,6 +173,28 @@ int lhcb_get_geom(const lhcb_ctx* c, lhcb_geom_t* out) {
 size_t lhcb_workspace_bytes(const lhcb_ctx* c, int n_events, size_t n_scifi_hits) {
   (void)c; (void)n_events; (void)n_scifi_hits;
   return 0;   // every intermediate lives in shared memory
+}
+
+int lhcb_prepare(lhcb_ctx* c, const lhcb_raw_t* raw, uint32_t* zone_off, float* hit_x, uint32_t* perm,
+                 uint32_t* status, void* stream) {
+  if (!c) return LHCB_ERR_NOT_INITIALISED;
+  if (!raw || raw->n_events < 0 || !zone_off) return LHCB_ERR_BAD_ARGUMENT;
+  c->last_launches = 0;
+  if (raw->n_events == 0) return LHCB_OK;                    // zone_off[0] is then the caller's to set
+  if (!raw->off || !status || (raw->n_hits && (!raw->x || !raw->zone || !hit_x))) return LHCB_ERR_BAD_ARGUMENT;
+  LHCB_CUDA(c, cudaSetDevice(c->device));
+  lhcb::PrepParams p;
+  // bins span +-3.2 m (the SciFi acceptance is |x| < 3 m, BASELINE.json configs[1]); x outside lands in
+  // the first or last bin, which costs time, not correctness
+  p.x_lo = -3200.0f; p.scale = (float)lhcb::kPrepBins / 6400.0f;
+  p.max_hits = 2 * c->geom.max_hits_per_half;
+  p.n_events = raw->n_events;
+  p.raw_off = raw->off; p.raw_x = raw->x; p.raw_zone = raw->zone;
+  p.zone_off = zone_off; p.hit_x = hit_x; p.perm = perm; p.status = status;
+  lhcb::prepare_kernel<<<raw->n_events, lhcb::kPrepThreads, c->prep_smem, (cudaStream_t)stream>>>(p);
+  LHCB_CUDA(c, cudaGetLastError());
+  c->last_launches = 1;
+  return LHCB_OK;
 }
 
 int lhcb_seeding(lhcb_ctx* c, const lhcb_events_t* ev, lhcb_seeds_t* out, void* workspace, void* stream) {
