@@ -197,6 +197,27 @@ def main():
                                 "combined_events_per_s": nb / (np.median(ts) + np.median(tm)) * 1e3}
             del sub, s2, l2
 
+    # ---- the step before the path, timed on its own: raw unsorted hits -> sorted zones ------
+    prepare = None
+    if rank == 0:
+        from lhcb_gen import shuffle_raw
+        raw = shuffle_raw(ev, seed=9)
+        up = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a, dt).view(np.int32 if dt == np.uint32 else dt)).to(f"cuda:{local_rank}")
+        ro, rx, rz = up(raw["raw_off"], np.uint32), up(raw["raw_x"], np.float32), up(raw["raw_zone"], np.uint8)
+        pout = ctx.lhcb_prepare(ro, rx, rz)
+        e = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        tp = []
+        for i in range(13):
+            e[0].record(stream); ctx.lhcb_prepare(ro, rx, rz, pout); e[1].record(stream); torch.cuda.synchronize()
+            if i >= 3:
+                tp.append(e[0].elapsed_time(e[1]))
+        assert int(pout["status"].max().item()) == 0 and torch.equal(pout["hit_x"], dev.hit_x), "lhcb_prepare output differs"
+        pb = 13 * rx.numel() + 4 * (ro.numel() + pout["zone_off"].numel())      # x, zone read; x, perm written; offsets
+        prepare = {"kernel": "prepare_kernel", "ms": float(np.median(tp)), "events_per_s": n / float(np.median(tp)) * 1e3,
+                   "algorithmic_bytes": pb, "achieved_gbs": pb / float(np.median(tp)) / 1e6,
+                   "note": "not part of the timed step (BASELINE metric = Seeding+Matching); HBM-bound row, see DESIGN.md"}
+        del raw, ro, rx, rz, pout
+
     # ---- end to end through the host-buffer C-ABI call ---------------------------------------------------
     e2e = None
     if not args.no_e2e:
@@ -261,7 +282,7 @@ def main():
             "long_tracks_per_s": n_long_all / (ms_per_step * 1e-3), "seeds_per_event": n_seeds / n, "long_per_event": n_long / n,
             "seeding_events_per_s": n / float(np.median(seed_ms)) * 1e3, "matching_events_per_s": n / float(np.median(match_ms)) * 1e3,
             "min_ms": {"seeding": float(seed_ms.min()), "matching": float(match_ms.min())},
-            "batches": batches, "clocks": clocks, "e2e": e2e, "gpu_launches": 2 * K, "roofline": roofline, "cpu_baseline": cpu}
+            "batches": batches, "prepare": prepare, "clocks": clocks, "e2e": e2e, "gpu_launches": 2 * K, "roofline": roofline, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

@@ -6,9 +6,10 @@
 //   P1  histogram over 24 zones x 256 x-bins (the bin is monotone in x)         one shared atomic per hit
 //   P2  exclusive scan of the 6,144 cells (24 per thread + block scan); the cells at the zone starts are
 //       the event's zone offsets
-//   P3  scatter (x, raw index) into its cell's range                              one shared atomic per hit
-//   P4  rank inside the cell (about 0.6 hits per cell at nominal occupancy) by the literal comparison
-//       (x, raw index) < (x', raw index'), write hit_x and perm at cell start + rank
+//   P3  scatter (x, raw index, cell) into the cell's range                        one shared atomic per hit
+//   P4  thread per scattered hit: rank inside its cell (about 0.6 hits per cell at nominal occupancy) by
+//       the literal comparison (x, raw index) < (x', raw index'); hit_x and perm are written at cell start
+//       + rank, i.e. within a few elements of the thread's own position: nearly coalesced stores
 // Bins only group; the order is decided by exact float comparisons, so the output is bit-identical to a
 // stable sort whatever the rounding of the bin function.
 #pragma once
@@ -19,7 +20,7 @@
 
 namespace lhcb {
 
-constexpr int kPrepThreads = 256;
+constexpr int kPrepThreads = 512;
 constexpr int kPrepBins = 256;                    // x bins per zone
 constexpr int kPrepCells = 24 * kPrepBins;        // 24 cells per thread
 static_assert(kPrepCells % kPrepThreads == 0, "whole cells per thread");
@@ -40,7 +41,7 @@ struct PrepParams {
 __host__ __device__ inline size_t prep_smem_bytes(int max_hits) {
   size_t b = (size_t)kPrepCells * 4 + 256;                       // cells, scan scratch, flags
   b += (((size_t)max_hits * 4 + 15) & ~(size_t)15);              // x by cell
-  b += (((size_t)max_hits * 2 + 15) & ~(size_t)15);              // raw index (event-local) by cell
+  b += 2 * (((size_t)max_hits * 2 + 15) & ~(size_t)15);          // raw index (event-local) and cell, by cell
   return b;
 }
 
@@ -55,10 +56,12 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
   extern __shared__ __align__(16) unsigned char smem[];
   unsigned int* cnt = reinterpret_cast<unsigned int*>(smem);
   int* warp_sums = reinterpret_cast<int*>(smem + (size_t)kPrepCells * 4);        // [kPrepThreads / 32 + 1]
-  int* flag = warp_sums + 16;
+  int* flag = warp_sums + 48;
   float* sx = reinterpret_cast<float*>(smem + (size_t)kPrepCells * 4 + 256);
   uint16_t* sidx = reinterpret_cast<uint16_t*>(reinterpret_cast<unsigned char*>(sx) +
                                                (((size_t)p.max_hits * 4 + 15) & ~(size_t)15));
+  uint16_t* scell = reinterpret_cast<uint16_t*>(reinterpret_cast<unsigned char*>(sidx) +
+                                                (((size_t)p.max_hits * 2 + 15) & ~(size_t)15));
   constexpr int T = kPrepThreads, per = kPrepCells / kPrepThreads;
   const int tid = threadIdx.x, e = blockIdx.x;
   const uint32_t b = p.raw_off[e];
@@ -71,6 +74,7 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
   __syncthreads();
   // P1
   if (!too_many)
+#pragma unroll 4
     for (int i = tid; i < n; i += T) {
       const float x = p.raw_x[b + i];
       const int z = p.raw_zone[b + i];
@@ -104,22 +108,25 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
   if (tid == 0) p.status[e] = 0u;
   __syncthreads();
   // P3
-  for (int i = tid; i < n; i += T) {
-    const float x = p.raw_x[b + i];
-    const unsigned int pos = atomicAdd(&cnt[prep_cell(p, x, p.raw_zone[b + i])], 1u);
-    sx[pos] = x;
-    sidx[pos] = (uint16_t)i;
-  }
-  __syncthreads();
-  // P4: cnt[c] is now the end of cell c = the start of cell c + 1
+#pragma unroll 4
   for (int i = tid; i < n; i += T) {
     const float x = p.raw_x[b + i];
     const int c = prep_cell(p, x, p.raw_zone[b + i]);
+    const unsigned int pos = atomicAdd(&cnt[c], 1u);
+    sx[pos] = x;
+    sidx[pos] = (uint16_t)i;
+    scell[pos] = (uint16_t)c;
+  }
+  __syncthreads();
+  // P4: cnt[c] is now the end of cell c = the start of cell c + 1
+  for (int q = tid; q < n; q += T) {
+    const float x = sx[q];
+    const int i = sidx[q], c = scell[q];
     const int start = c ? (int)cnt[c - 1] : 0, end = (int)cnt[c];
     int rank = 0;
-    for (int q = start; q < end; ++q) {
-      const float xq = sx[q];
-      rank += (xq < x || (xq == x && (int)sidx[q] < i)) ? 1 : 0;
+    for (int r = start; r < end; ++r) {
+      const float xr = sx[r];
+      rank += (xr < x || (xr == x && (int)sidx[r] < i)) ? 1 : 0;
     }
     const uint32_t out = b + (uint32_t)(start + rank);
     p.hit_x[out] = x;
