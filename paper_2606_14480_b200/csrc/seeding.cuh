@@ -430,13 +430,17 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     H.zi[tid] = z;
   }
   __syncthreads();
-  for (int z = warp; z < 12; z += nwarps) {
+  // 24 units (zone, half of its hits) over the warps: each hit fills the bins (bin of its predecessor, its bin]
+  for (int u = warp; u < 24; u += nwarps) {
+    const int z = u >> 1, part = u & 1;
     const Zone zz = H.zi[z];
     uint16_t* L = lut + z * (kLutBins + 1);
     if (zz.e == zz.b) {
-      for (int k = lane; k <= kLutBins; k += 32) L[k] = (uint16_t)zz.b;
+      for (int k = lane + part * 32; k <= kLutBins; k += 64) L[k] = (uint16_t)zz.b;
     } else {
-      for (int i = zz.b + lane; i < zz.e; i += 32) {
+      const int mid = zz.b + ((zz.e - zz.b + 1) >> 1);
+      const int ib = part ? mid : zz.b, ie = part ? zz.e : mid;
+      for (int i = ib + lane; i < ie; i += 32) {
         const int k1 = zone_bin(zz, hx[i]);
         const int k0 = i == zz.b ? -1 : zone_bin(zz, hx[i - 1]);
         for (int k = k0 + 1; k <= k1; ++k) L[k] = (uint16_t)i;
