@@ -115,7 +115,7 @@ __host__ __device__ inline size_t seed_off_hits(int nt, int max_cand) {
 }
 __host__ __device__ inline size_t seed_smem_bytes(int nt, int max_hits, int max_cand, int max_trip) {
   size_t b = seed_off_hits(nt, max_cand);
-  b += seed_align16(((size_t)max_hits + 8) * 4);           // hits tile (16-byte aligned superset)
+  b += seed_align16(((size_t)max_hits + 8) * 4 + 16);      // hits tile (16-byte aligned superset) + padding
   b += seed_align16((size_t)max_trip * 8);                 // work region W (minimum)
   b += (size_t)max_cand * 32;                              // candidates
   return b;
@@ -392,6 +392,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   }
   // tail (and the whole tile when the source is not 16-byte aligned) with plain loads
   for (uint32_t i = a1 + tid; i < g_end; i += T) hx[i - a0] = p.hit_x[i];
+  if (tid < 4) hx[(g_end > a1 ? g_end : a1) - a0 + tid] = __int_as_float(0x7f800000);
   {
     uint32_t done = 0;
     while (!done) {
@@ -408,7 +409,8 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   LHCB_CLK(0)
   const int* zl = H.zl;
   // work region W: from the end of the staged tile to the first candidate slot
-  const int off_w = (int)seed_align16((size_t)off_hits + (size_t)((g_end > a1 ? g_end : a1) - a0) * 4);
+  // (16 bytes of +inf padding after the tile: the three-probe searches may read up to 3 floats past a zone)
+  const int off_w = (int)seed_align16((size_t)off_hits + (size_t)((g_end > a1 ? g_end : a1) - a0) * 4 + 16);
   const int w_stat = p.smem_total - p.max_cand * (int)sizeof(Cand) - off_w;   // bytes of W with every candidate slot used
   Triplet* trip = reinterpret_cast<Triplet*>(smem + off_w);
   unsigned long long* tbl = reinterpret_cast<unsigned long long*>(smem + off_w);   // aliases trip
