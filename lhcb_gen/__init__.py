@@ -7,6 +7,7 @@ from .geometry import DEFAULT_GEOM, default_geom, X_LAYERS, UV_LAYERS, TAN5
 from .events import GenConfig, Events, config, generate, slice_events
 from . import truth
 from .raw import shuffle_raw
+from .ghost_nn import ghost_nn
 
 __all__ = ["DEFAULT_GEOM", "default_geom", "X_LAYERS", "UV_LAYERS", "TAN5",
-           "GenConfig", "Events", "config", "generate", "slice_events", "truth", "shuffle_raw"]
+           "GenConfig", "Events", "config", "generate", "slice_events", "truth", "shuffle_raw", "ghost_nn"]

@@ -68,6 +68,12 @@ class Oracle:
         L.orc_ctx_size.restype = C.c_size_t
         L.orc_seeding.restype = C.c_int64
         L.orc_matching.restype = C.c_int64
+        L.orc_matching_nn.restype = C.c_int64
+        for fn in (L.orc_spec_exp, L.orc_spec_log):
+            fn.restype = D; fn.argtypes = [D]
+        L.orc_eta_velo.restype = D; L.orc_eta_velo.argtypes = [D, D]
+        L.orc_ghost_prob.restype = D
+        L.orc_ghost_prob.argtypes = [C.POINTER(D), C.POINTER(D)]
         L.orc_clone_key.restype = C.c_uint64
         L.orc_clone_key.argtypes = [D, D, C.c_int, C.c_int]
         L.orc_ut_window.restype = D
@@ -105,8 +111,10 @@ class Oracle:
         return dict(n=n, event=o_event[:n], half=o_half[:n], state=o_state[:n], par=o_par[:n], hits=o_hits[:n],
                     nx=o_nx[:n], nuv=o_nuv[:n], counters=dict(zip(COUNTER_NAMES, cnt.tolist())))
 
-    def matching(self, n_events, seed_off, state, ev, use_ut=True, cap: int | None = None):
-        """seed_off u32[n_events+1], state [n][5]; VELO/UT/polarity from ev."""
+    def matching(self, n_events, seed_off, state, ev, use_ut=True, cap: int | None = None, nn=None, nhits=None):
+        """seed_off u32[n_events+1], state [n][5]; VELO/UT/polarity from ev.
+        nn: the 339 packed values of the ghost-killing network (reading A14b) or None (A14: chi2 ranking);
+        nhits: u8 per seed (nHits_SciFi), None = 12."""
         cap = cap or max(1024, 400 * n_events)
         r = self.real
         state = np.ascontiguousarray(state, r)
@@ -123,6 +131,23 @@ class Oracle:
         o_ut = np.zeros((cap, 4), np.uint32); o_nut = np.zeros(cap, np.uint8)
         o_qop = np.zeros(cap, r); o_chi2 = np.zeros(cap, r)
         cnt = np.zeros(len(COUNTER_NAMES), np.uint64)
+        if nn is not None:
+            nnr = np.ascontiguousarray(nn, r)
+            assert nnr.size == 339
+            nh = np.ascontiguousarray(nhits, np.uint8) if nhits is not None else None
+            o_ghost = np.zeros(cap, r)
+            n = self.lib.orc_matching_nn(self.ctx, C.c_int(n_events), _p(so, C.c_uint32), _p(state, self.creal),
+                                         _p(vo, C.c_uint32), _p(vx, self.creal), _p(vy, self.creal), _p(vtx, self.creal),
+                                         _p(vty, self.creal), _p(uo, C.c_uint32), _p(ux, self.creal), _p(ul, self.creal),
+                                         _p(uh, self.creal), _p(pol, C.c_int8), C.c_int64(cap), _p(o_event, C.c_int32),
+                                         _p(o_seed, C.c_uint32), _p(o_velo, C.c_uint32), _p(o_ut, C.c_uint32),
+                                         _p(o_nut, C.c_uint8), _p(o_qop, self.creal), _p(o_chi2, self.creal),
+                                         _p(cnt, C.c_uint64), _p(nh, C.c_uint8), _p(nnr, self.creal), _p(o_ghost, self.creal))
+            if n > cap:
+                raise RuntimeError(f"oracle long-track capacity {cap} < {n}")
+            return dict(n=n, event=o_event[:n], seed=o_seed[:n], velo=o_velo[:n], ut=o_ut[:n], n_ut=o_nut[:n],
+                        qop=o_qop[:n], chi2=o_chi2[:n], ghost=o_ghost[:n],
+                        counters=dict(zip(COUNTER_NAMES, cnt.tolist())))
         n = self.lib.orc_matching(self.ctx, C.c_int(n_events), _p(so, C.c_uint32), _p(state, self.creal),
                                   _p(vo, C.c_uint32), _p(vx, self.creal), _p(vy, self.creal), _p(vtx, self.creal),
                                   _p(vty, self.creal), _p(uo, C.c_uint32), _p(ux, self.creal), _p(ul, self.creal),
@@ -144,6 +169,15 @@ class Oracle:
         return s, m
 
     # ------------------------------------------------------------------ probes (pins)
+    def spec_exp(self, y): return self.lib.orc_spec_exp(float(y))
+    def spec_log(self, x): return self.lib.orc_spec_log(float(x))
+    def eta_velo(self, tx, ty): return self.lib.orc_eta_velo(float(tx), float(ty))
+
+    def ghost_prob(self, nn, inputs):
+        a = np.ascontiguousarray(nn, np.float64); b = np.ascontiguousarray(inputs, np.float64)
+        assert a.size == 339 and b.size == 8
+        return self.lib.orc_ghost_prob(_p(a, D), _p(b, D))
+
     def seeding_debug(self, ev, event, half, cap_t=200000, cap_c=50000):
         hx = self._hits(ev)
         zo = np.ascontiguousarray(ev.zone_off, np.uint32)

@@ -630,16 +630,85 @@ static int ut_search(const orc_ctx* C, REAL xV, REAL yV, REAL txV, REAL tyV, REA
   return have && best->n >= C->g.min_ut_hits;
 }
 
-typedef struct { int seed, velo; REAL chi2, qop; int n_ut; uint32_t ut[NUT]; int alive; } mcand_t;
+/* ---- ghost-killing network (L344-348; reading A14b) -------------------------------------
+ * A fully connected network 8 -> 32 -> 1 on (z_match, dx, dy, dtx, dty, chi2_match, eta_VELO, nHits_SciFi)
+ * gives the "ghost probability".  The paper fixes the shape and the inputs, not the activation, the input
+ * scaling or the weights: hidden ReLU, output logistic, inputs standardised as (v - mu) * isig, all passed
+ * in by the caller as one packed array
+ *   nn = mu[8], isig[8], W1[32][8], b1[32], W2[32], b2, cut (0.8), margin (0.05)          (339 values).
+ * exp and log are spelled out (same single-rounded operations on both sides of the parity test, no libm):
+ *   exp(y) = 2^n * P6(r),  n = floor(y log2(e) + 1/2),  r = (y - n c1) - n c2   (Cody-Waite),  |y| <= 87
+ *   log(x) = e ln2 + s (2 + s^2 (2/3 + s^2 (2/5 + s^2 (2/7 + s^2 2/9)))),  x = m 2^e, m in [sqrt(1/2), sqrt 2),
+ *            s = (m - 1) / (m + 1)                                                                          */
+#define NN_IN 8
+#define NN_HID 32
+#define NN_SIZE (NN_IN + NN_IN + NN_HID * NN_IN + NN_HID + NN_HID + 3)
+
+static REAL spec_exp(REAL y) {
+  REAL n, r, p;
+  if (y > (REAL)87.0) y = (REAL)87.0;
+  if (y < (REAL)-87.0) y = (REAL)-87.0;
+  n = (REAL)floor((double)(y * (REAL)1.44269504f + (REAL)0.5));
+  r = (y - n * (REAL)0.693359375f) - n * (REAL)-2.12194440e-4f;
+  p = (REAL)(1.0f / 720.0f);
+  p = p * r + (REAL)(1.0f / 120.0f);
+  p = p * r + (REAL)(1.0f / 24.0f);
+  p = p * r + (REAL)(1.0f / 6.0f);
+  p = p * r + (REAL)0.5;
+  p = p * r + (REAL)1.0;
+  p = p * r + (REAL)1.0;
+  return (REAL)ldexp((double)p, (int)n);                   /* exact: |n| <= 126 */
+}
+
+static REAL spec_log(REAL x) {
+  int e; REAL m, s, s2, q;
+  m = (REAL)frexp((double)x, &e);                           /* exact: x = m 2^e, m in [1/2, 1) */
+  if (m < (REAL)0.70710678f) { m = m * (REAL)2.0; e -= 1; }
+  s = (m - (REAL)1.0) / (m + (REAL)1.0);
+  s2 = s * s;
+  q = (REAL)(2.0f / 9.0f);
+  q = q * s2 + (REAL)(2.0f / 7.0f);
+  q = q * s2 + (REAL)(2.0f / 5.0f);
+  q = q * s2 + (REAL)(2.0f / 3.0f);
+  q = q * s2 + (REAL)2.0;
+  return (REAL)e * (REAL)0.69314718f + s * q;
+}
+
+/* pseudorapidity of a VELO segment from its slopes: eta = ln((1 + sqrt(1 + rho^2)) / rho), rho = tan(theta) */
+static REAL eta_velo(REAL tx, REAL ty) {
+  REAL rho2 = tx * tx + ty * ty;
+  REAL rho = (REAL)sqrt((double)rho2);                      /* correctly rounded in either precision */
+  REAL sh = (REAL)sqrt((double)((REAL)1.0 + rho2));
+  if (rho < (REAL)1e-6f) rho = (REAL)1e-6f;
+  return spec_log(((REAL)1.0 + sh) / rho);
+}
+
+static REAL ghost_prob(const REAL* nn, const REAL* in /* [8] */) {
+  const REAL *mu = nn, *isig = nn + NN_IN, *W1 = nn + 2 * NN_IN, *b1 = W1 + NN_HID * NN_IN, *W2 = b1 + NN_HID;
+  REAL u[NN_IN], t = W2[NN_HID];                            /* b2 */
+  int j, k;
+  for (k = 0; k < NN_IN; k++) u[k] = (in[k] - mu[k]) * isig[k];
+  for (j = 0; j < NN_HID; j++) {
+    REAL h = b1[j];
+    for (k = 0; k < NN_IN; k++) h = h + W1[j * NN_IN + k] * u[k];
+    if (h < 0) h = 0;
+    t = t + W2[j] * h;
+  }
+  return (REAL)1.0 / ((REAL)1.0 + spec_exp(-t));
+}
+
+typedef struct { int seed, velo; REAL chi2, qop, ghost; int n_ut; uint32_t ut[NUT]; int alive; } mcand_t;
 typedef VEC(mcand_t) vmc;
 
 /* Matching over a batch.  Seeds: per-event offsets seed_off[n_events+1] into state[n][5].
  * ut_off may be NULL (no UT).  Returns number of long tracks (only cap written). */
-int64_t orc_matching(const orc_ctx* C, int n_events, const uint32_t* seed_off, const REAL* state,
+static int64_t matching_impl(const orc_ctx* C, int n_events, const uint32_t* seed_off, const REAL* state,
                      const uint32_t* velo_off, const REAL* vx, const REAL* vy, const REAL* vtx, const REAL* vty,
                      const uint32_t* ut_off, const REAL* ux, const REAL* uylo, const REAL* uyhi,
                      const int8_t* polarity, int64_t cap, int32_t* o_event, uint32_t* o_seed, uint32_t* o_velo,
-                     uint32_t* o_ut /* [n][4] */, uint8_t* o_nut, REAL* o_qop, REAL* o_chi2, uint64_t* counters) {
+                     uint32_t* o_ut /* [n][4] */, uint8_t* o_nut, REAL* o_qop, REAL* o_chi2, uint64_t* counters,
+                     const uint8_t* seed_nhits /* per seed, NULL = 12 */, const REAL* nn /* NULL = A14 */,
+                     REAL* o_ghost /* may be NULL */) {
   uint64_t cnt[C_N] = { 0 };
   vmc mc = { 0 };
   int64_t n_out = 0; int e; size_t i;
@@ -658,7 +727,7 @@ int64_t orc_matching(const orc_ctx* C, int n_events, const uint32_t* seed_off, c
         if (!(pr.chi2 < C->chi2m_max)) continue;                                /* L301 */
         cnt[C_CHI2_OK]++;
         q0 = pr.dtx * C->inv_KB;                                                /* A10 */
-        m.seed = (int)s; m.velo = (int)v; m.chi2 = pr.chi2; m.alive = 1; m.n_ut = 0;
+        m.seed = (int)s; m.velo = (int)v; m.chi2 = pr.chi2; m.alive = 1; m.n_ut = 0; m.ghost = 0;
         m.qop = pol > 0 ? q0 : -q0;
         for (k = 0; k < NUT; k++) m.ut[k] = NO_HIT;
         if (use_ut) {
@@ -669,8 +738,30 @@ int64_t orc_matching(const orc_ctx* C, int n_events, const uint32_t* seed_off, c
           q1 = (h.gamma - C->Ag) * C->inv_Bg;
           m.qop = pol > 0 ? q1 : -q1;
         }
+        if (nn) {                                                               /* L346: ghost probability */
+          REAL in[NN_IN];
+          in[0] = pr.zm; in[1] = pr.dx; in[2] = pr.dy; in[3] = pr.dtx; in[4] = pr.dty; in[5] = pr.chi2;
+          in[6] = eta_velo(vtx[v], vty[v]);
+          in[7] = (REAL)(seed_nhits ? seed_nhits[s] : 12);
+          m.ghost = ghost_prob(nn, in);
+        }
         PUSH(&mc, m);
       }
+    if (nn) {
+      /* O14b (L348): keep ghost probability < cut; then a track that shares its VELO or its SciFi segment
+       * with another kept track is removed if its ghost probability is at least `margin` higher */
+      const REAL cut = nn[NN_SIZE - 2], margin = nn[NN_SIZE - 1];
+      for (i = 0; i < mc.n; i++) if (!(mc.p[i].ghost < cut)) mc.p[i].alive = 0;
+      for (i = 0; i < mc.n; i++) {
+        size_t j;
+        if (!mc.p[i].alive) continue;
+        for (j = 0; j < mc.n; j++) {
+          if (j == i || !mc.p[j].alive) continue;             /* alive is 1 or 2 for tracks that passed the cut */
+          if (mc.p[j].seed != mc.p[i].seed && mc.p[j].velo != mc.p[i].velo) continue;
+          if (mc.p[i].ghost >= mc.p[j].ghost + margin) mc.p[i].alive = 2;   /* mark only: the comparison set stays fixed */
+        }
+      }
+    } else {
     /* O14 (A14): each seed keeps its min (chi2, velo) candidate ... */
     for (i = 0; i < mc.n; i++) {
       size_t j;
@@ -691,6 +782,7 @@ int64_t orc_matching(const orc_ctx* C, int n_events, const uint32_t* seed_off, c
       }
       if (lose) mc.p[i].alive = 2;                          /* mark, do not change the survivor set mid-pass */
     }
+    }
     for (i = 0; i < mc.n; i++) {
       const mcand_t* m = &mc.p[i];
       if (m->alive != 1) continue;
@@ -699,6 +791,7 @@ int64_t orc_matching(const orc_ctx* C, int n_events, const uint32_t* seed_off, c
         o_event[n_out] = e; o_seed[n_out] = (uint32_t)m->seed; o_velo[n_out] = (uint32_t)m->velo;
         memcpy(o_ut + NUT * n_out, m->ut, sizeof(m->ut)); o_nut[n_out] = (uint8_t)m->n_ut;
         o_qop[n_out] = m->qop; o_chi2[n_out] = m->chi2;
+        if (o_ghost) o_ghost[n_out] = m->ghost;
       }
       n_out++;
     }
@@ -706,6 +799,37 @@ int64_t orc_matching(const orc_ctx* C, int n_events, const uint32_t* seed_off, c
   if (counters) for (i = 0; i < C_N; i++) counters[i] += cnt[i];
   free(mc.p);
   return n_out;
+}
+
+int64_t orc_matching(const orc_ctx* C, int n_events, const uint32_t* seed_off, const REAL* state,
+                     const uint32_t* velo_off, const REAL* vx, const REAL* vy, const REAL* vtx, const REAL* vty,
+                     const uint32_t* ut_off, const REAL* ux, const REAL* uylo, const REAL* uyhi,
+                     const int8_t* polarity, int64_t cap, int32_t* o_event, uint32_t* o_seed, uint32_t* o_velo,
+                     uint32_t* o_ut /* [n][4] */, uint8_t* o_nut, REAL* o_qop, REAL* o_chi2, uint64_t* counters) {
+  return matching_impl(C, n_events, seed_off, state, velo_off, vx, vy, vtx, vty, ut_off, ux, uylo, uyhi, polarity, cap,
+                       o_event, o_seed, o_velo, o_ut, o_nut, o_qop, o_chi2, counters, NULL, NULL, NULL);
+}
+
+/* The same with the ghost-killing network in place of the chi2 ranking (A14b).  nn: NN_SIZE packed values. */
+int64_t orc_matching_nn(const orc_ctx* C, int n_events, const uint32_t* seed_off, const REAL* state,
+                        const uint32_t* velo_off, const REAL* vx, const REAL* vy, const REAL* vtx, const REAL* vty,
+                        const uint32_t* ut_off, const REAL* ux, const REAL* uylo, const REAL* uyhi,
+                        const int8_t* polarity, int64_t cap, int32_t* o_event, uint32_t* o_seed, uint32_t* o_velo,
+                        uint32_t* o_ut, uint8_t* o_nut, REAL* o_qop, REAL* o_chi2, uint64_t* counters,
+                        const uint8_t* seed_nhits, const REAL* nn, REAL* o_ghost) {
+  return matching_impl(C, n_events, seed_off, state, velo_off, vx, vy, vtx, vty, ut_off, ux, uylo, uyhi, polarity, cap,
+                       o_event, o_seed, o_velo, o_ut, o_nut, o_qop, o_chi2, counters, seed_nhits, nn, o_ghost);
+}
+
+/* probes of the network arithmetic (pins) */
+double orc_spec_exp(double y) { return (double)spec_exp((REAL)y); }
+double orc_spec_log(double x) { return (double)spec_log((REAL)x); }
+double orc_eta_velo(double tx, double ty) { return (double)eta_velo((REAL)tx, (REAL)ty); }
+double orc_ghost_prob(const double* nn, const double* in) {
+  REAL w[NN_SIZE], v[NN_IN]; int i;
+  for (i = 0; i < NN_SIZE; i++) w[i] = (REAL)nn[i];
+  for (i = 0; i < NN_IN; i++) v[i] = (REAL)in[i];
+  return (double)ghost_prob(w, v);
 }
 
 /* ------------------------------------------------------------------------------------------ */

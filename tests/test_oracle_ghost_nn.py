@@ -1,0 +1,91 @@
+"""Pins of the ghost-killing network in the oracle (reading A14b)."""
+import numpy as np
+import pytest
+
+from lhcb_gen import config, default_geom, generate, ghost_nn
+from lhcb_gen.ghost_nn import unpack
+from oracle.binding import Oracle
+
+
+@pytest.fixture(scope="module")
+def o32():
+    return Oracle(default_geom(), "f32")
+
+
+def test_spelled_out_exp_and_log_against_libm(o32):
+    ys = np.linspace(-30, 30, 2001)
+    e = np.array([o32.spec_exp(y) for y in ys])
+    assert np.max(np.abs(e / np.exp(ys.astype(np.float32).astype(np.float64)) - 1)) < 3e-6
+    assert o32.spec_exp(0.0) == 1.0
+    assert o32.spec_exp(-1000.0) == o32.spec_exp(-87.0) and o32.spec_exp(1000.0) == o32.spec_exp(87.0)   # clamped
+    xs = np.exp(np.linspace(-12, 12, 2001)).astype(np.float32).astype(np.float64)
+    l = np.array([o32.spec_log(x) for x in xs])
+    assert np.max(np.abs(l - np.log(xs))) < 3e-6
+    assert o32.spec_log(1.0) == 0.0
+    o64 = Oracle(default_geom(), "f64")
+    assert abs(o64.spec_log(7.5) - np.log(7.5)) < 1e-7 and abs(o64.spec_exp(1.0) / np.e - 1) < 1e-6
+
+
+def test_eta_is_the_pseudorapidity(o32):
+    for tx, ty in [(0.1, 0.0), (0.0, -0.02), (0.25, 0.25), (0.003, 0.004), (-0.05, 0.12)]:
+        theta = np.arctan(np.hypot(tx, ty))
+        assert abs(o32.eta_velo(tx, ty) + np.log(np.tan(theta / 2))) < 5e-6 * (1 + abs(np.log(np.tan(theta / 2))))
+
+
+def test_ghost_prob_is_the_mlp(o32):
+    """8 -> 32 (ReLU) -> 1 (logistic) on standardised inputs, against a numpy float64 evaluation."""
+    rng = np.random.default_rng(3)
+    for trial in range(20):
+        w = np.concatenate([rng.normal(0, 1, 8), rng.uniform(0.5, 2, 8), rng.normal(0, 0.5, 256), rng.normal(0, 0.5, 32),
+                            rng.normal(0, 0.5, 32), rng.normal(0, 1, 1), [0.8, 0.05]]).astype(np.float32)
+        x = rng.normal(0, 2, 8).astype(np.float32)
+        n = unpack(w.astype(np.float64))
+        u = (x.astype(np.float64) - n["mu"]) * n["isig"]
+        t = n["b2"] + n["W2"] @ np.maximum(n["W1"] @ u + n["b1"], 0)
+        assert abs(o32.ghost_prob(w, x) - 1 / (1 + np.exp(-t))) < 2e-5
+    # special cases: all-zero weights -> 1/2 exactly; a dropped hidden bias or a transposed W1 would show above
+    z = np.zeros(339, np.float32); z[8:16] = 1
+    assert o32.ghost_prob(z, np.ones(8)) == 0.5
+    z[336] = 3.0
+    assert abs(o32.ghost_prob(z, np.ones(8)) - 1 / (1 + np.exp(-3.0))) < 1e-6
+
+
+def run(o, ev, nn):
+    s = o.seeding(ev)
+    seed_off = np.zeros(ev.n_events + 1, np.uint32)
+    np.cumsum(np.bincount(s["event"], minlength=ev.n_events), out=seed_off[1:])
+    nhits = (s["nx"] + s["nuv"]).astype(np.uint8)
+    return s, seed_off, nhits, o.matching(ev.n_events, seed_off, s["state"], ev, use_ut=True, nn=nn, nhits=nhits)
+
+
+def test_selection_equals_the_literal_rule_of_L348():
+    """Brute force in Python from the unfiltered candidate list: keep p < 0.8; drop a track that shares its
+    seed or its VELO segment with another kept track whose ghost probability is lower by >= 0.05."""
+    ev = generate(config(2, 40))
+    o = Oracle(ev.geom, "f32")
+    w = ghost_nn()
+    open_w = w.copy(); open_w[337] = np.inf; open_w[338] = np.inf
+    s, seed_off, nhits, allc = run(o, ev, open_w)
+    _, _, _, sel = run(o, ev, w)
+    # every candidate's ghost probability = the MLP on its own features
+    for i in range(0, allc["n"], 97):
+        sd, v = allc["seed"][i], allc["velo"][i]
+        r = o.match_pair(s["state"][sd, :4], [ev.velo_x[v], ev.velo_y[v], ev.velo_tx[v], ev.velo_ty[v]])
+        x = [r["zm"], r["dx"], r["dy"], r["dtx"], r["dty"], r["chi2"], o.eta_velo(ev.velo_tx[v], ev.velo_ty[v]), nhits[sd]]
+        assert abs(o.ghost_prob(w, x) - allc["ghost"][i]) < 1e-6
+    cut, margin = np.float32(w[337]), np.float32(w[338])
+    p = allc["ghost"].astype(np.float32)
+    kept = p < cut
+    expect = set()
+    for i in np.flatnonzero(kept):
+        share = kept & ((allc["seed"] == allc["seed"][i]) | (allc["velo"] == allc["velo"][i]))
+        share[i] = False
+        if not (p[i] >= (p[share] + margin).astype(np.float32)).any():
+            expect.add((int(allc["seed"][i]), int(allc["velo"][i])))
+    got = set(zip(sel["seed"].tolist(), sel["velo"].tolist()))
+    assert got == expect and len(got) > 50 * 40
+    assert (sel["ghost"] < cut).all()
+    assert len(got) < allc["n"]                                 # the selection does remove something
+    # without the network the chi2 ranking (A14) is unchanged
+    m0 = o.matching(ev.n_events, seed_off, s["state"], ev, use_ut=True)
+    assert "ghost" not in m0 and m0["n"] > 0
