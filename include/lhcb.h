@@ -172,6 +172,8 @@ typedef struct {
   float* qop;          /* [cap_total] q/p: UT-refined (Eq. 20) if UT hits were added, else the kick estimate */
   float* chi2;         /* [cap_total] chi2_match of Eq. 22 */
   uint32_t* status;    /* [n_events] LHCB_ST_* bits */
+  float* ghost;        /* [cap_total] ghost probability (L346); written only while a network is set
+                          (lhcb_set_ghost_nn); may be NULL */
 } lhcb_long_t;
 
 /* Host only.  Fills `out` from `g` (no CUDA call).  Returns LHCB_OK or LHCB_ERR_BAD_GEOMETRY /
@@ -202,6 +204,17 @@ size_t lhcb_workspace_bytes(const lhcb_ctx* ctx, int n_events, size_t n_scifi_hi
  * Enqueues one kernel on cuda_stream; does not synchronise or allocate. */
 int lhcb_prepare(lhcb_ctx* ctx, const lhcb_raw_t* raw, uint32_t* zone_off, float* hit_x, uint32_t* perm,
                  uint32_t* status, void* cuda_stream);
+
+/* Final selection with the ghost-killing network (reading A14b).
+ * nn: HOST array of LHCB_GHOST_NN_SIZE floats  mu[8], isig[8], W1[32][8], b1[32], W2[32], b2, cut, margin
+ * for the inputs (z_match, dx, dy, dtx, dty, chi2_match, eta_VELO, nHits_SciFi), standardised as
+ * (v - mu) * isig; hidden ReLU, output logistic = ghost probability.  lhcb_matching then keeps the
+ * candidates with ghost probability < cut (0.8) and removes a track that shares its VELO or its SciFi
+ * segment with another kept track whose ghost probability is lower by at least margin (0.05; must be > 0)
+ * -- instead of the chi2 ranking (A14).  nHits_SciFi = nx + nuv of the seed (12 if those arrays are NULL).
+ * nn == NULL switches back to the chi2 ranking.  Copied to the device by this call (synchronous). */
+#define LHCB_GHOST_NN_SIZE 339
+int lhcb_set_ghost_nn(lhcb_ctx* ctx, const float* nn);
 
 /* Seeding: x-z two-/three-hit search, extension, fit, clone kill, u/v addition, y fit (section 3).
  * One CTA per event-half.  `out` arrays must have cap_total = n_events*2*max_seeds_per_half slots. */

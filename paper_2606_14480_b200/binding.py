@@ -24,7 +24,7 @@ ST_BITS = {1: "triplet_overflow", 2: "cand_overflow", 4: "seed_overflow", 8: "hi
 EXPORTS = ["lhcb_geom_derive", "lhcb_geom_init", "lhcb_destroy", "lhcb_get_geom", "lhcb_workspace_bytes",
            "lhcb_seeding", "lhcb_matching", "lhcb_error_string", "lhcb_last_cuda_error",
            "lhcb_last_launch_count", "lhcb_pipeline_create", "lhcb_pipeline_destroy", "lhcb_reconstruct_host",
-           "lhcb_pipeline_last_bytes", "lhcb_launch_config", "lhcb_prepare"]
+           "lhcb_pipeline_last_bytes", "lhcb_launch_config", "lhcb_prepare", "lhcb_set_ghost_nn"]
 
 
 class LhcbGeom(C.Structure):
@@ -88,7 +88,7 @@ class LhcbUt(C.Structure):
 
 class LhcbLong(C.Structure):
     _fields_ = [("count", VP), ("seed_idx", VP), ("velo_idx", VP), ("ut_idx", VP), ("n_ut", VP), ("qop", VP),
-                ("chi2", VP), ("status", VP)]
+                ("chi2", VP), ("status", VP), ("ghost", VP)]
 
 
 def fill_geom(geom: dict) -> LhcbGeom:
@@ -135,6 +135,7 @@ def load_library(build: bool = True) -> C.CDLL:
         lib.lhcb_last_launch_count.argtypes = [VP]
         lib.lhcb_launch_config.argtypes = [VP, C.POINTER(C.c_int * 4)]
         lib.lhcb_prepare.argtypes = [VP, C.POINTER(LhcbRaw), VP, VP, VP, VP, VP]
+        lib.lhcb_set_ghost_nn.argtypes = [VP, C.POINTER(C.c_float)]
         lib.lhcb_pipeline_create.argtypes = [VP, C.c_int, C.c_size_t, C.c_size_t, C.c_size_t, C.c_int, C.POINTER(VP)]
         lib.lhcb_pipeline_destroy.argtypes = [VP]
         lib.lhcb_pipeline_destroy.restype = None
@@ -266,7 +267,7 @@ class Context:
                     seed_idx=t.empty(cap, dtype=t.int32, **kw), velo_idx=t.empty(cap, dtype=t.int32, **kw),
                     ut_idx=t.empty((4, cap), dtype=t.int32, **kw), n_ut=t.empty(cap, dtype=t.uint8, **kw),
                     qop=t.empty(cap, dtype=t.float32, **kw), chi2=t.empty(cap, dtype=t.float32, **kw),
-                    status=t.empty(n_events, dtype=t.int32, **kw))
+                    status=t.empty(n_events, dtype=t.int32, **kw), ghost=t.zeros(cap, dtype=t.float32, **kw))
 
     @staticmethod
     def _seeds_struct(s):
@@ -307,10 +308,21 @@ class Context:
         if use_ut and dev.ut_off is not None:
             u = C.byref(LhcbUt(dev.ut_x0.numel(), _ptr(dev.ut_off), _ptr(dev.ut_x0), _ptr(dev.ut_ylo), _ptr(dev.ut_yhi)))
         l = LhcbLong(_ptr(out["count"]), _ptr(out["seed_idx"]), _ptr(out["velo_idx"]), _ptr(out["ut_idx"]),
-                     _ptr(out["n_ut"]), _ptr(out["qop"]), _ptr(out["chi2"]), _ptr(out["status"]))
+                     _ptr(out["n_ut"]), _ptr(out["qop"]), _ptr(out["chi2"]), _ptr(out["status"]), _ptr(out.get("ghost")))
         rc = self.lib.lhcb_matching(self._ctx, C.byref(s), C.byref(v), u, C.byref(l), VP(0), self._stream())
         _check(self.lib, self._ctx, rc, "lhcb_matching")
         return out
+
+    def lhcb_set_ghost_nn(self, nn):
+        """nn: 339 float32 (mu, isig, W1, b1, W2, b2, cut, margin) or None (back to the chi2 ranking, A14)."""
+        if nn is None:
+            rc = self.lib.lhcb_set_ghost_nn(self._ctx, None)
+        else:
+            a = np.ascontiguousarray(nn, np.float32)
+            if a.size != 339:
+                raise ValueError("the packed network has 339 values")
+            rc = self.lib.lhcb_set_ghost_nn(self._ctx, a.ctypes.data_as(C.POINTER(C.c_float)))
+        _check(self.lib, self._ctx, rc, "lhcb_set_ghost_nn")
 
     def last_launch_count(self):
         return int(self.lib.lhcb_last_launch_count(self._ctx))
@@ -340,6 +352,7 @@ class Context:
         count[0::2] = np.minimum(cnt, ms); count[1::2] = np.maximum(cnt - ms, 0)
         out["state"].copy_(t.from_numpy(st)); out["count"].copy_(t.from_numpy(count))
         out["status"].zero_()
+        out["nx"].fill_(6); out["nuv"].fill_(6)             # states without hits count as full 12-hit seeds (nHits_SciFi input)
         return out, slot
 
     def seeds_to_host(self, s):
@@ -365,7 +378,8 @@ class Context:
         g = lambda name: l[name].cpu().numpy()
         return dict(n=len(slot), event=ev, seed=g("seed_idx").view(np.uint32)[slot], velo=g("velo_idx").view(np.uint32)[slot],
                     ut=g("ut_idx").view(np.uint32)[:, slot].T, n_ut=g("n_ut")[slot], qop=g("qop")[slot],
-                    chi2=g("chi2")[slot], status=g("status").view(np.uint32))
+                    chi2=g("chi2")[slot], status=g("status").view(np.uint32),
+                    ghost=g("ghost")[slot] if l.get("ghost") is not None else None)
 
 
 class HostPipeline:
@@ -408,7 +422,7 @@ class HostPipeline:
         self._ut = LhcbUt(len(ev.ut_x0), _ptr(h["ut_off"]), _ptr(h["ut_x0"]), _ptr(h["ut_ylo"]), _ptr(h["ut_yhi"])) if self.has_ut else None
         o = self.out
         self._long = LhcbLong(_ptr(o["count"]), _ptr(o["seed_idx"]), _ptr(o["velo_idx"]), _ptr(o["ut_idx"]),
-                              _ptr(o["n_ut"]), _ptr(o["qop"]), _ptr(o["chi2"]), _ptr(o["status"]))
+                              _ptr(o["n_ut"]), _ptr(o["qop"]), _ptr(o["chi2"]), _ptr(o["status"]), VP(0))
 
     def lhcb_reconstruct_host(self):
         """One end-to-end pass; returns (h2d_bytes, d2h_bytes, kernel launches).  Results are in self.out."""

@@ -19,6 +19,8 @@ struct lhcb_ctx {
   int device;
   float* d_P;
   float* d_Q;
+  float* d_nn;        // ghost-killing network on the device
+  int nn_on;
   size_t seed_smem, match_smem, prep_smem;
   int match_threads;  // 128 when six CTAs fit an SM, else 256
   int seed_threads;   // 256 when four CTAs fit the SM's shared memory, else 512
@@ -145,10 +147,11 @@ int lhcb_geom_init(const lhcb_geom_t* g, int device, lhcb_ctx** out) {
     e = cudaFuncSetAttribute(lhcb::prepare_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->prep_smem);
   if (e == cudaSuccess) e = cudaMalloc(&c->d_P, sizeof(c->der.P));
   if (e == cudaSuccess) e = cudaMalloc(&c->d_Q, sizeof(c->der.Q));
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_nn, LHCB_GHOST_NN_SIZE * sizeof(float));
   if (e == cudaSuccess) e = cudaMemcpy(c->d_P, c->der.P, sizeof(c->der.P), cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemcpy(c->d_Q, c->der.Q, sizeof(c->der.Q), cudaMemcpyHostToDevice);
   if (e != cudaSuccess) {
-    cudaFree(c->d_P); cudaFree(c->d_Q);
+    cudaFree(c->d_P); cudaFree(c->d_Q); cudaFree(c->d_nn);
     delete c;
     return LHCB_ERR_CUDA;
   }
@@ -161,6 +164,7 @@ void lhcb_destroy(lhcb_ctx* c) {
   cudaSetDevice(c->device);
   cudaFree(c->d_P);
   cudaFree(c->d_Q);
+  cudaFree(c->d_nn);
   delete c;
 }
 
@@ -173,6 +177,16 @@ int lhcb_get_geom(const lhcb_ctx* c, lhcb_geom_t* out) {
 size_t lhcb_workspace_bytes(const lhcb_ctx* c, int n_events, size_t n_scifi_hits) {
   (void)c; (void)n_events; (void)n_scifi_hits;
   return 0;   // every intermediate lives in shared memory
+}
+
+int lhcb_set_ghost_nn(lhcb_ctx* c, const float* nn) {
+  if (!c) return LHCB_ERR_NOT_INITIALISED;
+  if (!nn) { c->nn_on = 0; return LHCB_OK; }
+  if (!(nn[LHCB_GHOST_NN_SIZE - 1] > 0.0f)) return LHCB_ERR_BAD_ARGUMENT;     // margin must be positive
+  LHCB_CUDA(c, cudaSetDevice(c->device));
+  LHCB_CUDA(c, cudaMemcpy(c->d_nn, nn, LHCB_GHOST_NN_SIZE * sizeof(float), cudaMemcpyHostToDevice));
+  c->nn_on = 1;
+  return LHCB_OK;
 }
 
 int lhcb_prepare(lhcb_ctx* c, const lhcb_raw_t* raw, uint32_t* zone_off, float* hit_x, uint32_t* perm,
@@ -247,6 +261,7 @@ int lhcb_matching(lhcb_ctx* c, const lhcb_seeds_t* seeds, const lhcb_velo_t* vel
   if (ut) { p.ut_off = ut->off; p.ux = ut->x0; p.uylo = ut->y_lo; p.uyhi = ut->y_hi; p.n_ut_total = ut->n_hits; }
   p.count = out->count; p.seed_idx = out->seed_idx; p.velo_idx = out->velo_idx; p.ut_idx = out->ut_idx;
   p.n_ut = out->n_ut; p.qop = out->qop; p.chi2 = out->chi2; p.status = out->status;
+  p.nn = c->nn_on ? c->d_nn : nullptr; p.snx = seeds->nx; p.snuv = seeds->nuv; p.ghost = out->ghost;
   p.long_cap_total = (size_t)velo->n_events * (size_t)c->geom.max_long_per_event;
   if (c->match_threads == 128)
     lhcb::matching_kernel<128, 6><<<velo->n_events, 128, c->match_smem, (cudaStream_t)stream>>>(p);
@@ -434,7 +449,7 @@ int lhcb_reconstruct_host(lhcb_pipeline* p, const lhcb_events_t* ev, const lhcb_
     p->launches += c->last_launches;
     lhcb_velo_t dev_v = {ne, p->velo_off + e0, p->vx, p->vy, p->vtx, p->vty, ev->polarity ? p->pol + e0 : nullptr};
     lhcb_ut_t dev_u = {(uint32_t)n_ut, p->ut_off + (size_t)e0 * 4, p->ux, p->uylo, p->uyhi};
-    lhcb_long_t dev_l = {S.l_count, S.l_seed, S.l_velo, S.l_ut, S.l_nut, S.l_qop, S.l_chi2, S.l_status};
+    lhcb_long_t dev_l = {S.l_count, S.l_seed, S.l_velo, S.l_ut, S.l_nut, S.l_qop, S.l_chi2, S.l_status, nullptr};
     rc = lhcb_matching(c, &dev_s, &dev_v, ut ? &dev_u : nullptr, &dev_l, nullptr, s);
     if (rc != LHCB_OK) return rc;
     p->launches += c->last_launches;

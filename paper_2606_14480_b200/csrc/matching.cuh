@@ -53,6 +53,10 @@ struct MatchParams {
   float* chi2;
   uint32_t* status;
   size_t long_cap_total;
+  // ghost-killing network (reading A14b): packed weights on the device or NULL; seed hit counts; output
+  const float* nn;
+  const uint8_t *snx, *snuv;
+  float* ghost;
 };
 
 struct __align__(8) MatchCand {
@@ -60,8 +64,10 @@ struct __align__(8) MatchCand {
   float chi2, q0, gamma;    // chi2_match, kick q/p (A10), gamma_x of the best UT hypothesis
   unsigned long long key;   // best UT hypothesis: (4 - n_ut) << 50 | f32 bits of sum res^2 << 18 | layer << 16 | first hit
   uint16_t ut[4];           // its hits, relative to the event's first UT hit (0xFFFF = none)
+  float ghost;              // ghost probability (network set) 
+  uint32_t pad;
 };
-static_assert(sizeof(MatchCand) == 32, "MatchCand is 32 bytes");
+static_assert(sizeof(MatchCand) == 40, "MatchCand is 40 bytes");
 
 __host__ __device__ inline size_t match_smem_bytes(int kMatchThreads, int max_seeds, int max_mc, int max_velo, int max_ut) {
   size_t b = 64;
@@ -78,6 +84,59 @@ __host__ __device__ inline size_t match_smem_bytes(int kMatchThreads, int max_se
   b += (size_t)2 * max_seeds * 8;            // best key per seed
   b += (size_t)max_velo * 8;                 // best key per VELO track
   return b;
+}
+
+// ---- ghost-killing network (L344-348, reading A14b).  exp and log are spelled out operation by operation
+// (DESIGN.md "Arithmetic specification"): no libm, no fast-math intrinsics, -fmad=false.
+__device__ __forceinline__ float nn_exp(float y) {
+  y = y > 87.f ? 87.f : y;
+  y = y < -87.f ? -87.f : y;
+  const float n = floorf(y * 1.44269504f + 0.5f);
+  const float r = (y - n * 0.693359375f) - n * -2.12194440e-4f;       // Cody-Waite reduction
+  float q = 1.0f / 720.0f;
+  q = q * r + 1.0f / 120.0f;
+  q = q * r + 1.0f / 24.0f;
+  q = q * r + 1.0f / 6.0f;
+  q = q * r + 0.5f;
+  q = q * r + 1.0f;
+  q = q * r + 1.0f;
+  return q * __int_as_float(((int)n + 127) << 23);                    // times 2^n, |n| <= 126: exact scaling
+}
+__device__ __forceinline__ float nn_log(float x) {                     // x normal and positive
+  const unsigned int b = __float_as_uint(x);
+  int e = (int)((b >> 23) & 0xFFu) - 126;
+  float m = __uint_as_float((b & 0x807FFFFFu) | 0x3F000000u);          // x = m 2^e, m in [1/2, 1)
+  if (m < 0.70710678f) { m = m * 2.0f; e -= 1; }
+  const float s = (m - 1.0f) / (m + 1.0f);
+  const float s2 = s * s;
+  float q = 2.0f / 9.0f;
+  q = q * s2 + 2.0f / 7.0f;
+  q = q * s2 + 2.0f / 5.0f;
+  q = q * s2 + 2.0f / 3.0f;
+  q = q * s2 + 2.0f;
+  return (float)e * 0.69314718f + s * q;
+}
+__device__ __forceinline__ float nn_eta(float tx, float ty) {          // pseudorapidity from the slopes
+  const float rho2 = tx * tx + ty * ty;
+  float rho = sqrtf(rho2);
+  const float sh = sqrtf(1.0f + rho2);
+  rho = rho < 1e-6f ? 1e-6f : rho;
+  return nn_log((1.0f + sh) / rho);
+}
+// nn = mu[8], isig[8], W1[32][8], b1[32], W2[32], b2, cut, margin
+__device__ __forceinline__ float nn_ghost_prob(const float* __restrict__ nn, const float* in) {
+  float u[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) u[k] = (in[k] - __ldg(nn + k)) * __ldg(nn + 8 + k);
+  float t = __ldg(nn + 336);
+  for (int j = 0; j < 32; ++j) {
+    float h = __ldg(nn + 272 + j);
+#pragma unroll
+    for (int k = 0; k < 8; ++k) h = h + __ldg(nn + 16 + j * 8 + k) * u[k];
+    h = h < 0.f ? 0.f : h;
+    t = t + __ldg(nn + 304 + j) * h;
+  }
+  return 1.0f / (1.0f + nn_exp(-t));
 }
 
 struct UtHyp { int n; int idx[4]; float gamma, ssq; };      // idx: position in the searched x0 array, -1 = none
@@ -303,7 +362,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
         if (k < p.max_mc) {
           MatchCand m;
           m.seed = (uint16_t)s; m.velo = (uint16_t)v; m.chi2 = chi2; m.q0 = dtx * p.inv_KB;   // A10
-          m.gamma = 0.f; m.key = kNoKey;
+          m.gamma = 0.f; m.key = kNoKey; m.ghost = 0.f; m.pad = 0u;
 #pragma unroll
           for (int l = 0; l < 4; ++l) m.ut[l] = 0xFFFF;
           mc[k] = m;
@@ -399,6 +458,37 @@ matching_kernel(const __grid_constant__ MatchParams p) {
   }
   // a pair is valid if its best hypothesis has enough UT hits (L311); without UT every pair is
   const unsigned long long key_ok = p.use_ut ? (unsigned long long)(4 - p.min_ut_hits) : ~0ull >> 50;
+  const bool use_nn = p.nn != nullptr;
+  float nn_cut = 0.f, nn_margin = 0.f;
+  if (use_nn) {
+    // ---- M4 (O14b, L346-348): ghost probability of every valid pair; minimum per seed and per VELO over
+    // the pairs below the cut
+    nn_cut = __ldg(p.nn + 337); nn_margin = __ldg(p.nn + 338);
+    for (int k = tid; k < nm; k += kMatchThreads) {
+      MatchCand& m = mc[k];
+      if ((m.key >> 50) > key_ok) continue;
+      const int s = m.seed, v = m.velo;
+      const size_t slot = s < c0 ? (size_t)(2 * e) * p.max_seeds + s : (size_t)(2 * e + 1) * p.max_seeds + (s - c0);
+      const float xS = p.state[slot], yS = p.state[sct + slot], txS = p.state[2 * sct + slot], tyS = p.state[3 * sct + slot];
+      const float xV = svx[v], yV = svy[v], txV = svtx[v], tyV = svty[v];
+      const float dtx = txS - txV, dty = tyS - tyV, adtx = fabsf(dtx);
+      const float zm = (((p.mag[0] + p.mag[1] * adtx) + p.mag[2] * (dtx * dtx)) + p.mag[3] * fabsf(xS)) +
+                       p.mag[4] * (txV * txV);                                     // Eq. 18
+      const float xs = xS + (zm - p.zS) * txS, xv = xV + (zm - p.zV) * txV;        // Eq. 17
+      const float ys = yS + p.dzyS * tyS, yv = yV + p.dzyV * tyV;
+      float in[8];
+      in[0] = zm; in[1] = xs - xv; in[2] = ys - yv; in[3] = dtx; in[4] = dty; in[5] = m.chi2;
+      in[6] = nn_eta(txV, tyV);
+      in[7] = (float)(p.snx && p.snuv ? (int)p.snx[slot] + (int)p.snuv[slot] : 12);
+      const float g = nn_ghost_prob(p.nn, in);
+      m.ghost = g;
+      if (g < nn_cut) {
+        atomicMin(&seed_best[s], (unsigned long long)__float_as_uint(g));
+        atomicMin(&velo_best[sorig[v]], (unsigned long long)__float_as_uint(g));
+      }
+    }
+    __syncthreads();
+  } else {
   for (int k = tid; k < nm; k += kMatchThreads) {
     const MatchCand& m = mc[k];
     if ((m.key >> 50) <= key_ok)
@@ -415,13 +505,20 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     atomicMin(&velo_best[sorig[m.velo]], cb | m.seed);
   }
   __syncthreads();
+  }
   const int pol = p.pol ? (int)p.pol[e] : p.polarity;
   for (int k = tid; k < nm; k += kMatchThreads) {
     const MatchCand& m = mc[k];
     if ((m.key >> 50) > key_ok) continue;
     const unsigned long long cb = (unsigned long long)__float_as_uint(m.chi2) << 32;
     const int vo = sorig[m.velo];
-    if (seed_best[m.seed] != (cb | vo) || velo_best[vo] != (cb | m.seed)) continue;
+    if (use_nn) {
+      // kept if below the cut and no track sharing its seed or its VELO is better by the margin (the minimum
+      // includes the track itself, which never satisfies g >= g + margin)
+      if (!(m.ghost < nn_cut)) continue;
+      const float gs = __uint_as_float((unsigned int)seed_best[m.seed]), gv = __uint_as_float((unsigned int)velo_best[vo]);
+      if (m.ghost >= gs + nn_margin || m.ghost >= gv + nn_margin) continue;
+    } else if (seed_best[m.seed] != (cb | vo) || velo_best[vo] != (cb | m.seed)) continue;
     const int slot = atomicAdd(&hdr[1], 1);
     if (slot >= p.max_long) continue;
     const size_t o = (size_t)e * p.max_long + slot, ct = p.long_cap_total;
@@ -442,6 +539,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     }
     p.qop[o] = pol > 0 ? q : -q;
     p.chi2[o] = m.chi2;
+    if (use_nn && p.ghost) p.ghost[o] = m.ghost;
   }
   __syncthreads();
   LHCB_CLK(13)
