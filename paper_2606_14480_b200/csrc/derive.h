@@ -60,7 +60,7 @@ inline void resolve_defaults(lhcb_geom_t& g) {
   g.max_long_per_event = resolve_capacity(g.max_long_per_event, 256);
   g.max_hits_per_half = resolve_capacity(g.max_hits_per_half, 6144);
   g.max_triplets_per_half = resolve_capacity(g.max_triplets_per_half, 4096);
-  g.max_match_cand_per_event = resolve_capacity(g.max_match_cand_per_event, 768);
+  g.max_match_cand_per_event = resolve_capacity(g.max_match_cand_per_event, 384);
   g.max_velo_per_event = resolve_capacity(g.max_velo_per_event, 512);
   g.max_ut_per_event = resolve_capacity(g.max_ut_per_event, 6144);
 }
