@@ -168,6 +168,14 @@ class Oracle:
         m = self.matching(ev.n_events, seed_off, s["state"], ev, use_ut=use_ut)
         return s, m
 
+    def set_uv_hough(self, on: bool):
+        """Hough-cluster UV seeding (reading A20) instead of the iterative default."""
+        self.lib.orc_set_uv_hough(self.ctx, C.c_int(1 if on else 0))
+
+    def hough_constants(self):
+        o = self._dout(4); self.lib.orc_hough_constants(self.ctx, _p(o, D))
+        return dict(zip(["tlo0", "tlo1", "w", "invw"], o))
+
     # ------------------------------------------------------------------ probes (pins)
     def spec_exp(self, y): return self.lib.orc_spec_exp(float(y))
     def spec_log(self, x): return self.lib.orc_spec_log(float(x))

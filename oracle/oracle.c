@@ -80,6 +80,9 @@ typedef struct {
   REAL zS, zV, dzyS, dzyV, mag[5], presel[4], cx0, cx1, cy0, cy1, inv_tol_tx, inv_tol_ty, chi2m_max;
   REAL inv_KB, Ag, Bg, inv_Bg, ut_dz[NUT], ut_dz2[NUT], ut_dz4[NUT], ut_tan[NUT], ut_y_tol;
   REAL ut_loose[NUT][4], ut_tight[NUT][4];
+  /* Hough-cluster UV seeding (L217, reading A20): off unless orc_set_uv_hough(ctx, 1) */
+  int uv_hough;
+  REAL hough_tlo[2], hough_invw, hough_w;   /* t_y bins per half: b = floor((t - tlo) * invw), 64 bins of width w */
 } orc_ctx;
 
 enum { C_T1 = 0, C_PAIRS, C_TRIPLETS, C_EXT_OK, C_FIT_OK, C_XZ_KEPT, C_UV_FIRST, C_UV_STEPS,
@@ -247,6 +250,15 @@ int orc_init(const orc_geom_t* gin, orc_ctx* C) {
     for (k = 0; k < 4; k++) { C->ut_loose[i][k] = (REAL)g->ut_loose[i][k]; C->ut_tight[i][k] = (REAL)g->ut_tight[i][k]; }
   }
   C->ut_y_tol = (REAL)g->ut_y_tol;
+  {                                                         /* A20: t_y = y / z range of each half over the stereo layers */
+    double zmin = g->scifi_z[C->ul[0]], tol = fabs(g->y_half_tol);
+    double ylo[2], yhi[2]; int h;
+    ylo[0] = -tol; yhi[0] = g->y_max; ylo[1] = g->y_min; yhi[1] = tol;
+    for (h = 0; h < 2; h++) C->hough_tlo[h] = (REAL)rnd(ylo[h] / zmin);
+    C->hough_w = (REAL)rnd((yhi[0] - ylo[0]) / zmin / 64.0);
+    C->hough_invw = (REAL)rnd(64.0 / ((yhi[0] - ylo[0]) / zmin));
+    C->uv_hough = 0;
+  }
   return 0;
 }
 
@@ -432,6 +444,61 @@ static void seed_half(const orc_ctx* C, const uint32_t* zoff, const REAL* hx, in
     if (!cd->keep) continue;
     cnt[C_XZ_KEPT]++;
     for (s = 0; s < NX; s++) xp[s] = xz_at(C, cd->ax, cd->bx, cd->cx, C->ul[s]);
+    if (C->uv_hough) {
+      /* O8h (L217, reading A20): one-dimensional Hough transform in t_y over all six stereo layers.
+       * Every hit inside its layer's window (Eq. 16, the half's y range) votes for the bin of t_y = y / z;
+       * a layer counts once per bin ("bitwise").  A cluster is a bin together with its upper neighbour; its
+       * population is the number of layers with a vote in it.  Up to eight clusters with population >=
+       * min_uv_hits are taken, most populated first (then lower t_y); each is cut into four finer t_y
+       * hypotheses; per hypothesis the closest hit within tol_uv (2 mm) of the straight line is attached in
+       * every layer; fit and choice of the best combination as in the iterative version. */
+      uint64_t vote[NX]; int pop[64], sel[8], nsel = 0, b, level, r, k;
+      for (s = 0; s < NX; s++) {
+        int l = C->ul[s]; uint32_t ih;
+        REAL wa = xp[s] - C->ywin_a[half][l], wb = xp[s] - C->ywin_b[half][l];
+        REAL wlo = rmin(wa, wb), whi = rmax(wa, wb);
+        vote[s] = 0;
+        for (ih = zoff[l]; ih < zoff[l + 1]; ih++) {
+          REAL xh = hx[ih], t, tb;
+          if (!(wlo <= xh && xh <= whi)) continue;
+          cnt[C_UV_FIRST]++;
+          t = ((xp[s] - xh) * C->inv_tan[l]) * C->inv_z[l];                     /* Eq. 16, A7 */
+          tb = (t - C->hough_tlo[half]) * C->hough_invw;
+          tb = rmin(rmax(tb, (REAL)0), (REAL)63);
+          vote[s] |= (uint64_t)1 << (int)tb;
+        }
+      }
+      for (b = 0; b < 64; b++) {
+        pop[b] = 0;
+        for (s = 0; s < NX; s++)
+          pop[b] += (int)(((vote[s] >> b) & 1) | (b < 63 ? (vote[s] >> (b + 1)) & 1 : 0));
+      }
+      for (level = NX; level >= C->g.min_uv_hits && level >= 1; level--)
+        for (b = 0; b < 64; b++)
+          if (pop[b] == level && nsel < 8) sel[nsel++] = b;
+      for (r = 0; r < nsel; r++)
+        for (k = 0; k < 4; k++) {
+          REAL f = (REAL)k * (REAL)0.5 + (REAL)0.25;
+          REAL ty = C->hough_tlo[half] + ((REAL)sel[r] + f) * C->hough_w;
+          REAL m[NX], ay, by, chi2y; uint32_t hit[NX]; int n = 0, mask = 0;
+          for (s = 0; s < NX; s++) {
+            int l = C->ul[s]; REAL xe; int64_t h;
+            cnt[C_UV_STEPS]++;
+            hit[s] = NO_HIT;
+            xe = xp[s] - ty * C->zt[l];
+            h = closest_hit(hx, zoff[l], zoff[l + 1], xe, C->tol_uv);           /* L217: the same 2 mm */
+            if (h >= 0) { hit[s] = (uint32_t)h; m[s] = hx[h] - xp[s]; mask |= 1 << s; n++; }
+          }
+          if (n < C->g.min_uv_hits) continue;
+          cnt[C_YFITS]++;
+          chi2y = fit_y(C, mask, m, n, &ay, &by);
+          if (chi2y > C->chi2y_max) continue;
+          if (!have || n > best_n || (n == best_n && chi2y < best_chi2)) {      /* ties: earlier (cluster, k) */
+            have = 1; best_n = n; best_chi2 = chi2y; best_ay = ay; best_by = by;
+            memcpy(best_hit, hit, sizeof(hit));
+          }
+        }
+    } else
     for (pp = 0; pp < 2; pp++) {
       int lf = C->g.uv_first_layer[pp], sf = C->slot_of_layer[lf];
       REAL wa = xp[sf] - C->ywin_a[half][lf], wb = xp[sf] - C->ywin_b[half][lf];
@@ -819,6 +886,12 @@ int64_t orc_matching_nn(const orc_ctx* C, int n_events, const uint32_t* seed_off
                         const uint8_t* seed_nhits, const REAL* nn, REAL* o_ghost) {
   return matching_impl(C, n_events, seed_off, state, velo_off, vx, vy, vtx, vty, ut_off, ux, uylo, uyhi, polarity, cap,
                        o_event, o_seed, o_velo, o_ut, o_nut, o_qop, o_chi2, counters, seed_nhits, nn, o_ghost);
+}
+
+/* Hough-cluster UV seeding (reading A20) on / off; the default is the iterative version (L204) */
+void orc_set_uv_hough(orc_ctx* C, int on) { C->uv_hough = on ? 1 : 0; }
+void orc_hough_constants(const orc_ctx* C, double* out /* tlo0, tlo1, w, invw */) {
+  out[0] = C->hough_tlo[0]; out[1] = C->hough_tlo[1]; out[2] = C->hough_w; out[3] = C->hough_invw;
 }
 
 /* probes of the network arithmetic (pins) */
