@@ -205,6 +205,14 @@ size_t lhcb_workspace_bytes(const lhcb_ctx* ctx, int n_events, size_t n_scifi_hi
 int lhcb_prepare(lhcb_ctx* ctx, const lhcb_raw_t* raw, uint32_t* zone_off, float* hit_x, uint32_t* perm,
                  uint32_t* status, void* cuda_stream);
 
+/* UV seeding version: 0 = iterative over the hits of a first stereo layer (the paper's
+ * default, and the default here), 1 = Hough clusters (reading A20): a one-dimensional Hough
+ * transform in t_y over all six stereo layers with 64 bins per detector half, a layer voting once per bin;
+ * clusters of two adjacent bins ranked by the number of voting layers; up to eight clusters, each cut into
+ * four finer t_y hypotheses; per hypothesis the closest hit within tol_uv in every layer; fit and choice of
+ * the best combination as in the iterative version.  Takes effect from the next lhcb_seeding call. */
+int lhcb_set_uv_hough(lhcb_ctx* ctx, int on);
+
 /* Final selection with the ghost-killing network (reading A14b).
  * nn: HOST array of LHCB_GHOST_NN_SIZE floats  mu[8], isig[8], W1[32][8], b1[32], W2[32], b2, cut, margin
  * for the inputs (z_match, dx, dy, dtx, dty, chi2_match, eta_VELO, nHits_SciFi), standardised as

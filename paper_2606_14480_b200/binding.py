@@ -24,7 +24,7 @@ ST_BITS = {1: "triplet_overflow", 2: "cand_overflow", 4: "seed_overflow", 8: "hi
 EXPORTS = ["lhcb_geom_derive", "lhcb_geom_init", "lhcb_destroy", "lhcb_get_geom", "lhcb_workspace_bytes",
            "lhcb_seeding", "lhcb_matching", "lhcb_error_string", "lhcb_last_cuda_error",
            "lhcb_last_launch_count", "lhcb_pipeline_create", "lhcb_pipeline_destroy", "lhcb_reconstruct_host",
-           "lhcb_pipeline_last_bytes", "lhcb_launch_config", "lhcb_prepare", "lhcb_set_ghost_nn"]
+           "lhcb_pipeline_last_bytes", "lhcb_launch_config", "lhcb_prepare", "lhcb_set_ghost_nn", "lhcb_set_uv_hough"]
 
 
 class LhcbGeom(C.Structure):
@@ -136,6 +136,7 @@ def load_library(build: bool = True) -> C.CDLL:
         lib.lhcb_launch_config.argtypes = [VP, C.POINTER(C.c_int * 4)]
         lib.lhcb_prepare.argtypes = [VP, C.POINTER(LhcbRaw), VP, VP, VP, VP, VP]
         lib.lhcb_set_ghost_nn.argtypes = [VP, C.POINTER(C.c_float)]
+        lib.lhcb_set_uv_hough.argtypes = [VP, C.c_int]
         lib.lhcb_pipeline_create.argtypes = [VP, C.c_int, C.c_size_t, C.c_size_t, C.c_size_t, C.c_int, C.POINTER(VP)]
         lib.lhcb_pipeline_destroy.argtypes = [VP]
         lib.lhcb_pipeline_destroy.restype = None
@@ -312,6 +313,10 @@ class Context:
         rc = self.lib.lhcb_matching(self._ctx, C.byref(s), C.byref(v), u, C.byref(l), VP(0), self._stream())
         _check(self.lib, self._ctx, rc, "lhcb_matching")
         return out
+
+    def lhcb_set_uv_hough(self, on: bool):
+        """Hough-cluster UV seeding (reading A20) instead of the iterative default."""
+        _check(self.lib, self._ctx, self.lib.lhcb_set_uv_hough(self._ctx, 1 if on else 0), "lhcb_set_uv_hough")
 
     def lhcb_set_ghost_nn(self, nn):
         """nn: 339 float32 (mu, isig, W1, b1, W2, b2, cut, margin) or None (back to the chi2 ranking, A14)."""

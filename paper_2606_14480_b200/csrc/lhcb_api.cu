@@ -3,6 +3,7 @@
 //   nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo -fmad=false -shared -Xcompiler -fPIC
 #include <cuda_runtime.h>
 
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -21,6 +22,7 @@ struct lhcb_ctx {
   float* d_Q;
   float* d_nn;        // ghost-killing network on the device
   int nn_on;
+  int uv_hough;       // Hough-cluster UV seeding instead of the iterative one
   size_t seed_smem, match_smem, prep_smem;
   int match_threads;  // 128 when six CTAs fit an SM, else 256
   int seed_threads;   // 256 when four CTAs fit the SM's shared memory, else 512
@@ -69,6 +71,15 @@ void fill_seed_params(const lhcb_ctx* c, lhcb::SeedParams& p) {
   p.max_seeds = g.max_seeds_per_half; p.max_cand = g.max_xz_cand_per_half; p.max_hits = g.max_hits_per_half;
   p.max_trip = g.max_triplets_per_half;
   p.P = c->d_P; p.Q = c->d_Q;
+  // Hough-cluster UV seeding (reading A20): 64 t_y = y / z bins per half over the stereo layers, in double
+  // from the float geometry, rounded once
+  {
+    const double zmin = (double)g.scifi_z[D.ul[0]], tol = std::fabs((double)g.y_half_tol);
+    const double range = ((double)g.y_max + tol) / zmin;
+    p.uv_hough = c->uv_hough;
+    p.h_tlo[0] = (float)(-tol / zmin); p.h_tlo[1] = (float)((double)g.y_min / zmin);
+    p.h_w = (float)(range / 64.0); p.h_invw = (float)(64.0 / range);
+  }
 }
 
 void fill_match_params(const lhcb_ctx* c, lhcb::MatchParams& p) {
@@ -177,6 +188,12 @@ int lhcb_get_geom(const lhcb_ctx* c, lhcb_geom_t* out) {
 size_t lhcb_workspace_bytes(const lhcb_ctx* c, int n_events, size_t n_scifi_hits) {
   (void)c; (void)n_events; (void)n_scifi_hits;
   return 0;   // every intermediate lives in shared memory
+}
+
+int lhcb_set_uv_hough(lhcb_ctx* c, int on) {
+  if (!c) return LHCB_ERR_NOT_INITIALISED;
+  c->uv_hough = on ? 1 : 0;
+  return LHCB_OK;
 }
 
 int lhcb_set_ghost_nn(lhcb_ctx* c, const float* nn) {

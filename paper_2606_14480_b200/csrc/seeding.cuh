@@ -62,6 +62,8 @@ struct SeedParams {
   float zbS, gS, gpS;
   int min_x_hits, min_uv_hits, uv_first[2], polarity;
   int max_seeds, max_cand, max_hits, max_trip;
+  int uv_hough;                       // Hough-cluster UV seeding (L217, reading A20) instead of the iterative one
+  float h_tlo[2], h_w, h_invw;        // its t_y bins: b = clamp((t - tlo[half]) * invw, 0, 63), width w
   int smem_total;   // dynamic shared memory of the launch = seed_smem_bytes(threads, capacities)
   const float* P;   // [7][3][6]
   const float* Q;   // [64][2][6]
@@ -667,7 +669,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   uint32_t* items = reinterpret_cast<uint32_t*>(xps + (size_t)nk * 8);
   UvLive* live = reinterpret_cast<UvLive*>(items + C);
   UvSuccess* succ = reinterpret_cast<UvSuccess*>(live + C);
-  const int succ_cap = (rest - C * 20) / (int)sizeof(UvSuccess);
+  int succ_cap = (rest - C * 20) / (int)sizeof(UvSuccess);
   __syncthreads();
   for (int k = tid; k < nk; k += T) {
     best[k] = kNoKey;
@@ -684,6 +686,105 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   // is queued as (owner, hit); phase A walks the first three other stereo layers of every item (dense),
   // the walks that can still reach min_uv_hits are queued with their state; phase B finishes them.
   const int sf0 = p.slot_of_layer[p.uv_first[0]], sf1 = p.slot_of_layer[p.uv_first[1]];
+  if (p.uv_hough) {
+    // ---- S4h: Hough-cluster version (O8h).  The queue space after the predictions is laid out as
+    //   [votes u64[nk][6] | selected clusters u8[nk][8] + count | hypothesis list u32 | success queue]
+    unsigned long long* vote = reinterpret_cast<unsigned long long*>(items);      // items is 16-byte aligned
+    uint8_t* selb = reinterpret_cast<uint8_t*>(vote + (size_t)nk * 6);            // [nk][9]: 8 bins, then how many
+    uint32_t* hyp = reinterpret_cast<uint32_t*>(selb + (((size_t)nk * 9 + 15) & ~(size_t)15));
+    const int hrest = rest - nk * 48 - (int)(((size_t)nk * 9 + 15) & ~(size_t)15);
+    int hyp_cap = nk * 32;                                                        // 8 clusters x 4 finer hypotheses
+    if (hyp_cap * 4 > hrest / 2) hyp_cap = hrest / 8;
+    UvSuccess* hsucc = reinterpret_cast<UvSuccess*>(hyp + ((hyp_cap + 3) & ~3));
+    const int hsucc_cap = (hrest - ((hyp_cap + 3) & ~3) * 4) / (int)sizeof(UvSuccess);
+    if (tid == 0) H.n_live = 0;
+    // H1: votes.  Owner = (survivor, stereo slot); every hit in the slot's window of Eq. 16 sets the bit of
+    // its t_y bin (a layer counts once per bin)
+    for (int w = tid; w < 6 * nk; w += T) {
+      const int k = w / 6, sl = w - 6 * k;
+      const float4 cf = H.uvc[sl];                                                // {z tan, 1/tan, 1/z, layer}
+      const int l = __float_as_int(cf.w);
+      const float xpl = xps[k * 8 + sl];
+      const float wa = xpl - p.ywin_a[h][l], wb = xpl - p.ywin_b[h][l];
+      const Zone zf = H.zi[l];
+      const uint16_t* lutf = lut + l * (kLutBins + 1);
+      float xh;
+      int i = lower_bound_v(hx, lutf, zf, fminf(wa, wb), xh);
+      const float whi = fmaxf(wa, wb);
+      unsigned long long m = 0ull;
+      while (xh <= whi) {
+        const float t = ((xpl - xh) * cf.y) * cf.z;                               // Eq. 16, A7
+        float tb = (t - p.h_tlo[h]) * p.h_invw;
+        tb = fminf(fmaxf(tb, 0.f), 63.f);
+        m |= 1ull << (int)tb;
+        ++i;
+        xh = i < zf.e ? hx[i] : __int_as_float(0x7f800000);
+      }
+      vote[w] = m;
+    }
+    __syncthreads();
+    // H2: cluster = bin + upper neighbour; population = layers voting in it, counted for all 64 bins at once
+    // with a bit-sliced adder; up to eight clusters, most populated first, then lower t_y
+    for (int k = tid; k < nk; k += T) {
+      unsigned long long ones = 0ull, twos = 0ull, fours = 0ull;
+#pragma unroll
+      for (int sl = 0; sl < 6; ++sl) {
+        const unsigned long long m = vote[k * 6 + sl];
+        const unsigned long long cm = m | (m >> 1);
+        const unsigned long long c1 = ones & cm;
+        ones ^= cm;
+        const unsigned long long c2 = twos & c1;
+        twos ^= c1;
+        fours |= c2;
+      }
+      int nsel = 0;
+      for (int level = 6; level >= p.min_uv_hits && level >= 1 && nsel < 8; --level) {
+        unsigned long long lm = ((level & 4) ? fours : ~fours) & ((level & 2) ? twos : ~twos) & ((level & 1) ? ones : ~ones);
+        while (lm && nsel < 8) {
+          selb[k * 9 + nsel++] = (uint8_t)(__ffsll((long long)lm) - 1);
+          lm &= lm - 1;
+        }
+      }
+      selb[k * 9 + 8] = (uint8_t)nsel;
+      const int base = atomicAdd(&H.n_live, 4 * nsel);
+      for (int j = 0; j < 4 * nsel; ++j)
+        if (base + j < hyp_cap) hyp[base + j] = ((uint32_t)k << 8) | (uint32_t)j;   // j = cluster rank * 4 + finer index
+    }
+    __syncthreads();
+    int nhyp = H.n_live;
+    if (nhyp > hyp_cap) { nhyp = hyp_cap; if (tid == 0) H.status |= LHCB_ST_UV_QUEUE_OVERFLOW; }
+    // H3: thread per hypothesis: closest hit within tol_uv of the fixed line in every stereo layer
+    for (int i = tid; i < nhyp; i += T) {
+      const uint32_t hq = hyp[i];
+      const int k = (int)(hq >> 8), j = (int)(hq & 0xFFu);
+      const float* xpk = xps + k * 8;
+      const float f = (float)(j & 3) * 0.5f + 0.25f;
+      const float ty = p.h_tlo[h] + ((float)selb[k * 9 + (j >> 2)] + f) * p.h_w;
+      int n = 0, hh[6];
+#pragma unroll
+      for (int sl = 0; sl < 6; ++sl) {
+        hh[sl] = -1;
+        if (n + (6 - sl) < p.min_uv_hits) continue;                               // cannot reach min_uv_hits any more
+        const float4 cf = H.uvc[sl];
+        const int l = __float_as_int(cf.w);
+        const Zone z = H.zi[l];
+        float xhh;
+        hh[sl] = closest_hit(hx, lut + l * (kLutBins + 1), z, xpk[sl] - ty * cf.x, p.tol_uv, xhh);
+        n += hh[sl] >= 0;
+      }
+      if (n < p.min_uv_hits) continue;
+      const int slot = atomicAdd(&H.n_trip, 1);
+      if (slot < hsucc_cap) {
+        UvSuccess& u = hsucc[slot];
+        u.k = (uint16_t)k; u.pp = (uint8_t)j; u.n = (uint8_t)n;
+#pragma unroll
+        for (int sl = 0; sl < 6; ++sl) u.hit[sl] = (uint16_t)hh[sl];
+      }
+    }
+    __syncthreads();
+    succ = hsucc;
+    succ_cap = hsucc_cap;
+  } else
   for (int tile0 = 0; tile0 < 2 * nk; tile0 += T) {
     const int nown = 2 * nk - tile0 < T ? 2 * nk - tile0 : T;
     int cnt = 0, fst = 0;
@@ -775,12 +876,16 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     chi2y = fit_y(p, c, ay, by);
     key = kNoKey;
     if (!(chi2y > p.chi2y_max)) {
-      const int sf = p.slot_of_layer[p.uv_first[u.pp]];
-      int first_local = 0;
+      // ties: earlier pass, then lower first hit (iterative); earlier (cluster, finer index) (Hough)
+      unsigned long long tie = u.pp;
+      if (!p.uv_hough) {
+        const int sf = p.slot_of_layer[p.uv_first[u.pp]];
+        int first_local = 0;
 #pragma unroll
-      for (int s = 0; s < 6; ++s) first_local = (s == sf) ? (int)u.hit[s] - zl[p.ul[s]] : first_local;
-      key = ((unsigned long long)(6 - u.n) << 49) | ((unsigned long long)__float_as_uint(chi2y) << 17) |
-            ((unsigned long long)u.pp << 16) | (unsigned long long)first_local;
+        for (int s = 0; s < 6; ++s) first_local = (s == sf) ? (int)u.hit[s] - zl[p.ul[s]] : first_local;
+        tie = ((unsigned long long)u.pp << 16) | (unsigned long long)first_local;
+      }
+      key = ((unsigned long long)(6 - u.n) << 49) | ((unsigned long long)__float_as_uint(chi2y) << 17) | tie;
     }
   };
   for (int i = tid; i < nsucc; i += T) {
