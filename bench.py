@@ -236,6 +236,25 @@ def main():
                  "long_per_event": n_long_nn / n, "note": "lhcb_matching with lhcb_set_ghost_nn (reading A14b); "
                  "the timed step uses the chi2 ranking (A14)"}
 
+    # ---- seeding with the Hough-cluster UV version, timed on its own --------------------------
+    hough = None
+    if rank == 0:
+        ctx.lhcb_set_uv_hough(True)
+        s_h = ctx.alloc_seeds(n)
+        e = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        th_ = []
+        for i in range(13):
+            e[0].record(stream); ctx.lhcb_seeding(dev, s_h); e[1].record(stream); torch.cuda.synchronize()
+            if i >= 3:
+                th_.append(e[0].elapsed_time(e[1]))
+        ctx.lhcb_set_uv_hough(False)
+        if int(s_h["status"].max().item()) != 0:
+            raise SystemExit("capacity overflow in the Hough-cluster seeding")
+        hough = {"seeding_ms": float(np.median(th_)), "seeding_events_per_s": n / float(np.median(th_)) * 1e3,
+                 "seeds_per_event": int(s_h["count"].sum().item()) / n,
+                 "note": "lhcb_seeding with lhcb_set_uv_hough (reading A20); the timed step uses the iterative default"}
+        del s_h
+
     # ---- end to end through the host-buffer C-ABI call ---------------------------------------------------
     e2e = None
     if not args.no_e2e:
@@ -300,7 +319,7 @@ def main():
             "long_tracks_per_s": n_long_all / (ms_per_step * 1e-3), "seeds_per_event": n_seeds / n, "long_per_event": n_long / n,
             "seeding_events_per_s": n / float(np.median(seed_ms)) * 1e3, "matching_events_per_s": n / float(np.median(match_ms)) * 1e3,
             "min_ms": {"seeding": float(seed_ms.min()), "matching": float(match_ms.min())},
-            "batches": batches, "prepare": prepare, "ghost_nn": ghost, "clocks": clocks, "e2e": e2e, "gpu_launches": 2 * K, "roofline": roofline, "cpu_baseline": cpu}
+            "batches": batches, "prepare": prepare, "ghost_nn": ghost, "uv_hough": hough, "clocks": clocks, "e2e": e2e, "gpu_launches": 2 * K, "roofline": roofline, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

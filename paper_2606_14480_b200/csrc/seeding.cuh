@@ -688,16 +688,13 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   const int sf0 = p.slot_of_layer[p.uv_first[0]], sf1 = p.slot_of_layer[p.uv_first[1]];
   if (p.uv_hough) {
     // ---- S4h: Hough-cluster version (O8h).  The queue space after the predictions is laid out as
-    //   [votes u64[nk][6] | selected clusters u8[nk][8] + count | hypothesis list u32 | success queue]
+    //   [votes u64[nk][6] | first hypothesis of each survivor int[nk + 1] | selected clusters u8[nk][8] | success queue]
     unsigned long long* vote = reinterpret_cast<unsigned long long*>(items);      // items is 16-byte aligned
-    uint8_t* selb = reinterpret_cast<uint8_t*>(vote + (size_t)nk * 6);            // [nk][9]: 8 bins, then how many
-    uint32_t* hyp = reinterpret_cast<uint32_t*>(selb + (((size_t)nk * 9 + 15) & ~(size_t)15));
-    const int hrest = rest - nk * 48 - (int)(((size_t)nk * 9 + 15) & ~(size_t)15);
-    int hyp_cap = nk * 32;                                                        // 8 clusters x 4 finer hypotheses
-    if (hyp_cap * 4 > hrest / 2) hyp_cap = hrest / 8;
-    UvSuccess* hsucc = reinterpret_cast<UvSuccess*>(hyp + ((hyp_cap + 3) & ~3));
-    const int hsucc_cap = (hrest - ((hyp_cap + 3) & ~3) * 4) / (int)sizeof(UvSuccess);
-    if (tid == 0) H.n_live = 0;
+    int* hoff = reinterpret_cast<int*>(vote + (size_t)nk * 6);
+    uint8_t* selb = reinterpret_cast<uint8_t*>(hoff + nk + 1);
+    const int hused = nk * 48 + (int)((((size_t)nk + 1) * 4 + (size_t)nk * 8 + 15) & ~(size_t)15);
+    UvSuccess* hsucc = reinterpret_cast<UvSuccess*>(reinterpret_cast<unsigned char*>(items) + hused);
+    const int hsucc_cap = (rest - hused) / (int)sizeof(UvSuccess);
     // H1: votes.  Owner = (survivor, stereo slot); every hit in the slot's window of Eq. 16 sets the bit of
     // its t_y bin (a layer counts once per bin)
     for (int w = tid; w < 6 * nk; w += T) {
@@ -724,42 +721,45 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     }
     __syncthreads();
     // H2: cluster = bin + upper neighbour; population = layers voting in it, counted for all 64 bins at once
-    // with a bit-sliced adder; up to eight clusters, most populated first, then lower t_y
-    for (int k = tid; k < nk; k += T) {
-      unsigned long long ones = 0ull, twos = 0ull, fours = 0ull;
-#pragma unroll
-      for (int sl = 0; sl < 6; ++sl) {
-        const unsigned long long m = vote[k * 6 + sl];
-        const unsigned long long cm = m | (m >> 1);
-        const unsigned long long c1 = ones & cm;
-        ones ^= cm;
-        const unsigned long long c2 = twos & c1;
-        twos ^= c1;
-        fours |= c2;
-      }
+    // with a bit-sliced adder; up to eight clusters, most populated first, then lower t_y.  A block scan
+    // gives every survivor the index of its first hypothesis (4 per cluster).
+    int nhyp = 0;
+    for (int tile0 = 0; tile0 < nk; tile0 += T) {
+      const int k = tile0 + tid;
       int nsel = 0;
-      for (int level = 6; level >= p.min_uv_hits && level >= 1 && nsel < 8; --level) {
-        unsigned long long lm = ((level & 4) ? fours : ~fours) & ((level & 2) ? twos : ~twos) & ((level & 1) ? ones : ~ones);
-        while (lm && nsel < 8) {
-          selb[k * 9 + nsel++] = (uint8_t)(__ffsll((long long)lm) - 1);
-          lm &= lm - 1;
+      if (k < nk) {
+        unsigned long long ones = 0ull, twos = 0ull, fours = 0ull;
+#pragma unroll
+        for (int sl = 0; sl < 6; ++sl) {
+          const unsigned long long m = vote[k * 6 + sl];
+          const unsigned long long cm = m | (m >> 1);
+          const unsigned long long c1 = ones & cm;
+          ones ^= cm;
+          const unsigned long long c2 = twos & c1;
+          twos ^= c1;
+          fours |= c2;
+        }
+        for (int level = 6; level >= p.min_uv_hits && level >= 1 && nsel < 8; --level) {
+          unsigned long long lm = ((level & 4) ? fours : ~fours) & ((level & 2) ? twos : ~twos) & ((level & 1) ? ones : ~ones);
+          while (lm && nsel < 8) {
+            selb[k * 8 + nsel++] = (uint8_t)(__ffsll((long long)lm) - 1);
+            lm &= lm - 1;
+          }
         }
       }
-      selb[k * 9 + 8] = (uint8_t)nsel;
-      const int base = atomicAdd(&H.n_live, 4 * nsel);
-      for (int j = 0; j < 4 * nsel; ++j)
-        if (base + j < hyp_cap) hyp[base + j] = ((uint32_t)k << 8) | (uint32_t)j;   // j = cluster rank * 4 + finer index
+      int total;
+      const int ex = block_exscan<NT>(4 * nsel, H.warp_sums, total);
+      if (k < nk) hoff[k] = nhyp + ex;
+      nhyp += total;
     }
+    if (tid == 0) hoff[nk] = nhyp;
     __syncthreads();
-    int nhyp = H.n_live;
-    if (nhyp > hyp_cap) { nhyp = hyp_cap; if (tid == 0) H.status |= LHCB_ST_UV_QUEUE_OVERFLOW; }
     // H3: thread per hypothesis: closest hit within tol_uv of the fixed line in every stereo layer
     for (int i = tid; i < nhyp; i += T) {
-      const uint32_t hq = hyp[i];
-      const int k = (int)(hq >> 8), j = (int)(hq & 0xFFu);
+      const int k = owner_of(hoff, nk, i), j = i - hoff[k];                       // j = cluster rank * 4 + finer index
       const float* xpk = xps + k * 8;
       const float f = (float)(j & 3) * 0.5f + 0.25f;
-      const float ty = p.h_tlo[h] + ((float)selb[k * 9 + (j >> 2)] + f) * p.h_w;
+      const float ty = p.h_tlo[h] + ((float)selb[k * 8 + (j >> 2)] + f) * p.h_w;
       int n = 0, hh[6];
 #pragma unroll
       for (int sl = 0; sl < 6; ++sl) {
