@@ -456,7 +456,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   __syncthreads();
   LHCB_CLK(1)
 
-  // ---- S1 + S2 per iteration -----------------------------------------------------------
+  // ---- S1 per iteration: two- and three-hit search, triplets of both iterations in one queue ----------
   for (int it = 0; it < 2; ++it) {
     const int l1 = p.l1[it], l2 = p.l2[it], l3 = p.l3[it];
     const Zone z1n = H.zi[l1], z2n = H.zi[l2], z3n = H.zi[l3];
@@ -525,16 +525,21 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
       __syncthreads();
       LHCB_CLK(3)
     }
+  }
+  // ---- S2: extension of the queued triplets of both iterations (O5) ---------------------------------
+  {
     int nt = H.n_trip;
     LHCB_DBG_MAX(0, nt)
     if (nt > trip_cap) { nt = trip_cap; if (tid == 0) H.status |= LHCB_ST_TRIPLET_OVERFLOW; }
 
-    for (int t = tid; t < nt; t += T) {                                          // O5 + O6
+    for (int t = tid; t < nt; t += T) {
       const Triplet tr = trip[t];
-      const int i1 = b1 + tr.i1, i2 = b2 + tr.i2, i3 = b3 + tr.i3;
+      const int it = tr.it;                                  // the queue holds iteration 0 first: warps are uniform in it
+      const int l1 = p.l1[it], l2 = p.l2[it], l3 = p.l3[it];
+      const int i1 = H.zi[l1].b + tr.i1, i2 = H.zi[l2].b + tr.i2, i3 = H.zi[l3].b + tr.i3;
       const float x1 = hx[i1], x2 = hx[i2], x3 = hx[i3];
-      const float t13 = (x3 - x1) * idz;
-      const float x2c = x1 + dz12 * t13;
+      const float t13 = (x3 - x1) * p.inv_dz13[it];
+      const float x2c = x1 + p.dz12[it] * t13;
       float cx = (x2 - x2c) * p.inv_K[it];
       float bx = t13 - cx * p.G13[it];
       float ax = (x1 - bx * p.zb[l1]) - cx * p.gz[l1];
@@ -571,8 +576,6 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     }
     __syncthreads();
     LHCB_CLK(4)
-    if (tid == 0) H.n_trip = 0;
-    __syncthreads();
   }
 
   int nc = H.n_cand;

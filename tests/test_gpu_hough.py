@@ -24,8 +24,8 @@ def check(ev, nominal):
     os_, om = o.reconstruct(ev)
     r = compare_seeds(os_, gs)
     assert r["n_orc"] == r["n_gpu"] == r["n_common"] and r["bit_equal"], r
-    ok = dict(zip(range(os_["n"]), seed_keys(os_["event"], os_["half"], os_["hits"])))
-    gk = dict(zip((int(x) for x in gs["slot"]), seed_keys(gs["event"], gs["half"], gs["hits"])))
+    ok = dict(zip(range(os_["n"]), seed_keys(os_["event"], os_["half"], os_["hits"], os_["state"])))
+    gk = dict(zip((int(x) for x in gs["slot"]), seed_keys(gs["event"], gs["half"], gs["hits"], gs["state"])))
     rl = compare_long(om, gl, ok, gk)
     assert rl["n_orc"] == rl["n_gpu"] == rl["n_common"] and rl["bit_equal"], rl
     # back to the iterative default: a different (larger) seed collection on these events

@@ -39,8 +39,8 @@ def check_chain(ctx, oracle32, ev, use_ut):
     n_diff = len(r["only_orc"]) + len(r["only_gpu"])
     assert n_diff <= 1e-3 * r["n_orc"], r
     assert r["max_rel"] <= 1e-4 and r["max_dx"] <= 5e-3, r
-    ok = dict(zip(range(os_["n"]), seed_keys(os_["event"], os_["half"], os_["hits"])))
-    gk = dict(zip((int(s) for s in gs["slot"]), seed_keys(gs["event"], gs["half"], gs["hits"])))
+    ok = dict(zip(range(os_["n"]), seed_keys(os_["event"], os_["half"], os_["hits"], os_["state"])))
+    gk = dict(zip((int(s) for s in gs["slot"]), seed_keys(gs["event"], gs["half"], gs["hits"], gs["state"])))
     rl = compare_long(om, gl, ok, gk)
     assert len(rl["only_orc"]) + len(rl["only_gpu"]) <= 1e-3 * max(rl["n_orc"], 1) + n_diff, rl
     assert rl["max_rel_qop"] <= 1e-4 and rl["max_rel_chi2"] <= 1e-4, rl
@@ -158,8 +158,8 @@ def test_cfg3_full_size_bench_configuration(oracle32):
         assert r["n_orc"] == r["n_gpu"] == r["n_common"] and r["bit_equal"], (e, r)
         n_s += r["n_common"]
         # long tracks of this event: (seed identity, velo, UT hits) sets
-        ok = dict(zip(range(os_["n"]), seed_keys(os_["event"], os_["half"], os_["hits"])))
-        gk = dict(zip((int(s) for s in g1["slot"]), seed_keys(g1["event"], g1["half"], g1["hits"])))
+        ok = dict(zip(range(os_["n"]), seed_keys(os_["event"], os_["half"], os_["hits"], os_["state"])))
+        gk = dict(zip((int(s) for s in g1["slot"]), seed_keys(g1["event"], g1["half"], g1["hits"], g1["state"])))
         lsel = gl["event"] == e
         l1 = {k: (v[lsel] if isinstance(v, np.ndarray) and v.shape[:1] == lsel.shape else v) for k, v in gl.items()}
         l1["velo"] = l1["velo"] - int(ev.velo_off[e])
