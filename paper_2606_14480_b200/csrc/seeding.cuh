@@ -4,17 +4,24 @@
 // with one bulk async copy (cp.async.bulk + mbarrier) and stay there for every step (L370).
 // Stages, separated by __syncthreads():
 //   S0  staging + bin tables           per zone, a 256-bin table "first hit with bin >= k" turns every
-//                                      lower/upper bound into one lookup plus a short forward scan
-//   S1  two-hit + three-hit search     thread per T1 hit finds its T3 window (Eq. 8-11); a block scan
-//                                      flattens all pairs; each thread walks a contiguous chunk of
-//                                      pairs: Eq. 3-5 and the T2 band (Eq. 12-13, A3/A4); triplets are
-//                                      queued in shared memory
-//   S2  extension + fit                thread per queued triplet: exact parabola, +-1 mm closest hit in
-//                                      the other three x-layers, >=5 hits, fixed-matrix least squares (L90)
-//   S3  clone kill                     64-bit atomicMin table per x-hit, vote pass (L183-200, Eq. 15)
-//   S4  u/v addition                   (survivor, pass, first-layer hit) items flattened the same way
-//                                      (Eq. 16); best combination by packed-key atomicMin
-//   S5  seed output                    thread per survivor: rebuild the winning combination, y fit, store
+//                                      lower/upper bound and closest-hit search into one lookup plus a
+//                                      short scan (about 0.6 hits per bin)
+//   S1  two-hit + three-hit search     per iteration: thread per T1 hit finds its T3 window (Eq. 8-11); a
+//                                      block scan flattens all pairs; each thread walks a contiguous chunk
+//                                      of pairs: Eq. 3-5 and the T2 band (Eq. 12-13, A3/A4); the triplets of
+//                                      both iterations go to one queue in shared memory
+//   S2  extension                      thread per queued triplet: exact parabola, +-1 mm closest hit in
+//                                      the other three x-layers, >= 5 hits -> queued candidate (L90)
+//   S2b fit                            dense pass over the candidates: fixed-matrix least squares, chi2 cut
+//   S3  clone kill                     64-bit atomicMin table per x-hit, vote pass (L183-200, Eq. 15);
+//                                      survivors are compacted to the bottom of the work region
+//   S4  u/v addition, iterative        (survivor, pass, first-layer hit) items flattened the same way
+//                                      (Eq. 16): phase A walks three stereo layers of every
+//                                      item, phase B finishes the walks that can still succeed
+//   S4h u/v addition, Hough clusters   (lhcb_set_uv_hough, L217, reading A20) votes as 64-bit masks per
+//                                      (survivor, layer), bit-sliced populations, hypothesis pass
+//   S5  y fit + seed output            thread per queued combination: y fit, best per survivor by
+//                                      packed-key atomicMin, the winner writes the seed
 //
 // Arithmetic: every formula follows DESIGN.md "Arithmetic specification" operation by operation;
 // this translation unit is compiled with -fmad=false so that no multiply-add is contracted.
