@@ -6,10 +6,13 @@
 //   P1  histogram over 24 zones x 256 x-bins (the bin is monotone in x)         one shared atomic per hit
 //   P2  exclusive scan of the 6,144 cells (24 per thread + block scan); the cells at the zone starts are
 //       the event's zone offsets
-//   P3  scatter (x, raw index, cell) into the cell's range                        one shared atomic per hit
-//   P4  thread per scattered hit: rank inside its cell (about 0.6 hits per cell at nominal occupancy) by
-//       the literal comparison (x, raw index) < (x', raw index'); hit_x and perm are written at cell start
-//       + rank, i.e. within a few elements of the thread's own position: nearly coalesced stores
+//   P3  scatter (x, raw index) into the cell's range                              one shared atomic per hit
+//   P4  thread per scattered hit: its zone from the 24 zone starts, its cell from x; rank inside the cell
+//       (about 0.6 hits per cell at nominal occupancy) by the literal comparison (x, raw index) <
+//       (x', raw index'); hit_x and perm are written at cell start + rank, i.e. within a few elements of the
+//       thread's own position: nearly coalesced stores
+// The 6,144 cell counters are 16-bit (an event has at most 65,535 hits), two per 32-bit word, so that four
+// 512-thread CTAs fit an SM at the nominal capacity.
 // Bins only group; the order is decided by exact float comparisons, so the output is bit-identical to a
 // stable sort whatever the rounding of the bin function.
 #pragma once
@@ -39,10 +42,19 @@ struct PrepParams {
 };
 
 __host__ __device__ inline size_t prep_smem_bytes(int max_hits) {
-  size_t b = (size_t)kPrepCells * 4 + 256;                       // cells, scan scratch, flags
+  size_t b = (size_t)kPrepCells * 2 + 512;                       // packed cells; scan scratch, zone starts, flag
   b += (((size_t)max_hits * 4 + 15) & ~(size_t)15);              // x by cell
-  b += 2 * (((size_t)max_hits * 2 + 15) & ~(size_t)15);          // raw index (event-local) and cell, by cell
+  b += (((size_t)max_hits * 2 + 15) & ~(size_t)15);              // raw index (event-local) by cell
   return b;
+}
+
+// 16-bit cell c lives in half (c & 1) of word c >> 1
+__device__ __forceinline__ unsigned int cell_add(unsigned int* cw, int c) {
+  const int sh = (c & 1) << 4;
+  return (atomicAdd(&cw[c >> 1], 1u << sh) >> sh) & 0xFFFFu;
+}
+__device__ __forceinline__ int cell_get(const unsigned int* cw, int c) {
+  return (int)((cw[c >> 1] >> ((c & 1) << 4)) & 0xFFFFu);
 }
 
 __device__ __forceinline__ int prep_cell(const PrepParams& p, float x, int zone) {
@@ -54,14 +66,13 @@ __device__ __forceinline__ int prep_cell(const PrepParams& p, float x, int zone)
 __global__ void __launch_bounds__(kPrepThreads)
 prepare_kernel(const __grid_constant__ PrepParams p) {
   extern __shared__ __align__(16) unsigned char smem[];
-  unsigned int* cnt = reinterpret_cast<unsigned int*>(smem);
-  int* warp_sums = reinterpret_cast<int*>(smem + (size_t)kPrepCells * 4);        // [kPrepThreads / 32 + 1]
-  int* flag = warp_sums + 48;
-  float* sx = reinterpret_cast<float*>(smem + (size_t)kPrepCells * 4 + 256);
+  unsigned int* cw = reinterpret_cast<unsigned int*>(smem);                       // kPrepCells / 2 words
+  int* warp_sums = reinterpret_cast<int*>(smem + (size_t)kPrepCells * 2);         // [kPrepThreads / 32 + 1]
+  int* zs = warp_sums + 40;                                                        // [25] zone starts in the event
+  int* flag = warp_sums + 72;
+  float* sx = reinterpret_cast<float*>(smem + (size_t)kPrepCells * 2 + 512);
   uint16_t* sidx = reinterpret_cast<uint16_t*>(reinterpret_cast<unsigned char*>(sx) +
                                                (((size_t)p.max_hits * 4 + 15) & ~(size_t)15));
-  uint16_t* scell = reinterpret_cast<uint16_t*>(reinterpret_cast<unsigned char*>(sidx) +
-                                                (((size_t)p.max_hits * 2 + 15) & ~(size_t)15));
   constexpr int T = kPrepThreads, per = kPrepCells / kPrepThreads;
   const int tid = threadIdx.x, e = blockIdx.x;
   const uint32_t b = p.raw_off[e];
@@ -69,7 +80,7 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
   uint32_t* zo = p.zone_off + (size_t)e * 24;
   if (e == p.n_events - 1 && tid == 0) p.zone_off[(size_t)p.n_events * 24] = b + (uint32_t)n;
   const bool too_many = n > p.max_hits || n > 65535;
-  for (int c = tid; c < kPrepCells; c += T) cnt[c] = 0u;
+  for (int c = tid; c < kPrepCells / 2; c += T) cw[c] = 0u;
   if (tid == 0) *flag = 0;
   __syncthreads();
   // P1
@@ -79,7 +90,7 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
       const float x = p.raw_x[b + i];
       const int z = p.raw_zone[b + i];
       if (z >= 24 || !(fabsf(x) <= 3.0e38f)) *flag = 1;          // invalid zone, NaN or infinity
-      else atomicAdd(&cnt[prep_cell(p, x, z)], 1u);
+      else cell_add(cw, prep_cell(p, x, z));
     }
   __syncthreads();
   if (too_many || *flag) {
@@ -94,35 +105,47 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
   }
   // P2
   {
+    static_assert(per % 2 == 0, "whole words per thread");
     unsigned int v[per];
     int sum = 0;
 #pragma unroll
-    for (int k = 0; k < per; ++k) { v[k] = cnt[tid * per + k]; sum += (int)v[k]; }
+    for (int k = 0; k < per / 2; ++k) {
+      const unsigned int w = cw[tid * (per / 2) + k];
+      v[2 * k] = w & 0xFFFFu; v[2 * k + 1] = w >> 16;
+      sum += (int)(v[2 * k] + v[2 * k + 1]);
+    }
     int total;
     int run = block_exscan<T>(sum, warp_sums, total);
 #pragma unroll
-    for (int k = 0; k < per; ++k) { cnt[tid * per + k] = (unsigned int)run; run += (int)v[k]; }
+    for (int k = 0; k < per / 2; ++k) {
+      const unsigned int lo = (unsigned int)run; run += (int)v[2 * k];
+      const unsigned int hi = (unsigned int)run; run += (int)v[2 * k + 1];
+      cw[tid * (per / 2) + k] = lo | (hi << 16);
+    }
   }
   __syncthreads();
-  if (tid < 24) zo[tid] = b + cnt[tid * kPrepBins];
+  if (tid < 24) { const int z0 = cell_get(cw, tid * kPrepBins); zs[tid] = z0; zo[tid] = b + (uint32_t)z0; }
+  if (tid == 24) zs[24] = n;
   if (tid == 0) p.status[e] = 0u;
   __syncthreads();
   // P3
 #pragma unroll 4
   for (int i = tid; i < n; i += T) {
     const float x = p.raw_x[b + i];
-    const int c = prep_cell(p, x, p.raw_zone[b + i]);
-    const unsigned int pos = atomicAdd(&cnt[c], 1u);
+    const unsigned int pos = cell_add(cw, prep_cell(p, x, p.raw_zone[b + i]));
     sx[pos] = x;
     sidx[pos] = (uint16_t)i;
-    scell[pos] = (uint16_t)c;
   }
   __syncthreads();
-  // P4: cnt[c] is now the end of cell c = the start of cell c + 1
+  // P4: the cell counters now hold the end of each cell = the start of the next one
   for (int q = tid; q < n; q += T) {
     const float x = sx[q];
-    const int i = sidx[q], c = scell[q];
-    const int start = c ? (int)cnt[c - 1] : 0, end = (int)cnt[c];
+    const int i = sidx[q];
+    int z = 0;                                               // largest z with zs[z] <= q  (zs ascending, zs[0] = 0)
+#pragma unroll
+    for (int st = 16; st > 0; st >>= 1) z = (z + st < 24 && zs[z + st] <= q) ? z + st : z;
+    const int c = prep_cell(p, x, z);
+    const int start = c ? cell_get(cw, c - 1) : 0, end = cell_get(cw, c);
     int rank = 0;
     for (int r = start; r < end; ++r) {
       const float xr = sx[r];
