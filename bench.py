@@ -100,7 +100,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--events", type=int, default=16384, help="events per GPU batch (cfg3: 16384)")
-    ap.add_argument("--cpu-sample", type=int, default=1024, help="events the oracle is timed on")
+    ap.add_argument("--cpu-sample", type=int, default=4096, help="events the oracle is timed on (about 17 s on one core)")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
