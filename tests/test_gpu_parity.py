@@ -142,7 +142,24 @@ def test_cfg3_full_size_bench_configuration(oracle32):
     assert cfgl["seed_threads"] == 256 and cfgl["match_threads"] == 128
     gs, gl = run_gpu(c, ev, True)
     assert (gs["status"] == 0).all() and (gl["status"] == 0).all(), "capacity overflow at nominal occupancy"
+    # properties that hold at any size, on the whole batch
+    zo = ev.zone_off.astype(np.int64)
+    hits = gs["hits"].astype(np.int64)
+    zbase = (gs["event"].astype(np.int64) * 2 + gs["half"]) * 12
+    for l in range(12):                                   # every hit of a seed lies in its own half's zone of that layer
+        h = hits[:, l]; has = h != 0xFFFFFFFF
+        assert ((h >= zo[zbase + l]) & (h < zo[zbase + l + 1]))[has].all()
+    nx = (hits[:, [0, 3, 4, 7, 8, 11]] != 0xFFFFFFFF).sum(1); nuv = (hits[:, [1, 2, 5, 6, 9, 10]] != 0xFFFFFFFF).sum(1)
+    assert np.array_equal(nx, gs["nx"]) and np.array_equal(nuv, gs["nuv"])
+    assert np.isin(nx, (5, 6)).all() and np.isin(nuv, (4, 5, 6)).all()              # L90, A9
+    assert (gs["par"][:, 5] <= 8.0).all() and (gs["par"][:, 6] <= 8.0).all()        # chi2 cuts (A6)
+    assert len({(int(e), int(h)) + tuple(r) for e, h, r in zip(gs["event"], gs["half"], hits.tolist())}) == gs["n"]
+    assert (gl["chi2"] < 2.0).all() and (gl["n_ut"] >= 3).all()                     # L301, L311
+    assert len(np.unique(gl["seed"])) == gl["n"] and len(np.unique(gl["velo"])) == gl["n"]   # one-to-one (A14)
+    vo = ev.velo_off.astype(np.int64)
+    assert ((gl["velo"] >= vo[gl["event"]]) & (gl["velo"] < vo[gl["event"] + 1])).all()
     ms, ml = c.max_seeds, c.max_long
+    assert (gl["seed"] // (2 * ms) == gl["event"]).all()                             # a long track's seed is of its event
     sample = [0, 1, 63, 64, 1023, 4097, 8191, 12345, 16320, 16383] + list(range(5000, 5022))
     n_s = n_l = 0
     for e in sample:
