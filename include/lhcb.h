@@ -90,7 +90,7 @@ typedef struct {
   int32_t max_hits_per_half;                   /* [6144] SciFi hits staged per event-half (<= 32768) */
   int32_t max_triplets_per_half;               /* [4096] three-hit combinations per half, both iterations together (the queue also takes the
                                                   room a half leaves unused below max_hits_per_half) */
-  int32_t max_match_cand_per_event;            /* [384]  chi2-accepted seed-VELO pairs per event */
+  int32_t max_match_cand_per_event;            /* [384]  chi2-accepted seed-VELO pairs per event (>= 256) */
   int32_t max_velo_per_event;                  /* [512] */
   int32_t max_ut_per_event;                    /* [6144] UT hits staged in shared memory per event; events with
                                                   more are searched in global memory (slower, same result) */

@@ -3,9 +3,9 @@
 // One CTA per event.  The event's VELO states are staged in shared memory; the x0 of the event's UT
 // hits (four sorted layers, contiguous in memory) is fetched with one bulk async copy that lands while
 // the all-pairs loop runs, so the UT searches are shared-memory binary searches.
-//   M0     VELO states are rank-sorted by t_y into shared memory
+//   M0     VELO states are counting-sorted into 256 t_y bins in shared memory
 //   M1/M2  "all seed x VELO pairs" (L279) without touching most of them: the |dty| cut of Eq. 21 selects
-//          a contiguous range of the t_y-sorted VELO states (found by binary search with a safety
+//          a contiguous range of the t_y-binned VELO states (the bins of the window edges, with a safety
 //          margin; the literal cut is still applied to every pair in the range, so the accepted set
 //          is exactly that of the exhaustive loop).  Pairs in range are flattened over the CTA:
 //          kink extrapolation (Eq. 17-18), preselection (Eq. 21), chi2_match (Eq. 22-23) < 2; accepted
@@ -26,6 +26,8 @@
 
 namespace lhcb {
 
+
+constexpr int kTyBins = 256;                 // t_y bins of the VELO states (counting sort of M0)
 
 struct MatchParams {
   float zS, zV, dzyS, dzyV, mag[5], presel[4], cx0, cx1, cy0, cy1, inv_tol_tx, inv_tol_ty, chi2m_max;
@@ -73,7 +75,7 @@ __host__ __device__ inline size_t match_smem_bytes(int kMatchThreads, int max_se
   size_t b = 64;
   b += ((size_t)max_ut + 8) * 4;             // UT x0 tile (16-byte aligned superset)
   b += (size_t)max_velo * 16;                // VELO states, sorted by ty
-  b += (size_t)max_velo * 4;                 // unsorted ty (rank sort input)
+  b += (size_t)(kTyBins + 1) * 4;            // start of each t_y bin of the VELO states
   b += (size_t)max_velo * 2;                 // original index of each sorted state
   b = (b + 15) & ~(size_t)15;
   b += (kMatchThreads + 1) * 4 + kMatchThreads * 2 + 64;   // work-list scan scratch
@@ -209,9 +211,9 @@ matching_kernel(const __grid_constant__ MatchParams p) {
   float* svy = svx + p.max_velo;
   float* svtx = svy + p.max_velo;
   float* svty = svtx + p.max_velo;
-  float* tmp_ty = svty + p.max_velo;
-  uint16_t* sorig = reinterpret_cast<uint16_t*>(tmp_ty + p.max_velo);
-  size_t off = 64 + ((size_t)p.max_ut + 8) * 4 + (size_t)p.max_velo * 22;
+  int* vbin = reinterpret_cast<int*>(svty + p.max_velo);                  // [kTyBins + 1]
+  uint16_t* sorig = reinterpret_cast<uint16_t*>(vbin + kTyBins + 1);
+  size_t off = 64 + ((size_t)p.max_ut + 8) * 4 + (size_t)p.max_velo * 18 + (size_t)(kTyBins + 1) * 4;
   off = (off + 15) & ~(size_t)15;
   int* offs = reinterpret_cast<int*>(smem + off);                         // [kMatchThreads + 1]
   uint16_t* firsts = reinterpret_cast<uint16_t*>(offs + kMatchThreads + 1);
@@ -284,17 +286,33 @@ matching_kernel(const __grid_constant__ MatchParams p) {
       hdr[4 + tid] = (int)p.ut_off[(size_t)e * 4 + tid];
     }
   }
-  for (int v = tid; v < nv; v += kMatchThreads) { tmp_ty[v] = p.vty[v0 + v]; velo_best[v] = kNoKey; }
+  // t_y bin of a VELO state or of a window edge: monotone in t, so the states with t in [a, b] lie in the bins
+  // [bin(a), bin(b)] whatever the rounding; values outside +-0.4 land in the edge bins
+  auto ty_bin = [](float t) { return (int)fminf(fmaxf((t + 0.4f) * ((float)kTyBins / 0.8f), 0.f), (float)(kTyBins - 1)); };
+  int* vcur = reinterpret_cast<int*>(hyq);                                 // [kTyBins] scatter cursors (hyq is free until M3)
+  for (int v = tid; v < nv; v += kMatchThreads) velo_best[v] = kNoKey;
   for (int s = tid; s < ns; s += kMatchThreads) seed_best[s] = kNoKey;
+  for (int b = tid; b <= kTyBins; b += kMatchThreads) vbin[b] = 0;
   __syncthreads();
-  // ---- M0: rank sort of the VELO states by ty (ties by index) ---------------------------------
+  // ---- M0: counting sort of the VELO states into t_y bins (order inside a bin is irrelevant: the bins
+  // only delimit, per seed, a superset of the states that can pass the |dty| cut of Eq. 21) -----------
+  for (int v = tid; v < nv; v += kMatchThreads) atomicAdd(&vbin[ty_bin(p.vty[v0 + v]) + 1], 1);
+  __syncthreads();
+  {
+    constexpr int per = kTyBins / kMatchThreads;
+    static_assert(per * kMatchThreads == kTyBins, "whole bins per thread");
+    int c[per], sum = 0;
+#pragma unroll
+    for (int k = 0; k < per; ++k) { c[k] = vbin[tid * per + k + 1]; sum += c[k]; }
+    int total;
+    int run = block_exscan<kMatchThreads>(sum, warp_sums, total);
+#pragma unroll
+    for (int k = 0; k < per; ++k) { vcur[tid * per + k] = run; run += c[k]; vbin[tid * per + k + 1] = run; }
+  }
+  __syncthreads();
   for (int v = tid; v < nv; v += kMatchThreads) {
-    const float t = tmp_ty[v];
-    int r = 0;
-    for (int u = 0; u < nv; ++u) {
-      const float tu = tmp_ty[u];
-      r += (tu < t || (tu == t && u < v)) ? 1 : 0;
-    }
+    const float t = p.vty[v0 + v];
+    const int r = atomicAdd(&vcur[ty_bin(t)], 1);
     svx[r] = p.vx[v0 + v]; svy[r] = p.vy[v0 + v]; svtx[r] = p.vtx[v0 + v]; svty[r] = t;
     sorig[r] = (uint16_t)v;
   }
@@ -313,10 +331,8 @@ matching_kernel(const __grid_constant__ MatchParams p) {
       const float tyS = p.state[3 * sct + slot];
       // superset of {v : |tyS - tyV| < presel[3]} whatever the rounding of the subtraction
       const float w = p.presel[3] + 1e-6f * (fabsf(tyS) + p.presel[3]) + 1e-30f;
-      fst = lower_bound(svty, 0, nv, tyS - w);
-      int lst = fst;
-      { int n = nv - fst; const float hi = tyS + w;
-        while (n > 0) { const int hh = n >> 1; const bool le = svty[lst + hh] <= hi; lst = le ? lst + hh + 1 : lst; n = le ? n - hh - 1 : hh; } }
+      fst = vbin[ty_bin(tyS - w)];
+      const int lst = vbin[ty_bin(tyS + w) + 1];
       cnt = lst - fst;
     }
     int total;
