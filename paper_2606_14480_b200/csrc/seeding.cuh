@@ -3,9 +3,9 @@
 // One CTA per event-half (L372): the half's twelve sorted hit zones are staged into shared memory
 // with one bulk async copy (cp.async.bulk + mbarrier) and stay there for every step (L370).
 // Stages, separated by __syncthreads():
-//   S0  staging + bin tables           per zone, a 256-bin table "first hit with bin >= k" turns every
+//   S0  staging + bin tables           per zone, a 320-bin table "first hit with bin >= k" turns every
 //                                      lower/upper bound and closest-hit search into one lookup plus a
-//                                      short scan (about 0.6 hits per bin)
+//                                      short scan (about 0.5 hits per bin)
 //   S1  two-hit + three-hit search     per iteration: thread per T1 hit finds its T3 window (Eq. 8-11); a
 //                                      block scan flattens all pairs; each thread walks a contiguous chunk
 //                                      of pairs: Eq. 3-5 and the T2 band (Eq. 12-13, A3/A4); the triplets of
@@ -32,8 +32,11 @@
 
 namespace lhcb {
 
+#ifndef LHCB_PROBES
+#define LHCB_PROBES 3     // hits probed without a branch by closest_hit
+#endif
 #ifndef LHCB_LUT_BINS
-#define LHCB_LUT_BINS 256
+#define LHCB_LUT_BINS 320
 #endif
 constexpr int kSeedThreadsMax = 512;          // the kernel is instantiated for 256 x 4 CTAs/SM and 512 x 2 CTAs/SM
 constexpr int kLutBins = LHCB_LUT_BINS;       // bins of the per-zone search table
@@ -218,7 +221,7 @@ __device__ __forceinline__ int closest_hit(const float* __restrict__ x, const ui
   int best = -1;
   float bd = 0.f, xlast = 0.f;
 #pragma unroll
-  for (int k = 0; k < 3; ++k) {
+  for (int k = 0; k < LHCB_PROBES; ++k) {
     const float v = x[i0 + k];                               // at most 3 floats past the zone: still shared memory
     const float xi = i0 + k < z.e ? v : __int_as_float(0x7f800000);
     const float d = fabsf(xi - xp);
@@ -227,7 +230,7 @@ __device__ __forceinline__ int closest_hit(const float* __restrict__ x, const ui
     xlast = xi;
   }
   if (xlast <= hi) {
-    int i = i0 + 3;
+    int i = i0 + LHCB_PROBES;
     while (i < z.e) {
       const float xi = x[i];
       if (xi > hi) break;
