@@ -6,8 +6,8 @@
 //   P1  histogram over 24 zones x 256 x-bins (the bin is monotone in x)         one shared atomic per hit
 //   P2  exclusive scan of the 6,144 cells (24 per thread + block scan); the cells at the zone starts are
 //       the event's zone offsets
-//   P3  scatter (x, raw index) into the cell's range                              one shared atomic per hit
-//   P4  thread per scattered hit: its zone from the 24 zone starts, its cell from x; rank inside the cell
+//   P3  scatter (x, raw index, zone) into the cell's range                        one shared atomic per hit
+//   P4  thread per scattered hit: its cell from its zone and x; rank inside the cell
 //       (about 0.6 hits per cell at nominal occupancy) by the literal comparison (x, raw index) <
 //       (x', raw index'); hit_x and perm are written at cell start + rank, i.e. within a few elements of the
 //       thread's own position: nearly coalesced stores
@@ -24,7 +24,10 @@
 namespace lhcb {
 
 constexpr int kPrepThreads = 512;
-constexpr int kPrepBins = 256;                    // x bins per zone
+#ifndef LHCB_PREP_BINS
+#define LHCB_PREP_BINS 256
+#endif
+constexpr int kPrepBins = LHCB_PREP_BINS;         // x bins per zone
 constexpr int kPrepCells = 24 * kPrepBins;        // 24 cells per thread
 static_assert(kPrepCells % kPrepThreads == 0, "whole cells per thread");
 
@@ -45,6 +48,7 @@ __host__ __device__ inline size_t prep_smem_bytes(int max_hits) {
   size_t b = (size_t)kPrepCells * 2 + 512;                       // packed cells; scan scratch, zone starts, flag
   b += (((size_t)max_hits * 4 + 15) & ~(size_t)15);              // x by cell
   b += (((size_t)max_hits * 2 + 15) & ~(size_t)15);              // raw index (event-local) by cell
+  b += (((size_t)max_hits + 15) & ~(size_t)15);                  // zone by cell
   return b;
 }
 
@@ -68,11 +72,11 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
   extern __shared__ __align__(16) unsigned char smem[];
   unsigned int* cw = reinterpret_cast<unsigned int*>(smem);                       // kPrepCells / 2 words
   int* warp_sums = reinterpret_cast<int*>(smem + (size_t)kPrepCells * 2);         // [kPrepThreads / 32 + 1]
-  int* zs = warp_sums + 40;                                                        // [25] zone starts in the event
   int* flag = warp_sums + 72;
   float* sx = reinterpret_cast<float*>(smem + (size_t)kPrepCells * 2 + 512);
   uint16_t* sidx = reinterpret_cast<uint16_t*>(reinterpret_cast<unsigned char*>(sx) +
                                                (((size_t)p.max_hits * 4 + 15) & ~(size_t)15));
+  uint8_t* szone = reinterpret_cast<uint8_t*>(sidx) + (((size_t)p.max_hits * 2 + 15) & ~(size_t)15);
   constexpr int T = kPrepThreads, per = kPrepCells / kPrepThreads;
   const int tid = threadIdx.x, e = blockIdx.x;
   const uint32_t b = p.raw_off[e];
@@ -124,26 +128,25 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
     }
   }
   __syncthreads();
-  if (tid < 24) { const int z0 = cell_get(cw, tid * kPrepBins); zs[tid] = z0; zo[tid] = b + (uint32_t)z0; }
-  if (tid == 24) zs[24] = n;
+  if (tid < 24) zo[tid] = b + (uint32_t)cell_get(cw, tid * kPrepBins);
   if (tid == 0) p.status[e] = 0u;
   __syncthreads();
   // P3
 #pragma unroll 4
   for (int i = tid; i < n; i += T) {
     const float x = p.raw_x[b + i];
-    const unsigned int pos = cell_add(cw, prep_cell(p, x, p.raw_zone[b + i]));
+    const int z = p.raw_zone[b + i];
+    const unsigned int pos = cell_add(cw, prep_cell(p, x, z));
     sx[pos] = x;
     sidx[pos] = (uint16_t)i;
+    szone[pos] = (uint8_t)z;
   }
   __syncthreads();
   // P4: the cell counters now hold the end of each cell = the start of the next one
   for (int q = tid; q < n; q += T) {
     const float x = sx[q];
     const int i = sidx[q];
-    int z = 0;                                               // largest z with zs[z] <= q  (zs ascending, zs[0] = 0)
-#pragma unroll
-    for (int st = 16; st > 0; st >>= 1) z = (z + st < 24 && zs[z + st] <= q) ? z + st : z;
+    const int z = szone[q];
     const int c = prep_cell(p, x, z);
     const int start = c ? cell_get(cw, c - 1) : 0, end = cell_get(cw, c);
     int rank = 0;
