@@ -231,8 +231,11 @@ int lhcb_seeding(lhcb_ctx* ctx, const lhcb_events_t* events, lhcb_seeds_t* out, 
                  void* cuda_stream);
 
 /* Matching: kink extrapolation, preselection, chi2_match, UT hit search, one-to-one selection
- * (section 4).  `ut` may be NULL (no UT in the data taking, L307).  Only seeds->count and
- * seeds->state are read. */
+ * (section 4).  `ut` may be NULL (no UT in the data taking, L307).  Of the seeds, count and state are
+ * read; nx / nuv if given and a ghost network is set; hits if given: two seeds with bit-identical states
+ * (twins from duplicate hits at the same x) tie exactly in chi2_match, and the tie is decided by their hit
+ * lists in lexicographic order (layer 0 first), without hit lists by the lower slot (reading A21),
+ * so the set of long tracks does not depend on the order in which lhcb_seeding wrote the seeds. */
 int lhcb_matching(lhcb_ctx* ctx, const lhcb_seeds_t* seeds, const lhcb_velo_t* velo, const lhcb_ut_t* ut,
                   lhcb_long_t* out, void* workspace, void* cuda_stream);
 

@@ -111,8 +111,11 @@ class Oracle:
         return dict(n=n, event=o_event[:n], half=o_half[:n], state=o_state[:n], par=o_par[:n], hits=o_hits[:n],
                     nx=o_nx[:n], nuv=o_nuv[:n], counters=dict(zip(COUNTER_NAMES, cnt.tolist())))
 
-    def matching(self, n_events, seed_off, state, ev, use_ut=True, cap: int | None = None, nn=None, nhits=None):
+    def matching(self, n_events, seed_off, state, ev, use_ut=True, cap: int | None = None, nn=None, nhits=None,
+                 hits=None):
         """seed_off u32[n_events+1], state [n][5]; VELO/UT/polarity from ev.
+        hits: u32 [n][12] hit indices of the seeds (exact chi2 ties between twin seeds are then broken by the
+        hit lists, reading A21) or None (ties to the lower seed index).
         nn: the 339 packed values of the ghost-killing network (reading A14b) or None (A14: chi2 ranking);
         nhits: u8 per seed (nHits_SciFi), None = 12."""
         cap = cap or max(1024, 400 * n_events)
@@ -154,7 +157,8 @@ class Oracle:
                                   _p(uh, self.creal), _p(pol, C.c_int8), C.c_int64(cap), _p(o_event, C.c_int32),
                                   _p(o_seed, C.c_uint32), _p(o_velo, C.c_uint32), _p(o_ut, C.c_uint32),
                                   _p(o_nut, C.c_uint8), _p(o_qop, self.creal), _p(o_chi2, self.creal),
-                                  _p(cnt, C.c_uint64))
+                                  _p(cnt, C.c_uint64),
+                                  _p(np.ascontiguousarray(hits, np.uint32), C.c_uint32) if hits is not None else None)
         if n > cap:
             raise RuntimeError(f"oracle long-track capacity {cap} < {n}")
         return dict(n=n, event=o_event[:n], seed=o_seed[:n], velo=o_velo[:n], ut=o_ut[:n], n_ut=o_nut[:n],
@@ -165,7 +169,7 @@ class Oracle:
         s = self.seeding(ev)
         seed_off = np.zeros(ev.n_events + 1, np.uint32)
         np.cumsum(np.bincount(s["event"], minlength=ev.n_events), out=seed_off[1:])
-        m = self.matching(ev.n_events, seed_off, s["state"], ev, use_ut=use_ut)
+        m = self.matching(ev.n_events, seed_off, s["state"], ev, use_ut=use_ut, hits=s["hits"])
         return s, m
 
     def set_uv_hough(self, on: bool):

@@ -6,7 +6,7 @@
  * constant generator with the CUDA path under paper_2606_14480_b200/ and neither includes the other.
  *
  * What it is: the paper's algorithm written out step by step (PAPER.md sections 3 and 4), in the
- * order and notation of the paper, with the readings DESIGN.md lists (A1..A17) where the paper is
+ * order and notation of the paper, with the readings DESIGN.md lists (A1..A21) where the paper is
  * silent or garbled.  Searches are linear scans with the literal predicate; there is no binary
  * search, no blocking, no fusion.  Steps are labelled O1..O14 as in DESIGN.md.
  *
@@ -767,6 +767,21 @@ static REAL ghost_prob(const REAL* nn, const REAL* in /* [8] */) {
 typedef struct { int seed, velo; REAL chi2, qop, ghost; int n_ut; uint32_t ut[NUT]; int alive; } mcand_t;
 typedef VEC(mcand_t) vmc;
 
+/* A21: order of two seeds whose candidates tie exactly in chi2_match (twin seeds: bit-identical states from
+ * duplicate hits at the same x).  The seed whose twelve hit indices (layer 0 first, NO_HIT = largest) come
+ * first in lexicographic order wins; seeds without hit lists (or with equal ones) fall back to the seed index.
+ * Unlike the index, the hit list does not depend on the order in which the seeds were written. */
+static int seed_before(const uint32_t* seed_hits, int a, int b) {
+  if (seed_hits) {
+    int l;
+    for (l = 0; l < NL; l++) {
+      uint32_t ha = seed_hits[(size_t)a * NL + l], hb = seed_hits[(size_t)b * NL + l];
+      if (ha != hb) return ha < hb;
+    }
+  }
+  return a < b;
+}
+
 /* Matching over a batch.  Seeds: per-event offsets seed_off[n_events+1] into state[n][5].
  * ut_off may be NULL (no UT).  Returns number of long tracks (only cap written). */
 static int64_t matching_impl(const orc_ctx* C, int n_events, const uint32_t* seed_off, const REAL* state,
@@ -775,7 +790,7 @@ static int64_t matching_impl(const orc_ctx* C, int n_events, const uint32_t* see
                      const int8_t* polarity, int64_t cap, int32_t* o_event, uint32_t* o_seed, uint32_t* o_velo,
                      uint32_t* o_ut /* [n][4] */, uint8_t* o_nut, REAL* o_qop, REAL* o_chi2, uint64_t* counters,
                      const uint8_t* seed_nhits /* per seed, NULL = 12 */, const REAL* nn /* NULL = A14 */,
-                     REAL* o_ghost /* may be NULL */) {
+                     REAL* o_ghost /* may be NULL */, const uint32_t* seed_hits /* [n][12] or NULL (A21) */) {
   uint64_t cnt[C_N] = { 0 };
   vmc mc = { 0 };
   int64_t n_out = 0; int e; size_t i;
@@ -844,7 +859,8 @@ static int64_t matching_impl(const orc_ctx* C, int n_events, const uint32_t* see
       if (!mc.p[i].alive) continue;
       for (j = 0; j < mc.n; j++) {
         if (j == i || !mc.p[j].alive || mc.p[j].velo != mc.p[i].velo) continue;
-        if (mc.p[j].chi2 < mc.p[i].chi2 || (mc.p[j].chi2 == mc.p[i].chi2 && mc.p[j].seed < mc.p[i].seed))
+        if (mc.p[j].chi2 < mc.p[i].chi2 ||
+            (mc.p[j].chi2 == mc.p[i].chi2 && seed_before(seed_hits, mc.p[j].seed, mc.p[i].seed)))
           lose = 1;
       }
       if (lose) mc.p[i].alive = 2;                          /* mark, do not change the survivor set mid-pass */
@@ -872,9 +888,10 @@ int64_t orc_matching(const orc_ctx* C, int n_events, const uint32_t* seed_off, c
                      const uint32_t* velo_off, const REAL* vx, const REAL* vy, const REAL* vtx, const REAL* vty,
                      const uint32_t* ut_off, const REAL* ux, const REAL* uylo, const REAL* uyhi,
                      const int8_t* polarity, int64_t cap, int32_t* o_event, uint32_t* o_seed, uint32_t* o_velo,
-                     uint32_t* o_ut /* [n][4] */, uint8_t* o_nut, REAL* o_qop, REAL* o_chi2, uint64_t* counters) {
+                     uint32_t* o_ut /* [n][4] */, uint8_t* o_nut, REAL* o_qop, REAL* o_chi2, uint64_t* counters,
+                     const uint32_t* seed_hits /* [n][12] or NULL: tie-break of reading A21 */) {
   return matching_impl(C, n_events, seed_off, state, velo_off, vx, vy, vtx, vty, ut_off, ux, uylo, uyhi, polarity, cap,
-                       o_event, o_seed, o_velo, o_ut, o_nut, o_qop, o_chi2, counters, NULL, NULL, NULL);
+                       o_event, o_seed, o_velo, o_ut, o_nut, o_qop, o_chi2, counters, NULL, NULL, NULL, seed_hits);
 }
 
 /* The same with the ghost-killing network in place of the chi2 ranking (A14b).  nn: NN_SIZE packed values. */
@@ -885,7 +902,7 @@ int64_t orc_matching_nn(const orc_ctx* C, int n_events, const uint32_t* seed_off
                         uint32_t* o_ut, uint8_t* o_nut, REAL* o_qop, REAL* o_chi2, uint64_t* counters,
                         const uint8_t* seed_nhits, const REAL* nn, REAL* o_ghost) {
   return matching_impl(C, n_events, seed_off, state, velo_off, vx, vy, vtx, vty, ut_off, ux, uylo, uyhi, polarity, cap,
-                       o_event, o_seed, o_velo, o_ut, o_nut, o_qop, o_chi2, counters, seed_nhits, nn, o_ghost);
+                       o_event, o_seed, o_velo, o_ut, o_nut, o_qop, o_chi2, counters, seed_nhits, nn, o_ghost, NULL);
 }
 
 /* Hough-cluster UV seeding (reading A20) on / off; the default is the iterative version (L204) */

@@ -358,6 +358,7 @@ class Context:
         out["state"].copy_(t.from_numpy(st)); out["count"].copy_(t.from_numpy(count))
         out["status"].zero_()
         out["nx"].fill_(6); out["nuv"].fill_(6)             # states without hits count as full 12-hit seeds (nHits_SciFi input)
+        out["hits"] = None; out["par"] = None               # no hit lists: chi2 ties go to the lower seed index (A21)
         return out, slot
 
     def seeds_to_host(self, s):

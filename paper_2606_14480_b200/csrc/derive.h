@@ -82,6 +82,12 @@ inline int derive(const lhcb_geom_t& g, lhcb_derived_t& D) {
   if (g.min_x_hits < 5 || g.min_x_hits > 6 || g.min_uv_hits < 2 || g.min_uv_hits > 6) return LHCB_ERR_BAD_GEOMETRY;
   if (!(g.sigma_hit > 0) || !(g.kappa_cx != 0) || !(g.kick_pt != 0) || g.gamma_ab[1] == 0)
     return LHCB_ERR_BAD_GEOMETRY;
+  for (int pp = 0; pp < 2; ++pp) {                           // first layer of each UV pass: a stereo layer
+    const int lf = g.uv_first_layer[pp];
+    if (lf < 0 || lf >= 12 || g.scifi_tan_alpha[lf] == 0.0f) return LHCB_ERR_BAD_GEOMETRY;
+  }
+  if (g.min_ut_hits < 1 || g.min_ut_hits > 4) return LHCB_ERR_BAD_GEOMETRY;
+  if (!(g.y_max > 0) || !(g.y_min < 0) || !(g.y_half_tol >= 0)) return LHCB_ERR_BAD_GEOMETRY;
   const double zref = g.z_ref, dr = g.d_ratio;
   for (int l = 0; l < 12; ++l) {
     const double z = g.scifi_z[l], zb = z - zref, ta = g.scifi_tan_alpha[l];
@@ -109,6 +115,8 @@ inline int derive(const lhcb_geom_t& g, lhcb_derived_t& D) {
     const double ratio = z1 / (z3 - z1);
     const double acorr = (double)g.alpha0 / (ratio * (pmin - (double)g.alpha1));  // Eq. 9-10
     const double K = (g2 - g1) - (z2 - z1) / (z3 - z1) * (g3 - g1);              // reading A3
+    if (!std::isfinite(dx3) || !std::isfinite(acorr) || !std::isfinite(K) || K == 0.0)
+      return LHCB_ERR_BAD_GEOMETRY;                          // e.g. p_min below the real root of Eq. 8
     D.l1[it] = l1; D.l2[it] = l2; D.l3[it] = l3;
     D.dx3max[it] = (float)dx3;
     D.alpha_corr[it] = (float)acorr;

@@ -75,7 +75,8 @@ void fill_seed_params(const lhcb_ctx* c, lhcb::SeedParams& p) {
   // from the float geometry, rounded once
   {
     const double zmin = (double)g.scifi_z[D.ul[0]], tol = std::fabs((double)g.y_half_tol);
-    const double range = ((double)g.y_max + tol) / zmin;
+    const double range = ((double)g.y_max + tol) / zmin;       // the lower half spans [y_min, tol]: the same width when
+                                                               // y_min = -y_max; wider halves land in the edge bins
     p.uv_hough = c->uv_hough;
     p.h_tlo[0] = (float)(-tol / zmin); p.h_tlo[1] = (float)((double)g.y_min / zmin);
     p.h_w = (float)(range / 64.0); p.h_invw = (float)(64.0 / range);
@@ -279,6 +280,7 @@ int lhcb_matching(lhcb_ctx* c, const lhcb_seeds_t* seeds, const lhcb_velo_t* vel
   p.count = out->count; p.seed_idx = out->seed_idx; p.velo_idx = out->velo_idx; p.ut_idx = out->ut_idx;
   p.n_ut = out->n_ut; p.qop = out->qop; p.chi2 = out->chi2; p.status = out->status;
   p.nn = c->nn_on ? c->d_nn : nullptr; p.snx = seeds->nx; p.snuv = seeds->nuv; p.ghost = out->ghost;
+  p.shits = seeds->hits;
   p.long_cap_total = (size_t)velo->n_events * (size_t)c->geom.max_long_per_event;
   if (c->match_threads == 128)
     lhcb::matching_kernel<128, 6><<<velo->n_events, 128, c->match_smem, (cudaStream_t)stream>>>(p);

@@ -59,6 +59,7 @@ struct MatchParams {
   const float* nn;
   const uint8_t *snx, *snuv;
   float* ghost;
+  const uint32_t* shits;    // [12][seed_cap_total] hit indices of the seeds or NULL (tie-break of reading A21)
 };
 
 struct __align__(8) MatchCand {
@@ -204,7 +205,7 @@ template <int kMatchThreads, int MIN_CTAS>
 __global__ void __launch_bounds__(kMatchThreads, MIN_CTAS)
 matching_kernel(const __grid_constant__ MatchParams p) {
   extern __shared__ __align__(16) unsigned char smem[];
-  int* hdr = reinterpret_cast<int*>(smem);                  // [0] n_mc, [1] n_long, [2] status, [3] n_hyp, [4..8] UT offsets
+  int* hdr = reinterpret_cast<int*>(smem);                  // [0] n_mc, [1] n_long, [2] status, [3] n_hyp, [4..8] UT offsets, [9] tie flag
   unsigned long long* mbar = reinterpret_cast<unsigned long long*>(smem + 48);
   float* sux = reinterpret_cast<float*>(smem + 64);
   float* svx = sux + p.max_ut + 8;
@@ -242,6 +243,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     return;
   }
   if (tid < 4) hdr[tid] = 0;
+  if (tid == 4) hdr[9] = 0;                                  // chi2 tie seen (reading A21)
   // ---- UT x0 of this event: one bulk copy, overlapped with the all-pairs loop -----------------
   uint32_t u_begin = 0, u_end = 0, ua0 = 0, ua1 = 0;
   bool ut_in_smem = false;
@@ -521,6 +523,40 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     atomicMin(&velo_best[sorig[m.velo]], cb | m.seed);
   }
   __syncthreads();
+  // Reading A21: an exact chi2 tie between two seeds for one VELO state (twin seeds: bit-identical states
+  // from duplicate hits) is decided by the seeds' hit lists, not by their slot order.  Ties are detected by
+  // every thread; the (rare) event that has one resolves it serially.
+  for (int k = tid; k < nm; k += kMatchThreads) {
+    const MatchCand& m = mc[k];
+    if ((m.key >> 50) > key_ok) continue;
+    const unsigned long long cb = (unsigned long long)__float_as_uint(m.chi2) << 32;
+    if (seed_best[m.seed] != (cb | sorig[m.velo])) continue;
+    const unsigned long long vb = velo_best[sorig[m.velo]];
+    if ((vb >> 32) == (cb >> 32) && (uint32_t)vb != (uint32_t)m.seed) hdr[9] = 1;
+  }
+  __syncthreads();
+  if (hdr[9]) {
+    if (tid == 0) {
+      auto slot_of = [&](int s) { return s < c0 ? (size_t)(2 * e) * p.max_seeds + s : (size_t)(2 * e + 1) * p.max_seeds + (s - c0); };
+      auto before = [&](int a, int b) {                        // hit lists in lexicographic order, then the index
+        if (p.shits)
+          for (int l = 0; l < 12; ++l) {
+            const uint32_t ha = p.shits[(size_t)l * sct + slot_of(a)], hb = p.shits[(size_t)l * sct + slot_of(b)];
+            if (ha != hb) return ha < hb;
+          }
+        return a < b;
+      };
+      for (int k = 0; k < nm; ++k) {
+        const MatchCand& m = mc[k];
+        if ((m.key >> 50) > key_ok) continue;
+        const unsigned long long cb = (unsigned long long)__float_as_uint(m.chi2) << 32;
+        if (seed_best[m.seed] != (cb | sorig[m.velo])) continue;
+        const unsigned long long vb = velo_best[sorig[m.velo]];
+        if ((vb >> 32) == (cb >> 32) && before((int)m.seed, (int)(uint32_t)vb)) velo_best[sorig[m.velo]] = cb | m.seed;
+      }
+    }
+    __syncthreads();
+  }
   }
   const int pol = p.pol ? (int)p.pol[e] : p.polarity;
   for (int k = tid; k < nm; k += kMatchThreads) {

@@ -4,19 +4,9 @@ import numpy as np
 NO_HIT = 0xFFFFFFFF
 
 
-class SeedKey(tuple):
-    """(event, half, 12 hit indices) -- the identity of a seed -- plus, optionally, the bytes of its state."""
-    alt = None
-
-
 def seed_keys(event, half, hits, state=None):
-    out = []
-    for i, (e, h, row) in enumerate(zip(event, half, hits)):
-        k = SeedKey((int(e), int(h)) + tuple(int(x) for x in row))
-        if state is not None:
-            k.alt = (int(e), np.ascontiguousarray(state[i], np.float32).tobytes())
-        out.append(k)
-    return out
+    """(event, half, 12 hit indices): the identity of a seed (`state` is accepted and ignored)."""
+    return [(int(e), int(h)) + tuple(int(x) for x in row) for e, h, row in zip(event, half, hits)]
 
 
 def compare_seeds(orc, gpu, rtol=1e-4, x_atol=5e-3):
@@ -57,24 +47,10 @@ def compare_long(orc_m, gpu_m, orc_seed_key, gpu_seed_key):
     ko = long_keys(orc_m, orc_seed_key); kg = long_keys(gpu_m, gpu_seed_key)
     io = {k: i for i, k in enumerate(ko)}; ig = {k: i for i, k in enumerate(kg)}
     assert len(io) == len(ko) and len(ig) == len(kg)
+    # strict: since reading A21 (exact chi2 ties between twin seeds are decided by their hit lists) the set of
+    # long tracks is unique, whatever the order in which the seeds were written
     common = [(k, k) for k in ko if k in ig]
     only_orc = [k for k in ko if k not in ig]; only_gpu = [k for k in kg if k not in io]
-    # Where several results are correct, compare what is unique: two seeds of an event with bit-identical
-    # states (duplicate hits at the same x give twin candidates that the clone kill keeps, equal keys) tie
-    # exactly in chi2_match, and which twin carries the long track depends on the unspecified order of the
-    # seeds.  Leftovers are therefore paired by (seed state, VELO, UT hits).
-    if only_orc and only_gpu:
-        def alt(k):
-            return (k[0].alt,) + tuple(k[1:]) if getattr(k[0], "alt", None) is not None else None
-        pool = {}
-        for k in only_gpu:
-            if alt(k) is not None:
-                pool.setdefault(alt(k), []).append(k)
-        for k in list(only_orc):
-            m = pool.get(alt(k)) if alt(k) is not None else None
-            if m:
-                g = m.pop()
-                common.append((k, g)); only_orc.remove(k); only_gpu.remove(g)
     a = np.array([io[k] for k, _ in common], np.int64); b = np.array([ig[g] for _, g in common], np.int64)
     res = dict(n_orc=len(ko), n_gpu=len(kg), n_common=len(common), only_orc=only_orc, only_gpu=only_gpu,
                max_rel_qop=0.0, max_rel_chi2=0.0, bit_equal=True, pairs=(a, b))

@@ -41,6 +41,11 @@ def test_error_paths_without_gpu():
     bad = default_geom(iter_layers=[[0, 5, 8], [3, 7, 11]])        # layer 5 is a stereo layer
     with pytest.raises(ValueError):
         lhcb_geom_derive(bad)
+    # geometry validation: first stereo layers, UT hit minimum, Eq. 8 domain, half ranges
+    for kw in (dict(uv_first_layer=[1, 12]), dict(uv_first_layer=[0, 6]), dict(min_ut_hits=0), dict(min_ut_hits=5),
+               dict(p_min=700.0), dict(y_max=-1.0), dict(y_half_tol=-5.0)):
+        with pytest.raises(ValueError):
+            lhcb_geom_derive(default_geom(**kw))
     assert lib.lhcb_seeding(None, None, None, None, None) == -4
     assert lib.lhcb_last_launch_count(None) == 0
 
