@@ -82,15 +82,17 @@ typedef struct {
   float ut_loose[LHCB_N_UT_LAYERS][4];         /* A, B [mm GeV], min, max per layer: Table 2 (L323-340) */
   float ut_tight[LHCB_N_UT_LAYERS][4];
   float ut_y_tol;                              /* strip y-coverage tolerance (O13) */
+  float ut_row_y0, ut_row_pitch;               /* UT strips come in sensor rows: row r covers y in [ut_row_y0 + r*ut_row_pitch,
+                                                  that + ut_row_pitch] (lhcb_ut_t.row; BASELINE.json configs[1]: 14 rows of 100 mm) */
   int32_t min_ut_hits, ut_enabled;             /* 3 (L311); 0 disables the UT search (L307) */
   /* capacities; 0 selects the default in brackets */
   int32_t max_seeds_per_half;                  /* [256]  output slots per event-half */
   int32_t max_xz_cand_per_half;                /* [1024] fitted x-z candidates per event-half */
   int32_t max_long_per_event;                  /* [256]  output slots per event */
-  int32_t max_hits_per_half;                   /* [6144] SciFi hits staged per event-half (<= 32768) */
+  int32_t max_hits_per_half;                   /* [6144] SciFi hits staged per event-half (<= 8000) */
   int32_t max_triplets_per_half;               /* [4096] three-hit combinations per half, both iterations together (the queue also takes the
                                                   room a half leaves unused below max_hits_per_half) */
-  int32_t max_match_cand_per_event;            /* [384]  chi2-accepted seed-VELO pairs per event (>= 256) */
+  int32_t max_match_cand_per_event;            /* [384]  chi2-accepted seed-VELO pairs per event */
   int32_t max_velo_per_event;                  /* [512] */
   int32_t max_ut_per_event;                    /* [6144] UT hits staged in shared memory per event; events with
                                                   more are searched in global memory (slower, same result) */
@@ -155,11 +157,15 @@ typedef struct {
   const int8_t* polarity;    /* [n_events] or NULL -> geom.polarity */
 } lhcb_velo_t;
 
-/* UT hits (L305-342): per (event, layer) sorted by x0 = x at y=0; strip covers [y_lo, y_hi]. */
+/* UT hits (L305-342): per (event, layer) sorted by x0 = x at y=0; strip covers [y_lo, y_hi].  The y coverage
+ * comes either as the sensor row of the strip (one byte per hit: y_lo = ut_row_y0 + row * ut_row_pitch and
+ * y_hi = y_lo + ut_row_pitch, evaluated in float32; y_lo / y_hi may then be NULL) or, when row is NULL, as two
+ * floats per hit.  Rows are staged in shared memory beside x0; the float form is read from global memory. */
 typedef struct {
-  uint32_t n_hits;           /* length of x0, y_lo, y_hi */
+  uint32_t n_hits;           /* length of x0, y_lo, y_hi, row */
   const uint32_t* off;       /* [n_events*4+1] */
   const float *x0, *y_lo, *y_hi;
+  const uint8_t* row;        /* [n_hits] or NULL */
 } lhcb_ut_t;
 
 /* Long tracks.  Event e owns slots [e*max_long_per_event, +count[e]); order unspecified.

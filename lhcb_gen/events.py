@@ -20,7 +20,7 @@ Layout produced (all SoA, float32 unless noted):
   hit_x64   f64[n_hits]          the same values before rounding (for f64 oracle checks)
   hit_pid   i32[n_hits]          global particle id, -1 for noise
   velo_off  u32[n_events+1];  velo_x, velo_y, velo_tx, velo_ty at z_velo;  velo_pid
-  ut_off    u32[n_events*4+1];  ut_x0 ascending per (event, layer);  ut_ylo, ut_yhi;  ut_pid
+  ut_off    u32[n_events*4+1];  ut_x0 ascending per (event, layer);  ut_ylo, ut_yhi;  ut_row u8;  ut_pid
   polarity  i8[n_events]
 """
 from __future__ import annotations
@@ -116,6 +116,7 @@ class Events:
     ut_yhi: np.ndarray
     ut_pid: np.ndarray
     particles: Dict[str, np.ndarray] = field(default_factory=dict)
+    ut_row: Optional[np.ndarray] = None       # u8 strip row per UT hit: y_lo = ut_row_y0 + row * ut_row_pitch
     # cfg5: seeds given directly as states at z_scifi_state
     seed_off: Optional[np.ndarray] = None
     seed_state: Optional[np.ndarray] = None   # [5, n_seeds] x, y, tx, ty, qop
@@ -211,13 +212,18 @@ def _pack_ut(n_events, parts):
     order = np.lexsort((x0.astype(np.float32), zone))
     off = np.zeros(n_events * N_UT + 1, np.uint32)
     np.cumsum(np.bincount(zone, minlength=n_events * N_UT), out=off[1:])
-    return (off, x0[order].astype(np.float32), ylo[order].astype(np.float32),
-            yhi[order].astype(np.float32), pid[order].astype(np.int32))
+    # strip rows: one byte per hit.  The float form of the y coverage is DERIVED from the rows with the float32
+    # operations the ABI states (y_lo = y0 + row * pitch, y_hi = y_lo + pitch), so both forms agree bit for bit.
+    row = np.rint((ylo[order] + UT_Y_MAX) / UT_ROW).astype(np.uint8)
+    ylo32 = np.float32(-UT_Y_MAX) + row.astype(np.float32) * np.float32(UT_ROW)
+    yhi32 = ylo32 + np.float32(UT_ROW)
+    return (off, x0[order].astype(np.float32), ylo32.astype(np.float32),
+            yhi32.astype(np.float32), pid[order].astype(np.int32), row)
 
 
 def _empty_ut(n_events):
     z = np.zeros(0, np.float32)
-    return np.zeros(n_events * N_UT + 1, np.uint32), z, z.copy(), z.copy(), np.zeros(0, np.int32)
+    return np.zeros(n_events * N_UT + 1, np.uint32), z, z.copy(), z.copy(), np.zeros(0, np.int32), np.zeros(0, np.uint8)
 
 
 def _shuffle_within(rng, ev):
@@ -471,6 +477,7 @@ def generate(cfg: GenConfig, geom: Optional[dict] = None, workers: int = 1, firs
         ut_yhi=np.concatenate([c["ut"][3] for c in chunks]),
         ut_pid=np.concatenate([c["ut"][4] for c in chunks]),
         particles=parts,
+        ut_row=np.concatenate([c["ut"][5] for c in chunks]),
     )
     if cfg.direct_seeds:
         evs.seed_off = _cat_off(chunks, "seed_off")
@@ -495,7 +502,7 @@ def slice_events(ev: Events, start: int, stop: int) -> Events:
         velo_ty=ev.velo_ty[v0:v1], velo_pid=ev.velo_pid[v0:v1],
         ut_off=(ev.ut_off[start * 4:stop * 4 + 1] - ev.ut_off[start * 4]).astype(np.uint32),
         ut_x0=ev.ut_x0[u0:u1], ut_ylo=ev.ut_ylo[u0:u1], ut_yhi=ev.ut_yhi[u0:u1],
-        ut_pid=ev.ut_pid[u0:u1],
+        ut_pid=ev.ut_pid[u0:u1], ut_row=ev.ut_row[u0:u1] if ev.ut_row is not None else None,
     )
     if ev.seed_off is not None:
         s0, s1 = int(ev.seed_off[start]), int(ev.seed_off[stop])

@@ -37,7 +37,7 @@ class LhcbGeom(C.Structure):
         ("z_velo", F), ("z_scifi_state", F), ("z_match_y", F), ("mag", F * 5), ("gamma_ab", F * 2),
         ("kick_pt", F), ("polarity", I), ("presel", F * 4), ("match_tol", F * 8), ("chi2_match_max", F),
         ("ut_z", F * 4), ("ut_tan_alpha", F * 4), ("ut_loose", (F * 4) * 4), ("ut_tight", (F * 4) * 4),
-        ("ut_y_tol", F), ("min_ut_hits", I), ("ut_enabled", I),
+        ("ut_y_tol", F), ("ut_row_y0", F), ("ut_row_pitch", F), ("min_ut_hits", I), ("ut_enabled", I),
         ("max_seeds_per_half", I), ("max_xz_cand_per_half", I), ("max_long_per_event", I),
         ("max_hits_per_half", I), ("max_triplets_per_half", I), ("max_match_cand_per_event", I),
         ("max_velo_per_event", I), ("max_ut_per_event", I),
@@ -83,7 +83,7 @@ class LhcbVelo(C.Structure):
 
 
 class LhcbUt(C.Structure):
-    _fields_ = [("n_hits", C.c_uint32), ("off", VP), ("x0", VP), ("y_lo", VP), ("y_hi", VP)]
+    _fields_ = [("n_hits", C.c_uint32), ("off", VP), ("x0", VP), ("y_lo", VP), ("y_hi", VP), ("row", VP)]
 
 
 class LhcbLong(C.Structure):
@@ -184,6 +184,7 @@ class DeviceEvents:
     ut_x0: Optional["torch.Tensor"] = None
     ut_ylo: Optional["torch.Tensor"] = None
     ut_yhi: Optional["torch.Tensor"] = None
+    ut_row: Optional["torch.Tensor"] = None     # u8 strip rows: used instead of ut_ylo / ut_yhi when present
 
     @staticmethod
     def from_host(ev, device="cuda:0"):
@@ -202,12 +203,14 @@ class DeviceEvents:
             ut_off=up(ev.ut_off, np.uint32) if has_ut else None,
             ut_x0=up(ev.ut_x0, np.float32) if has_ut else None,
             ut_ylo=up(ev.ut_ylo, np.float32) if has_ut else None,
-            ut_yhi=up(ev.ut_yhi, np.float32) if has_ut else None)
+            ut_yhi=up(ev.ut_yhi, np.float32) if has_ut else None,
+            ut_row=up(ev.ut_row, np.uint8) if has_ut and getattr(ev, "ut_row", None) is not None else None)
 
     def input_bytes(self):
         n = 0
         for t in (self.zone_off, self.hit_x, self.polarity, self.velo_off, self.velo_x, self.velo_y, self.velo_tx,
-                  self.velo_ty, self.ut_off, self.ut_x0, self.ut_ylo, self.ut_yhi):
+                  self.velo_ty, self.ut_off, self.ut_x0, self.ut_row if self.ut_row is not None else self.ut_ylo,
+                  None if self.ut_row is not None else self.ut_yhi):
             if t is not None:
                 n += t.numel() * t.element_size()
         return n
@@ -307,7 +310,8 @@ class Context:
                      _ptr(dev.velo_ty), _ptr(dev.polarity))
         u = None
         if use_ut and dev.ut_off is not None:
-            u = C.byref(LhcbUt(dev.ut_x0.numel(), _ptr(dev.ut_off), _ptr(dev.ut_x0), _ptr(dev.ut_ylo), _ptr(dev.ut_yhi)))
+            u = C.byref(LhcbUt(dev.ut_x0.numel(), _ptr(dev.ut_off), _ptr(dev.ut_x0), _ptr(dev.ut_ylo), _ptr(dev.ut_yhi),
+                               _ptr(dev.ut_row)))
         l = LhcbLong(_ptr(out["count"]), _ptr(out["seed_idx"]), _ptr(out["velo_idx"]), _ptr(out["ut_idx"]),
                      _ptr(out["n_ut"]), _ptr(out["qop"]), _ptr(out["chi2"]), _ptr(out["status"]), _ptr(out.get("ghost")))
         rc = self.lib.lhcb_matching(self._ctx, C.byref(s), C.byref(v), u, C.byref(l), VP(0), self._stream())

@@ -14,6 +14,10 @@
 #include "prepare.cuh"
 #include "seeding.cuh"
 
+#ifndef LHCB_SEED_CTAS
+#define LHCB_SEED_CTAS 4   // CTAs per SM the 256-thread seeding kernel is compiled for (64 registers per thread)
+#endif
+
 struct lhcb_ctx {
   lhcb_geom_t geom;
   lhcb_derived_t der;
@@ -70,6 +74,15 @@ void fill_seed_params(const lhcb_ctx* c, lhcb::SeedParams& p) {
   p.min_x_hits = g.min_x_hits; p.min_uv_hits = g.min_uv_hits; p.polarity = g.polarity;
   p.max_seeds = g.max_seeds_per_half; p.max_cand = g.max_xz_cand_per_half; p.max_hits = g.max_hits_per_half;
   p.max_trip = g.max_triplets_per_half;
+  for (int it = 0; it < 2; ++it) {                         // the three x-layers an iteration extends to, slots of all six
+    const int seedl[3] = {D.l1[it], D.l2[it], D.l3[it]};
+    int n = 0;
+    for (int s = 0; s < 6; ++s) {
+      const int l = D.xl[s];
+      if (l != seedl[0] && l != seedl[1] && l != seedl[2] && n < 3) { p.ol[it][n] = l; p.os[it][n] = s; ++n; }
+    }
+    for (int k = 0; k < 3; ++k) p.ss[it][k] = D.slot_of_layer[seedl[k]];
+  }
   p.P = c->d_P; p.Q = c->d_Q;
   // Hough-cluster UV seeding (reading A20): 64 t_y = y / z bins per half over the stereo layers, in double
   // from the float geometry, rounded once
@@ -94,6 +107,7 @@ void fill_match_params(const lhcb_ctx* c, lhcb::MatchParams& p) {
   p.inv_KB = D.inv_KB; p.Ag = D.Ag; p.Bg = D.Bg; p.inv_Bg = D.inv_Bg;
   copy_arr(p.ut_dz, D.ut_dz); copy_arr(p.ut_dz2, D.ut_dz2); copy_arr(p.ut_dz4, D.ut_dz4);
   copy_arr(p.ut_tan, D.ut_tan); p.ut_y_tol = D.ut_y_tol;
+  p.row_y0 = g.ut_row_y0; p.row_pitch = g.ut_row_pitch;
   std::memcpy(p.ut_loose, D.ut_loose, sizeof(p.ut_loose)); std::memcpy(p.ut_tight, D.ut_tight, sizeof(p.ut_tight));
   p.min_ut_hits = g.min_ut_hits; p.polarity = g.polarity;
   p.max_seeds = g.max_seeds_per_half; p.max_long = g.max_long_per_event;
@@ -121,17 +135,14 @@ int lhcb_geom_init(const lhcb_geom_t* g, int device, lhcb_ctx** out) {
   const lhcb_geom_t& G = c->geom;
   int rc = lhcb::derive(G, c->der);
   if (rc != LHCB_OK) { delete c; return rc; }
-  if (G.max_hits_per_half > 32768 || G.max_xz_cand_per_half > 65535 || G.max_seeds_per_half > 32767 ||
-      G.max_velo_per_event > 65535 || G.max_ut_per_event > 65534 || G.max_match_cand_per_event > 16383 || G.max_match_cand_per_event < lhcb::kTyBins || G.max_triplets_per_half < G.max_xz_cand_per_half) { delete c; return LHCB_ERR_BAD_ARGUMENT; }
+  if (G.max_hits_per_half > 8000 || G.max_xz_cand_per_half > 65535 || G.max_seeds_per_half > 32767 ||
+      G.max_velo_per_event > 65535 || G.max_ut_per_event > 65534 || G.max_match_cand_per_event > 16383 || G.max_triplets_per_half < G.max_xz_cand_per_half) { delete c; return LHCB_ERR_BAD_ARGUMENT; }
   // 256-thread CTAs, four per SM, when their shared memory fits (228 KB per SM, 1 KB reserved per
   // CTA); else 512-thread CTAs, two (or one) per SM
   c->seed_threads = 256;
-  c->seed_smem = lhcb::seed_smem_bytes(256, G.max_hits_per_half, G.max_xz_cand_per_half, G.max_triplets_per_half);
-  c->seed_ctas = 4;   // (five 48-register CTAs per SM measured slower than four 64-register ones)
-  if (c->seed_smem > (size_t)(228 * 1024 / 4 - 1024)) {
-    c->seed_threads = 512; c->seed_ctas = 2;
-    c->seed_smem = lhcb::seed_smem_bytes(512, G.max_hits_per_half, G.max_xz_cand_per_half, G.max_triplets_per_half);
-  }
+  c->seed_smem = lhcb::seed_smem_bytes(G.max_hits_per_half, G.max_xz_cand_per_half, G.max_triplets_per_half);
+  c->seed_ctas = LHCB_SEED_CTAS;
+  if (c->seed_smem > (size_t)(228 * 1024 / LHCB_SEED_CTAS - 1024)) { c->seed_threads = 512; c->seed_ctas = 2; }
   c->match_threads = 128;
   c->match_smem = lhcb::match_smem_bytes(128, G.max_seeds_per_half, G.max_match_cand_per_event, G.max_velo_per_event,
                                          G.max_ut_per_event);
@@ -147,7 +158,7 @@ int lhcb_geom_init(const lhcb_geom_t* g, int device, lhcb_ctx** out) {
   if (e != cudaSuccess) { c->last_cuda_error = (int)e; delete c; return LHCB_ERR_CUDA; }
   if (c->seed_smem > (size_t)max_optin || c->match_smem > (size_t)max_optin || c->prep_smem > (size_t)max_optin) { delete c; return LHCB_ERR_CAPACITY; }
   {
-    const void* fn = c->seed_ctas == 4 ? (const void*)lhcb::seeding_kernel<256, 4>
+    const void* fn = c->seed_ctas == LHCB_SEED_CTAS ? (const void*)lhcb::seeding_kernel<256, LHCB_SEED_CTAS>
                                        : (const void*)lhcb::seeding_kernel<512, 2>;
     e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->seed_smem);
   }
@@ -247,8 +258,8 @@ int lhcb_seeding(lhcb_ctx* c, const lhcb_events_t* ev, lhcb_seeds_t* out, void* 
   p.nuv = out->nuv; p.status = out->status;
   p.cap_total = (size_t)ev->n_events * 2 * (size_t)c->geom.max_seeds_per_half;
   p.smem_total = (int)c->seed_smem;
-  if (c->seed_ctas == 4)
-    lhcb::seeding_kernel<256, 4><<<ev->n_events * 2, 256, c->seed_smem, (cudaStream_t)stream>>>(p);
+  if (c->seed_ctas == LHCB_SEED_CTAS)
+    lhcb::seeding_kernel<256, LHCB_SEED_CTAS><<<ev->n_events * 2, 256, c->seed_smem, (cudaStream_t)stream>>>(p);
   else
     lhcb::seeding_kernel<512, 2><<<ev->n_events * 2, 512, c->seed_smem, (cudaStream_t)stream>>>(p);
   LHCB_CUDA(c, cudaGetLastError());
@@ -267,7 +278,7 @@ int lhcb_matching(lhcb_ctx* c, const lhcb_seeds_t* seeds, const lhcb_velo_t* vel
   if (!seeds->count || !seeds->state || !velo->off || !out->count || !out->seed_idx || !out->velo_idx ||
       !out->ut_idx || !out->n_ut || !out->qop || !out->chi2 || !out->status)
     return LHCB_ERR_BAD_ARGUMENT;
-  if (ut && (!ut->off || !ut->x0 || !ut->y_lo || !ut->y_hi)) return LHCB_ERR_BAD_ARGUMENT;
+  if (ut && (!ut->off || !ut->x0 || (!ut->row && (!ut->y_lo || !ut->y_hi)))) return LHCB_ERR_BAD_ARGUMENT;
   LHCB_CUDA(c, cudaSetDevice(c->device));
   lhcb::MatchParams p;
   fill_match_params(c, p);
@@ -276,7 +287,7 @@ int lhcb_matching(lhcb_ctx* c, const lhcb_seeds_t* seeds, const lhcb_velo_t* vel
   p.seed_count = seeds->count; p.state = seeds->state;
   p.seed_cap_total = (size_t)velo->n_events * 2 * (size_t)c->geom.max_seeds_per_half;
   p.velo_off = velo->off; p.vx = velo->x; p.vy = velo->y; p.vtx = velo->tx; p.vty = velo->ty; p.pol = velo->polarity;
-  if (ut) { p.ut_off = ut->off; p.ux = ut->x0; p.uylo = ut->y_lo; p.uyhi = ut->y_hi; p.n_ut_total = ut->n_hits; }
+  if (ut) { p.ut_off = ut->off; p.ux = ut->x0; p.uylo = ut->y_lo; p.uyhi = ut->y_hi; p.urow = ut->row; p.n_ut_total = ut->n_hits; }
   p.count = out->count; p.seed_idx = out->seed_idx; p.velo_idx = out->velo_idx; p.ut_idx = out->ut_idx;
   p.n_ut = out->n_ut; p.qop = out->qop; p.chi2 = out->chi2; p.status = out->status;
   p.nn = c->nn_on ? c->d_nn : nullptr; p.snx = seeds->nx; p.snuv = seeds->nuv; p.ghost = out->ghost;

@@ -33,6 +33,7 @@ struct MatchParams {
   float zS, zV, dzyS, dzyV, mag[5], presel[4], cx0, cx1, cy0, cy1, inv_tol_tx, inv_tol_ty, chi2m_max;
   float inv_KB, Ag, Bg, inv_Bg, ut_dz[4], ut_dz2[4], ut_dz4[4], ut_tan[4], ut_y_tol;
   float ut_loose[4][4], ut_tight[4][4];
+  float row_y0, row_pitch;  // strip row r covers y in [row_y0 + r * row_pitch, that + row_pitch]
   int min_ut_hits, use_ut, polarity;
   int max_seeds, max_long, max_mc, max_velo, max_ut;
   uint32_t n_ut_total;
@@ -46,6 +47,7 @@ struct MatchParams {
   const int8_t* pol;
   const uint32_t* ut_off;
   const float *ux, *uylo, *uyhi;
+  const uint8_t* urow;      // strip row per UT hit (then uylo / uyhi are not read) or NULL
   uint32_t* count;
   uint32_t* seed_idx;
   uint32_t* velo_idx;
@@ -67,23 +69,37 @@ struct __align__(8) MatchCand {
   float chi2, q0, gamma;    // chi2_match, kick q/p (A10), gamma_x of the best UT hypothesis
   unsigned long long key;   // best UT hypothesis: (4 - n_ut) << 50 | f32 bits of sum res^2 << 18 | layer << 16 | first hit
   uint16_t ut[4];           // its hits, relative to the event's first UT hit (0xFFFF = none)
-  float ghost;              // ghost probability (network set) 
-  uint32_t pad;
 };
-static_assert(sizeof(MatchCand) == 40, "MatchCand is 40 bytes");
+static_assert(sizeof(MatchCand) == 32, "MatchCand is 32 bytes");
 
-__host__ __device__ inline size_t match_smem_bytes(int kMatchThreads, int max_seeds, int max_mc, int max_velo, int max_ut) {
+// Shared-memory map of one CTA (T threads):
+//   [header 64 | UT x0 tile | UT strip rows | VELO states sorted by t_y (x, y, tx, ty) | original index u16 |
+//    t_y bin starts u16[257] | scan scratch | region X | pair records | best key per seed | best key per VELO]
+// Region X is used in turn as the scatter cursors of M0, the seed states of the current tile (M1/M2), the UT
+// hypothesis queue (M3) and the ghost probabilities (M4).  After M3 the UT tile is dead: M4 keeps the network
+// weights and the seed states there.
+__host__ __device__ inline size_t match_align16(size_t b) { return (b + 15) & ~(size_t)15; }
+__host__ __device__ inline size_t match_x_bytes(int T, int max_mc) {
+  size_t b = (size_t)T * 16;                                   // float4 per owner of a tile
+  if (b < (size_t)kTyBins * 4) b = (size_t)kTyBins * 4;        // scatter cursors
+  if (b < (size_t)max_mc * 8) b = (size_t)max_mc * 8;          // 2 * max_mc hypotheses / max_mc ghost probabilities
+  return b;
+}
+__host__ __device__ inline size_t match_ut_bytes(int max_seeds, int max_ut) {
+  size_t b = ((size_t)max_ut + 8) * 4;                         // x0 tile (16-byte aligned superset)
+  const size_t m4 = 1360 + (size_t)2 * max_seeds * 16;         // M4: network weights + seed states
+  return match_align16(b > m4 ? b : m4);
+}
+__host__ __device__ inline size_t match_smem_bytes(int T, int max_seeds, int max_mc, int max_velo, int max_ut) {
   size_t b = 64;
-  b += ((size_t)max_ut + 8) * 4;             // UT x0 tile (16-byte aligned superset)
+  b += match_ut_bytes(max_seeds, max_ut);
+  b += match_align16((size_t)max_ut + 32);   // strip rows (16-byte aligned superset)
   b += (size_t)max_velo * 16;                // VELO states, sorted by ty
-  b += (size_t)(kTyBins + 1) * 4;            // start of each t_y bin of the VELO states
-  b += (size_t)max_velo * 2;                 // original index of each sorted state
-  b = (b + 15) & ~(size_t)15;
-  b += (kMatchThreads + 1) * 4 + kMatchThreads * 2 + 64;   // work-list scan scratch
-  b = (b + 15) & ~(size_t)15;
+  b += match_align16((size_t)max_velo * 2);  // original index of each sorted state
+  b += match_align16((size_t)(kTyBins + 1) * 2);   // start of each t_y bin
+  b += match_align16((size_t)(T + 1) * 4 + (size_t)T * 2 + 144);   // work-list scan scratch (two warp_sums buffers)
+  b += match_align16(match_x_bytes(T, max_mc));
   b += (size_t)max_mc * sizeof(MatchCand);
-  b += (size_t)max_mc * 4;                   // UT hypothesis queue
-  b = (b + 15) & ~(size_t)15;
   b += (size_t)2 * max_seeds * 8;            // best key per seed
   b += (size_t)max_velo * 8;                 // best key per VELO track
   return b;
@@ -126,18 +142,20 @@ __device__ __forceinline__ float nn_eta(float tx, float ty) {          // pseudo
   rho = rho < 1e-6f ? 1e-6f : rho;
   return nn_log((1.0f + sh) / rho);
 }
-// nn = mu[8], isig[8], W1[32][8], b1[32], W2[32], b2, cut, margin
+// nn = mu[8], isig[8], W1[32][8], b1[32], W2[32], b2, cut, margin (a copy in shared memory: every lane reads
+// the same weight, a broadcast)
 __device__ __forceinline__ float nn_ghost_prob(const float* __restrict__ nn, const float* in) {
   float u[8];
 #pragma unroll
-  for (int k = 0; k < 8; ++k) u[k] = (in[k] - __ldg(nn + k)) * __ldg(nn + 8 + k);
-  float t = __ldg(nn + 336);
+  for (int k = 0; k < 8; ++k) u[k] = (in[k] - nn[k]) * nn[8 + k];
+  float t = nn[336];
+#pragma unroll 4
   for (int j = 0; j < 32; ++j) {
-    float h = __ldg(nn + 272 + j);
+    float h = nn[272 + j];
 #pragma unroll
-    for (int k = 0; k < 8; ++k) h = h + __ldg(nn + 16 + j * 8 + k) * u[k];
+    for (int k = 0; k < 8; ++k) h = h + nn[16 + j * 8 + k] * u[k];
     h = h < 0.f ? 0.f : h;
-    t = t + __ldg(nn + 304 + j) * h;
+    t = t + nn[304 + j] * h;
   }
   return 1.0f / (1.0f + nn_exp(-t));
 }
@@ -150,14 +168,28 @@ __device__ __forceinline__ float ut_window(const float* w, float invpG) {
   return lo < w[3] ? lo : w[3];
 }
 
+// Does the strip of UT hit i (index into the searched x0 array) cover y within ut_y_tol (reading A18)?
+// Strip rows (one byte per hit, staged in shared memory): y_lo = row_y0 + row * row_pitch, y_hi = y_lo +
+// row_pitch, the same float operations that produced the y_lo / y_hi arrays the float form carries.
+struct UtCover {
+  const uint8_t* __restrict__ row;     // shared-memory rows or NULL
+  const float* __restrict__ ylo;       // global arrays (already offset to the indexing of the x0 array)
+  const float* __restrict__ yhi;
+  float y0, pitch, tol;
+  __device__ __forceinline__ bool operator()(int i, float y) const {
+    float lo, hi;
+    if (row) { lo = y0 + (float)row[i] * pitch; hi = lo + pitch; }
+    else { lo = ylo[i]; hi = yhi[i]; }
+    return lo - tol <= y && y <= hi + tol;
+  }
+};
+
 // O13, second half: hypothesis (layer i0, hit j) of one accepted pair.  The remaining layers use tight
 // windows and the closest hit; gamma_x is refitted after each hit (L309).  ux is the searched x0 array
-// (shared-memory tile or the global array), uo[] its layer offsets; the y-range of hit i of ux is
-// (uylo[i], uyhi[i]) (global memory, already offset to the indexing of ux).
+// (shared-memory tile or the global array), uo[] its layer offsets.
 __device__ __forceinline__ void ut_tight_walk(const MatchParams& p, float xV, float yV, float txV, float tyV,
                                               float invpG, int i0, int j, const float* __restrict__ ux,
-                                              const float* __restrict__ uylo, const float* __restrict__ uyhi,
-                                              const int* uo, UtHyp& hy) {
+                                              const UtCover& cover, const int* uo, UtHyp& hy) {
   float dj[4];
   float num = 0.f, den = 0.f, gam = 0.f;
   hy.n = 0;
@@ -177,7 +209,7 @@ __device__ __forceinline__ void ut_tight_walk(const MatchParams& p, float xV, fl
       const int bb = uo[i], ee = uo[i + 1];
       float bd = 0.f;
       for (int jj = lower_bound(ux, bb, ee, tlo); jj < ee && ux[jj] <= thi; ++jj) {
-        if (!(uylo[jj] - p.ut_y_tol <= yt && yt <= uyhi[jj] + p.ut_y_tol)) continue;
+        if (!cover(jj, yt)) continue;
         const float dd = fabsf(ux[jj] - xe);
         if (bj < 0 || dd < bd) { bj = jj; bd = dd; }
       }
@@ -201,36 +233,54 @@ __device__ __forceinline__ void ut_tight_walk(const MatchParams& p, float xV, fl
     }
 }
 
+// one bulk async copy global -> shared signalling mbar
+__device__ __forceinline__ void bulk_copy(void* dst, const void* src, uint32_t bytes, uint32_t mbar_addr) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   (uint32_t)__cvta_generic_to_shared(dst)),
+               "l"(src), "r"(bytes), "r"(mbar_addr)
+               : "memory");
+}
+
 template <int kMatchThreads, int MIN_CTAS>
 __global__ void __launch_bounds__(kMatchThreads, MIN_CTAS)
 matching_kernel(const __grid_constant__ MatchParams p) {
   extern __shared__ __align__(16) unsigned char smem[];
+  constexpr int T = kMatchThreads;
   int* hdr = reinterpret_cast<int*>(smem);                  // [0] n_mc, [1] n_long, [2] status, [3] n_hyp, [4..8] UT offsets, [9] tie flag
   unsigned long long* mbar = reinterpret_cast<unsigned long long*>(smem + 48);
-  float* sux = reinterpret_cast<float*>(smem + 64);
-  float* svx = sux + p.max_ut + 8;
+  size_t off = 64;
+  float* sux = reinterpret_cast<float*>(smem + off);                       // UT x0 tile; M4: network weights + seed states
+  off += match_ut_bytes(p.max_seeds, p.max_ut);
+  uint8_t* srow = smem + off;                                              // UT strip rows
+  off += match_align16((size_t)p.max_ut + 32);
+  float* svx = reinterpret_cast<float*>(smem + off);
   float* svy = svx + p.max_velo;
   float* svtx = svy + p.max_velo;
   float* svty = svtx + p.max_velo;
-  int* vbin = reinterpret_cast<int*>(svty + p.max_velo);                  // [kTyBins + 1]
-  uint16_t* sorig = reinterpret_cast<uint16_t*>(vbin + kTyBins + 1);
-  size_t off = 64 + ((size_t)p.max_ut + 8) * 4 + (size_t)p.max_velo * 18 + (size_t)(kTyBins + 1) * 4;
-  off = (off + 15) & ~(size_t)15;
-  int* offs = reinterpret_cast<int*>(smem + off);                         // [kMatchThreads + 1]
-  uint16_t* firsts = reinterpret_cast<uint16_t*>(offs + kMatchThreads + 1);
-  int* warp_sums = reinterpret_cast<int*>(smem + off + (kMatchThreads + 1) * 4 + kMatchThreads * 2);
-  off += (kMatchThreads + 1) * 4 + kMatchThreads * 2 + 64;
-  off = (off + 15) & ~(size_t)15;
+  off += (size_t)p.max_velo * 16;
+  uint16_t* sorig = reinterpret_cast<uint16_t*>(smem + off);
+  off += match_align16((size_t)p.max_velo * 2);
+  uint16_t* vbin = reinterpret_cast<uint16_t*>(smem + off);               // [kTyBins + 1]
+  off += match_align16((size_t)(kTyBins + 1) * 2);
+  int* offs = reinterpret_cast<int*>(smem + off);                         // [T + 1]
+  uint16_t* firsts = reinterpret_cast<uint16_t*>(offs + T + 1);
+  int* warp_sums = reinterpret_cast<int*>(smem + off + (T + 1) * 4 + T * 2);
+  off += match_align16((size_t)(T + 1) * 4 + (size_t)T * 2 + 144);
+  unsigned char* regx = smem + off;
+  int* vcur = reinterpret_cast<int*>(regx);                                // M0: [kTyBins] scatter cursors
+  float4* sown = reinterpret_cast<float4*>(regx);                          // M1/M2: (x, y at z_match_y, tx, ty) of the tile's seeds
+  uint32_t* hyq = reinterpret_cast<uint32_t*>(regx);                       // M3: (pair << 18) | (layer << 16) | first hit
+  float* sghost = reinterpret_cast<float*>(regx);                          // M4: ghost probability per pair
+  const int hyp_cap = (int)(match_x_bytes(T, p.max_mc) / 4);
+  off += match_align16(match_x_bytes(T, p.max_mc));
   MatchCand* mc = reinterpret_cast<MatchCand*>(smem + off);
   off += (size_t)p.max_mc * sizeof(MatchCand);
-  uint32_t* hyq = reinterpret_cast<uint32_t*>(smem + off);                 // (pair << 18) | (layer << 16) | first hit
-  off += (size_t)p.max_mc * 4;
-  off = (off + 15) & ~(size_t)15;
   unsigned long long* seed_best = reinterpret_cast<unsigned long long*>(smem + off);
   unsigned long long* velo_best = seed_best + 2 * p.max_seeds;
 
   const int tid = threadIdx.x;
   const int e = blockIdx.x;
+  int flip = 0;                                            // warp_sums buffer of the next block scan
   LHCB_CLK_INIT
   const uint32_t v0 = p.velo_off[e];
   const int nv = (int)(p.velo_off[e + 1] - v0);
@@ -244,9 +294,9 @@ matching_kernel(const __grid_constant__ MatchParams p) {
   }
   if (tid < 4) hdr[tid] = 0;
   if (tid == 4) hdr[9] = 0;                                  // chi2 tie seen (reading A21)
-  // ---- UT x0 of this event: one bulk copy, overlapped with the all-pairs loop -----------------
-  uint32_t u_begin = 0, u_end = 0, ua0 = 0, ua1 = 0;
-  bool ut_in_smem = false;
+  // ---- UT x0 (and strip rows) of this event: bulk copies, overlapped with the all-pairs loop ----------
+  uint32_t u_begin = 0, u_end = 0, ua0 = 0;
+  bool ut_in_smem = false, rows_in_smem = false;
   const uint32_t mbar_addr = (uint32_t)__cvta_generic_to_shared(mbar);
   if (p.use_ut) {
     u_begin = p.ut_off[(size_t)e * 4]; u_end = p.ut_off[(size_t)e * 4 + 4];
@@ -256,33 +306,34 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     }
     ua0 = u_begin & ~3u;
     ut_in_smem = (int)(u_end - u_begin) <= p.max_ut;
+    rows_in_smem = ut_in_smem && p.urow != nullptr;
     if (ut_in_smem) {
+      // x0: floats [ua0, ua1) by one bulk copy, the unaligned tail of the array by plain loads;
+      // rows: bytes [ra0, ra1), srow[i - ra0] = row of hit i
       const bool aligned = (reinterpret_cast<uintptr_t>(p.ux) & 15) == 0;
-      ua1 = (u_end + 3u) & ~3u;
+      uint32_t ua1 = (u_end + 3u) & ~3u;
       if (ua1 > (p.n_ut_total & ~3u)) ua1 = p.n_ut_total & ~3u;
       if (!aligned || ua1 < ua0) ua1 = ua0;
+      const bool raligned = rows_in_smem && (reinterpret_cast<uintptr_t>(p.urow) & 15) == 0;
+      const uint32_t ra0 = u_begin & ~15u;
+      uint32_t ra1 = (u_end + 15u) & ~15u;
+      if (ra1 > (p.n_ut_total & ~15u)) ra1 = p.n_ut_total & ~15u;
+      if (!raligned || ra1 < ra0) ra1 = ra0;
       if (tid == 0) {
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar_addr));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        const uint32_t bytes = (ua1 - ua0) * 4u;
+        const uint32_t bytes = (ua1 - ua0) * 4u + (ra1 - ra0);
         if (bytes > 0) {
           asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar_addr), "r"(bytes) : "memory");
-          asm volatile(
-              "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                  (uint32_t)__cvta_generic_to_shared(sux)),
-              "l"(p.ux + ua0), "r"(bytes), "r"(mbar_addr)
-              : "memory");
+          if (ua1 > ua0) bulk_copy(sux, p.ux + ua0, (ua1 - ua0) * 4u, mbar_addr);
+          if (ra1 > ra0) bulk_copy(srow, p.urow + ra0, ra1 - ra0, mbar_addr);
         } else {
           asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(mbar_addr) : "memory");
         }
       }
-      if (tid == 32 && aligned && ua1 > ua0 && ((reinterpret_cast<uintptr_t>(p.uylo) | reinterpret_cast<uintptr_t>(p.uyhi)) & 15) == 0) {
-        // the y ranges of the hits the UT search will touch: pull the event's slice into L2 while M0-M2 run
-        const uint32_t bytes = (ua1 - ua0) * 4u;
-        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p.uylo + ua0), "r"(bytes) : "memory");
-        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p.uyhi + ua0), "r"(bytes) : "memory");
-      }
-      for (uint32_t i = ua1 + tid; i < u_end; i += kMatchThreads) sux[i - ua0] = p.ux[i];
+      for (uint32_t i = (ua1 > u_begin ? ua1 : u_begin) + tid; i < u_end; i += T) sux[i - ua0] = p.ux[i];
+      if (rows_in_smem)
+        for (uint32_t i = (ra1 > u_begin ? ra1 : u_begin) + tid; i < u_end; i += T) srow[i - ra0] = p.urow[i];
       if (tid < 5) hdr[4 + tid] = (int)(p.ut_off[(size_t)e * 4 + tid] - ua0);
     } else if (tid < 5) {
       hdr[4 + tid] = (int)p.ut_off[(size_t)e * 4 + tid];
@@ -291,28 +342,28 @@ matching_kernel(const __grid_constant__ MatchParams p) {
   // t_y bin of a VELO state or of a window edge: monotone in t, so the states with t in [a, b] lie in the bins
   // [bin(a), bin(b)] whatever the rounding; values outside +-0.4 land in the edge bins
   auto ty_bin = [](float t) { return (int)fminf(fmaxf((t + 0.4f) * ((float)kTyBins / 0.8f), 0.f), (float)(kTyBins - 1)); };
-  int* vcur = reinterpret_cast<int*>(hyq);                                 // [kTyBins] scatter cursors (hyq is free until M3)
-  for (int v = tid; v < nv; v += kMatchThreads) velo_best[v] = kNoKey;
-  for (int s = tid; s < ns; s += kMatchThreads) seed_best[s] = kNoKey;
-  for (int b = tid; b <= kTyBins; b += kMatchThreads) vbin[b] = 0;
+  for (int v = tid; v < nv; v += T) velo_best[v] = kNoKey;
+  for (int s = tid; s < ns; s += T) seed_best[s] = kNoKey;
+  for (int b = tid; b < kTyBins; b += T) vcur[b] = 0;
   __syncthreads();
   // ---- M0: counting sort of the VELO states into t_y bins (order inside a bin is irrelevant: the bins
   // only delimit, per seed, a superset of the states that can pass the |dty| cut of Eq. 21) -----------
-  for (int v = tid; v < nv; v += kMatchThreads) atomicAdd(&vbin[ty_bin(p.vty[v0 + v]) + 1], 1);
+  for (int v = tid; v < nv; v += T) atomicAdd(&vcur[ty_bin(p.vty[v0 + v])], 1);
   __syncthreads();
   {
-    constexpr int per = kTyBins / kMatchThreads;
-    static_assert(per * kMatchThreads == kTyBins, "whole bins per thread");
+    constexpr int per = kTyBins / T;
+    static_assert(per * T == kTyBins, "whole bins per thread");
     int c[per], sum = 0;
 #pragma unroll
-    for (int k = 0; k < per; ++k) { c[k] = vbin[tid * per + k + 1]; sum += c[k]; }
+    for (int k = 0; k < per; ++k) { c[k] = vcur[tid * per + k]; sum += c[k]; }
     int total;
-    int run = block_exscan<kMatchThreads>(sum, warp_sums, total);
+    int run = block_exscan<T>(sum, warp_sums, flip, total);
+    if (tid == 0) vbin[0] = 0;
 #pragma unroll
-    for (int k = 0; k < per; ++k) { vcur[tid * per + k] = run; run += c[k]; vbin[tid * per + k + 1] = run; }
+    for (int k = 0; k < per; ++k) { vcur[tid * per + k] = run; run += c[k]; vbin[tid * per + k + 1] = (uint16_t)run; }
   }
   __syncthreads();
-  for (int v = tid; v < nv; v += kMatchThreads) {
+  for (int v = tid; v < nv; v += T) {
     const float t = p.vty[v0 + v];
     const int r = atomicAdd(&vcur[ty_bin(t)], 1);
     svx[r] = p.vx[v0 + v]; svy[r] = p.vy[v0 + v]; svtx[r] = p.vtx[v0 + v]; svty[r] = t;
@@ -323,14 +374,14 @@ matching_kernel(const __grid_constant__ MatchParams p) {
 
   // ---- M1/M2: all seed x VELO pairs (L279), restricted to the |dty| range of each seed ----------
   const size_t sct = p.seed_cap_total;
-  constexpr int T = kMatchThreads;
+  auto slot_of = [&](int s) { return s < c0 ? (size_t)(2 * e) * p.max_seeds + s : (size_t)(2 * e + 1) * p.max_seeds + (s - c0); };
   for (int tile0 = 0; tile0 < ns; tile0 += T) {
     const int nown = ns - tile0 < T ? ns - tile0 : T;
     int cnt = 0, fst = 0;
     if (tid < nown) {
-      const int s = tile0 + tid;
-      const size_t slot = s < c0 ? (size_t)(2 * e) * p.max_seeds + s : (size_t)(2 * e + 1) * p.max_seeds + (s - c0);
-      const float tyS = p.state[3 * sct + slot];
+      const size_t slot = slot_of(tile0 + tid);
+      const float xS = p.state[slot], yS = p.state[sct + slot], txS = p.state[2 * sct + slot], tyS = p.state[3 * sct + slot];
+      sown[tid] = make_float4(xS, yS + p.dzyS * tyS, txS, tyS);                    // L231: y at z_match_y
       // superset of {v : |tyS - tyV| < presel[3]} whatever the rounding of the subtraction
       const float w = p.presel[3] + 1e-6f * (fabsf(tyS) + p.presel[3]) + 1e-30f;
       fst = vbin[ty_bin(tyS - w)];
@@ -338,7 +389,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
       cnt = lst - fst;
     }
     int total;
-    const int ex = block_exscan<T>(cnt, warp_sums, total);
+    const int ex = block_exscan<T>(cnt, warp_sums, flip, total);
     offs[tid] = ex; firsts[tid] = (uint16_t)fst;
     if (tid == T - 1) offs[T] = total;
     __syncthreads();
@@ -347,17 +398,14 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     const int p0 = tid * chunk, p1 = p0 + chunk < total ? p0 + chunk : total;
     if (p0 < p1) {
       int t = owner_of(offs, nown, p0) - 1;
-      int nxt = -1, f = 0, s = 0;
+      int nxt = -1, f = 0;
       float xS = 0.f, txS = 0.f, tyS = 0.f, axS = 0.f, ys = 0.f;
       for (int q = p0; q < p1; ++q) {
         if (q >= nxt) {
           do { ++t; nxt = offs[t + 1]; } while (q >= nxt);
-          s = tile0 + t;
-          const size_t slot = s < c0 ? (size_t)(2 * e) * p.max_seeds + s : (size_t)(2 * e + 1) * p.max_seeds + (s - c0);
-          xS = p.state[slot]; const float yS = p.state[sct + slot]; txS = p.state[2 * sct + slot];
-          tyS = p.state[3 * sct + slot];
+          const float4 o = sown[t];
+          xS = o.x; ys = o.y; txS = o.z; tyS = o.w;
           axS = fabsf(xS);
-          ys = yS + p.dzyS * tyS;                                                  // L231
           f = (int)firsts[t] - offs[t];
         }
         const int v = f + q;                                                       // rank in ty order
@@ -376,11 +424,11 @@ matching_kernel(const __grid_constant__ MatchParams p) {
         const float chi2 = (((dx * dx) / tolx + (dy * dy) / toly) + (dtx * dtx) * p.inv_tol_tx) +
                            (dty * dty) * p.inv_tol_ty;                             // Eq. 22
         if (!(chi2 < p.chi2m_max)) continue;                                       // L301
-        const int k = atomicAdd(&hdr[0], 1);
+        const int k = smem_inc(&hdr[0]);
         if (k < p.max_mc) {
           MatchCand m;
-          m.seed = (uint16_t)s; m.velo = (uint16_t)v; m.chi2 = chi2; m.q0 = dtx * p.inv_KB;   // A10
-          m.gamma = 0.f; m.key = kNoKey; m.ghost = 0.f; m.pad = 0u;
+          m.seed = (uint16_t)(tile0 + t); m.velo = (uint16_t)v; m.chi2 = chi2; m.q0 = dtx * p.inv_KB;   // A10
+          m.gamma = 0.f; m.key = kNoKey;
 #pragma unroll
           for (int l = 0; l < 4; ++l) m.ut[l] = 0xFFFF;
           mc[k] = m;
@@ -390,7 +438,6 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     __syncthreads();
     LHCB_CLK(11)
   }
-  __syncthreads();
   int nm = hdr[0];
   LHCB_DBG_MAX(4, nm)
   if (nm > p.max_mc) { nm = p.max_mc; if (tid == 0) hdr[2] |= LHCB_ST_MATCH_OVERFLOW; }
@@ -409,16 +456,20 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     }
   }
   LHCB_CLK(14)
-  // searched x0 array (shared tile or global), its y ranges, and the index of its element 0 relative to
+  // searched x0 array (shared tile or global), its y coverage, and the index of its element 0 relative to
   // the event's first UT hit
   const float* __restrict__ ux = ut_in_smem ? sux : p.ux;
-  const float* __restrict__ uylo = p.uylo + (ut_in_smem ? ua0 : 0u);
-  const float* __restrict__ uyhi = p.uyhi + (ut_in_smem ? ua0 : 0u);
   const int rel0 = ut_in_smem ? (int)(ua0 - u_begin) : -(int)u_begin;
+  UtCover cover;
+  cover.row = rows_in_smem ? srow + (ua0 - (u_begin & ~15u)) : nullptr;             // row of x0-tile element i at cover.row[i]
+  cover.ylo = p.urow ? nullptr : p.uylo + (ut_in_smem ? ua0 : 0u);
+  cover.yhi = p.urow ? nullptr : p.uyhi + (ut_in_smem ? ua0 : 0u);
+  cover.y0 = p.row_y0; cover.pitch = p.row_pitch; cover.tol = p.ut_y_tol;
+  if (p.urow && !rows_in_smem) cover.row = p.urow + (ut_in_smem ? ua0 : 0u);       // event too large for the tile: rows from global memory
   const int* uo = hdr + 4;
   if (p.use_ut) {
     // M3a: loose windows, layer by layer until one has hits; each hit is a hypothesis (A13)
-    for (int k = tid; k < nm; k += kMatchThreads) {
+    for (int k = tid; k < nm; k += T) {
       MatchCand& m = mc[k];
       const int v = m.velo;
       const float xV = svx[v], yV = svy[v], txV = svtx[v], tyV = svty[v], q0 = m.q0;
@@ -434,21 +485,21 @@ matching_kernel(const __grid_constant__ MatchParams p) {
         const float lo = x0e - w, hi = x0e + w;
         const int b = uo[i0], ee = uo[i0 + 1];
         for (int j = lower_bound(ux, b, ee, lo); j < ee && ux[j] <= hi; ++j) {
-          if (!(uylo[j] - p.ut_y_tol <= yi && yi <= uyhi[j] + p.ut_y_tol)) continue;
+          if (!cover(j, yi)) continue;
           found = true;
-          const int slot = atomicAdd(&hdr[3], 1);
-          if (slot < p.max_mc) hyq[slot] = ((uint32_t)k << 18) | ((uint32_t)i0 << 16) | (uint32_t)(j + rel0);
+          const int slot = smem_inc(&hdr[3]);
+          if (slot < hyp_cap) hyq[slot] = ((uint32_t)k << 18) | ((uint32_t)i0 << 16) | (uint32_t)(j + rel0);
         }
       }
     }
     __syncthreads();
     int nh = hdr[3];
     LHCB_DBG_MAX(5, nh)
-    if (nh > p.max_mc) { nh = p.max_mc; if (tid == 0) hdr[2] |= LHCB_ST_MATCH_OVERFLOW; }
+    if (nh > hyp_cap) { nh = hyp_cap; if (tid == 0) hdr[2] |= LHCB_ST_MATCH_OVERFLOW; }
     // M3b: tight walk of every hypothesis; the best one of each pair wins the atomicMin and, after the
     // barrier, leaves its hits and gamma_x in the pair's record (a better hypothesis of a later round
     // overwrites them)
-    for (int i0r = 0; i0r < nh; i0r += kMatchThreads) {
+    for (int i0r = 0; i0r < nh; i0r += T) {
       const int i = i0r + tid;
       UtHyp hy;
       unsigned long long key = kNoKey;
@@ -459,7 +510,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
         const int i0 = (int)((hq >> 16) & 3u), jrel = (int)(hq & 0xFFFFu);
         const MatchCand& m = mc[k];
         const int v = m.velo;
-        ut_tight_walk(p, svx[v], svy[v], svtx[v], svty[v], fabsf(m.q0) * 1000.f, i0, jrel - rel0, ux, uylo, uyhi, uo, hy);
+        ut_tight_walk(p, svx[v], svy[v], svtx[v], svty[v], fabsf(m.q0) * 1000.f, i0, jrel - rel0, ux, cover, uo, hy);
         key = ((unsigned long long)(4 - hy.n) << 50) | ((unsigned long long)__float_as_uint(hy.ssq) << 18) |
               (hq & 0x3FFFFu);
         atomicMin(&mc[k].key, key);
@@ -474,20 +525,29 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     }
     __syncthreads();
   }
+  LHCB_CLK(12)
   // a pair is valid if its best hypothesis has enough UT hits (L311); without UT every pair is
   const unsigned long long key_ok = p.use_ut ? (unsigned long long)(4 - p.min_ut_hits) : ~0ull >> 50;
   const bool use_nn = p.nn != nullptr;
   float nn_cut = 0.f, nn_margin = 0.f;
   if (use_nn) {
     // ---- M4 (O14b, L346-348): ghost probability of every valid pair; minimum per seed and per VELO over
-    // the pairs below the cut
-    nn_cut = __ldg(p.nn + 337); nn_margin = __ldg(p.nn + 338);
-    for (int k = tid; k < nm; k += kMatchThreads) {
-      MatchCand& m = mc[k];
+    // the pairs below the cut.  The UT tile is dead: the network and the seed states are staged over it.
+    float* snn = sux;                                                              // [339] (+ padding to 340)
+    float4* sst = reinterpret_cast<float4*>(sux + 340);                            // [ns] x, y, tx, ty
+    for (int i = tid; i < LHCB_GHOST_NN_SIZE; i += T) snn[i] = __ldg(p.nn + i);
+    for (int s = tid; s < ns; s += T) {
+      const size_t slot = slot_of(s);
+      sst[s] = make_float4(p.state[slot], p.state[sct + slot], p.state[2 * sct + slot], p.state[3 * sct + slot]);
+    }
+    __syncthreads();
+    nn_cut = snn[337]; nn_margin = snn[338];
+    for (int k = tid; k < nm; k += T) {
+      const MatchCand& m = mc[k];
       if ((m.key >> 50) > key_ok) continue;
       const int s = m.seed, v = m.velo;
-      const size_t slot = s < c0 ? (size_t)(2 * e) * p.max_seeds + s : (size_t)(2 * e + 1) * p.max_seeds + (s - c0);
-      const float xS = p.state[slot], yS = p.state[sct + slot], txS = p.state[2 * sct + slot], tyS = p.state[3 * sct + slot];
+      const float4 st = sst[s];
+      const float xS = st.x, yS = st.y, txS = st.z, tyS = st.w;
       const float xV = svx[v], yV = svy[v], txV = svtx[v], tyV = svty[v];
       const float dtx = txS - txV, dty = tyS - tyV, adtx = fabsf(dtx);
       const float zm = (((p.mag[0] + p.mag[1] * adtx) + p.mag[2] * (dtx * dtx)) + p.mag[3] * fabsf(xS)) +
@@ -497,9 +557,10 @@ matching_kernel(const __grid_constant__ MatchParams p) {
       float in[8];
       in[0] = zm; in[1] = xs - xv; in[2] = ys - yv; in[3] = dtx; in[4] = dty; in[5] = m.chi2;
       in[6] = nn_eta(txV, tyV);
+      const size_t slot = slot_of(s);
       in[7] = (float)(p.snx && p.snuv ? (int)p.snx[slot] + (int)p.snuv[slot] : 12);
-      const float g = nn_ghost_prob(p.nn, in);
-      m.ghost = g;
+      const float g = nn_ghost_prob(snn, in);
+      sghost[k] = g;
       if (g < nn_cut) {
         atomicMin(&seed_best[s], (unsigned long long)__float_as_uint(g));
         atomicMin(&velo_best[sorig[v]], (unsigned long long)__float_as_uint(g));
@@ -507,37 +568,27 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     }
     __syncthreads();
   } else {
-  for (int k = tid; k < nm; k += kMatchThreads) {
+  for (int k = tid; k < nm; k += T) {
     const MatchCand& m = mc[k];
     if ((m.key >> 50) <= key_ok)
       atomicMin(&seed_best[m.seed], ((unsigned long long)__float_as_uint(m.chi2) << 32) | sorig[m.velo]);
   }
   __syncthreads();
-  LHCB_CLK(12)
   // ---- M4: one-to-one selection (O14) -------------------------------------------------------------
-  for (int k = tid; k < nm; k += kMatchThreads) {
+  for (int k = tid; k < nm; k += T) {
     const MatchCand& m = mc[k];
     if ((m.key >> 50) > key_ok) continue;
     const unsigned long long cb = (unsigned long long)__float_as_uint(m.chi2) << 32;
     if (seed_best[m.seed] != (cb | sorig[m.velo])) continue;
-    atomicMin(&velo_best[sorig[m.velo]], cb | m.seed);
-  }
-  __syncthreads();
-  // Reading A21: an exact chi2 tie between two seeds for one VELO state (twin seeds: bit-identical states
-  // from duplicate hits) is decided by the seeds' hit lists, not by their slot order.  Ties are detected by
-  // every thread; the (rare) event that has one resolves it serially.
-  for (int k = tid; k < nm; k += kMatchThreads) {
-    const MatchCand& m = mc[k];
-    if ((m.key >> 50) > key_ok) continue;
-    const unsigned long long cb = (unsigned long long)__float_as_uint(m.chi2) << 32;
-    if (seed_best[m.seed] != (cb | sorig[m.velo])) continue;
-    const unsigned long long vb = velo_best[sorig[m.velo]];
-    if ((vb >> 32) == (cb >> 32) && (uint32_t)vb != (uint32_t)m.seed) hdr[9] = 1;
+    const unsigned long long old = atomicMin(&velo_best[sorig[m.velo]], cb | m.seed);
+    // Reading A21: an exact chi2 tie between two seeds for one VELO state (twin seeds: bit-identical states
+    // from duplicate hits) is decided by the seeds' hit lists, not by their slot order.  Whoever meets a
+    // different seed at its own chi2 reports the tie; the (rare) event that has one resolves it serially.
+    if ((old >> 32) == (cb >> 32) && (uint32_t)old != (uint32_t)m.seed) hdr[9] = 1;
   }
   __syncthreads();
   if (hdr[9]) {
     if (tid == 0) {
-      auto slot_of = [&](int s) { return s < c0 ? (size_t)(2 * e) * p.max_seeds + s : (size_t)(2 * e + 1) * p.max_seeds + (s - c0); };
       auto before = [&](int a, int b) {                        // hit lists in lexicographic order, then the index
         if (p.shits)
           for (int l = 0; l < 12; ++l) {
@@ -559,23 +610,24 @@ matching_kernel(const __grid_constant__ MatchParams p) {
   }
   }
   const int pol = p.pol ? (int)p.pol[e] : p.polarity;
-  for (int k = tid; k < nm; k += kMatchThreads) {
+  for (int k = tid; k < nm; k += T) {
     const MatchCand& m = mc[k];
     if ((m.key >> 50) > key_ok) continue;
     const unsigned long long cb = (unsigned long long)__float_as_uint(m.chi2) << 32;
     const int vo = sorig[m.velo];
+    float g = 0.f;
     if (use_nn) {
       // kept if below the cut and no track sharing its seed or its VELO is better by the margin (the minimum
       // includes the track itself, which never satisfies g >= g + margin)
-      if (!(m.ghost < nn_cut)) continue;
+      g = sghost[k];
+      if (!(g < nn_cut)) continue;
       const float gs = __uint_as_float((unsigned int)seed_best[m.seed]), gv = __uint_as_float((unsigned int)velo_best[vo]);
-      if (m.ghost >= gs + nn_margin || m.ghost >= gv + nn_margin) continue;
+      if (g >= gs + nn_margin || g >= gv + nn_margin) continue;
     } else if (seed_best[m.seed] != (cb | vo) || velo_best[vo] != (cb | m.seed)) continue;
-    const int slot = atomicAdd(&hdr[1], 1);
+    const int slot = smem_inc(&hdr[1]);
     if (slot >= p.max_long) continue;
     const size_t o = (size_t)e * p.max_long + slot, ct = p.long_cap_total;
-    const int s = m.seed;
-    p.seed_idx[o] = s < c0 ? (uint32_t)((2 * e) * p.max_seeds + s) : (uint32_t)((2 * e + 1) * p.max_seeds + (s - c0));
+    p.seed_idx[o] = (uint32_t)slot_of(m.seed);
     p.velo_idx[o] = v0 + vo;
     float q = m.q0;                                                              // A10
     if (p.use_ut) {
@@ -591,7 +643,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     }
     p.qop[o] = pol > 0 ? q : -q;
     p.chi2[o] = m.chi2;
-    if (use_nn && p.ghost) p.ghost[o] = m.ghost;
+    if (use_nn && p.ghost) p.ghost[o] = g;
   }
   __syncthreads();
   LHCB_CLK(13)

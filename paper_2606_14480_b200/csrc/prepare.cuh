@@ -119,7 +119,8 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
       sum += (int)(v[2 * k] + v[2 * k + 1]);
     }
     int total;
-    int run = block_exscan<T>(sum, warp_sums, total);
+    int flip = 0;                                          // a single scan: only the first warp_sums buffer is used
+    int run = block_exscan<T>(sum, warp_sums, flip, total);
 #pragma unroll
     for (int k = 0; k < per / 2; ++k) {
       const unsigned int lo = (unsigned int)run; run += (int)v[2 * k];

@@ -1,23 +1,25 @@
 // SciFi Seeding kernel (section 3) for sm_100a.
 //
-// One CTA per event-half (L372): the half's twelve sorted hit zones are staged into shared memory
-// with one bulk async copy (cp.async.bulk + mbarrier) and stay there for every step (L370).
-// Stages, separated by __syncthreads():
-//   S0  staging + bin tables           per zone, a 320-bin table "first hit with bin >= k" turns every
-//                                      lower/upper bound and closest-hit search into one lookup plus a
-//                                      short scan (about 0.5 hits per bin)
-//   S1  two-hit + three-hit search     per iteration: thread per T1 hit finds its T3 window (Eq. 8-11); a
-//                                      block scan flattens all pairs; each thread walks a contiguous chunk
-//                                      of pairs: Eq. 3-5 and the T2 band (Eq. 12-13, A3/A4); the triplets of
-//                                      both iterations go to one queue in shared memory
+// One CTA per event-half (L372): the half's twelve sorted hit zones are staged into shared memory and stay
+// there for every step (L370).  In the staged tile every zone is framed by a -inf and a +inf sentinel, so
+// that no search needs a bounds check.  Stages, separated by __syncthreads():
+//   S0  staging + bin tables           per zone, a 320-bin table "first hit with bin >= k" turns every lower
+//                                      bound into one lookup plus a short forward scan (about 0.5 hits per
+//                                      bin); the table is built by marking the first hit of every occupied
+//                                      bin and a ballot-based suffix fill, one warp per zone
+//   S1  two-hit + three-hit search     per iteration: thread per T1 hit finds its T3 window (Eq. 8-11) and
+//                                      cuts it into items of at most 8 consecutive T3 hits; thread per item:
+//                                      Eq. 3-5 and the T2 band (Eq. 12-13, A3/A4) for its pairs, with one
+//                                      T2 pointer that only moves forward (the band moves monotonically with
+//                                      x3); the triplets of both iterations go to one queue in shared memory
 //   S2  extension                      thread per queued triplet: exact parabola, +-1 mm closest hit in
 //                                      the other three x-layers, >= 5 hits -> queued candidate (L90)
 //   S2b fit                            dense pass over the candidates: fixed-matrix least squares, chi2 cut
 //   S3  clone kill                     64-bit atomicMin table per x-hit, vote pass (L183-200, Eq. 15);
 //                                      survivors are compacted to the bottom of the work region
-//   S4  u/v addition, iterative        (survivor, pass, first-layer hit) items flattened the same way
-//                                      (Eq. 16): phase A walks three stereo layers of every
-//                                      item, phase B finishes the walks that can still succeed
+//   S4  u/v addition, iterative        (survivor, pass, first-layer hit) items (Eq. 16): phase A
+//                                      walks three stereo layers of every item, phase B finishes the walks
+//                                      that can still succeed
 //   S4h u/v addition, Hough clusters   (lhcb_set_uv_hough, L217, reading A20) votes as 64-bit masks per
 //                                      (survivor, layer), bit-sliced populations, hypothesis pass
 //   S5  y fit + seed output            thread per queued combination: y fit, best per survivor by
@@ -32,21 +34,26 @@
 
 namespace lhcb {
 
-#ifndef LHCB_PROBES
-#define LHCB_PROBES 3     // hits probed without a branch by closest_hit
-#endif
 #ifndef LHCB_LUT_BINS
 #define LHCB_LUT_BINS 320
 #endif
+#ifndef LHCB_ITEM_PAIRS
+#define LHCB_ITEM_PAIRS 8   // T3 hits per item of the pair walk (a power of two, at most 8)
+#endif
 constexpr int kSeedThreadsMax = 512;          // the kernel is instantiated for 256 x 4 CTAs/SM and 512 x 2 CTAs/SM
 constexpr int kLutBins = LHCB_LUT_BINS;       // bins of the per-zone search table
+constexpr int kItemPairs = LHCB_ITEM_PAIRS;
+constexpr int kTileIndexBits = 13;            // tile indices fit 13 bits: max_hits_per_half + 172 <= 8192
 constexpr unsigned long long kNoKey = ~0ull;
+static_assert(kLutBins % 32 == 0, "the suffix fill of the bin tables works on whole warps of bins");
+static_assert(kItemPairs == 2 || kItemPairs == 4 || kItemPairs == 8, "item length");
 
-// Optional per-stage cycle counters (diagnostic builds only: -DLHCB_STAGE_CLOCKS).  Thread 0 of every
-// CTA adds the cycles since its previous mark to g_stage_clk[i]; lhcb_debug_stage_clocks() reads them.
+// Optional per-stage cycle counters (diagnostic build only: -DLHCB_STAGE_CLOCKS, bench.py --stage-clocks).
+// Thread 0 of every CTA adds the cycles since its previous mark to g_stage_clk[i];
+// lhcb_debug_stage_clocks() reads them.
 #ifdef LHCB_STAGE_CLOCKS
 __device__ unsigned long long g_stage_clk[16];
-__device__ unsigned int g_dbg_max[8];     // maxima over CTAs: triplets per iteration, candidates, survivors, queued u/v combinations
+__device__ unsigned int g_dbg_max[8];     // maxima over CTAs: triplets, candidates, survivors, queued u/v combinations, ...
 #define LHCB_DBG_MAX(i, v) if (threadIdx.x == 0) atomicMax(&g_dbg_max[i], (unsigned int)(v));
 #define LHCB_CLK_INIT long long clk_prev__ = clock64();
 #define LHCB_CLK(i)                                                                         \
@@ -66,6 +73,7 @@ struct SeedParams {
   float ywin_a[2][12], ywin_b[2][12];
   int xl[6], ul[6], slot_of_layer[12];
   int l1[2], l2[2], l3[2];
+  int ol[2][3], os[2][3], ss[2][3];   // per iteration: the three other x-layers, their x-slots, the x-slots of l1 l2 l3
   float dx3max[2], r13[2], inv_dz13[2], z1[2], dz12[2], K[2], inv_K[2], G13[2];
   float a, b, kappa, inv_kappa, f_lo, f_hi, d_lo, d_hi, tol_x, tol_uv, chi2x_max, chi2y_max;
   float wx[7], wy[7];
@@ -74,7 +82,7 @@ struct SeedParams {
   int max_seeds, max_cand, max_hits, max_trip;
   int uv_hough;                       // Hough-cluster UV seeding (L217, reading A20) instead of the iterative one
   float h_tlo[2], h_w, h_invw;        // its t_y bins: b = clamp((t - tlo[half]) * invw, 0, 63), width w
-  int smem_total;   // dynamic shared memory of the launch = seed_smem_bytes(threads, capacities)
+  int smem_total;   // dynamic shared memory of the launch = seed_smem_bytes(capacities)
   const float* P;   // [7][3][6]
   const float* Q;   // [64][2][6]
   // batch
@@ -83,6 +91,7 @@ struct SeedParams {
   const uint32_t* zone_off;
   const float* hit_x;
   const int8_t* pol;
+  const uint32_t* order;   // optional CTA -> event-half map (heaviest halves first) or NULL
   uint32_t* count;
   float* state;
   float* par;
@@ -93,95 +102,91 @@ struct SeedParams {
   size_t cap_total;
 };
 
-struct __align__(8) Triplet { uint16_t i1, i2, i3, it; };                 // zone-local indices
+// all hit references inside the kernel are TILE indices (position in the staged, sentinel-framed tile)
+struct __align__(8) Triplet { uint16_t i1, i2, i3, it; };
 struct __align__(16) Cand { float ax, bx, cx, chi2; uint16_t hit[6]; uint8_t nx, it, keep, pattern; };   // nx = 0: rejected by the fit
 
-struct __align__(16) Zone { int b, e; float x0, invw; };   // one 16-byte shared-memory load
+struct __align__(16) Zone { int b, e; float x0, invw; };   // hits [b, e) of the tile; one 16-byte shared-memory load
 
 struct SeedSmemHeader {
   unsigned long long mbar;
-  int zl[13];          // zone offsets relative to the staged tile
-  int xbase[7];        // prefix of x-zone sizes (clone-table index base per x-slot)
+  unsigned long long pad_;
   Zone zi[12];         // per zone: [b, e) in the tile and bin(v) = clamp((v - x0) * invw, 0, kLutBins-1)
   float4 uvc[6];       // per stereo slot: {z tan(alpha), 1/tan(alpha), 1/z, layer index (int bits)}
+  uint32_t zg[12];     // global hit index = tile index + zg[layer]
+  int xoff[6];         // clone-table index of an x-hit = tile index + xoff[x-slot]
+  int n_xhits;
   int n_trip, n_cand, n_kept, n_seed, n_live;
   unsigned int status;
-  int warp_sums[kSeedThreadsMax / 32 + 1];
+  int warp_sums[2][kSeedThreadsMax / 32 + 1];   // two buffers: consecutive block scans never share one
 };
 
 constexpr int kSeedHeaderBytes = 640;
 static_assert(sizeof(SeedSmemHeader) <= kSeedHeaderBytes, "shared-memory header overflows its slot");
 
-// Shared-memory map of one CTA (NT threads), all offsets 16-byte aligned:
-//   [header | bin tables | scan scratch: int offs[NT+1], u16 first[NT], later the kept list u16[max_cand] |
-//    hits tile (the half's ACTUAL size) | work region W ... | x-z candidates, filled downward from the end]
-// W holds the triplet queue, then the clone table, then the u/v queues; it starts right after the staged
-// hits and ends where the candidates begin, so a half with fewer hits or candidates than the capacities
-// leaves more room for the queues.  The capacities guarantee W >= max_trip * 8 bytes.
+// Shared-memory map of one CTA, all offsets 16-byte aligned:
+//   [header | bin tables | kept list u16[max_cand] | hits tile (the half's ACTUAL size) | work region W ... |
+//    x-z candidates, filled downward from the end]
+// The tile holds, per zone, [..., -inf, hits ..., +inf, ...].  W holds the triplet queue, then the clone table, then the
+// u/v queues; it starts right after the tile and ends where the candidates begin, so a half with fewer hits or
+// candidates than the capacities leaves more room for the queues.  The capacities guarantee
+// W >= max_trip * 8 bytes.  During S1 the (still empty) candidate slots hold the items of the pair walk.
 __host__ __device__ inline size_t seed_align16(size_t b) { return (b + 15) & ~(size_t)15; }
-__host__ __device__ inline size_t seed_off_scan() { return kSeedHeaderBytes + seed_align16(12 * (kLutBins + 1) * 2); }
-// the kept list (clone-kill survivors, used from S3 on) shares its slot with the scan scratch (used by S1 only)
-__host__ __device__ inline size_t seed_off_hits(int nt, int max_cand) {
-  const size_t scan = (size_t)(nt + 1) * 4 + (size_t)nt * 2, kept = (size_t)max_cand * 2;
-  return seed_off_scan() + seed_align16(scan > kept ? scan : kept);
-}
-__host__ __device__ inline size_t seed_smem_bytes(int nt, int max_hits, int max_cand, int max_trip) {
-  size_t b = seed_off_hits(nt, max_cand);
-  b += seed_align16(((size_t)max_hits + 8) * 4 + 16);      // hits tile (16-byte aligned superset) + padding
+__host__ __device__ inline size_t seed_off_kept() { return kSeedHeaderBytes + seed_align16(12 * (kLutBins + 1) * 2); }
+__host__ __device__ inline size_t seed_off_hits(int max_cand) { return seed_off_kept() + seed_align16((size_t)max_cand * 2); }
+// tile: per zone [4 floats | aligned superset of the zone (at most 6 floats more than its hits) | 4 floats]
+__host__ __device__ inline size_t seed_tile_bytes(int n_hits) { return seed_align16(((size_t)n_hits + 12 * 14) * 4 + 16); }
+__host__ __device__ inline size_t seed_smem_bytes(int max_hits, int max_cand, int max_trip) {
+  size_t b = seed_off_hits(max_cand);
+  b += seed_tile_bytes(max_hits);                           // hits tile with its 24 sentinels
   b += seed_align16((size_t)max_trip * 8);                 // work region W (minimum)
   b += (size_t)max_cand * 32;                              // candidates
   return b;
 }
 
 // ------------------------------------------------------------------------------------ searches
-// Sorted zone + bin table.  lut[k] = first tile index whose bin is >= k (lut[kLutBins] = zone end).
-// bin() is monotone in v, so every hit before lut[bin(v)] is < v: the exact lower/upper bound is
-// lut[bin(v)] plus a forward scan inside one bin (about one hit per bin).  Pure comparisons: the
-// result is identical to a binary search, whatever the rounding of bin().
+// Sorted zone framed by sentinels + bin table.  lut[k] = first tile index whose bin is >= k
+// (lut[kLutBins] = zone end, the +inf sentinel).  bin() is monotone in v, so every hit before lut[bin(v)] is
+// < v: the exact lower/upper bound is lut[bin(v)] plus a forward scan inside one bin (about half a hit per
+// bin), which the +inf sentinel ends.  Pure comparisons: the result is identical to a binary search, whatever
+// the rounding of bin().
+// bin(v): any monotone function of v used alike by the table build and the lookups.  Rounded to the nearest
+// integer by adding 2^23 (one FADD instead of a conversion on the slower XU pipe); NaN lands in bin 0.
 __device__ __forceinline__ int zone_bin(const Zone& z, float v) {
   float t = (v - z.x0) * z.invw;
   t = fminf(fmaxf(t, 0.f), (float)(kLutBins - 1));
-  return (int)t;
+  return __float_as_int(t + 8388608.f) & 0x3FF;
 }
-// first index in [b, e) with x[i] >= v
-__device__ __forceinline__ int lower_bound(const float* __restrict__ x, const uint16_t* __restrict__ lut,
-                                           const Zone& z, float v) {
-  int i = lut[zone_bin(z, v)];
-  // about one hit per bin: two predicated steps cover almost every call, the loop is the rare tail
-  bool m = i < z.e && x[i] < v;
-  i += m;
-  m = m && i < z.e && x[i] < v;
-  i += m;
-  if (m)
-    while (i < z.e && x[i] < v) ++i;
-  return i;
+static_assert(kLutBins <= 1024, "zone_bin keeps ten bits");
+
+// shared-memory counter + 1, returning the old value: one ATOMS per lane (the compiler's warp-aggregated
+// atomicAdd costs about twenty instructions on the divergent paths where the queues are appended)
+__device__ __forceinline__ int smem_inc(int* counter) {
+  int old;
+  asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(old) : "r"((uint32_t)__cvta_generic_to_shared(counter)) : "memory");
+  return old;
 }
-// the same, also returning x[i] (+inf when i == e)
+// first index in [b, e] with x[i] >= v, also returning x[i] (+inf at e)
 __device__ __forceinline__ int lower_bound_v(const float* __restrict__ x, const uint16_t* __restrict__ lut,
                                              const Zone& z, float v, float& xv) {
-  const float inf = __int_as_float(0x7f800000);
   int i = lut[zone_bin(z, v)];
-  float xi = i < z.e ? x[i] : inf;
-  if (xi < v) {
-    ++i; xi = i < z.e ? x[i] : inf;
-    if (xi < v) {
-      ++i; xi = i < z.e ? x[i] : inf;
-      while (xi < v) { ++i; xi = i < z.e ? x[i] : inf; }
-    }
-  }
+  float xi = x[i];
+  while (xi < v) { ++i; xi = x[i]; }
   xv = xi;
   return i;
 }
-// first index in [b, e) with x[i] > v
+__device__ __forceinline__ int lower_bound(const float* __restrict__ x, const uint16_t* __restrict__ lut,
+                                           const Zone& z, float v) {
+  float xv;
+  return lower_bound_v(x, lut, z, v, xv);
+}
+// first index in [b, e] with x[i] > v
 __device__ __forceinline__ int upper_bound(const float* __restrict__ x, const uint16_t* __restrict__ lut,
                                            const Zone& z, float v) {
+  v = fminf(v, 3.4028235e38f);                               // the +inf sentinel must end the scan
   int i = lut[zone_bin(z, v)];
-  bool m = i < z.e && x[i] <= v;
-  i += m;
-  m = m && i < z.e && x[i] <= v;
-  i += m;
-  if (m)
-    while (i < z.e && x[i] <= v) ++i;
+  float xi = x[i];
+  while (xi <= v) { ++i; xi = x[i]; }
   return i;
 }
 // plain binary searches (global-memory arrays without a bin table)
@@ -206,66 +211,59 @@ __device__ __forceinline__ int owner_of(const int* offs, int n, int p) {
   }
   return b;
 }
-// index of the hit closest to xp with |x - xp| <= tol, ties to the lower index; -1 if none.
-// The scan starts at the bin of (xp - tol - guard), so every hit that can pass the literal predicate
-// fabsf(x - xp) <= tol is visited (the guard of 1/64 mm is far above one rounding of x - xp at
-// |x| < 2^15 mm), and ends at the first hit above xp + tol + guard.  Strict "<" keeps the lowest index
-// among equal distances, like the oracle's linear scan.  With about 0.6 hits per bin the first three
-// hits from the bin start almost always reach past the window: they are probed without a branch (every
-// lane of the warp does the same work); the loop is the rare tail.
+// Index of the hit closest to xp with |x - xp| <= tol, ties to the lower index; -1 if none.  The zone is
+// sorted, so with R the first hit >= xp and L = R - 1, every hit left of L is at least as far as L and every
+// hit right of R at least as far as R (float subtraction is monotone): the minimum of |x - xp| is at L or R,
+// "L if d_L <= d_R" keeps the lower index on a tie, and the only other hits with that same distance are equal
+// neighbours further left (duplicates), which the walk back finds.  This is the hit the oracle's linear scan
+// with "strictly closer replaces" selects.  The sentinels (-inf before, +inf after the zone) make every
+// access safe and give the distance +inf.
 __device__ __forceinline__ int closest_hit(const float* __restrict__ x, const uint16_t* __restrict__ lut,
                                            const Zone& z, float xp, float tol, float& xbest) {
-  const float guard = tol + 0.015625f;
-  const float hi = xp + guard;
-  const int i0 = lut[zone_bin(z, xp - guard)];
-  int best = -1;
-  float bd = 0.f, xlast = 0.f;
-#pragma unroll
-  for (int k = 0; k < LHCB_PROBES; ++k) {
-    const float v = x[i0 + k];                               // at most 3 floats past the zone: still shared memory
-    const float xi = i0 + k < z.e ? v : __int_as_float(0x7f800000);
-    const float d = fabsf(xi - xp);
-    const bool ok = d <= tol && (best < 0 || d < bd);
-    best = ok ? i0 + k : best; bd = ok ? d : bd; xbest = ok ? xi : xbest;
-    xlast = xi;
+  int i = lut[zone_bin(z, xp)];
+  float xr = x[i];
+  while (xr < xp) { ++i; xr = x[i]; }
+  const float xl = x[i - 1], xll = x[i - 2];                 // (i - 2 is at worst a sentinel or padding)
+  const float dl = fabsf(xl - xp), dr = fabsf(xr - xp);
+  const bool left = dl <= dr;
+  const float d = left ? dl : dr;
+  const bool ok = d <= tol;
+  xbest = left ? xl : xr;
+  i -= left;
+  if (left && ok && fabsf(xll - xp) == d) {                 // duplicates: the lowest index among equal distances
+    --i;
+    while (fabsf(x[i - 1] - xp) == d) --i;
   }
-  if (xlast <= hi) {
-    int i = i0 + LHCB_PROBES;
-    while (i < z.e) {
-      const float xi = x[i];
-      if (xi > hi) break;
-      const float d = fabsf(xi - xp);
-      if (d <= tol && (best < 0 || d < bd)) { best = i; bd = d; xbest = xi; }
-      ++i;
-    }
-  }
-  return best;
+  return ok ? i : -1;
 }
 
-// exclusive prefix sum of one int per thread over the CTA; total returned to every thread
+// exclusive prefix sum of one int per thread over the CTA; total returned to every thread.  `flip` selects
+// one of the two warp_sums buffers and is toggled: a call may follow the previous one without a barrier.
 template <int NT>
-__device__ __forceinline__ int block_exscan(int v, int* warp_sums, int& total) {
+__device__ __forceinline__ int block_exscan(int v, int* warp_sums /* [2][kSeedThreadsMax / 32 + 1] */, int& flip, int& total) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  int* ws = warp_sums + flip * (kSeedThreadsMax / 32 + 1);
+  flip ^= 1;
   int inc = v;
 #pragma unroll
   for (int o = 1; o < 32; o <<= 1) {
     const int t = __shfl_up_sync(0xffffffffu, inc, o);
     if (lane >= o) inc += t;
   }
-  if (lane == 31) warp_sums[warp] = inc;
+  if (lane == 31) ws[warp] = inc;
   __syncthreads();
   if (warp == 0) {
-    int w = lane < NT / 32 ? warp_sums[lane] : 0;
+    int w = lane < NT / 32 ? ws[lane] : 0;
 #pragma unroll
     for (int o = 1; o < NT / 32; o <<= 1) {
       const int t = __shfl_up_sync(0xffffffffu, w, o);
       if (lane >= o) w += t;
     }
-    if (lane < NT / 32) warp_sums[lane] = w;                 // inclusive warp totals
+    if (lane < NT / 32) ws[lane] = w;                        // inclusive warp totals
   }
   __syncthreads();
-  total = warp_sums[NT / 32 - 1];
-  const int base = warp ? warp_sums[warp - 1] : 0;
+  total = ws[NT / 32 - 1];
+  const int base = warp ? ws[warp - 1] : 0;
   return base + inc - v;
 }
 
@@ -346,65 +344,96 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   extern __shared__ __align__(16) unsigned char smem[];
   SeedSmemHeader& H = *reinterpret_cast<SeedSmemHeader*>(smem);
   uint16_t* lut = reinterpret_cast<uint16_t*>(smem + kSeedHeaderBytes);
-  int* scan_offs = reinterpret_cast<int*>(smem + seed_off_scan());            // [NT + 1] exclusive offsets
-  uint16_t* scan_first = reinterpret_cast<uint16_t*>(scan_offs + NT + 1);      // [NT] first index per owner
-  uint16_t* kept = reinterpret_cast<uint16_t*>(smem + seed_off_scan());         // aliases the scan scratch
-  const int off_hits = (int)seed_off_hits(NT, p.max_cand);
+  uint16_t* kept = reinterpret_cast<uint16_t*>(smem + seed_off_kept());
+  const int off_hits = (int)seed_off_hits(p.max_cand);
   float* hx = reinterpret_cast<float*>(smem + off_hits);
   Cand* cand_end = reinterpret_cast<Cand*>(smem + p.smem_total);               // candidate c lives at cand_end[-1 - c]
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   constexpr int T = NT, nwarps = NT / 32;
+  const float inf = __int_as_float(0x7f800000);
+  int flip = 0;                                            // buffer of the next block scan
   LHCB_CLK_INIT
-  const int half_id = blockIdx.x, event = half_id >> 1, h = half_id & 1;
+  const int half_id = p.order ? (int)p.order[blockIdx.x] : (int)blockIdx.x, event = half_id >> 1, h = half_id & 1;
   const uint32_t* zo = p.zone_off + (size_t)half_id * 12;
 
-  const uint32_t g_begin = zo[0], g_end = zo[12];
-  const uint32_t a0 = g_begin & ~3u;                       // 16-byte aligned start of the staged tile
-  const int n_half = (int)(g_end - g_begin);
+  // ---- S0: stage the half's hits, every zone framed by sentinels ----------------------------------
+  // One bulk async copy per zone (cp.async.bulk needs 16-byte aligned addresses and sizes: each copy takes
+  // the aligned superset of its zone, so up to three hits of the neighbouring zones land beside it; the
+  // region of a zone is [4 floats | superset | 4 floats] and the sentinels are written over the neighbours
+  // once the copies have landed).  Zone z: region start rb (multiple of 4), first hit at rb + 4 + (zoff & 3).
+  uint32_t zoff[13];
+#pragma unroll
+  for (int z = 0; z < 13; ++z) zoff[z] = __ldg(zo + z);
+  const int n_half = (int)(zoff[12] - zoff[0]);
   const uint32_t slot0 = (uint32_t)half_id * (uint32_t)p.max_seeds;
-
   if (n_half > p.max_hits) {                               // uniform: whole CTA leaves
     if (tid == 0) { p.count[half_id] = 0; p.status[half_id] = LHCB_ST_HITS_OVERFLOW; }
     return;
   }
-
-  // ---- S0: stage the half's hits -----------------------------------------------------
-  const bool aligned = ((reinterpret_cast<uintptr_t>(p.hit_x) & 15) == 0);
-  uint32_t a1 = (g_end + 3u) & ~3u;                        // end of the bulk part (multiple of 4 floats)
-  if (a1 > (p.n_hits & ~3u)) a1 = p.n_hits & ~3u;
-  if (!aligned || a1 < a0) a1 = a0;
+  const bool aligned = (reinterpret_cast<uintptr_t>(p.hit_x) & 15) == 0;
+  const uint32_t n_al = p.n_hits & ~3u;                    // bulk copies stay inside the array
   const uint32_t mbar_addr = (uint32_t)__cvta_generic_to_shared(&H.mbar);
   if (tid == 0) {
     H.n_trip = 0; H.n_cand = 0; H.n_kept = 0; H.n_seed = 0; H.status = 0;
     asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar_addr));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    uint32_t bytes = 0;
+    if (aligned) {
+#pragma unroll
+      for (int z = 0; z < 12; ++z) {
+        const uint32_t s0 = zoff[z] & ~3u;
+        uint32_t s1 = (zoff[z + 1] + 3u) & ~3u;
+        if (s1 > n_al) s1 = n_al;
+        if (zoff[z + 1] > zoff[z] && s1 > s0) bytes += (s1 - s0) * 4u;
+      }
+    }
+    if (bytes) asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar_addr), "r"(bytes) : "memory");
+    else asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(mbar_addr) : "memory");
+    int acc = 0, rb = 0, xs = 0;
+#pragma unroll
+    for (int z = 0; z < 12; ++z) {                         // the copies; x-hits are numbered densely for the clone table
+      const int n = (int)(zoff[z + 1] - zoff[z]);
+      const uint32_t s0 = zoff[z] & ~3u;
+      uint32_t s1 = (zoff[z + 1] + 3u) & ~3u;
+      const int span = (int)(s1 - s0);
+      if (s1 > n_al) s1 = n_al;
+      if (aligned && n > 0 && s1 > s0)
+        asm volatile(
+            "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                (uint32_t)__cvta_generic_to_shared(hx + rb + 4)),
+            "l"(p.hit_x + s0), "r"((s1 - s0) * 4u), "r"(mbar_addr)
+            : "memory");
+      const int pos = rb + 4 + (int)(zoff[z] & 3u);
+      if (xs < 6 && p.xl[xs] == z) { H.xoff[xs] = acc - pos; acc += n; ++xs; }
+      rb += (n > 0 ? span : 0) + 8;
+    }
+    H.n_xhits = acc;
   }
-  if (tid < 13) H.zl[tid] = (int)(zo[tid] - a0);
-  if (tid >= 32 && tid < 38) {
-    const int l = p.ul[tid - 32];
-    H.uvc[tid - 32] = make_float4(p.zt[l], p.inv_tan[l], p.inv_z[l], __int_as_float(l));
+  if (tid >= 64 && tid < 70) {
+    const int l = p.ul[tid - 64];
+    H.uvc[tid - 64] = make_float4(p.zt[l], p.inv_tan[l], p.inv_z[l], __int_as_float(l));
   }
-  __syncthreads();
-  if (tid == 0) {
-    int acc = 0;
-    for (int s = 0; s < 6; ++s) { H.xbase[s] = acc; acc += H.zl[p.xl[s] + 1] - H.zl[p.xl[s]]; }
-    H.xbase[6] = acc;
-    const uint32_t bytes = (a1 - a0) * 4u;
-    if (bytes > 0) {
-      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar_addr), "r"(bytes) : "memory");
-      asm volatile(
-          "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-              (uint32_t)__cvta_generic_to_shared(hx)),
-          "l"(p.hit_x + a0), "r"(bytes), "r"(mbar_addr)
-          : "memory");
-    } else {
-      asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(mbar_addr) : "memory");
+  {                                                        // bin tables: every entry "unmarked"
+    uint32_t* L32 = reinterpret_cast<uint32_t*>(lut);
+    constexpr int nw = (12 * (kLutBins + 1) + 1) / 2;
+    for (int i = tid; i < nw; i += T) L32[i] = 0xFFFFFFFFu;
+  }
+  {
+    // what the bulk copies do not cover: everything when the source is not 16-byte aligned, else the last
+    // (at most three) hits of a zone that ends in the unaligned tail of the array
+    int rb = 0;
+#pragma unroll
+    for (int z = 0; z < 12; ++z) {
+      const int n = (int)(zoff[z + 1] - zoff[z]);
+      const uint32_t s0 = zoff[z] & ~3u;
+      const uint32_t s1 = (zoff[z + 1] + 3u) & ~3u;
+      const int pos = rb + 4 + (int)(zoff[z] & 3u);
+      uint32_t from = aligned ? (s1 > n_al ? (n_al > zoff[z] ? n_al : zoff[z]) : zoff[z + 1]) : zoff[z];
+      for (uint32_t i = from + tid; i < zoff[z + 1]; i += T) hx[pos + (int)(i - zoff[z])] = __ldg(p.hit_x + i);
+      rb += (n > 0 ? (int)(s1 - s0) : 0) + 8;
     }
   }
-  // tail (and the whole tile when the source is not 16-byte aligned) with plain loads
-  for (uint32_t i = a1 + tid; i < g_end; i += T) hx[i - a0] = p.hit_x[i];
-  if (tid < 4) hx[(g_end > a1 ? g_end : a1) - a0 + tid] = __int_as_float(0x7f800000);
   {
     uint32_t done = 0;
     while (!done) {
@@ -417,97 +446,119 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
           : "memory");
     }
   }
+  if (tid >= 32 && tid < 44) {                             // sentinels, bin function and index map of zone tid - 32
+    int rb = 0, pos = 0, n = 0;
+    uint32_t z0 = 0;
+#pragma unroll
+    for (int z = 0; z < 12; ++z) {
+      const int nz = (int)(zoff[z + 1] - zoff[z]);
+      if (z == tid - 32) { pos = rb + 4 + (int)(zoff[z] & 3u); n = nz; z0 = zoff[z]; }
+      rb += (nz > 0 ? (int)(((zoff[z + 1] + 3u) & ~3u) - (zoff[z] & ~3u)) : 0) + 8;
+    }
+    float x0 = 0.f, invw = 0.f;
+    if (n > 0) {
+      x0 = hx[pos];
+      const float span = hx[pos + n - 1] - x0;
+      invw = span > 0.f ? (float)kLutBins / span : 0.f;
+    }
+    // (the two stores below may hit hits of the neighbouring zones that the aligned superset brought along;
+    // a tail hit written by another thread is never at pos - 1 / pos + n of this zone)
+    hx[pos - 2] = -inf; hx[pos - 1] = -inf; hx[pos + n] = inf;
+    Zone zn; zn.b = pos; zn.e = pos + n; zn.x0 = x0; zn.invw = invw;
+    H.zi[tid - 32] = zn;
+    H.zg[tid - 32] = z0 - (uint32_t)pos;
+  }
   __syncthreads();
   LHCB_CLK(0)
-  const int* zl = H.zl;
-  // work region W: from the end of the staged tile to the first candidate slot
-  // (16 bytes of +inf padding after the tile: the three-probe searches may read up to 3 floats past a zone)
-  const int off_w = (int)seed_align16((size_t)off_hits + (size_t)((g_end > a1 ? g_end : a1) - a0) * 4 + 16);
+  // work region W: from the end of the tile to the first candidate slot
+  const int off_w = off_hits + (int)seed_tile_bytes(n_half);
   const int w_stat = p.smem_total - p.max_cand * (int)sizeof(Cand) - off_w;   // bytes of W with every candidate slot used
   Triplet* trip = reinterpret_cast<Triplet*>(smem + off_w);
   unsigned long long* tbl = reinterpret_cast<unsigned long long*>(smem + off_w);   // aliases trip
   const int trip_cap = w_stat / 8;
-  if (H.xbase[6] > trip_cap) {                              // clone table would not fit
+  if (H.n_xhits > trip_cap) {                               // clone table would not fit
     if (tid == 0) { p.count[half_id] = 0; p.status[half_id] = LHCB_ST_HITS_OVERFLOW; }
     return;
   }
-  // bin tables: per zone, bins span [first hit, last hit]
-  if (tid < 12) {
-    const int b = zl[tid], e = zl[tid + 1];
-    float x0 = 0.f, invw = 0.f;
-    if (e > b) {
-      x0 = hx[b];
-      const float span = hx[e - 1] - x0;
-      invw = span > 0.f ? (float)kLutBins / span : 0.f;
-    }
-    Zone z; z.b = b; z.e = e; z.x0 = x0; z.invw = invw;
-    H.zi[tid] = z;
-  }
-  __syncthreads();
-  // 24 units (zone, half of its hits) over the warps: each hit fills the bins (bin of its predecessor, its bin]
-  for (int u = warp; u < 24; u += nwarps) {
-    const int z = u >> 1, part = u & 1;
+  // the first hit of every occupied bin marks its entry ...
+#pragma unroll 1
+  for (int z = 0; z < 12; ++z) {
     const Zone zz = H.zi[z];
     uint16_t* L = lut + z * (kLutBins + 1);
-    if (zz.e == zz.b) {
-      for (int k = lane + part * 32; k <= kLutBins; k += 64) L[k] = (uint16_t)zz.b;
-    } else {
-      const int mid = zz.b + ((zz.e - zz.b + 1) >> 1);
-      const int ib = part ? mid : zz.b, ie = part ? zz.e : mid;
-      for (int i = ib + lane; i < ie; i += 32) {
-        const int k1 = zone_bin(zz, hx[i]);
-        const int k0 = i == zz.b ? -1 : zone_bin(zz, hx[i - 1]);
-        for (int k = k0 + 1; k <= k1; ++k) L[k] = (uint16_t)i;
-        if (i == zz.e - 1)
-          for (int k = k1 + 1; k <= kLutBins; ++k) L[k] = (uint16_t)zz.e;
-      }
+    for (int i = zz.b + tid; i < zz.e; i += T) {
+      const int k1 = zone_bin(zz, hx[i]);
+      const int k0 = zone_bin(zz, hx[i - 1]);              // -inf in front of the first hit: bin 0
+      if (i == zz.b || k1 != k0) L[k1] = (uint16_t)i;
+    }
+  }
+  __syncthreads();
+  // ... and every empty bin takes the entry of the next marked bin above it (zone end after the last one):
+  // one warp per zone, 32 bins at a time from the top, the next marked bin of a lane from a ballot
+  for (int z = warp; z < 12; z += nwarps) {
+    uint16_t* L = lut + z * (kLutBins + 1);
+    unsigned carry = (unsigned)H.zi[z].e;
+    if (lane == 0) L[kLutBins] = (uint16_t)carry;
+#pragma unroll 2
+    for (int c = kLutBins / 32 - 1; c >= 0; --c) {
+      const unsigned v = L[c * 32 + lane];
+      const unsigned above = __ballot_sync(0xffffffffu, v != 0xFFFFu) >> lane;   // marked bins at or above mine
+      const unsigned w = __shfl_sync(0xffffffffu, v, (lane + __ffs(above) - 1) & 31);
+      const unsigned r = above ? w : carry;
+      L[c * 32 + lane] = (uint16_t)r;
+      carry = __shfl_sync(0xffffffffu, r, 0);
     }
   }
   __syncthreads();
   LHCB_CLK(1)
 
   // ---- S1 per iteration: two- and three-hit search, triplets of both iterations in one queue ----------
+  // items of the pair walk live in the candidate slots (empty until S2): (i1 | first i3 << 13 | (n - 1) << 26)
+  // one item buffer per iteration: the walk of iteration 0 needs no barrier before the T3 windows of iteration 1
+  const int item_cap = p.max_cand * (int)(sizeof(Cand) / 8);
   for (int it = 0; it < 2; ++it) {
+    uint32_t* items = reinterpret_cast<uint32_t*>(smem + p.smem_total - p.max_cand * (int)sizeof(Cand)) + it * item_cap;
     const int l1 = p.l1[it], l2 = p.l2[it], l3 = p.l3[it];
     const Zone z1n = H.zi[l1], z2n = H.zi[l2], z3n = H.zi[l3];
     const uint16_t* lut2 = lut + l2 * (kLutBins + 1);
     const uint16_t* lut3 = lut + l3 * (kLutBins + 1);
-    const int b1 = z1n.b, n1 = z1n.e - z1n.b, b2 = z2n.b, e2 = z2n.e, b3 = z3n.b;
+    const int b1 = z1n.b, n1 = z1n.e - z1n.b;
     const float r13 = p.r13[it], dx3 = p.dx3max[it], idz = p.inv_dz13[it], z1 = p.z1[it], dz12 = p.dz12[it];
     const float K = p.K[it];
 
     for (int tile0 = 0; tile0 < n1; tile0 += T) {
-      // O2: T3 window of this thread's T1 hit
-      const int nt1 = n1 - tile0 < T ? n1 - tile0 : T;
+      // O2: T3 window of this thread's T1 hit, cut into items of at most kItemPairs T3 hits
       int cnt = 0, fst = 0;
-      if (tid < nt1) {
+      if (tile0 + tid < n1) {
         const float x1 = hx[b1 + tile0 + tid];
         const float c = x1 * r13;                                                // Eq. 11
         const float lo = c - dx3, hi = c + dx3;
         fst = lower_bound(hx, lut3, z3n, lo);
         cnt = upper_bound(hx, lut3, z3n, hi) - fst;
       }
+      const int nit = (cnt + kItemPairs - 1) / kItemPairs;
       int total;
-      const int ex = block_exscan<NT>(cnt, H.warp_sums, total);
-      scan_offs[tid] = ex; scan_first[tid] = (uint16_t)fst;
-      if (tid == T - 1) scan_offs[T] = total;
+      const int ex = block_exscan<NT>(nit, &H.warp_sums[0][0], flip, total);
+      if (total > item_cap) { total = item_cap; if (tid == 0) H.status |= LHCB_ST_TRIPLET_OVERFLOW; }
+      {
+        const uint32_t base = (uint32_t)(b1 + tile0 + tid) | ((uint32_t)fst << kTileIndexBits);
+        int left = cnt;
+        for (int q = 0; q < nit && ex + q < item_cap; ++q, left -= kItemPairs) {
+          const int n = left < kItemPairs ? left : kItemPairs;
+          items[ex + q] = base + ((uint32_t)(q * kItemPairs) << kTileIndexBits) + ((uint32_t)(n - 1) << (2 * kTileIndexBits));
+        }
+      }
       __syncthreads();
       LHCB_CLK(2)
-      // flattened pairs: thread owns pairs [p0, p1)
-      const int chunk = (total + T - 1) / T;
-      const int p0 = tid * chunk, p1 = p0 + chunk < total ? p0 + chunk : total;
-      if (p0 < p1) {
-        int t = owner_of(scan_offs, nt1, p0);
-        int nxt = scan_offs[t + 1];
-        int i1 = b1 + tile0 + t;
-        float x1 = hx[i1];
-        int f = (int)scan_first[t] - scan_offs[t];
-        for (int pp = p0; pp < p1; ++pp) {
-          while (pp >= nxt) {
-            ++t; nxt = scan_offs[t + 1]; i1 = b1 + tile0 + t; x1 = hx[i1]; f = (int)scan_first[t] - scan_offs[t];
-          }
-          const int i3 = f + pp;
-          const float x3 = hx[i3];
+      for (int i = tid; i < total; i += T) {
+        const uint32_t item = items[i];
+        const int i1 = (int)(item & ((1u << kTileIndexBits) - 1)), i3f = (int)((item >> kTileIndexBits) & ((1u << kTileIndexBits) - 1));
+        const int n = (int)(item >> (2 * kTileIndexBits)) + 1;
+        const float x1 = hx[i1];
+        const int e2 = z2n.e;
+        int j = e2;
+        float xj = inf, lo2p = inf;
+        for (int k = 0; k < n; ++k) {
+          const float x3 = hx[i3f + k];
           const float t13 = (x3 - x1) * idz;                                     // O3, Eq. 4
           const float x0 = x1 - z1 * t13;                                        // Eq. 3
           const float invp = p.a * fabsf(x0) + p.b * (x0 * x0);                  // Eq. 5
@@ -518,70 +569,71 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
           const float cxlo = fminf(ca, cb) - p.d_lo, cxhi = fmaxf(ca, cb) + p.d_hi;
           const float ea = x2c + K * cxlo, eb = x2c + K * cxhi;
           const float lo2 = fminf(ea, eb), hi2 = fmaxf(ea, eb);
-          float xj;
-          int j = lower_bound_v(hx, lut2, z2n, lo2, xj);
-          while (xj <= hi2) {
-            const int k = atomicAdd(&H.n_trip, 1);
-            if (k < trip_cap) {
+          // the T2 interval moves up with x3: the pointer of the previous pair is a valid start; the first
+          // pair of the item (and a lower edge that moved down, a rounding event) starts from the bin table
+          if (lo2 < lo2p) { j = lut2[zone_bin(z2n, lo2)]; xj = hx[j]; }
+          lo2p = lo2;
+          while (xj < lo2) { ++j; xj = hx[j]; }
+          int jj = j;
+          float xjj = xj;
+          while (xjj <= hi2) {
+            if (jj >= e2) break;                                                 // hi2 = +inf: stop at the sentinel
+            const int slot = smem_inc(&H.n_trip);
+            if (slot < trip_cap) {
               Triplet tr;
-              tr.i1 = (uint16_t)(i1 - b1); tr.i2 = (uint16_t)(j - b2); tr.i3 = (uint16_t)(i3 - b3); tr.it = (uint16_t)it;
-              trip[k] = tr;
+              tr.i1 = (uint16_t)i1; tr.i2 = (uint16_t)jj; tr.i3 = (uint16_t)(i3f + k); tr.it = (uint16_t)it;
+              trip[slot] = tr;
             }
-            ++j;
-            xj = j < e2 ? hx[j] : __int_as_float(0x7f800000);
+            ++jj;
+            xjj = hx[jj];
           }
         }
       }
-      __syncthreads();
+      if (it == 1 || tile0 + T < n1) __syncthreads();
       LHCB_CLK(3)
     }
   }
+  __syncthreads();
   // ---- S2: extension of the queued triplets of both iterations (O5) ---------------------------------
   {
     int nt = H.n_trip;
     LHCB_DBG_MAX(0, nt)
     if (nt > trip_cap) { nt = trip_cap; if (tid == 0) H.status |= LHCB_ST_TRIPLET_OVERFLOW; }
+    const int miss_max = 6 - p.min_x_hits;
 
     for (int t = tid; t < nt; t += T) {
       const Triplet tr = trip[t];
       const int it = tr.it;                                  // the queue holds iteration 0 first: warps are uniform in it
-      const int l1 = p.l1[it], l2 = p.l2[it], l3 = p.l3[it];
-      const int i1 = H.zi[l1].b + tr.i1, i2 = H.zi[l2].b + tr.i2, i3 = H.zi[l3].b + tr.i3;
-      const float x1 = hx[i1], x2 = hx[i2], x3 = hx[i3];
+      const int l1 = p.l1[it];
+      const float x1 = hx[tr.i1], x2 = hx[tr.i2], x3 = hx[tr.i3];
       const float t13 = (x3 - x1) * p.inv_dz13[it];
       const float x2c = x1 + p.dz12[it] * t13;
-      float cx = (x2 - x2c) * p.inv_K[it];
-      float bx = t13 - cx * p.G13[it];
-      float ax = (x1 - bx * p.zb[l1]) - cx * p.gz[l1];
-      int hit[6];
-      int nx = 0, pattern = 0;
+      const float cx = (x2 - x2c) * p.inv_K[it];
+      const float bx = t13 - cx * p.G13[it];
+      const float ax = (x1 - bx * p.zb[l1]) - cx * p.gz[l1];
+      int ho[3];
+      int miss = 0, pattern = 0;
 #pragma unroll
-      for (int s = 0; s < 6; ++s) {
-        const int l = p.xl[s];
-        int hh;
-        if (l == l1) hh = i1;
-        else if (l == l2) hh = i2;
-        else if (l == l3) hh = i3;
-        else {
-          const Zone z = H.zi[l];
-          float xh;
-          hh = closest_hit(hx, lut + l * (kLutBins + 1), z, xz_at(p, ax, bx, cx, l), p.tol_x, xh);
-        }
-        if (hh < 0) { hit[s] = -1; pattern = 1 + s; }
-        else { hit[s] = hh - zl[l]; ++nx; }
-        if (s + 1 - nx > 6 - p.min_x_hits) break;               // too many layers missed already
+      for (int q = 0; q < 3; ++q) {                          // the three other x-layers in z order
+        ho[q] = -1;
+        if (miss > miss_max) continue;                        // too many layers missed already
+        const int l = p.ol[it][q];
+        const Zone z = H.zi[l];
+        float xh;
+        ho[q] = closest_hit(hx, lut + l * (kLutBins + 1), z, xz_at(p, ax, bx, cx, l), p.tol_x, xh);
+        if (ho[q] < 0) { ++miss; pattern = 1 + p.os[it][q]; }
       }
-      if (nx < p.min_x_hits) continue;
+      if (miss > miss_max) continue;
       // enough x-hits: queue the three-point parabola and its hits; the least-squares fit runs as a dense
       // pass over the queued candidates of both iterations (S2b)
-      const int k = atomicAdd(&H.n_cand, 1);
+      const int k = smem_inc(&H.n_cand);
       if (k < p.max_cand) {
-        Cand cd;
+        Cand& cd = cand_end[-1 - k];
         cd.ax = ax; cd.bx = bx; cd.cx = cx; cd.chi2 = 0.f;
+        cd.hit[p.ss[it][0]] = tr.i1; cd.hit[p.ss[it][1]] = tr.i2; cd.hit[p.ss[it][2]] = tr.i3;
 #pragma unroll
-        for (int s = 0; s < 6; ++s) cd.hit[s] = hit[s] < 0 ? (uint16_t)0xFFFF : (uint16_t)hit[s];
-        cd.nx = (uint8_t)nx; cd.it = (uint8_t)it; cd.keep = 0; cd.pattern = (uint8_t)pattern;
-        cand_end[-1 - k] = cd;
+        for (int q = 0; q < 3; ++q) cd.hit[p.os[it][q]] = (uint16_t)ho[q];     // -1 -> 0xFFFF
+        cd.nx = (uint8_t)(6 - miss); cd.it = (uint8_t)it; cd.keep = 0; cd.pattern = (uint8_t)pattern;
       }
     }
     __syncthreads();
@@ -602,7 +654,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     for (int s = 0; s < 6; ++s) {
       const int l = p.xl[s];
       r[s] = 0.f;
-      if (pattern != 1 + s) r[s] = hx[zl[l] + cd.hit[s]] - xz_at(p, ax, bx, cx, l);
+      if (pattern != 1 + s) r[s] = hx[cd.hit[s]] - xz_at(p, ax, bx, cx, l);
     }
     const float* __restrict__ P = p.P + pattern * 18;
     float d[3];
@@ -635,7 +687,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   }
   __syncthreads();
   // ---- S3: clone kill (O7) ------------------------------------------------------------------
-  const int n_xhits = H.xbase[6];
+  const int n_xhits = H.n_xhits;
   for (int i = tid; i < n_xhits; i += T) tbl[i] = kNoKey;
   __syncthreads();
   for (int c = tid; c < nc; c += T) {
@@ -644,7 +696,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     const unsigned long long key = clone_key(cd.chi2, cd.cx, cd.nx, cd.it);
 #pragma unroll
     for (int s = 0; s < 6; ++s)
-      if (cd.hit[s] != 0xFFFF) atomicMin(&tbl[H.xbase[s] + cd.hit[s]], key);
+      if (cd.hit[s] != 0xFFFF) atomicMin(&tbl[H.xoff[s] + cd.hit[s]], key);
   }
   __syncthreads();
   for (int c = tid; c < nc; c += T) {
@@ -654,10 +706,10 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     int own = 0;
 #pragma unroll
     for (int s = 0; s < 6; ++s)
-      if (cd.hit[s] != 0xFFFF && tbl[H.xbase[s] + cd.hit[s]] == key) ++own;
+      if (cd.hit[s] != 0xFFFF && tbl[H.xoff[s] + cd.hit[s]] == key) ++own;
     const bool keep = own >= 3 || (own >= 2 && cd.nx == 6);
     cd.keep = keep;
-    if (keep) kept[atomicAdd(&H.n_kept, 1)] = (uint16_t)c;
+    if (keep) kept[smem_inc(&H.n_kept)] = (uint16_t)c;
   }
   __syncthreads();
   int nk = H.n_kept;
@@ -665,9 +717,11 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   // The clone table is dead.  The survivors move to the bottom of W; after that every candidate slot is
   // dead too and W extends to the end of shared memory:
   //   [survivors | best key per survivor | predictions per survivor | item chunk | live walks | success queue]
+  // (Hough version: [... | votes | first hypothesis per survivor | selected clusters | success queue])
   const int wbytes = p.smem_total - off_w;
   {                                                            // survivors must fit below the candidate slots (the
-    int nk_max = (wbytes - 4096) / 72;                         // copy is in place) and leave room for the queues
+    // copy is in place) and leave room for the queues: 72 bytes per survivor, 132 with the Hough tables
+    int nk_max = (wbytes - 4096) / (p.uv_hough ? 136 : 72);
     if (nk_max > w_stat / 32) nk_max = w_stat / 32;
     if (nk > nk_max) { nk = nk_max > 0 ? nk_max : 0; if (tid == 0) H.status |= LHCB_ST_UV_QUEUE_OVERFLOW; }
   }
@@ -679,8 +733,8 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   int C = (rest / 2) / 20;                                                // items per chunk: 4 B item + 16 B live walk
   C = C >= T ? C / T * T : (C & ~31);                                     // whole rounds of the CTA when possible
   if (C < 32) C = 32;
-  uint32_t* items = reinterpret_cast<uint32_t*>(xps + (size_t)nk * 8);
-  UvLive* live = reinterpret_cast<UvLive*>(items + C);
+  uint32_t* uitems = reinterpret_cast<uint32_t*>(xps + (size_t)nk * 8);
+  UvLive* live = reinterpret_cast<UvLive*>(uitems + C);
   UvSuccess* succ = reinterpret_cast<UvSuccess*>(live + C);
   int succ_cap = (rest - C * 20) / (int)sizeof(UvSuccess);
   __syncthreads();
@@ -702,12 +756,12 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   if (p.uv_hough) {
     // ---- S4h: Hough-cluster version (O8h).  The queue space after the predictions is laid out as
     //   [votes u64[nk][6] | first hypothesis of each survivor int[nk + 1] | selected clusters u8[nk][8] | success queue]
-    unsigned long long* vote = reinterpret_cast<unsigned long long*>(items);      // items is 16-byte aligned
+    unsigned long long* vote = reinterpret_cast<unsigned long long*>(uitems);     // 16-byte aligned
     int* hoff = reinterpret_cast<int*>(vote + (size_t)nk * 6);
     uint8_t* selb = reinterpret_cast<uint8_t*>(hoff + nk + 1);
     const int hused = nk * 48 + (int)((((size_t)nk + 1) * 4 + (size_t)nk * 8 + 15) & ~(size_t)15);
-    UvSuccess* hsucc = reinterpret_cast<UvSuccess*>(reinterpret_cast<unsigned char*>(items) + hused);
-    const int hsucc_cap = (rest - hused) / (int)sizeof(UvSuccess);
+    UvSuccess* hsucc = reinterpret_cast<UvSuccess*>(reinterpret_cast<unsigned char*>(uitems) + hused);
+    const int hsucc_cap = (rest - hused) / (int)sizeof(UvSuccess);        // > 0: nk was clamped with the Hough tables in mind
     // H1: votes.  Owner = (survivor, stereo slot); every hit in the slot's window of Eq. 16 sets the bit of
     // its t_y bin (a layer counts once per bin)
     for (int w = tid; w < 6 * nk; w += T) {
@@ -720,7 +774,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
       const uint16_t* lutf = lut + l * (kLutBins + 1);
       float xh;
       int i = lower_bound_v(hx, lutf, zf, fminf(wa, wb), xh);
-      const float whi = fmaxf(wa, wb);
+      const float whi = fminf(fmaxf(wa, wb), 3.4028235e38f);
       unsigned long long m = 0ull;
       while (xh <= whi) {
         const float t = ((xpl - xh) * cf.y) * cf.z;                               // Eq. 16, A7
@@ -728,7 +782,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
         tb = fminf(fmaxf(tb, 0.f), 63.f);
         m |= 1ull << (int)tb;
         ++i;
-        xh = i < zf.e ? hx[i] : __int_as_float(0x7f800000);
+        xh = hx[i];
       }
       vote[w] = m;
     }
@@ -761,7 +815,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
         }
       }
       int total;
-      const int ex = block_exscan<NT>(4 * nsel, H.warp_sums, total);
+      const int ex = block_exscan<NT>(4 * nsel, &H.warp_sums[0][0], flip, total);
       if (k < nk) hoff[k] = nhyp + ex;
       nhyp += total;
     }
@@ -786,7 +840,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
         n += hh[sl] >= 0;
       }
       if (n < p.min_uv_hits) continue;
-      const int slot = atomicAdd(&H.n_trip, 1);
+      const int slot = smem_inc(&H.n_trip);
       if (slot < hsucc_cap) {
         UvSuccess& u = hsucc[slot];
         u.k = (uint16_t)k; u.pp = (uint8_t)j; u.n = (uint8_t)n;
@@ -813,19 +867,19 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
       cnt = upper_bound(hx, lutf, zf, whi) - fst;
     }
     int total;
-    const int ex = block_exscan<NT>(cnt, H.warp_sums, total);
+    const int ex = block_exscan<NT>(cnt, &H.warp_sums[0][0], flip, total);
     LHCB_CLK(6)
     for (int q0 = 0; q0 < total; q0 += C) {                  // uniform: chunks of C items
       if (tid == 0) H.n_live = 0;
       {
         int i = q0 - ex; if (i < 0) i = 0;
         int iend = q0 + C - ex; if (iend > cnt) iend = cnt;
-        for (; i < iend; ++i) items[ex + i - q0] = ((uint32_t)tid << 16) | (uint32_t)(fst + i);
+        for (; i < iend; ++i) uitems[ex + i - q0] = ((uint32_t)tid << 16) | (uint32_t)(fst + i);
       }
       __syncthreads();
       const int nitems = total - q0 < C ? total - q0 : C;
       for (int i = tid; i < nitems; i += T) {                // phase A
-        const uint32_t item = items[i];
+        const uint32_t item = uitems[i];
         const int w = tile0 + (int)(item >> 16), ih = (int)(item & 0xFFFFu);
         const int sf = (w & 1) ? sf1 : sf0;
         const float* xpk = xps + (w >> 1) * 8;
@@ -840,7 +894,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
         UvLive lv;
         lv.item = ((uint32_t)w << 16) | (uint32_t)ih; lv.ty = ty;
         lv.h[0] = (uint16_t)h0; lv.h[1] = (uint16_t)h1; lv.h[2] = (uint16_t)h2; lv.n = (uint16_t)n;
-        live[atomicAdd(&H.n_live, 1)] = lv;
+        live[smem_inc(&H.n_live)] = lv;
       }
       __syncthreads();
       const int nl = H.n_live;
@@ -854,7 +908,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
         const int h3 = uv_step(H, hx, lut, xpk, 3 + (3 >= sf), p.tol_uv, ty, n);
         const int h4 = (n + 1 < p.min_uv_hits) ? -1 : uv_step(H, hx, lut, xpk, 4 + (4 >= sf), p.tol_uv, ty, n);
         if (n < p.min_uv_hits) continue;
-        const int slot = atomicAdd(&H.n_trip, 1);            // enough hits: queue for the dense fit pass
+        const int slot = smem_inc(&H.n_trip);            // enough hits: queue for the dense fit pass
         if (slot < succ_cap) {
           UvSuccess& u = succ[slot];
           u.k = (uint16_t)(w >> 1); u.pp = (uint8_t)(w & 1); u.n = (uint8_t)n;
@@ -895,7 +949,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
         const int sf = p.slot_of_layer[p.uv_first[u.pp]];
         int first_local = 0;
 #pragma unroll
-        for (int s = 0; s < 6; ++s) first_local = (s == sf) ? (int)u.hit[s] - zl[p.ul[s]] : first_local;
+        for (int s = 0; s < 6; ++s) first_local = (s == sf) ? (int)u.hit[s] - H.zi[p.ul[s]].b : first_local;
         tie = ((unsigned long long)u.pp << 16) | (unsigned long long)first_local;
       }
       key = ((unsigned long long)(6 - u.n) << 49) | ((unsigned long long)__float_as_uint(chi2y) << 17) | tie;
@@ -910,7 +964,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     if (!single) fit_success(i);                               // more than one round: redo the (cheap) fit
     if (key == kNoKey || best[u.k] != key) continue;           // not the best combination of its survivor
     const Cand& cd = surv[u.k];
-    const int slot = atomicAdd(&H.n_seed, 1);
+    const int slot = smem_inc(&H.n_seed);
     if (slot >= p.max_seeds) continue;
     const size_t o = (size_t)slot0 + slot, ct = p.cap_total;
     p.state[0 * ct + o] = (cd.ax + cd.bx * p.zbS) + cd.cx * p.gS;
@@ -924,8 +978,8 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
 #pragma unroll
     for (int s = 0; s < 6; ++s) {
       const int lx = p.xl[s], lu = p.ul[s];
-      p.hits[(size_t)lx * ct + o] = cd.hit[s] == 0xFFFF ? LHCB_NO_HIT : a0 + (uint32_t)(zl[lx] + cd.hit[s]);
-      p.hits[(size_t)lu * ct + o] = u.hit[s] == 0xFFFF ? LHCB_NO_HIT : a0 + (uint32_t)u.hit[s];
+      p.hits[(size_t)lx * ct + o] = cd.hit[s] == 0xFFFF ? LHCB_NO_HIT : H.zg[lx] + (uint32_t)cd.hit[s];
+      p.hits[(size_t)lu * ct + o] = u.hit[s] == 0xFFFF ? LHCB_NO_HIT : H.zg[lu] + (uint32_t)u.hit[s];
     }
     p.nx[o] = cd.nx;
     p.nuv[o] = u.n;
