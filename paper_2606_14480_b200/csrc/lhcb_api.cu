@@ -136,7 +136,8 @@ int lhcb_geom_init(const lhcb_geom_t* g, int device, lhcb_ctx** out) {
   int rc = lhcb::derive(G, c->der);
   if (rc != LHCB_OK) { delete c; return rc; }
   if (G.max_hits_per_half > 8000 || G.max_xz_cand_per_half > 65535 || G.max_seeds_per_half > 32767 ||
-      G.max_velo_per_event > 65535 || G.max_ut_per_event > 65534 || G.max_match_cand_per_event > 16383 || G.max_triplets_per_half < G.max_xz_cand_per_half) { delete c; return LHCB_ERR_BAD_ARGUMENT; }
+      G.max_velo_per_event > 65535 || G.max_ut_per_event > 65534 || G.max_match_cand_per_event > 16383 || G.max_triplets_per_half < G.max_xz_cand_per_half ||
+      (size_t)G.max_triplets_per_half * 8 + (size_t)G.max_xz_cand_per_half * 32 < ((size_t)G.max_hits_per_half + 8) * 4 /* staging buffer */) { delete c; return LHCB_ERR_BAD_ARGUMENT; }
   // 256-thread CTAs, four per SM, when their shared memory fits (228 KB per SM, 1 KB reserved per
   // CTA); else 512-thread CTAs, two (or one) per SM
   c->seed_threads = 256;

@@ -8,7 +8,7 @@
 //                                      bin); the table is built by marking the first hit of every occupied
 //                                      bin and a ballot-based suffix fill, one warp per zone
 //   S1  two-hit + three-hit search     per iteration: thread per T1 hit finds its T3 window (Eq. 8-11) and
-//                                      cuts it into items of at most 8 consecutive T3 hits; thread per item:
+//                                      cuts it into items of at most 4 consecutive T3 hits; thread per item:
 //                                      Eq. 3-5 and the T2 band (Eq. 12-13, A3/A4) for its pairs, with one
 //                                      T2 pointer that only moves forward (the band moves monotonically with
 //                                      x3); the triplets of both iterations go to one queue in shared memory
@@ -38,12 +38,12 @@ namespace lhcb {
 #define LHCB_LUT_BINS 320
 #endif
 #ifndef LHCB_ITEM_PAIRS
-#define LHCB_ITEM_PAIRS 8   // T3 hits per item of the pair walk (a power of two, at most 8)
+#define LHCB_ITEM_PAIRS 4   // T3 hits per item of the pair walk (2, 4 or 8; measured 3.10 ms with 4 against 3.16 ms with 8)
 #endif
 constexpr int kSeedThreadsMax = 512;          // the kernel is instantiated for 256 x 4 CTAs/SM and 512 x 2 CTAs/SM
 constexpr int kLutBins = LHCB_LUT_BINS;       // bins of the per-zone search table
 constexpr int kItemPairs = LHCB_ITEM_PAIRS;
-constexpr int kTileIndexBits = 13;            // tile indices fit 13 bits: max_hits_per_half + 172 <= 8192
+constexpr int kTileIndexBits = 13;            // tile indices fit 13 bits: max_hits_per_half + 40 <= 8192
 constexpr unsigned long long kNoKey = ~0ull;
 static_assert(kLutBins % 32 == 0, "the suffix fill of the bin tables works on whole warps of bins");
 static_assert(kItemPairs == 2 || kItemPairs == 4 || kItemPairs == 8, "item length");
@@ -134,8 +134,8 @@ static_assert(sizeof(SeedSmemHeader) <= kSeedHeaderBytes, "shared-memory header 
 __host__ __device__ inline size_t seed_align16(size_t b) { return (b + 15) & ~(size_t)15; }
 __host__ __device__ inline size_t seed_off_kept() { return kSeedHeaderBytes + seed_align16(12 * (kLutBins + 1) * 2); }
 __host__ __device__ inline size_t seed_off_hits(int max_cand) { return seed_off_kept() + seed_align16((size_t)max_cand * 2); }
-// tile: per zone [4 floats | aligned superset of the zone (at most 6 floats more than its hits) | 4 floats]
-__host__ __device__ inline size_t seed_tile_bytes(int n_hits) { return seed_align16(((size_t)n_hits + 12 * 14) * 4 + 16); }
+// tile: per zone [-inf, -inf, hits ..., +inf]
+__host__ __device__ inline size_t seed_tile_bytes(int n_hits) { return seed_align16(((size_t)n_hits + 36) * 4 + 16); }
 __host__ __device__ inline size_t seed_smem_bytes(int max_hits, int max_cand, int max_trip) {
   size_t b = seed_off_hits(max_cand);
   b += seed_tile_bytes(max_hits);                           // hits tile with its 24 sentinels
@@ -358,10 +358,9 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   const uint32_t* zo = p.zone_off + (size_t)half_id * 12;
 
   // ---- S0: stage the half's hits, every zone framed by sentinels ----------------------------------
-  // One bulk async copy per zone (cp.async.bulk needs 16-byte aligned addresses and sizes: each copy takes
-  // the aligned superset of its zone, so up to three hits of the neighbouring zones land beside it; the
-  // region of a zone is [4 floats | superset | 4 floats] and the sentinels are written over the neighbours
-  // once the copies have landed).  Zone z: region start rb (multiple of 4), first hit at rb + 4 + (zoff & 3).
+  // The half is one contiguous run of hit_x: ONE bulk async copy brings its 16-byte aligned superset into a
+  // staging buffer (the work region, empty so far); the zones are then moved into the tile, each as
+  // [-inf, -inf, hits ..., +inf]: zone z starts at pos_z = 2 + sum_{k<z} (n_k + 3).
   uint32_t zoff[13];
 #pragma unroll
   for (int z = 0; z < 13; ++z) zoff[z] = __ldg(zo + z);
@@ -371,45 +370,39 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     if (tid == 0) { p.count[half_id] = 0; p.status[half_id] = LHCB_ST_HITS_OVERFLOW; }
     return;
   }
-  const bool aligned = (reinterpret_cast<uintptr_t>(p.hit_x) & 15) == 0;
-  const uint32_t n_al = p.n_hits & ~3u;                    // bulk copies stay inside the array
+  const int off_w = off_hits + (int)seed_tile_bytes(n_half);   // work region W: from the end of the tile to the first candidate slot
+  float* stg = reinterpret_cast<float*>(smem + off_w);
+  const uint32_t a0 = zoff[0] & ~3u;                       // 16-byte aligned start of the staged run
+  uint32_t a1 = (zoff[12] + 3u) & ~3u;                     // end of the bulk part (multiple of 4 floats)
+  if (a1 > (p.n_hits & ~3u)) a1 = p.n_hits & ~3u;
+  if ((reinterpret_cast<uintptr_t>(p.hit_x) & 15) != 0 || a1 < a0) a1 = a0;
   const uint32_t mbar_addr = (uint32_t)__cvta_generic_to_shared(&H.mbar);
   if (tid == 0) {
     H.n_trip = 0; H.n_cand = 0; H.n_kept = 0; H.n_seed = 0; H.status = 0;
     asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar_addr));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    uint32_t bytes = 0;
-    if (aligned) {
-#pragma unroll
-      for (int z = 0; z < 12; ++z) {
-        const uint32_t s0 = zoff[z] & ~3u;
-        uint32_t s1 = (zoff[z + 1] + 3u) & ~3u;
-        if (s1 > n_al) s1 = n_al;
-        if (zoff[z + 1] > zoff[z] && s1 > s0) bytes += (s1 - s0) * 4u;
-      }
+    const uint32_t bytes = (a1 - a0) * 4u;
+    if (bytes > 0) {
+      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar_addr), "r"(bytes) : "memory");
+      asm volatile(
+          "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+              (uint32_t)__cvta_generic_to_shared(stg)),
+          "l"(p.hit_x + a0), "r"(bytes), "r"(mbar_addr)
+          : "memory");
+    } else {
+      asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(mbar_addr) : "memory");
     }
-    if (bytes) asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar_addr), "r"(bytes) : "memory");
-    else asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(mbar_addr) : "memory");
-    int acc = 0, rb = 0, xs = 0;
+    int acc = 0, pos = 2, xs = 0;
 #pragma unroll
-    for (int z = 0; z < 12; ++z) {                         // the copies; x-hits are numbered densely for the clone table
+    for (int z = 0; z < 12; ++z) {                         // x-hits are numbered densely for the clone table
       const int n = (int)(zoff[z + 1] - zoff[z]);
-      const uint32_t s0 = zoff[z] & ~3u;
-      uint32_t s1 = (zoff[z + 1] + 3u) & ~3u;
-      const int span = (int)(s1 - s0);
-      if (s1 > n_al) s1 = n_al;
-      if (aligned && n > 0 && s1 > s0)
-        asm volatile(
-            "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                (uint32_t)__cvta_generic_to_shared(hx + rb + 4)),
-            "l"(p.hit_x + s0), "r"((s1 - s0) * 4u), "r"(mbar_addr)
-            : "memory");
-      const int pos = rb + 4 + (int)(zoff[z] & 3u);
       if (xs < 6 && p.xl[xs] == z) { H.xoff[xs] = acc - pos; acc += n; ++xs; }
-      rb += (n > 0 ? span : 0) + 8;
+      pos += n + 3;
     }
     H.n_xhits = acc;
   }
+  // tail (and the whole run when the source is not 16-byte aligned) with plain loads
+  for (uint32_t i = (a1 > zoff[0] ? a1 : zoff[0]) + tid; i < zoff[12]; i += T) stg[i - a0] = __ldg(p.hit_x + i);
   if (tid >= 64 && tid < 70) {
     const int l = p.ul[tid - 64];
     H.uvc[tid - 64] = make_float4(p.zt[l], p.inv_tan[l], p.inv_z[l], __int_as_float(l));
@@ -419,21 +412,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     constexpr int nw = (12 * (kLutBins + 1) + 1) / 2;
     for (int i = tid; i < nw; i += T) L32[i] = 0xFFFFFFFFu;
   }
-  {
-    // what the bulk copies do not cover: everything when the source is not 16-byte aligned, else the last
-    // (at most three) hits of a zone that ends in the unaligned tail of the array
-    int rb = 0;
-#pragma unroll
-    for (int z = 0; z < 12; ++z) {
-      const int n = (int)(zoff[z + 1] - zoff[z]);
-      const uint32_t s0 = zoff[z] & ~3u;
-      const uint32_t s1 = (zoff[z + 1] + 3u) & ~3u;
-      const int pos = rb + 4 + (int)(zoff[z] & 3u);
-      uint32_t from = aligned ? (s1 > n_al ? (n_al > zoff[z] ? n_al : zoff[z]) : zoff[z + 1]) : zoff[z];
-      for (uint32_t i = from + tid; i < zoff[z + 1]; i += T) hx[pos + (int)(i - zoff[z])] = __ldg(p.hit_x + i);
-      rb += (n > 0 ? (int)(s1 - s0) : 0) + 8;
-    }
-  }
+  __syncthreads();                                         // the mbarrier is initialised; the tail hits are in place
   {
     uint32_t done = 0;
     while (!done) {
@@ -446,32 +425,30 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
           : "memory");
     }
   }
-  if (tid >= 32 && tid < 44) {                             // sentinels, bin function and index map of zone tid - 32
-    int rb = 0, pos = 0, n = 0;
-    uint32_t z0 = 0;
+  {
+    int pos = 2;
 #pragma unroll
     for (int z = 0; z < 12; ++z) {
-      const int nz = (int)(zoff[z + 1] - zoff[z]);
-      if (z == tid - 32) { pos = rb + 4 + (int)(zoff[z] & 3u); n = nz; z0 = zoff[z]; }
-      rb += (nz > 0 ? (int)(((zoff[z + 1] + 3u) & ~3u) - (zoff[z] & ~3u)) : 0) + 8;
+      const int n = (int)(zoff[z + 1] - zoff[z]);
+      const float* src = stg + (zoff[z] - a0);
+      for (int i = tid; i < n; i += T) hx[pos + i] = src[i];
+      if (tid == 32 + z) {                                 // sentinels, bin function, index map of zone z
+        hx[pos - 2] = -inf; hx[pos - 1] = -inf; hx[pos + n] = inf;
+        float x0 = 0.f, invw = 0.f;
+        if (n > 0) {
+          x0 = src[0];
+          const float span = src[n - 1] - x0;
+          invw = span > 0.f ? (float)kLutBins / span : 0.f;
+        }
+        Zone zn; zn.b = pos; zn.e = pos + n; zn.x0 = x0; zn.invw = invw;
+        H.zi[z] = zn;
+        H.zg[z] = zoff[z] - (uint32_t)pos;
+      }
+      pos += n + 3;
     }
-    float x0 = 0.f, invw = 0.f;
-    if (n > 0) {
-      x0 = hx[pos];
-      const float span = hx[pos + n - 1] - x0;
-      invw = span > 0.f ? (float)kLutBins / span : 0.f;
-    }
-    // (the two stores below may hit hits of the neighbouring zones that the aligned superset brought along;
-    // a tail hit written by another thread is never at pos - 1 / pos + n of this zone)
-    hx[pos - 2] = -inf; hx[pos - 1] = -inf; hx[pos + n] = inf;
-    Zone zn; zn.b = pos; zn.e = pos + n; zn.x0 = x0; zn.invw = invw;
-    H.zi[tid - 32] = zn;
-    H.zg[tid - 32] = z0 - (uint32_t)pos;
   }
   __syncthreads();
   LHCB_CLK(0)
-  // work region W: from the end of the tile to the first candidate slot
-  const int off_w = off_hits + (int)seed_tile_bytes(n_half);
   const int w_stat = p.smem_total - p.max_cand * (int)sizeof(Cand) - off_w;   // bytes of W with every candidate slot used
   Triplet* trip = reinterpret_cast<Triplet*>(smem + off_w);
   unsigned long long* tbl = reinterpret_cast<unsigned long long*>(smem + off_w);   // aliases trip
