@@ -195,8 +195,19 @@ void lhcb_destroy(lhcb_ctx* ctx);
 /* The geometry the context holds, with capacity defaults resolved. */
 int lhcb_get_geom(const lhcb_ctx* ctx, lhcb_geom_t* out);
 
-/* Bytes of device scratch the two calls need for a batch (may be 0; pass NULL workspace then). */
+/* Bytes of the optional device workspace of a batch (see lhcb_order).  The two kernels keep every
+ * intermediate in shared memory and run without a workspace (pass NULL). */
 size_t lhcb_workspace_bytes(const lhcb_ctx* ctx, int n_events, size_t n_scifi_hits);
+
+/* Optional scheduling step (batches of about 1000 events): sorts the
+ * event-halves by their number of SciFi hits and the events by their number of UT hits (VELO states if
+ * ut == NULL), heaviest first, into `workspace` (device memory, lhcb_workspace_bytes(n_events) bytes).
+ * lhcb_seeding / lhcb_matching called with THIS workspace for THE SAME batch start their CTAs in that order,
+ * which shortens the last wave of a small batch; the results are the same in the same slots.  `velo` may be
+ * NULL (Seeding order only).  A workspace that lhcb_order has not filled for the batch must not be passed
+ * to the two calls.  Enqueues one small kernel; does not synchronise. */
+int lhcb_order(lhcb_ctx* ctx, const lhcb_events_t* events, const lhcb_velo_t* velo, const lhcb_ut_t* ut,
+               void* workspace, void* cuda_stream);
 
 /* Event preparation, the step before the hot path (hits tiled by detector half and layer;
  * the searches of section 3 need them sorted in x).  Inside each event the raw hits are
@@ -232,7 +243,8 @@ int lhcb_set_uv_hough(lhcb_ctx* ctx, int on);
 int lhcb_set_ghost_nn(lhcb_ctx* ctx, const float* nn);
 
 /* Seeding: x-z two-/three-hit search, extension, fit, clone kill, u/v addition, y fit (section 3).
- * One CTA per event-half.  `out` arrays must have cap_total = n_events*2*max_seeds_per_half slots. */
+ * One CTA per event-half.  `out` arrays must have cap_total = n_events*2*max_seeds_per_half slots.
+ * workspace: NULL, or the workspace lhcb_order filled for this batch. */
 int lhcb_seeding(lhcb_ctx* ctx, const lhcb_events_t* events, lhcb_seeds_t* out, void* workspace,
                  void* cuda_stream);
 
@@ -243,23 +255,52 @@ int lhcb_seeding(lhcb_ctx* ctx, const lhcb_events_t* events, lhcb_seeds_t* out, 
  * lists in lexicographic order (layer 0 first), without hit lists by the lower slot (reading A21),
  * so the set of long tracks does not depend on the order in which lhcb_seeding wrote the seeds. */
 int lhcb_matching(lhcb_ctx* ctx, const lhcb_seeds_t* seeds, const lhcb_velo_t* velo, const lhcb_ut_t* ut,
-                  lhcb_long_t* out, void* workspace, void* cuda_stream);
+                  lhcb_long_t* out, void* workspace /* NULL or lhcb_order's */, void* cuda_stream);
 
-/* ---- host-buffer pipeline (end-to-end path: H2D copies + seeding + matching + D2H copies) ---------
- * A pipeline owns device buffers sized at creation and two CUDA streams.  lhcb_reconstruct_host takes
- * the SAME descriptor structs as above but with HOST pointers (pinned memory for full copy/compute
- * overlap; pageable memory works, slower), splits the batch into event slices, and overlaps the
- * copies of one slice with the kernels of another.  It blocks until every output has landed in the
- * caller's host arrays.  Outputs: `out` (host arrays laid out for the whole batch, cap_total =
- * n_events*max_long_per_event) and, if non-NULL, seed_count[n_events*2].  The seeds themselves stay on
- * the device.  Returns LHCB_ERR_CAPACITY if the batch exceeds the sizes given at creation. */
+/* ---- host-buffer pipeline (end-to-end path: H2D copies + seeding + matching + compaction + D2H copies) ----
+ * A pipeline owns device buffers sized at creation, three CUDA streams (copies in, kernels, copies out) and one
+ * CUDA graph per slice of events.  lhcb_reconstruct_host takes lhcb_events_t / lhcb_velo_t / lhcb_ut_t with
+ * HOST pointers (pinned memory for full copy/compute overlap; pageable memory works, slower; lhcb_ut_t.row is
+ * required, y_lo / y_hi are not read), splits the batch into slices, and overlaps the input copies of later
+ * slices and the output copies of earlier ones with the kernels.  Per slice: lhcb_order, lhcb_seeding,
+ * lhcb_matching and two compaction kernels that move seeds and long tracks from their fixed slots to dense
+ * arrays, so that exactly the found entries are copied back.  It blocks until every output has landed.
+ *
+ * Outputs (HOST arrays owned by the caller, fully usable on their own):
+ *   seeds ("T tracks", L219: "made available to other algorithms"): event-half h owns the dense entries
+ *     [off[h], off[h+1]); the order inside a half is unspecified.
+ *   long tracks: event e owns [off[e], off[e+1]); seed_idx is an index into the dense seed arrays above,
+ *     velo_idx / ut_idx are indices into the caller's batch arrays.
+ * `cap` = entries the caller's arrays can hold (row stride of the [k][cap] arrays); n = entries written.
+ * Returns LHCB_ERR_CAPACITY if the batch exceeds the sizes given at creation or the dense arrays are too
+ * small; on any error every stream is drained before returning. */
+typedef struct {
+  uint32_t cap, n;
+  uint32_t* off;       /* [n_events*2+1] */
+  float* state;        /* [5][cap]  x, y, tx, ty, q/p at z_scifi_state */
+  uint32_t* hits;      /* [12][cap] global hit index per layer or LHCB_NO_HIT */
+  uint8_t *nx, *nuv;   /* [cap] */
+  float* par;          /* [7][cap] ax, bx, cx, ay, by, chi2x, chi2y, or NULL (not copied) */
+  uint32_t* status;    /* [n_events*2] LHCB_ST_* bits */
+} lhcb_host_seeds_t;
+typedef struct {
+  uint32_t cap, n;
+  uint32_t* off;       /* [n_events+1] */
+  uint32_t* seed_idx;  /* [cap] index into lhcb_host_seeds_t */
+  uint32_t* velo_idx;  /* [cap] */
+  uint32_t* ut_idx;    /* [4][cap] or LHCB_NO_HIT */
+  uint8_t* n_ut;       /* [cap] */
+  float *qop, *chi2;   /* [cap] */
+  uint32_t* status;    /* [n_events] LHCB_ST_* bits */
+} lhcb_host_long_t;
 typedef struct lhcb_pipeline lhcb_pipeline;
+/* max_seeds_total / max_long_total: entries of the device-side dense arrays (0: the slot capacity of the batch) */
 int lhcb_pipeline_create(lhcb_ctx* ctx, int max_events, size_t max_scifi_hits, size_t max_velo, size_t max_ut_hits,
-                         int slice_events, lhcb_pipeline** out);
+                         int slice_events, size_t max_seeds_total, size_t max_long_total, lhcb_pipeline** out);
 void lhcb_pipeline_destroy(lhcb_pipeline* p);
 int lhcb_reconstruct_host(lhcb_pipeline* p, const lhcb_events_t* host_events, const lhcb_velo_t* host_velo,
-                          const lhcb_ut_t* host_ut, lhcb_long_t* host_out, uint32_t* host_seed_count);
-/* bytes moved by the last lhcb_reconstruct_host call */
+                          const lhcb_ut_t* host_ut, lhcb_host_seeds_t* seeds_out, lhcb_host_long_t* long_out);
+/* bytes moved by the last lhcb_reconstruct_host call; returns the number of kernels it launched */
 int lhcb_pipeline_last_bytes(const lhcb_pipeline* p, uint64_t* h2d, uint64_t* d2h);
 
 const char* lhcb_error_string(int status);

@@ -24,7 +24,8 @@ ST_BITS = {1: "triplet_overflow", 2: "cand_overflow", 4: "seed_overflow", 8: "hi
 EXPORTS = ["lhcb_geom_derive", "lhcb_geom_init", "lhcb_destroy", "lhcb_get_geom", "lhcb_workspace_bytes",
            "lhcb_seeding", "lhcb_matching", "lhcb_error_string", "lhcb_last_cuda_error",
            "lhcb_last_launch_count", "lhcb_pipeline_create", "lhcb_pipeline_destroy", "lhcb_reconstruct_host",
-           "lhcb_pipeline_last_bytes", "lhcb_launch_config", "lhcb_prepare", "lhcb_set_ghost_nn", "lhcb_set_uv_hough"]
+           "lhcb_pipeline_last_bytes", "lhcb_launch_config", "lhcb_prepare", "lhcb_set_ghost_nn", "lhcb_set_uv_hough",
+           "lhcb_order"]
 
 
 class LhcbGeom(C.Structure):
@@ -91,6 +92,16 @@ class LhcbLong(C.Structure):
                 ("chi2", VP), ("status", VP), ("ghost", VP)]
 
 
+class LhcbHostSeeds(C.Structure):
+    _fields_ = [("cap", C.c_uint32), ("n", C.c_uint32), ("off", VP), ("state", VP), ("hits", VP), ("nx", VP), ("nuv", VP),
+                ("par", VP), ("status", VP)]
+
+
+class LhcbHostLong(C.Structure):
+    _fields_ = [("cap", C.c_uint32), ("n", C.c_uint32), ("off", VP), ("seed_idx", VP), ("velo_idx", VP), ("ut_idx", VP),
+                ("n_ut", VP), ("qop", VP), ("chi2", VP), ("status", VP)]
+
+
 def fill_geom(geom: dict) -> LhcbGeom:
     g = LhcbGeom()
     for name, _ in LhcbGeom._fields_:
@@ -137,11 +148,13 @@ def load_library(build: bool = True) -> C.CDLL:
         lib.lhcb_prepare.argtypes = [VP, C.POINTER(LhcbRaw), VP, VP, VP, VP, VP]
         lib.lhcb_set_ghost_nn.argtypes = [VP, C.POINTER(C.c_float)]
         lib.lhcb_set_uv_hough.argtypes = [VP, C.c_int]
-        lib.lhcb_pipeline_create.argtypes = [VP, C.c_int, C.c_size_t, C.c_size_t, C.c_size_t, C.c_int, C.POINTER(VP)]
+        lib.lhcb_order.argtypes = [VP, C.POINTER(LhcbEvents), C.POINTER(LhcbVelo), C.POINTER(LhcbUt), VP, VP]
+        lib.lhcb_pipeline_create.argtypes = [VP, C.c_int, C.c_size_t, C.c_size_t, C.c_size_t, C.c_int, C.c_size_t,
+                                             C.c_size_t, C.POINTER(VP)]
         lib.lhcb_pipeline_destroy.argtypes = [VP]
         lib.lhcb_pipeline_destroy.restype = None
         lib.lhcb_reconstruct_host.argtypes = [VP, C.POINTER(LhcbEvents), C.POINTER(LhcbVelo), C.POINTER(LhcbUt),
-                                              C.POINTER(LhcbLong), VP]
+                                              C.POINTER(LhcbHostSeeds), C.POINTER(LhcbHostLong)]
         lib.lhcb_pipeline_last_bytes.argtypes = [VP, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
         _LIB = lib
     return _LIB
@@ -295,15 +308,34 @@ class Context:
         _check(self.lib, self._ctx, rc, "lhcb_prepare")
         return out
 
-    def lhcb_seeding(self, dev: DeviceEvents, out: Optional[dict] = None) -> dict:
+    def lhcb_order(self, dev: DeviceEvents, workspace=None, use_ut: bool = True):
+        """CTA order "heaviest first" of a batch -> the workspace tensor to hand to lhcb_seeding / lhcb_matching."""
+        t = self.torch
+        nb = int(self.lib.lhcb_workspace_bytes(self._ctx, dev.n_events, 0))
+        if workspace is None:
+            workspace = t.empty(max(nb, 16), dtype=t.uint8, device=self.dev)
+        assert workspace.numel() * workspace.element_size() >= nb
+        e = LhcbEvents(dev.n_events, dev.n_hits, _ptr(dev.zone_off), _ptr(dev.hit_x), _ptr(dev.polarity))
+        v = LhcbVelo(dev.n_events, _ptr(dev.velo_off), _ptr(dev.velo_x), _ptr(dev.velo_y), _ptr(dev.velo_tx),
+                     _ptr(dev.velo_ty), _ptr(dev.polarity))
+        u = None
+        if use_ut and dev.ut_off is not None:
+            u = C.byref(LhcbUt(dev.ut_x0.numel(), _ptr(dev.ut_off), _ptr(dev.ut_x0), _ptr(dev.ut_ylo), _ptr(dev.ut_yhi),
+                               _ptr(dev.ut_row)))
+        rc = self.lib.lhcb_order(self._ctx, C.byref(e), C.byref(v), u, _ptr(workspace), self._stream())
+        _check(self.lib, self._ctx, rc, "lhcb_order")
+        return workspace
+
+    def lhcb_seeding(self, dev: DeviceEvents, out: Optional[dict] = None, workspace=None) -> dict:
         out = out if out is not None else self.alloc_seeds(dev.n_events)
         e = LhcbEvents(dev.n_events, dev.n_hits, _ptr(dev.zone_off), _ptr(dev.hit_x), _ptr(dev.polarity))
         s = self._seeds_struct(out)
-        rc = self.lib.lhcb_seeding(self._ctx, C.byref(e), C.byref(s), VP(0), self._stream())
+        rc = self.lib.lhcb_seeding(self._ctx, C.byref(e), C.byref(s), _ptr(workspace), self._stream())
         _check(self.lib, self._ctx, rc, "lhcb_seeding")
         return out
 
-    def lhcb_matching(self, seeds: dict, dev: DeviceEvents, out: Optional[dict] = None, use_ut: bool = True) -> dict:
+    def lhcb_matching(self, seeds: dict, dev: DeviceEvents, out: Optional[dict] = None, use_ut: bool = True,
+                      workspace=None) -> dict:
         out = out if out is not None else self.alloc_long(dev.n_events)
         s = self._seeds_struct(seeds)
         v = LhcbVelo(dev.n_events, _ptr(dev.velo_off), _ptr(dev.velo_x), _ptr(dev.velo_y), _ptr(dev.velo_tx),
@@ -314,7 +346,7 @@ class Context:
                                _ptr(dev.ut_row)))
         l = LhcbLong(_ptr(out["count"]), _ptr(out["seed_idx"]), _ptr(out["velo_idx"]), _ptr(out["ut_idx"]),
                      _ptr(out["n_ut"]), _ptr(out["qop"]), _ptr(out["chi2"]), _ptr(out["status"]), _ptr(out.get("ghost")))
-        rc = self.lib.lhcb_matching(self._ctx, C.byref(s), C.byref(v), u, C.byref(l), VP(0), self._stream())
+        rc = self.lib.lhcb_matching(self._ctx, C.byref(s), C.byref(v), u, C.byref(l), _ptr(workspace), self._stream())
         _check(self.lib, self._ctx, rc, "lhcb_matching")
         return out
 
@@ -394,14 +426,16 @@ class Context:
 
 class HostPipeline:
     """lhcb_pipeline_create / lhcb_reconstruct_host: host buffers in, host buffers out (the end-to-end
-    path: H2D copies, seeding, matching and D2H copies all inside one C-ABI call)."""
+    path: H2D copies, order, seeding, matching, compaction and D2H copies all inside one C-ABI call)."""
 
-    def __init__(self, ctx: Context, ev, slice_events: int = 2048, use_ut: bool = True):
+    def __init__(self, ctx: Context, ev, slice_events: int = 2048, use_ut: bool = True, want_par: bool = False,
+                 seeds_per_event: int = 256, long_per_event: int = 160):
         """ev: a host batch (lhcb_gen.Events-like).  Its arrays are copied once into pinned host memory;
-        the pipeline's device buffers are sized for this batch."""
+        the pipeline's device buffers are sized for this batch.  seeds_per_event / long_per_event size the dense
+        output arrays (LHCB_ERR_CAPACITY if a batch needs more)."""
         import torch
         self.ctx, self.torch = ctx, torch
-        self.n_events = ev.n_events
+        self.n_events = n = ev.n_events
 
         def pin(a, dt):
             a = np.ascontiguousarray(a, dt)
@@ -413,40 +447,58 @@ class HostPipeline:
                       velo_tx=pin(ev.velo_tx, np.float32), velo_ty=pin(ev.velo_ty, np.float32))
         self.has_ut = use_ut and len(ev.ut_x0) > 0
         if self.has_ut:
-            self.h.update(ut_off=pin(ev.ut_off, np.uint32), ut_x0=pin(ev.ut_x0, np.float32),
-                          ut_ylo=pin(ev.ut_ylo, np.float32), ut_yhi=pin(ev.ut_yhi, np.float32))
-        n, cap = ev.n_events, ev.n_events * ctx.max_long
+            self.h.update(ut_off=pin(ev.ut_off, np.uint32), ut_x0=pin(ev.ut_x0, np.float32), ut_row=pin(ev.ut_row, np.uint8))
+        cs, cl = n * seeds_per_event, n * long_per_event
         z = lambda shape, dt: torch.zeros(shape, dtype=dt).pin_memory()
-        self.out = dict(n_events=n, cap_total=cap, count=z(n, torch.int32), seed_idx=z(cap, torch.int32),
-                        velo_idx=z(cap, torch.int32), ut_idx=z((4, cap), torch.int32), n_ut=z(cap, torch.uint8),
-                        qop=z(cap, torch.float32), chi2=z(cap, torch.float32), status=z(n, torch.int32))
-        self.seed_count = z(2 * n, torch.int32)
+        self.seeds = dict(cap=cs, off=z(2 * n + 1, torch.int32), state=z((5, cs), torch.float32), hits=z((12, cs), torch.int32),
+                          nx=z(cs, torch.uint8), nuv=z(cs, torch.uint8), par=z((7, cs), torch.float32) if want_par else None,
+                          status=z(2 * n, torch.int32))
+        self.long = dict(cap=cl, off=z(n + 1, torch.int32), seed_idx=z(cl, torch.int32), velo_idx=z(cl, torch.int32),
+                         ut_idx=z((4, cl), torch.int32), n_ut=z(cl, torch.uint8), qop=z(cl, torch.float32),
+                         chi2=z(cl, torch.float32), status=z(n, torch.int32))
         self._p = VP(0)
-        rc = ctx.lib.lhcb_pipeline_create(ctx._ctx, n, ev.n_hits, len(ev.velo_x),
-                                          len(ev.ut_x0) if self.has_ut else 0, slice_events, C.byref(self._p))
+        rc = ctx.lib.lhcb_pipeline_create(ctx._ctx, n, ev.n_hits, len(ev.velo_x), len(ev.ut_x0) if self.has_ut else 0,
+                                          slice_events, cs, cl, C.byref(self._p))
         _check(ctx.lib, ctx._ctx, rc, "lhcb_pipeline_create")
         h = self.h
         self._ev = LhcbEvents(n, ev.n_hits, _ptr(h["zone_off"]), _ptr(h["hit_x"]), _ptr(h["polarity"]))
         self._velo = LhcbVelo(n, _ptr(h["velo_off"]), _ptr(h["velo_x"]), _ptr(h["velo_y"]), _ptr(h["velo_tx"]),
                               _ptr(h["velo_ty"]), _ptr(h["polarity"]))
-        self._ut = LhcbUt(len(ev.ut_x0), _ptr(h["ut_off"]), _ptr(h["ut_x0"]), _ptr(h["ut_ylo"]), _ptr(h["ut_yhi"])) if self.has_ut else None
-        o = self.out
-        self._long = LhcbLong(_ptr(o["count"]), _ptr(o["seed_idx"]), _ptr(o["velo_idx"]), _ptr(o["ut_idx"]),
-                              _ptr(o["n_ut"]), _ptr(o["qop"]), _ptr(o["chi2"]), _ptr(o["status"]), VP(0))
+        self._ut = LhcbUt(len(ev.ut_x0), _ptr(h["ut_off"]), _ptr(h["ut_x0"]), VP(0), VP(0), _ptr(h["ut_row"])) if self.has_ut else None
+        s, l = self.seeds, self.long
+        self._hs = LhcbHostSeeds(cs, 0, _ptr(s["off"]), _ptr(s["state"]), _ptr(s["hits"]), _ptr(s["nx"]), _ptr(s["nuv"]),
+                                 _ptr(s["par"]), _ptr(s["status"]))
+        self._hl = LhcbHostLong(cl, 0, _ptr(l["off"]), _ptr(l["seed_idx"]), _ptr(l["velo_idx"]), _ptr(l["ut_idx"]),
+                                _ptr(l["n_ut"]), _ptr(l["qop"]), _ptr(l["chi2"]), _ptr(l["status"]))
 
     def lhcb_reconstruct_host(self):
-        """One end-to-end pass; returns (h2d_bytes, d2h_bytes, kernel launches).  Results are in self.out."""
+        """One end-to-end pass; returns (h2d_bytes, d2h_bytes, kernel launches).  Results: seeds_to_host(), long_to_host()."""
         lib = self.ctx.lib
         rc = lib.lhcb_reconstruct_host(self._p, C.byref(self._ev), C.byref(self._velo),
-                                       C.byref(self._ut) if self._ut is not None else None, C.byref(self._long),
-                                       _ptr(self.seed_count))
+                                       C.byref(self._ut) if self._ut is not None else None, C.byref(self._hs), C.byref(self._hl))
         _check(lib, self.ctx._ctx, rc, "lhcb_reconstruct_host")
         a, b = C.c_uint64(0), C.c_uint64(0)
         launches = lib.lhcb_pipeline_last_bytes(self._p, C.byref(a), C.byref(b))
         return a.value, b.value, launches
 
+    def seeds_to_host(self):
+        """Dense seeds of the last pass in the form of Context.seeds_to_host (slot = dense index)."""
+        s, n = self.seeds, int(self._hs.n)
+        off = s["off"].numpy().view(np.uint32).astype(np.int64)
+        half = np.repeat(np.arange(2 * self.n_events), np.diff(off))
+        return dict(n=n, event=half // 2, half=half % 2, slot=np.arange(n), state=s["state"].numpy()[:, :n].T.copy(),
+                    par=s["par"].numpy()[:, :n].T.copy() if s["par"] is not None else None,
+                    hits=s["hits"].numpy().view(np.uint32)[:, :n].T.copy(), nx=s["nx"].numpy()[:n].copy(),
+                    nuv=s["nuv"].numpy()[:n].copy(), status=s["status"].numpy().view(np.uint32).copy(), off=off)
+
     def long_to_host(self):
-        return self.ctx.long_to_host(self.out)
+        l, n = self.long, int(self._hl.n)
+        off = l["off"].numpy().view(np.uint32).astype(np.int64)
+        ev = np.repeat(np.arange(self.n_events), np.diff(off))
+        g = lambda name: l[name].numpy()
+        return dict(n=n, event=ev, seed=g("seed_idx").view(np.uint32)[:n].copy(), velo=g("velo_idx").view(np.uint32)[:n].copy(),
+                    ut=g("ut_idx").view(np.uint32)[:, :n].T.copy(), n_ut=g("n_ut")[:n].copy(), qop=g("qop")[:n].copy(),
+                    chi2=g("chi2")[:n].copy(), status=g("status").view(np.uint32).copy(), ghost=None, off=off)
 
     def close(self):
         if self._p.value:

@@ -12,6 +12,7 @@
 #include "derive.h"
 #include "matching.cuh"
 #include "prepare.cuh"
+#include "schedule.cuh"
 #include "seeding.cuh"
 
 #ifndef LHCB_SEED_CTAS
@@ -199,8 +200,27 @@ int lhcb_get_geom(const lhcb_ctx* c, lhcb_geom_t* out) {
 }
 
 size_t lhcb_workspace_bytes(const lhcb_ctx* c, int n_events, size_t n_scifi_hits) {
-  (void)c; (void)n_events; (void)n_scifi_hits;
-  return 0;   // every intermediate lives in shared memory
+  (void)c; (void)n_scifi_hits;
+  // every intermediate of the two kernels lives in shared memory; the workspace holds only the optional CTA
+  // orders of lhcb_order: u32[2 n_events] for the Seeding, u32[n_events] for the Matching
+  return n_events > 0 ? (((size_t)n_events * 12 + 15) & ~(size_t)15) : 0;
+}
+
+int lhcb_order(lhcb_ctx* c, const lhcb_events_t* ev, const lhcb_velo_t* velo, const lhcb_ut_t* ut, void* workspace,
+               void* stream) {
+  if (!c) return LHCB_ERR_NOT_INITIALISED;
+  if (!ev || !workspace || ev->n_events < 0 || (velo && velo->n_events != ev->n_events)) return LHCB_ERR_BAD_ARGUMENT;
+  c->last_launches = 0;
+  if (ev->n_events == 0) return LHCB_OK;
+  if (!ev->zone_off || (velo && !velo->off) || (ut && !ut->off)) return LHCB_ERR_BAD_ARGUMENT;
+  LHCB_CUDA(c, cudaSetDevice(c->device));
+  uint32_t* so = static_cast<uint32_t*>(workspace);
+  lhcb::order_kernel<<<1, lhcb::kOrderThreads, 0, (cudaStream_t)stream>>>(ev->n_events, ev->zone_off, ut ? ut->off : nullptr,
+                                                                        velo ? velo->off : nullptr, so,
+                                                                        velo ? so + (size_t)ev->n_events * 2 : nullptr);
+  LHCB_CUDA(c, cudaGetLastError());
+  c->last_launches = 1;
+  return LHCB_OK;
 }
 
 int lhcb_set_uv_hough(lhcb_ctx* c, int on) {
@@ -242,7 +262,6 @@ int lhcb_prepare(lhcb_ctx* c, const lhcb_raw_t* raw, uint32_t* zone_off, float* 
 }
 
 int lhcb_seeding(lhcb_ctx* c, const lhcb_events_t* ev, lhcb_seeds_t* out, void* workspace, void* stream) {
-  (void)workspace;
   if (!c) return LHCB_ERR_NOT_INITIALISED;
   if (!ev || !out || ev->n_events < 0) return LHCB_ERR_BAD_ARGUMENT;
   c->last_launches = 0;
@@ -259,6 +278,7 @@ int lhcb_seeding(lhcb_ctx* c, const lhcb_events_t* ev, lhcb_seeds_t* out, void* 
   p.nuv = out->nuv; p.status = out->status;
   p.cap_total = (size_t)ev->n_events * 2 * (size_t)c->geom.max_seeds_per_half;
   p.smem_total = (int)c->seed_smem;
+  p.order = static_cast<const uint32_t*>(workspace);        // CTA order of lhcb_order, or NULL: CTA b takes half b
   if (c->seed_ctas == LHCB_SEED_CTAS)
     lhcb::seeding_kernel<256, LHCB_SEED_CTAS><<<ev->n_events * 2, 256, c->seed_smem, (cudaStream_t)stream>>>(p);
   else
@@ -270,7 +290,6 @@ int lhcb_seeding(lhcb_ctx* c, const lhcb_events_t* ev, lhcb_seeds_t* out, void* 
 
 int lhcb_matching(lhcb_ctx* c, const lhcb_seeds_t* seeds, const lhcb_velo_t* velo, const lhcb_ut_t* ut,
                   lhcb_long_t* out, void* workspace, void* stream) {
-  (void)workspace;
   if (!c) return LHCB_ERR_NOT_INITIALISED;
   if (!seeds || !velo || !out || velo->n_events < 0 || seeds->n_events != velo->n_events)
     return LHCB_ERR_BAD_ARGUMENT;
@@ -293,6 +312,7 @@ int lhcb_matching(lhcb_ctx* c, const lhcb_seeds_t* seeds, const lhcb_velo_t* vel
   p.n_ut = out->n_ut; p.qop = out->qop; p.chi2 = out->chi2; p.status = out->status;
   p.nn = c->nn_on ? c->d_nn : nullptr; p.snx = seeds->nx; p.snuv = seeds->nuv; p.ghost = out->ghost;
   p.shits = seeds->hits;
+  p.order = workspace ? static_cast<const uint32_t*>(workspace) + (size_t)velo->n_events * 2 : nullptr;
   p.long_cap_total = (size_t)velo->n_events * (size_t)c->geom.max_long_per_event;
   if (c->match_threads == 128)
     lhcb::matching_kernel<128, 6><<<velo->n_events, 128, c->match_smem, (cudaStream_t)stream>>>(p);
@@ -346,21 +366,32 @@ int lhcb_launch_config(const lhcb_ctx* c, int out[4]) {
 }  // extern "C"
 
 // ---------------------------------------------------------------------------------------------
-// Host-buffer pipeline: slices of events, two streams, copies of one slice overlap kernels of another.
+// Host-buffer pipeline: slices of events on three streams (H2D copies, kernels, D2H copies).  The kernels of
+// a slice (order, seeding, matching, compaction) are captured once in a CUDA graph and replayed.
 struct lhcb_pipeline {
   lhcb_ctx* ctx;
-  int max_events, slice;
+  int max_events, slice, n_slices;
   size_t max_hits, max_velo, max_ut;
-  cudaStream_t st[2];
+  uint32_t cap_s, cap_l;
+  cudaStream_t st_in, st_k, st_out;
+  cudaEvent_t *ev_in, *ev_k;          // per slice
   // inputs (whole batch, same offsets as on the host)
   uint32_t *zone_off, *velo_off, *ut_off;
-  float *hit_x, *vx, *vy, *vtx, *vty, *ux, *uylo, *uyhi;
+  float *hit_x, *vx, *vy, *vtx, *vty, *ux;
+  uint8_t* urow;
   int8_t* pol;
-  // per-stream seeds and long-track buffers (one slice each)
-  struct Slot {
-    uint32_t *s_count, *s_hits, *s_status; float *s_state, *s_par; uint8_t *s_nx, *s_nuv;
-    uint32_t *l_count, *l_seed, *l_velo, *l_ut, *l_status; uint8_t* l_nut; float *l_qop, *l_chi2;
-  } slot[2];
+  // slot buffers of one slice (lhcb_seeds_t / lhcb_long_t layout)
+  uint32_t *s_count, *s_hits, *s_status; float *s_state, *s_par; uint8_t *s_nx, *s_nuv;
+  uint32_t *l_count, *l_seed, *l_velo, *l_ut, *l_status; uint8_t* l_nut; float *l_qop, *l_chi2;
+  void* order_ws;
+  // dense outputs of the whole batch
+  uint32_t *d_s_off, *d_l_off, *d_s_status, *d_l_status;
+  float *d_state, *d_par; uint32_t* d_hits; uint8_t *d_nx, *d_nuv;
+  uint32_t *d_seed, *d_velo, *d_ut; uint8_t* d_nut; float *d_qop, *d_chi2;
+  uint32_t *totals, *slice_totals;    // device: [2], [n_slices][4]
+  uint32_t* h_totals;                 // pinned host mirror of slice_totals
+  // one graph per slice
+  struct Graph { cudaGraphExec_t exec; int ne; unsigned flags; } * graphs;
   uint64_t h2d, d2h;
   int launches;
 };
@@ -368,6 +399,44 @@ struct lhcb_pipeline {
 namespace {
 template <class T>
 cudaError_t dalloc(T** p, size_t n) { return cudaMalloc((void**)p, (n ? n : 1) * sizeof(T)); }
+
+// the kernels of one slice on the compute stream (captured into the slice's graph)
+int enqueue_slice(lhcb_pipeline* p, int k, int e0, int ne, bool has_ut, bool has_pol, bool want_par) {
+  lhcb_ctx* c = p->ctx;
+  cudaStream_t s = p->st_k;
+  const size_t z0 = (size_t)e0 * 24;
+  lhcb_events_t dev_ev = {ne, (uint32_t)p->max_hits, p->zone_off + z0, p->hit_x, has_pol ? p->pol + e0 : nullptr};
+  lhcb_velo_t dev_v = {ne, p->velo_off + e0, p->vx, p->vy, p->vtx, p->vty, has_pol ? p->pol + e0 : nullptr};
+  lhcb_ut_t dev_u = {(uint32_t)p->max_ut, p->ut_off + (size_t)e0 * 4, p->ux, nullptr, nullptr, p->urow};
+  lhcb_seeds_t dev_s = {ne, p->s_count, p->s_state, p->s_par, p->s_hits, p->s_nx, p->s_nuv, p->s_status};
+  lhcb_long_t dev_l = {p->l_count, p->l_seed, p->l_velo, p->l_ut, p->l_nut, p->l_qop, p->l_chi2, p->l_status, nullptr};
+  int rc = lhcb_order(c, &dev_ev, &dev_v, has_ut ? &dev_u : nullptr, p->order_ws, s);
+  if (rc != LHCB_OK) return rc;
+  rc = lhcb_seeding(c, &dev_ev, &dev_s, p->order_ws, s);
+  if (rc != LHCB_OK) return rc;
+  rc = lhcb_matching(c, &dev_s, &dev_v, has_ut ? &dev_u : nullptr, &dev_l, p->order_ws, s);
+  if (rc != LHCB_OK) return rc;
+  lhcb::CompactParams q;
+  std::memset(&q, 0, sizeof(q));
+  q.n_events = ne; q.max_seeds = c->geom.max_seeds_per_half; q.max_long = c->geom.max_long_per_event;
+  q.s_count = p->s_count; q.s_state = p->s_state; q.s_par = p->s_par; q.s_hits = p->s_hits; q.s_nx = p->s_nx; q.s_nuv = p->s_nuv;
+  q.l_count = p->l_count; q.l_seed = p->l_seed; q.l_velo = p->l_velo; q.l_ut = p->l_ut; q.l_nut = p->l_nut;
+  q.l_qop = p->l_qop; q.l_chi2 = p->l_chi2;
+  q.totals = p->totals; q.slice_totals = p->slice_totals + (size_t)k * 4;
+  q.s_off = p->d_s_off + (size_t)e0 * 2; q.l_off = p->d_l_off + e0;
+  q.cap_s = p->cap_s; q.cap_l = p->cap_l;
+  q.d_state = p->d_state; q.d_par = want_par ? p->d_par : nullptr; q.d_hits = p->d_hits; q.d_nx = p->d_nx; q.d_nuv = p->d_nuv;
+  q.d_seed = p->d_seed; q.d_velo = p->d_velo; q.d_ut = p->d_ut; q.d_nut = p->d_nut; q.d_qop = p->d_qop; q.d_chi2 = p->d_chi2;
+  lhcb::compact_scan_kernel<<<2, lhcb::kScanThreads, 0, s>>>(q);
+  const int groups = 3 * ne, per = lhcb::kGatherThreads / 32;
+  lhcb::compact_gather_kernel<<<(groups + per - 1) / per, lhcb::kGatherThreads, 0, s>>>(q);
+  LHCB_CUDA(c, cudaGetLastError());
+  // status words of the slice into the batch arrays, totals to the host mirror
+  LHCB_CUDA(c, cudaMemcpyAsync(p->d_s_status + (size_t)e0 * 2, p->s_status, (size_t)ne * 8, cudaMemcpyDeviceToDevice, s));
+  LHCB_CUDA(c, cudaMemcpyAsync(p->d_l_status + e0, p->l_status, (size_t)ne * 4, cudaMemcpyDeviceToDevice, s));
+  LHCB_CUDA(c, cudaMemcpyAsync(p->h_totals + (size_t)k * 4, p->slice_totals + (size_t)k * 4, 16, cudaMemcpyDeviceToHost, s));
+  return LHCB_OK;
+}
 }  // namespace
 
 extern "C" {
@@ -375,130 +444,193 @@ extern "C" {
 void lhcb_pipeline_destroy(lhcb_pipeline* p) {
   if (!p) return;
   cudaSetDevice(p->ctx->device);
-  for (int i = 0; i < 2; ++i) {
-    if (p->st[i]) { cudaStreamSynchronize(p->st[i]); cudaStreamDestroy(p->st[i]); }
-    lhcb_pipeline::Slot& s = p->slot[i];
-    cudaFree(s.s_count); cudaFree(s.s_hits); cudaFree(s.s_status); cudaFree(s.s_state); cudaFree(s.s_par);
-    cudaFree(s.s_nx); cudaFree(s.s_nuv); cudaFree(s.l_count); cudaFree(s.l_seed); cudaFree(s.l_velo);
-    cudaFree(s.l_ut); cudaFree(s.l_status); cudaFree(s.l_nut); cudaFree(s.l_qop); cudaFree(s.l_chi2);
+  for (cudaStream_t s : {p->st_in, p->st_k, p->st_out})
+    if (s) { cudaStreamSynchronize(s); cudaStreamDestroy(s); }
+  for (int k = 0; k < p->n_slices; ++k) {
+    if (p->ev_in && p->ev_in[k]) cudaEventDestroy(p->ev_in[k]);
+    if (p->ev_k && p->ev_k[k]) cudaEventDestroy(p->ev_k[k]);
+    if (p->graphs && p->graphs[k].exec) cudaGraphExecDestroy(p->graphs[k].exec);
   }
-  cudaFree(p->zone_off); cudaFree(p->velo_off); cudaFree(p->ut_off); cudaFree(p->hit_x); cudaFree(p->vx);
-  cudaFree(p->vy); cudaFree(p->vtx); cudaFree(p->vty); cudaFree(p->ux); cudaFree(p->uylo); cudaFree(p->uyhi);
-  cudaFree(p->pol);
+  delete[] p->ev_in; delete[] p->ev_k; delete[] p->graphs;
+  for (void* q : {(void*)p->zone_off, (void*)p->velo_off, (void*)p->ut_off, (void*)p->hit_x, (void*)p->vx, (void*)p->vy,
+                  (void*)p->vtx, (void*)p->vty, (void*)p->ux, (void*)p->urow, (void*)p->pol, (void*)p->s_count,
+                  (void*)p->s_hits, (void*)p->s_status, (void*)p->s_state, (void*)p->s_par, (void*)p->s_nx, (void*)p->s_nuv,
+                  (void*)p->l_count, (void*)p->l_seed, (void*)p->l_velo, (void*)p->l_ut, (void*)p->l_status, (void*)p->l_nut,
+                  (void*)p->l_qop, (void*)p->l_chi2, p->order_ws, (void*)p->d_s_off, (void*)p->d_l_off, (void*)p->d_s_status,
+                  (void*)p->d_l_status, (void*)p->d_state, (void*)p->d_par, (void*)p->d_hits, (void*)p->d_nx, (void*)p->d_nuv,
+                  (void*)p->d_seed, (void*)p->d_velo, (void*)p->d_ut, (void*)p->d_nut, (void*)p->d_qop, (void*)p->d_chi2,
+                  (void*)p->totals, (void*)p->slice_totals})
+    cudaFree(q);
+  if (p->h_totals) cudaFreeHost(p->h_totals);
   delete p;
 }
 
 int lhcb_pipeline_create(lhcb_ctx* c, int max_events, size_t max_hits, size_t max_velo, size_t max_ut,
-                         int slice_events, lhcb_pipeline** out) {
+                         int slice_events, size_t max_seeds_total, size_t max_long_total, lhcb_pipeline** out) {
   if (!c) return LHCB_ERR_NOT_INITIALISED;
-  if (!out || max_events <= 0 || slice_events <= 0) return LHCB_ERR_BAD_ARGUMENT;
+  if (!out || max_events <= 0 || slice_events <= 0 || max_seeds_total > 0xFFFFFFF0u || max_long_total > 0xFFFFFFF0u)
+    return LHCB_ERR_BAD_ARGUMENT;
   *out = nullptr;
   LHCB_CUDA(c, cudaSetDevice(c->device));
   lhcb_pipeline* p = new (std::nothrow) lhcb_pipeline();
   if (!p) return LHCB_ERR_BAD_ARGUMENT;
   std::memset(p, 0, sizeof(*p));
   p->ctx = c; p->max_events = max_events; p->slice = slice_events < max_events ? slice_events : max_events;
+  p->n_slices = (max_events + p->slice - 1) / p->slice;
   p->max_hits = max_hits; p->max_velo = max_velo; p->max_ut = max_ut;
   const size_t ms = c->geom.max_seeds_per_half, ml = c->geom.max_long_per_event, sl = p->slice;
+  p->cap_s = (uint32_t)(max_seeds_total ? max_seeds_total : (size_t)max_events * 2 * ms);
+  p->cap_l = (uint32_t)(max_long_total ? max_long_total : (size_t)max_events * ml);
+  const size_t cs = sl * 2 * ms, cl = sl * ml, CS = p->cap_s, CL = p->cap_l;
   cudaError_t e = cudaSuccess;
   auto ok = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
-  for (int i = 0; i < 2; ++i) ok(cudaStreamCreateWithFlags(&p->st[i], cudaStreamNonBlocking));
-  ok(dalloc(&p->zone_off, (size_t)max_events * 24 + 1)); ok(dalloc(&p->velo_off, (size_t)max_events + 1));
-  ok(dalloc(&p->ut_off, (size_t)max_events * 4 + 1)); ok(dalloc(&p->hit_x, max_hits + 4));
-  ok(dalloc(&p->vx, max_velo)); ok(dalloc(&p->vy, max_velo)); ok(dalloc(&p->vtx, max_velo)); ok(dalloc(&p->vty, max_velo));
-  ok(dalloc(&p->ux, max_ut)); ok(dalloc(&p->uylo, max_ut)); ok(dalloc(&p->uyhi, max_ut));
-  ok(dalloc(&p->pol, (size_t)max_events));
-  for (int i = 0; i < 2; ++i) {
-    lhcb_pipeline::Slot& s = p->slot[i];
-    const size_t cs = sl * 2 * ms, cl = sl * ml;
-    ok(dalloc(&s.s_count, sl * 2)); ok(dalloc(&s.s_status, sl * 2)); ok(dalloc(&s.s_state, 5 * cs));
-    ok(dalloc(&s.s_par, 7 * cs)); ok(dalloc(&s.s_hits, 12 * cs)); ok(dalloc(&s.s_nx, cs)); ok(dalloc(&s.s_nuv, cs));
-    ok(dalloc(&s.l_count, sl)); ok(dalloc(&s.l_status, sl)); ok(dalloc(&s.l_seed, cl)); ok(dalloc(&s.l_velo, cl));
-    ok(dalloc(&s.l_ut, 4 * cl)); ok(dalloc(&s.l_nut, cl)); ok(dalloc(&s.l_qop, cl)); ok(dalloc(&s.l_chi2, cl));
+  for (cudaStream_t* s : {&p->st_in, &p->st_k, &p->st_out}) ok(cudaStreamCreateWithFlags(s, cudaStreamNonBlocking));
+  p->ev_in = new (std::nothrow) cudaEvent_t[p->n_slices]();
+  p->ev_k = new (std::nothrow) cudaEvent_t[p->n_slices]();
+  p->graphs = new (std::nothrow) lhcb_pipeline::Graph[p->n_slices]();
+  if (!p->ev_in || !p->ev_k || !p->graphs) { lhcb_pipeline_destroy(p); return LHCB_ERR_BAD_ARGUMENT; }
+  for (int k = 0; k < p->n_slices; ++k) {
+    ok(cudaEventCreateWithFlags(&p->ev_in[k], cudaEventDisableTiming));
+    ok(cudaEventCreateWithFlags(&p->ev_k[k], cudaEventDisableTiming));
   }
+  ok(dalloc(&p->zone_off, (size_t)max_events * 24 + 1)); ok(dalloc(&p->velo_off, (size_t)max_events + 1));
+  ok(dalloc(&p->ut_off, (size_t)max_events * 4 + 1)); ok(dalloc(&p->hit_x, max_hits + 8));
+  ok(dalloc(&p->vx, max_velo)); ok(dalloc(&p->vy, max_velo)); ok(dalloc(&p->vtx, max_velo)); ok(dalloc(&p->vty, max_velo));
+  ok(dalloc(&p->ux, max_ut + 8)); ok(dalloc(&p->urow, max_ut + 32)); ok(dalloc(&p->pol, (size_t)max_events));
+  ok(dalloc(&p->s_count, sl * 2)); ok(dalloc(&p->s_status, sl * 2)); ok(dalloc(&p->s_state, 5 * cs));
+  ok(dalloc(&p->s_par, 7 * cs)); ok(dalloc(&p->s_hits, 12 * cs)); ok(dalloc(&p->s_nx, cs)); ok(dalloc(&p->s_nuv, cs));
+  ok(dalloc(&p->l_count, sl)); ok(dalloc(&p->l_status, sl)); ok(dalloc(&p->l_seed, cl)); ok(dalloc(&p->l_velo, cl));
+  ok(dalloc(&p->l_ut, 4 * cl)); ok(dalloc(&p->l_nut, cl)); ok(dalloc(&p->l_qop, cl)); ok(dalloc(&p->l_chi2, cl));
+  ok(cudaMalloc(&p->order_ws, lhcb_workspace_bytes(c, (int)sl, 0) + 16));
+  ok(dalloc(&p->d_s_off, (size_t)max_events * 2 + 1)); ok(dalloc(&p->d_l_off, (size_t)max_events + 1));
+  ok(dalloc(&p->d_s_status, (size_t)max_events * 2)); ok(dalloc(&p->d_l_status, (size_t)max_events));
+  ok(dalloc(&p->d_state, 5 * CS)); ok(dalloc(&p->d_par, 7 * CS)); ok(dalloc(&p->d_hits, 12 * CS));
+  ok(dalloc(&p->d_nx, CS)); ok(dalloc(&p->d_nuv, CS));
+  ok(dalloc(&p->d_seed, CL)); ok(dalloc(&p->d_velo, CL)); ok(dalloc(&p->d_ut, 4 * CL)); ok(dalloc(&p->d_nut, CL));
+  ok(dalloc(&p->d_qop, CL)); ok(dalloc(&p->d_chi2, CL));
+  ok(dalloc(&p->totals, 2)); ok(dalloc(&p->slice_totals, (size_t)p->n_slices * 4));
+  ok(cudaMallocHost((void**)&p->h_totals, (size_t)p->n_slices * 16));
   if (e != cudaSuccess) { c->last_cuda_error = (int)e; lhcb_pipeline_destroy(p); return LHCB_ERR_CUDA; }
   *out = p;
   return LHCB_OK;
 }
 
 int lhcb_reconstruct_host(lhcb_pipeline* p, const lhcb_events_t* ev, const lhcb_velo_t* velo, const lhcb_ut_t* ut,
-                          lhcb_long_t* out, uint32_t* host_seed_count) {
+                          lhcb_host_seeds_t* so, lhcb_host_long_t* lo) {
   if (!p) return LHCB_ERR_NOT_INITIALISED;
   lhcb_ctx* c = p->ctx;
-  if (!ev || !velo || !out || ev->n_events < 0 || velo->n_events != ev->n_events || !ev->zone_off || !velo->off ||
-      !out->count || !out->seed_idx || !out->velo_idx || !out->ut_idx || !out->n_ut || !out->qop || !out->chi2 ||
-      !out->status)
+  if (!ev || !velo || !so || !lo || ev->n_events < 0 || velo->n_events != ev->n_events || !ev->zone_off || !velo->off ||
+      !so->off || !so->state || !so->hits || !so->nx || !so->nuv || !so->status || !lo->off || !lo->seed_idx ||
+      !lo->velo_idx || !lo->ut_idx || !lo->n_ut || !lo->qop || !lo->chi2 || !lo->status)
     return LHCB_ERR_BAD_ARGUMENT;
+  if (ut && (!ut->off || !ut->x0 || !ut->row)) return LHCB_ERR_BAD_ARGUMENT;   // the pipeline ships strip rows, not two floats per hit
   const int n = ev->n_events;
   p->h2d = p->d2h = 0; p->launches = 0;
-  if (n == 0) return LHCB_OK;
+  so->n = 0; lo->n = 0;
+  if (n == 0) { so->off[0] = 0; lo->off[0] = 0; return LHCB_OK; }
   if (n > p->max_events || ev->n_hits > p->max_hits) return LHCB_ERR_CAPACITY;
   const size_t n_velo = velo->off[n];
   const size_t n_ut = ut ? ut->off[(size_t)n * 4] : 0;
   if (n_velo > p->max_velo || n_ut > p->max_ut) return LHCB_ERR_CAPACITY;
   LHCB_CUDA(c, cudaSetDevice(c->device));
-  const size_t ms = c->geom.max_seeds_per_half, ml = c->geom.max_long_per_event;
-  const size_t ct_all = (size_t)n * ml;
-  auto H2D = [&](void* d, const void* h, size_t bytes, cudaStream_t s) {
+  int rc = LHCB_OK;
+  cudaError_t ce = cudaSuccess;
+  auto H2D = [&](void* d, const void* h, size_t bytes) {
+    if (ce != cudaSuccess || !bytes) return;
     p->h2d += bytes;
-    return bytes ? cudaMemcpyAsync(d, h, bytes, cudaMemcpyHostToDevice, s) : cudaSuccess;
+    ce = cudaMemcpyAsync(d, h, bytes, cudaMemcpyHostToDevice, p->st_in);
   };
-  auto D2H = [&](void* h, const void* d, size_t bytes, cudaStream_t s) {
+  auto D2H = [&](void* h, const void* d, size_t bytes) {
+    if (ce != cudaSuccess || !bytes) return;
     p->d2h += bytes;
-    return bytes ? cudaMemcpyAsync(h, d, bytes, cudaMemcpyDeviceToHost, s) : cudaSuccess;
+    ce = cudaMemcpyAsync(h, d, bytes, cudaMemcpyDeviceToHost, p->st_out);
   };
-  int k = 0;
-  for (int e0 = 0; e0 < n; e0 += p->slice, ++k) {
-    const int ne = (n - e0) < p->slice ? (n - e0) : p->slice;
-    cudaStream_t s = p->st[k & 1];
-    lhcb_pipeline::Slot& S = p->slot[k & 1];
-    // ---- inputs of this slice, at the same offsets as on the host
+  auto D2H2D = [&](void* h, size_t hpitch, const void* d, size_t dpitch, size_t width, size_t rows) {
+    if (ce != cudaSuccess || !width) return;
+    p->d2h += width * rows;
+    ce = cudaMemcpy2DAsync(h, hpitch, d, dpitch, width, rows, cudaMemcpyDeviceToHost, p->st_out);
+  };
+  const bool has_pol = ev->polarity != nullptr, has_ut = ut != nullptr, want_par = so->par != nullptr;
+  const unsigned flags = (has_pol ? 1u : 0u) | (has_ut ? 2u : 0u) | (want_par ? 4u : 0u) | (c->nn_on ? 8u : 0u) | (c->uv_hough ? 16u : 0u);
+  const int ns = (n + p->slice - 1) / p->slice;
+  // ---- all input copies, slice by slice, on the copy-in stream
+  for (int k = 0; k < ns && ce == cudaSuccess; ++k) {
+    const int e0 = k * p->slice, ne = (n - e0) < p->slice ? (n - e0) : p->slice;
     const size_t z0 = (size_t)e0 * 24, z1 = (size_t)(e0 + ne) * 24;
     const size_t h0 = ev->zone_off[z0], h1 = ev->zone_off[z1];
     const size_t v0 = velo->off[e0], v1 = velo->off[e0 + ne];
-    LHCB_CUDA(c, H2D(p->zone_off + z0, ev->zone_off + z0, (z1 - z0 + 1) * 4, s));
-    LHCB_CUDA(c, H2D(p->hit_x + h0, ev->hit_x + h0, (h1 - h0) * 4, s));
-    if (ev->polarity) LHCB_CUDA(c, H2D(p->pol + e0, ev->polarity + e0, (size_t)ne, s));
-    LHCB_CUDA(c, H2D(p->velo_off + e0, velo->off + e0, ((size_t)ne + 1) * 4, s));
-    LHCB_CUDA(c, H2D(p->vx + v0, velo->x + v0, (v1 - v0) * 4, s));
-    LHCB_CUDA(c, H2D(p->vy + v0, velo->y + v0, (v1 - v0) * 4, s));
-    LHCB_CUDA(c, H2D(p->vtx + v0, velo->tx + v0, (v1 - v0) * 4, s));
-    LHCB_CUDA(c, H2D(p->vty + v0, velo->ty + v0, (v1 - v0) * 4, s));
-    if (ut) {
+    H2D(p->zone_off + z0, ev->zone_off + z0, (z1 - z0 + 1) * 4);
+    H2D(p->hit_x + h0, ev->hit_x + h0, (h1 - h0) * 4);
+    if (has_pol) H2D(p->pol + e0, ev->polarity + e0, (size_t)ne);
+    H2D(p->velo_off + e0, velo->off + e0, ((size_t)ne + 1) * 4);
+    H2D(p->vx + v0, velo->x + v0, (v1 - v0) * 4);
+    H2D(p->vy + v0, velo->y + v0, (v1 - v0) * 4);
+    H2D(p->vtx + v0, velo->tx + v0, (v1 - v0) * 4);
+    H2D(p->vty + v0, velo->ty + v0, (v1 - v0) * 4);
+    if (has_ut) {
       const size_t u0 = ut->off[(size_t)e0 * 4], u1 = ut->off[(size_t)(e0 + ne) * 4];
-      LHCB_CUDA(c, H2D(p->ut_off + (size_t)e0 * 4, ut->off + (size_t)e0 * 4, ((size_t)ne * 4 + 1) * 4, s));
-      LHCB_CUDA(c, H2D(p->ux + u0, ut->x0 + u0, (u1 - u0) * 4, s));
-      LHCB_CUDA(c, H2D(p->uylo + u0, ut->y_lo + u0, (u1 - u0) * 4, s));
-      LHCB_CUDA(c, H2D(p->uyhi + u0, ut->y_hi + u0, (u1 - u0) * 4, s));
+      H2D(p->ut_off + (size_t)e0 * 4, ut->off + (size_t)e0 * 4, ((size_t)ne * 4 + 1) * 4);
+      H2D(p->ux + u0, ut->x0 + u0, (u1 - u0) * 4);
+      H2D(p->urow + u0, ut->row + u0, u1 - u0);
     }
-    // ---- kernels
-    lhcb_events_t dev_ev = {ne, (uint32_t)p->max_hits, p->zone_off + z0, p->hit_x, ev->polarity ? p->pol + e0 : nullptr};
-    dev_ev.n_hits = ev->n_hits;
-    lhcb_seeds_t dev_s = {ne, S.s_count, S.s_state, S.s_par, S.s_hits, S.s_nx, S.s_nuv, S.s_status};
-    int rc = lhcb_seeding(c, &dev_ev, &dev_s, nullptr, s);
-    if (rc != LHCB_OK) return rc;
-    p->launches += c->last_launches;
-    lhcb_velo_t dev_v = {ne, p->velo_off + e0, p->vx, p->vy, p->vtx, p->vty, ev->polarity ? p->pol + e0 : nullptr};
-    lhcb_ut_t dev_u = {(uint32_t)n_ut, p->ut_off + (size_t)e0 * 4, p->ux, p->uylo, p->uyhi};
-    lhcb_long_t dev_l = {S.l_count, S.l_seed, S.l_velo, S.l_ut, S.l_nut, S.l_qop, S.l_chi2, S.l_status, nullptr};
-    rc = lhcb_matching(c, &dev_s, &dev_v, ut ? &dev_u : nullptr, &dev_l, nullptr, s);
-    if (rc != LHCB_OK) return rc;
-    p->launches += c->last_launches;
-    // ---- outputs of this slice
-    const size_t o = (size_t)e0 * ml, cl = (size_t)ne * ml;
-    LHCB_CUDA(c, D2H(out->count + e0, S.l_count, (size_t)ne * 4, s));
-    LHCB_CUDA(c, D2H(out->status + e0, S.l_status, (size_t)ne * 4, s));
-    LHCB_CUDA(c, D2H(out->seed_idx + o, S.l_seed, cl * 4, s));
-    LHCB_CUDA(c, D2H(out->velo_idx + o, S.l_velo, cl * 4, s));
-    for (int l = 0; l < 4; ++l) LHCB_CUDA(c, D2H(out->ut_idx + (size_t)l * ct_all + o, S.l_ut + (size_t)l * cl, cl * 4, s));
-    LHCB_CUDA(c, D2H(out->n_ut + o, S.l_nut, cl, s));
-    LHCB_CUDA(c, D2H(out->qop + o, S.l_qop, cl * 4, s));
-    LHCB_CUDA(c, D2H(out->chi2 + o, S.l_chi2, cl * 4, s));
-    if (host_seed_count) LHCB_CUDA(c, D2H(host_seed_count + (size_t)e0 * 2, S.s_count, (size_t)ne * 8, s));
+    if (ce == cudaSuccess) ce = cudaEventRecord(p->ev_in[k], p->st_in);
   }
-  LHCB_CUDA(c, cudaStreamSynchronize(p->st[0]));
-  LHCB_CUDA(c, cudaStreamSynchronize(p->st[1]));
-  (void)ms;
+  // ---- kernels: one graph per slice on the compute stream
+  if (ce == cudaSuccess) ce = cudaMemsetAsync(p->totals, 0, 8, p->st_k);
+  for (int k = 0; k < ns && ce == cudaSuccess && rc == LHCB_OK; ++k) {
+    const int e0 = k * p->slice, ne = (n - e0) < p->slice ? (n - e0) : p->slice;
+    lhcb_pipeline::Graph& G = p->graphs[k];
+    if (!G.exec || G.ne != ne || G.flags != flags) {
+      if (G.exec) { cudaGraphExecDestroy(G.exec); G.exec = nullptr; }
+      cudaGraph_t graph = nullptr;
+      ce = cudaStreamBeginCapture(p->st_k, cudaStreamCaptureModeThreadLocal);
+      if (ce != cudaSuccess) break;
+      rc = enqueue_slice(p, k, e0, ne, has_ut, has_pol, want_par);
+      const cudaError_t ec = cudaStreamEndCapture(p->st_k, &graph);
+      if (rc != LHCB_OK) { if (graph) cudaGraphDestroy(graph); break; }
+      ce = ec;
+      if (ce == cudaSuccess) ce = cudaGraphInstantiate(&G.exec, graph, 0);
+      if (graph) cudaGraphDestroy(graph);
+      if (ce != cudaSuccess) { G.exec = nullptr; break; }
+      G.ne = ne; G.flags = flags;
+    }
+    ce = cudaStreamWaitEvent(p->st_k, p->ev_in[k], 0);
+    if (ce == cudaSuccess) ce = cudaGraphLaunch(G.exec, p->st_k);
+    if (ce == cudaSuccess) ce = cudaEventRecord(p->ev_k[k], p->st_k);
+    p->launches += 5;                                        // order, seeding, matching, scan, gather
+  }
+  // ---- outputs: as soon as a slice's totals are known, exactly its entries are copied
+  uint32_t seeds_end = 0, long_end = 0;
+  for (int k = 0; k < ns && ce == cudaSuccess && rc == LHCB_OK; ++k) {
+    const int e0 = k * p->slice, ne = (n - e0) < p->slice ? (n - e0) : p->slice;
+    ce = cudaEventSynchronize(p->ev_k[k]);
+    if (ce != cudaSuccess) break;
+    const uint32_t sb = p->h_totals[k * 4], se = p->h_totals[k * 4 + 1], lb = p->h_totals[k * 4 + 2], le = p->h_totals[k * 4 + 3];
+    if (se > p->cap_s || le > p->cap_l || se > so->cap || le > lo->cap) { rc = LHCB_ERR_CAPACITY; break; }
+    seeds_end = se; long_end = le;
+    const size_t CS = p->cap_s, CL = p->cap_l, hs = so->cap, hl = lo->cap, nsd = se - sb, nl = le - lb;
+    D2H(so->off + (size_t)e0 * 2, p->d_s_off + (size_t)e0 * 2, ((size_t)ne * 2 + 1) * 4);
+    D2H(so->status + (size_t)e0 * 2, p->d_s_status + (size_t)e0 * 2, (size_t)ne * 8);
+    D2H2D(so->state + sb, hs * 4, p->d_state + sb, CS * 4, nsd * 4, 5);
+    D2H2D(so->hits + sb, hs * 4, p->d_hits + sb, CS * 4, nsd * 4, 12);
+    if (want_par) D2H2D(so->par + sb, hs * 4, p->d_par + sb, CS * 4, nsd * 4, 7);
+    D2H(so->nx + sb, p->d_nx + sb, nsd);
+    D2H(so->nuv + sb, p->d_nuv + sb, nsd);
+    D2H(lo->off + e0, p->d_l_off + e0, ((size_t)ne + 1) * 4);
+    D2H(lo->status + e0, p->d_l_status + e0, (size_t)ne * 4);
+    D2H(lo->seed_idx + lb, p->d_seed + lb, nl * 4);
+    D2H(lo->velo_idx + lb, p->d_velo + lb, nl * 4);
+    D2H2D(lo->ut_idx + lb, hl * 4, p->d_ut + lb, CL * 4, nl * 4, 4);
+    D2H(lo->n_ut + lb, p->d_nut + lb, nl);
+    D2H(lo->qop + lb, p->d_qop + lb, nl * 4);
+    D2H(lo->chi2 + lb, p->d_chi2 + lb, nl * 4);
+  }
+  // every stream is drained before returning, whatever happened: no copy is left in flight on the caller's buffers
+  const cudaError_t e1 = cudaStreamSynchronize(p->st_in), e2 = cudaStreamSynchronize(p->st_k), e3 = cudaStreamSynchronize(p->st_out);
+  if (ce == cudaSuccess) ce = e1 != cudaSuccess ? e1 : (e2 != cudaSuccess ? e2 : e3);
+  if (rc != LHCB_OK) return rc;
+  if (ce != cudaSuccess) return cuda_fail(c, ce);
+  so->n = seeds_end; lo->n = long_end;
   return LHCB_OK;
 }
 

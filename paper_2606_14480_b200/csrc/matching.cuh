@@ -62,6 +62,7 @@ struct MatchParams {
   const uint8_t *snx, *snuv;
   float* ghost;
   const uint32_t* shits;    // [12][seed_cap_total] hit indices of the seeds or NULL (tie-break of reading A21)
+  const uint32_t* order;    // optional CTA -> event map (heaviest events first) or NULL
 };
 
 struct __align__(8) MatchCand {
@@ -279,7 +280,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
   unsigned long long* velo_best = seed_best + 2 * p.max_seeds;
 
   const int tid = threadIdx.x;
-  const int e = blockIdx.x;
+  const int e = p.order ? (int)p.order[blockIdx.x] : (int)blockIdx.x;
   int flip = 0;                                            // warp_sums buffer of the next block scan
   LHCB_CLK_INIT
   const uint32_t v0 = p.velo_off[e];

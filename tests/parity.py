@@ -63,3 +63,50 @@ def compare_long(orc_m, gpu_m, orc_seed_key, gpu_seed_key):
                                 and np.array_equal(orc_m["chi2"][a].astype(np.float32).view(np.uint32), gpu_m["chi2"][b].view(np.uint32)))
         assert (orc_m["n_ut"][a] == gpu_m["n_ut"][b]).all()
     return res
+
+
+# ---------------------------------------------------------------------------------------- whole batches
+def _seed_matrix(s):
+    return np.column_stack([np.asarray(s["event"], np.int64), np.asarray(s["half"], np.int64), s["hits"].astype(np.int64)])
+
+
+def assert_batch_identical(orc_s, orc_m, gpu_s, gpu_m, what=""):
+    """Whole-batch, vectorised: the CUDA seeds and long tracks equal the oracle's as sets, with bit-identical
+    float32 parameters.  gpu_m["seed"] refers to gpu_s["slot"]; orc_m["seed"] to the row of orc_s.
+    Returns (n_seeds, n_long)."""
+    ko, kg = _seed_matrix(orc_s), _seed_matrix(gpu_s)
+    oo, og = np.lexsort(ko.T[::-1]), np.lexsort(kg.T[::-1])
+    assert ko.shape == kg.shape, (what, "seed counts differ", ko.shape, kg.shape)
+    assert np.array_equal(ko[oo], kg[og]), (what, "seed hit sets differ")
+    assert len(np.unique(ko, axis=0)) == len(ko), (what, "duplicate seeds")
+    for name in ("state", "par"):
+        a = np.ascontiguousarray(orc_s[name][oo], np.float32).view(np.uint32)
+        b = np.ascontiguousarray(gpu_s[name][og], np.float32).view(np.uint32)
+        assert np.array_equal(a, b), (what, name, "not bit-identical")
+    assert np.array_equal(orc_s["nx"][oo], gpu_s["nx"][og]) and np.array_equal(orc_s["nuv"][oo], gpu_s["nuv"][og])
+    # long tracks: (seed identity, velo, ut hits)
+    slot_sorted = np.argsort(gpu_s["slot"])
+    row_of_slot = slot_sorted[np.searchsorted(gpu_s["slot"][slot_sorted], gpu_m["seed"].astype(np.int64))]
+    lo = np.column_stack([ko[orc_m["seed"].astype(np.int64)], orc_m["velo"].astype(np.int64), orc_m["ut"].astype(np.int64)])
+    lg = np.column_stack([kg[row_of_slot], gpu_m["velo"].astype(np.int64), gpu_m["ut"].astype(np.int64)])
+    po, pg = np.lexsort(lo.T[::-1]), np.lexsort(lg.T[::-1])
+    assert lo.shape == lg.shape, (what, "long-track counts differ", lo.shape, lg.shape)
+    assert np.array_equal(lo[po], lg[pg]), (what, "long tracks differ")
+    for name in ("qop", "chi2"):
+        a = np.ascontiguousarray(orc_m[name][po], np.float32).view(np.uint32)
+        b = np.ascontiguousarray(gpu_m[name][pg], np.float32).view(np.uint32)
+        assert np.array_equal(a, b), (what, name, "not bit-identical")
+    assert np.array_equal(orc_m["n_ut"][po], gpu_m["n_ut"][pg])
+    return len(ko), len(lo)
+
+
+def select_events(s, m, keep_event, slot_key="slot"):
+    """Rows of a seeds dict / long-track dict whose event is flagged in keep_event (bool per event)."""
+    ks = keep_event[np.asarray(s["event"], np.int64)]
+    s2 = {k: (v[ks] if isinstance(v, np.ndarray) and v.shape[:1] == ks.shape else v) for k, v in s.items()}
+    km = keep_event[np.asarray(m["event"], np.int64)]
+    m2 = {k: (v[km] if isinstance(v, np.ndarray) and v.shape[:1] == km.shape else v) for k, v in m.items()}
+    if slot_key not in s:                       # oracle: m["seed"] is a row index -> renumber
+        new_row = np.cumsum(ks) - 1
+        m2["seed"] = new_row[m2["seed"].astype(np.int64)].astype(np.uint32)
+    return s2, m2

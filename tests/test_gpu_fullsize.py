@@ -1,0 +1,145 @@
+"""Parity at the sizes BASELINE.json states, on whole batches: cfg2 1,000 events, cfg3 16,384, cfg4 2,000,
+cfg5 1,000, in both launch configurations where the capacities allow.  The oracle runs as independent
+single-threaded processes over event shards (oracle/parallel.py); the comparison is vectorised and exact:
+identical hit-index sets, bit-identical float32 parameters (the north_star bar is 1e-4 / 5 um / 0.1% near a
+threshold; both sides follow one arithmetic specification, so equality is what is asserted)."""
+import numpy as np
+import pytest
+
+from lhcb_gen import config, generate
+from oracle.parallel import reconstruct_parallel
+from tests.parity import assert_batch_identical, select_events
+
+pytestmark = pytest.mark.gpu
+
+
+def run_gpu(geom, ev, caps=None, order=False, hough=False):
+    from paper_2606_14480_b200 import Context, DeviceEvents
+    g = dict(geom)
+    if caps:
+        g.update(caps)
+    c = Context(g)
+    if hough:
+        c.lhcb_set_uv_hough(True)
+    dev = DeviceEvents.from_host(ev)
+    ws = c.lhcb_order(dev) if order else None
+    s = c.lhcb_seeding(dev, workspace=ws)
+    l = c.lhcb_matching(s, dev, workspace=ws)
+    c.torch.cuda.synchronize()
+    out = c.seeds_to_host(s), c.long_to_host(l), c.lhcb_launch_config()
+    c.close()
+    return out
+
+
+def check_properties(ev, gs, gl, ms, ml):
+    """What must hold at any size (readings A6, A9, A14)."""
+    zo = ev.zone_off.astype(np.int64)
+    hits = gs["hits"].astype(np.int64)
+    zbase = (gs["event"].astype(np.int64) * 2 + gs["half"]) * 12
+    for l in range(12):                                   # every hit of a seed lies in its own half's zone of that layer
+        h = hits[:, l]; has = h != 0xFFFFFFFF
+        assert ((h >= zo[zbase + l]) & (h < zo[zbase + l + 1]))[has].all()
+    nx = (hits[:, [0, 3, 4, 7, 8, 11]] != 0xFFFFFFFF).sum(1); nuv = (hits[:, [1, 2, 5, 6, 9, 10]] != 0xFFFFFFFF).sum(1)
+    assert np.array_equal(nx, gs["nx"]) and np.array_equal(nuv, gs["nuv"])
+    assert np.isin(nx, (5, 6)).all() and np.isin(nuv, (4, 5, 6)).all()
+    assert (gs["par"][:, 5] <= 8.0).all() and (gs["par"][:, 6] <= 8.0).all()
+    assert (gl["chi2"] < 2.0).all() and (gl["n_ut"] >= 3).all()
+    assert len(np.unique(gl["seed"])) == gl["n"] and len(np.unique(gl["velo"])) == gl["n"]
+    vo = ev.velo_off.astype(np.int64)
+    assert ((gl["velo"] >= vo[gl["event"]]) & (gl["velo"] < vo[gl["event"] + 1])).all()
+    assert (gl["seed"] // (2 * ms) == gl["event"]).all()
+
+
+@pytest.fixture(scope="module")
+def cfg2_full():
+    ev = generate(config(2), workers=8)
+    assert ev.n_events == 1000
+    return ev, reconstruct_parallel(ev)
+
+
+def test_cfg2_1000_events_both_launch_configurations(cfg2_full):
+    from paper_2606_14480_b200 import capacities
+    ev, (os_, om, _) = cfg2_full
+    for caps, order, threads in ((None, False, (512, 256)), (capacities.NOMINAL, True, (256, 128))):
+        gs, gl, cfg = run_gpu(ev.geom, ev, caps, order)
+        assert (cfg["seed_threads"], cfg["match_threads"]) == threads
+        assert not gs["status"].any() and not gl["status"].any(), "capacity overflow"
+        n_s, n_l = assert_batch_identical(os_, om, gs, gl, f"cfg2 {threads}")
+        assert n_s > 150 * 1000 and n_l > 90 * 1000
+
+
+def test_cfg4_2000_events_default_capacities_and_nominal_overflow_report():
+    """High occupancy + displaced tracks.  The library defaults hold the whole sample; capacities.NOMINAL (sized
+    for mu ~ 5) overflow on part of it: every such half / event carries a status bit, and every event without
+    one is still identical to the oracle's."""
+    from paper_2606_14480_b200 import capacities
+    ev = generate(config(4), workers=8)
+    assert ev.n_events == 2000
+    os_, om, _ = reconstruct_parallel(ev)
+    gs, gl, cfg = run_gpu(ev.geom, ev)
+    assert cfg["seed_threads"] == 512 and not gs["status"].any() and not gl["status"].any()
+    n_s, n_l = assert_batch_identical(os_, om, gs, gl, "cfg4 defaults")
+    assert n_s > 200 * 2000
+    gs, gl, cfg = run_gpu(ev.geom, ev, capacities.NOMINAL, order=True)
+    assert cfg["seed_threads"] == 256
+    bad = (gs["status"].reshape(-1, 2) != 0).any(1) | (gl["status"] != 0)
+    print("cfg4 with NOMINAL capacities: %d of 2000 events report an overflow (bits %s)" %
+          (bad.sum(), sorted(set(np.unique(gs["status"])) | set(np.unique(gl["status"])))))
+    assert 0 < bad.sum() < 2000
+    o2 = select_events(os_, om, ~bad); g2 = select_events(gs, gl, ~bad)
+    assert_batch_identical(o2[0], o2[1], g2[0], g2[1], "cfg4 NOMINAL, events without a status bit")
+
+
+def test_cfg5_1000_events():
+    from paper_2606_14480_b200 import Context, DeviceEvents
+    ev = generate(config(5), workers=8)
+    assert ev.n_events == 1000
+    _, om, _ = reconstruct_parallel(ev, direct_seeds=True)
+    c = Context(ev.geom)
+    dev = DeviceEvents.from_host(ev)
+    seeds, slot = c.seeds_from_states(ev.n_events, ev.seed_off, ev.seed_state)
+    for order in (False, True):
+        ws = c.lhcb_order(dev) if order else None
+        gl = c.long_to_host(c.lhcb_matching(seeds, dev, use_ut=True, workspace=ws))
+        assert not gl["status"].any()
+        inv = np.full(int(slot.max()) + 1, -1, np.int64); inv[slot] = np.arange(len(slot))
+        a = np.column_stack([inv[gl["seed"].astype(np.int64)], gl["velo"].astype(np.int64), gl["ut"].astype(np.int64)])
+        b = np.column_stack([om["seed"].astype(np.int64), om["velo"].astype(np.int64), om["ut"].astype(np.int64)])
+        pa, pb = np.lexsort(a.T[::-1]), np.lexsort(b.T[::-1])
+        assert a.shape == b.shape and np.array_equal(a[pa], b[pb])
+        assert np.array_equal(gl["qop"][pa].view(np.uint32), om["qop"][pb].astype(np.float32).view(np.uint32))
+        assert np.array_equal(gl["chi2"][pa].view(np.uint32), om["chi2"][pb].astype(np.float32).view(np.uint32))
+        assert len(a) > 100 * 1000
+    c.close()
+
+
+def test_cfg3_16384_events_bench_configuration_and_defaults():
+    """BASELINE.json configs[2] at full size (16,384 events, seed 2): ALL events against the oracle, in the
+    launch configuration bench.py times (capacities.NOMINAL with lhcb_order: 256-thread seeding CTAs,
+    128-thread matching CTAs) and with the library defaults."""
+    from paper_2606_14480_b200 import capacities
+    n = 16384
+    ev = generate(config(3, n), workers=8)
+    os_, om, info = reconstruct_parallel(ev)
+    print("oracle: %d processes, %.1f s wall, %.1f core-seconds" % (info["workers"], info["wall_s"], info["cpu_s"]))
+    for caps, order, threads in ((capacities.NOMINAL, True, (256, 128)), (None, False, (512, 256))):
+        gs, gl, cfg = run_gpu(ev.geom, ev, caps, order)
+        assert (cfg["seed_threads"], cfg["match_threads"]) == threads
+        assert not gs["status"].any() and not gl["status"].any(), "capacity overflow at nominal occupancy"
+        g = dict(ev.geom); g.update(caps or {})
+        check_properties(ev, gs, gl, g["max_seeds_per_half"] or 256, g["max_long_per_event"] or 256)
+        n_s, n_l = assert_batch_identical(os_, om, gs, gl, f"cfg3 {threads}")
+        assert n_s > 170 * n and n_l > 100 * n
+
+
+def test_hough_busy_half_reports_overflow_instead_of_writing_out_of_bounds():
+    """a half with more clone-kill survivors than the Hough tables can hold : the survivors are clamped, LHCB_ST_UV_QUEUE_OVERFLOW is set,
+    nothing is written out of bounds; the iterative version (72 bytes per survivor) holds more of them.
+    Noise-free events of 440 tracks: about 190 survivors per half against room for about 150 with these capacities."""
+    from dataclasses import replace
+    ev = generate(replace(config(1), tracks_fixed=440, n_events=4, seed=5))
+    caps = dict(max_hits_per_half=2816, max_xz_cand_per_half=512, max_triplets_per_half=1024, max_seeds_per_half=256)
+    gs, gl, cfg = run_gpu(ev.geom, ev, caps, hough=True)
+    assert (gs["status"] & 256).any(), np.unique(gs["status"])
+    gs2, _, _ = run_gpu(ev.geom, ev, caps, hough=False)
+    assert gs2["n"] > gs["n"]                                     # 72 bytes per survivor: more of them fit

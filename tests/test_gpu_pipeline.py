@@ -1,0 +1,50 @@
+"""The end-to-end call lhcb_reconstruct_host (host buffers in, dense host buffers out, CUDA graph per slice)
+against the oracle: seeds and long tracks, several slices with a ragged last one."""
+import numpy as np
+import pytest
+
+from lhcb_gen import config, generate
+from oracle.parallel import reconstruct_parallel
+from tests.parity import assert_batch_identical
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("nominal", [False, True])
+def test_pipeline_output_equals_oracle(nominal):
+    from paper_2606_14480_b200 import Context, HostPipeline, capacities
+    ev = generate(config(2, 300), workers=4)
+    g = dict(ev.geom)
+    if nominal:
+        g.update(capacities.NOMINAL)
+    c = Context(g)
+    pipe = HostPipeline(c, ev, slice_events=128, want_par=True)          # slices of 128, 128, 44 events
+    for rep in range(2):                                                 # second pass replays the graphs
+        h2d, d2h, launches = pipe.lhcb_reconstruct_host()
+    gs, gl = pipe.seeds_to_host(), pipe.long_to_host()
+    assert not gs["status"].any() and not gl["status"].any()
+    os_, om, _ = reconstruct_parallel(ev, workers=4)
+    n_s, n_l = assert_batch_identical(os_, om, gs, gl, "pipeline")
+    assert n_s > 150 * 300 and n_l > 90 * 300 and launches == 15
+    # offsets: event-half h owns [off[h], off[h+1]) and the long tracks of event e refer to seeds of event e
+    assert gs["off"][-1] == n_s and gl["off"][-1] == n_l
+    ev_of_seed = np.repeat(np.arange(600), np.diff(gs["off"])) // 2
+    assert np.array_equal(ev_of_seed[gl["seed"]], gl["event"])
+    # exactly the found entries are copied back: record sizes 98 B per seed (state, hits, par, nx, nuv), 33 B per long track
+    want = n_s * (5 * 4 + 12 * 4 + 7 * 4 + 2) + n_l * (4 + 4 + 16 + 1 + 4 + 4) + (600 + 300 + 2 * 3) * 4 + 900 * 4
+    assert abs(d2h - want) <= 0.1 * want, (d2h, want)
+    # inputs: hits, offsets, VELO states, UT x0 + one row byte per UT hit
+    assert h2d < 4 * ev.n_hits + 16 * len(ev.velo_x) + 5 * len(ev.ut_x0) + 300 * 140
+    pipe.close()
+    c.close()
+
+
+def test_pipeline_reports_dense_capacity():
+    from paper_2606_14480_b200 import Context, HostPipeline
+    ev = generate(config(2, 8))
+    c = Context(ev.geom)
+    pipe = HostPipeline(c, ev, slice_events=4, seeds_per_event=20)
+    with pytest.raises(RuntimeError, match="capacit"):
+        pipe.lhcb_reconstruct_host()
+    pipe.close()
+    c.close()
