@@ -82,6 +82,7 @@ typedef struct {
   float ut_loose[LHCB_N_UT_LAYERS][4];         /* A, B [mm GeV], min, max per layer: Table 2 (L323-340) */
   float ut_tight[LHCB_N_UT_LAYERS][4];
   float ut_y_tol;                              /* strip y-coverage tolerance (O13) */
+  float ut_strip_x0, ut_strip_pitch;           /* UT strip number s <-> x0 = ut_strip_x0 + s*ut_strip_pitch in float32 (lhcb_ut_t.strip; L315: 190 um pitch) */
   float ut_row_y0, ut_row_pitch;               /* UT strips come in sensor rows: row r covers y in [ut_row_y0 + r*ut_row_pitch,
                                                   that + ut_row_pitch] (lhcb_ut_t.row; BASELINE.json configs[1]: 14 rows of 100 mm) */
   int32_t min_ut_hits, ut_enabled;             /* 3 (L311); 0 disables the UT search (L307) */
@@ -166,6 +167,9 @@ typedef struct {
   const uint32_t* off;       /* [n_events*4+1] */
   const float *x0, *y_lo, *y_hi;
   const uint8_t* row;        /* [n_hits] or NULL */
+  const uint16_t* strip;     /* [n_hits] or NULL: strip numbers, x0 = ut_strip_x0 + strip * ut_strip_pitch.  Read by
+                                lhcb_reconstruct_host only, which then ships 2 bytes per hit instead of the 4 of x0 and
+                                decodes on the device; lhcb_matching reads x0 */
 } lhcb_ut_t;
 
 /* Long tracks.  Event e owns slots [e*max_long_per_event, +count[e]); order unspecified.
@@ -260,8 +264,8 @@ int lhcb_matching(lhcb_ctx* ctx, const lhcb_seeds_t* seeds, const lhcb_velo_t* v
 /* ---- host-buffer pipeline (end-to-end path: H2D copies + seeding + matching + compaction + D2H copies) ----
  * A pipeline owns device buffers sized at creation, three CUDA streams (copies in, kernels, copies out) and one
  * CUDA graph per slice of events.  lhcb_reconstruct_host takes lhcb_events_t / lhcb_velo_t / lhcb_ut_t with
- * HOST pointers (pinned memory for full copy/compute overlap; pageable memory works, slower; lhcb_ut_t.row is
- * required, y_lo / y_hi are not read), splits the batch into slices, and overlaps the input copies of later
+ * HOST pointers (pinned memory for full copy/compute overlap; pageable memory works, slower; of lhcb_ut_t, row is
+ * required, y_lo / y_hi are not read, and strip is shipped instead of x0 when given), splits the batch into slices, and overlaps the input copies of later
  * slices and the output copies of earlier ones with the kernels.  Per slice: lhcb_order, lhcb_seeding,
  * lhcb_matching and two compaction kernels that move seeds and long tracks from their fixed slots to dense
  * arrays, so that exactly the found entries are copied back.  It blocks until every output has landed.
@@ -278,7 +282,9 @@ typedef struct {
   uint32_t cap, n;
   uint32_t* off;       /* [n_events*2+1] */
   float* state;        /* [5][cap]  x, y, tx, ty, q/p at z_scifi_state */
-  uint32_t* hits;      /* [12][cap] global hit index per layer or LHCB_NO_HIT */
+  uint16_t* hits;      /* [12][cap] per layer l: hit index relative to the first hit of the seed's (half, layer) zone, i.e.
+                          global index = host_events.zone_off[half*12 + l] + hits[l], or 0xFFFF for no hit (half the bytes
+                          of a global index on the way back) */
   uint8_t *nx, *nuv;   /* [cap] */
   float* par;          /* [7][cap] ax, bx, cx, ay, by, chi2x, chi2y, or NULL (not copied) */
   uint32_t* status;    /* [n_events*2] LHCB_ST_* bits */

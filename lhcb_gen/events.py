@@ -43,6 +43,7 @@ UT_X_MAX = 850.0
 UT_Y_MAX = 700.0
 UT_ROW = 100.0
 UT_PITCH = 0.190
+UT_STRIP0 = 4474                # strip number of x0 = 0
 
 
 @dataclass
@@ -117,6 +118,7 @@ class Events:
     ut_pid: np.ndarray
     particles: Dict[str, np.ndarray] = field(default_factory=dict)
     ut_row: Optional[np.ndarray] = None       # u8 strip row per UT hit: y_lo = ut_row_y0 + row * ut_row_pitch
+    ut_strip: Optional[np.ndarray] = None     # u16 strip number per UT hit: x0 = ut_strip_x0 + strip * ut_strip_pitch
     # cfg5: seeds given directly as states at z_scifi_state
     seed_off: Optional[np.ndarray] = None
     seed_state: Optional[np.ndarray] = None   # [5, n_seeds] x, y, tx, ty, qop
@@ -209,7 +211,11 @@ def _pack_ut(n_events, parts):
     x0 = np.concatenate([p[2] for p in parts]); ylo = np.concatenate([p[3] for p in parts])
     yhi = np.concatenate([p[4] for p in parts]); pid = np.concatenate([p[5] for p in parts])
     zone = ev * N_UT + lay
-    order = np.lexsort((x0.astype(np.float32), zone))
+    # strip numbers: the float x0 is DERIVED from them with the float32 operations the ABI states
+    # (x0 = ut_strip_x0 + strip * ut_strip_pitch), so both forms of a UT hit agree bit for bit
+    strip = (np.rint(x0 / UT_PITCH).astype(np.int64) + UT_STRIP0).astype(np.uint16)
+    x0 = np.float32(-UT_STRIP0 * UT_PITCH) + strip.astype(np.float32) * np.float32(UT_PITCH)
+    order = np.lexsort((strip, zone))
     off = np.zeros(n_events * N_UT + 1, np.uint32)
     np.cumsum(np.bincount(zone, minlength=n_events * N_UT), out=off[1:])
     # strip rows: one byte per hit.  The float form of the y coverage is DERIVED from the rows with the float32
@@ -218,12 +224,12 @@ def _pack_ut(n_events, parts):
     ylo32 = np.float32(-UT_Y_MAX) + row.astype(np.float32) * np.float32(UT_ROW)
     yhi32 = ylo32 + np.float32(UT_ROW)
     return (off, x0[order].astype(np.float32), ylo32.astype(np.float32),
-            yhi32.astype(np.float32), pid[order].astype(np.int32), row)
+            yhi32.astype(np.float32), pid[order].astype(np.int32), row, strip[order])
 
 
 def _empty_ut(n_events):
     z = np.zeros(0, np.float32)
-    return np.zeros(n_events * N_UT + 1, np.uint32), z, z.copy(), z.copy(), np.zeros(0, np.int32), np.zeros(0, np.uint8)
+    return np.zeros(n_events * N_UT + 1, np.uint32), z, z.copy(), z.copy(), np.zeros(0, np.int32), np.zeros(0, np.uint8), np.zeros(0, np.uint16)
 
 
 def _shuffle_within(rng, ev):
@@ -478,6 +484,7 @@ def generate(cfg: GenConfig, geom: Optional[dict] = None, workers: int = 1, firs
         ut_pid=np.concatenate([c["ut"][4] for c in chunks]),
         particles=parts,
         ut_row=np.concatenate([c["ut"][5] for c in chunks]),
+        ut_strip=np.concatenate([c["ut"][6] for c in chunks]),
     )
     if cfg.direct_seeds:
         evs.seed_off = _cat_off(chunks, "seed_off")
@@ -503,6 +510,7 @@ def slice_events(ev: Events, start: int, stop: int) -> Events:
         ut_off=(ev.ut_off[start * 4:stop * 4 + 1] - ev.ut_off[start * 4]).astype(np.uint32),
         ut_x0=ev.ut_x0[u0:u1], ut_ylo=ev.ut_ylo[u0:u1], ut_yhi=ev.ut_yhi[u0:u1],
         ut_pid=ev.ut_pid[u0:u1], ut_row=ev.ut_row[u0:u1] if ev.ut_row is not None else None,
+        ut_strip=ev.ut_strip[u0:u1] if ev.ut_strip is not None else None,
     )
     if ev.seed_off is not None:
         s0, s1 = int(ev.seed_off[start]), int(ev.seed_off[stop])

@@ -77,6 +77,8 @@ DEFAULT_GEOM = {
                  [0.4, 1.2, 1.0, 4.0],
                  [0.4, 1.2, 1.0, 4.0]],
     "ut_y_tol": 1.0,            # DESIGN.md O13
+    "ut_strip_x0": -4474 * 0.190,   # strip s sits at x0 = ut_strip_x0 + s * ut_strip_pitch; 8,949 strips over |x| < 850 mm
+    "ut_strip_pitch": 0.190,        # L315 / BASELINE.json configs[1]: 190 um pitch
     "ut_row_y0": -700.0,        # UT strips come in 14 sensor rows of 100 mm over |y| < 700 mm (BASELINE.json configs[1])
     "ut_row_pitch": 100.0,
     "min_ut_hits": 3,           # L311 ("more than two")

@@ -38,7 +38,7 @@ class LhcbGeom(C.Structure):
         ("z_velo", F), ("z_scifi_state", F), ("z_match_y", F), ("mag", F * 5), ("gamma_ab", F * 2),
         ("kick_pt", F), ("polarity", I), ("presel", F * 4), ("match_tol", F * 8), ("chi2_match_max", F),
         ("ut_z", F * 4), ("ut_tan_alpha", F * 4), ("ut_loose", (F * 4) * 4), ("ut_tight", (F * 4) * 4),
-        ("ut_y_tol", F), ("ut_row_y0", F), ("ut_row_pitch", F), ("min_ut_hits", I), ("ut_enabled", I),
+        ("ut_y_tol", F), ("ut_strip_x0", F), ("ut_strip_pitch", F), ("ut_row_y0", F), ("ut_row_pitch", F), ("min_ut_hits", I), ("ut_enabled", I),
         ("max_seeds_per_half", I), ("max_xz_cand_per_half", I), ("max_long_per_event", I),
         ("max_hits_per_half", I), ("max_triplets_per_half", I), ("max_match_cand_per_event", I),
         ("max_velo_per_event", I), ("max_ut_per_event", I),
@@ -84,7 +84,7 @@ class LhcbVelo(C.Structure):
 
 
 class LhcbUt(C.Structure):
-    _fields_ = [("n_hits", C.c_uint32), ("off", VP), ("x0", VP), ("y_lo", VP), ("y_hi", VP), ("row", VP)]
+    _fields_ = [("n_hits", C.c_uint32), ("off", VP), ("x0", VP), ("y_lo", VP), ("y_hi", VP), ("row", VP), ("strip", VP)]
 
 
 class LhcbLong(C.Structure):
@@ -122,11 +122,12 @@ def fill_geom(geom: dict) -> LhcbGeom:
 _LIB = None
 
 
-def load_library(build: bool = True) -> C.CDLL:
-    """dlopen the in-tree library (building it first if the sources are newer)."""
+def load_library(build: bool = True, stage_clocks: bool = False) -> C.CDLL:
+    """dlopen the in-tree library (building it first if the sources are newer).  stage_clocks=True selects the
+    diagnostic build with per-stage cycle counters; it must be the first load of the process."""
     global _LIB
     if _LIB is None:
-        path = _build.build() if build else _build.LIB
+        path = _build.build(stage_clocks=stage_clocks) if build else _build.LIB
         if not os.path.exists(path):
             raise RuntimeError(f"CUDA library {path} is missing: run python -m paper_2606_14480_b200.build")
         lib = C.CDLL(path)
@@ -429,7 +430,7 @@ class HostPipeline:
     path: H2D copies, order, seeding, matching, compaction and D2H copies all inside one C-ABI call)."""
 
     def __init__(self, ctx: Context, ev, slice_events: int = 2048, use_ut: bool = True, want_par: bool = False,
-                 seeds_per_event: int = 256, long_per_event: int = 160):
+                 seeds_per_event: int = 256, long_per_event: int = 160, ship_strips: bool = True):
         """ev: a host batch (lhcb_gen.Events-like).  Its arrays are copied once into pinned host memory;
         the pipeline's device buffers are sized for this batch.  seeds_per_event / long_per_event size the dense
         output arrays (LHCB_ERR_CAPACITY if a batch needs more)."""
@@ -448,9 +449,11 @@ class HostPipeline:
         self.has_ut = use_ut and len(ev.ut_x0) > 0
         if self.has_ut:
             self.h.update(ut_off=pin(ev.ut_off, np.uint32), ut_x0=pin(ev.ut_x0, np.float32), ut_row=pin(ev.ut_row, np.uint8))
+            if ship_strips and getattr(ev, "ut_strip", None) is not None:
+                self.h["ut_strip"] = pin(ev.ut_strip.view(np.int16), np.int16)
         cs, cl = n * seeds_per_event, n * long_per_event
         z = lambda shape, dt: torch.zeros(shape, dtype=dt).pin_memory()
-        self.seeds = dict(cap=cs, off=z(2 * n + 1, torch.int32), state=z((5, cs), torch.float32), hits=z((12, cs), torch.int32),
+        self.seeds = dict(cap=cs, off=z(2 * n + 1, torch.int32), state=z((5, cs), torch.float32), hits=z((12, cs), torch.int16),
                           nx=z(cs, torch.uint8), nuv=z(cs, torch.uint8), par=z((7, cs), torch.float32) if want_par else None,
                           status=z(2 * n, torch.int32))
         self.long = dict(cap=cl, off=z(n + 1, torch.int32), seed_idx=z(cl, torch.int32), velo_idx=z(cl, torch.int32),
@@ -464,7 +467,8 @@ class HostPipeline:
         self._ev = LhcbEvents(n, ev.n_hits, _ptr(h["zone_off"]), _ptr(h["hit_x"]), _ptr(h["polarity"]))
         self._velo = LhcbVelo(n, _ptr(h["velo_off"]), _ptr(h["velo_x"]), _ptr(h["velo_y"]), _ptr(h["velo_tx"]),
                               _ptr(h["velo_ty"]), _ptr(h["polarity"]))
-        self._ut = LhcbUt(len(ev.ut_x0), _ptr(h["ut_off"]), _ptr(h["ut_x0"]), VP(0), VP(0), _ptr(h["ut_row"])) if self.has_ut else None
+        self._ut = LhcbUt(len(ev.ut_x0), _ptr(h["ut_off"]), _ptr(h["ut_x0"]), VP(0), VP(0), _ptr(h["ut_row"]),
+                          _ptr(h.get("ut_strip"))) if self.has_ut else None
         s, l = self.seeds, self.long
         self._hs = LhcbHostSeeds(cs, 0, _ptr(s["off"]), _ptr(s["state"]), _ptr(s["hits"]), _ptr(s["nx"]), _ptr(s["nuv"]),
                                  _ptr(s["par"]), _ptr(s["status"]))
@@ -488,8 +492,14 @@ class HostPipeline:
         half = np.repeat(np.arange(2 * self.n_events), np.diff(off))
         return dict(n=n, event=half // 2, half=half % 2, slot=np.arange(n), state=s["state"].numpy()[:, :n].T.copy(),
                     par=s["par"].numpy()[:, :n].T.copy() if s["par"] is not None else None,
-                    hits=s["hits"].numpy().view(np.uint32)[:, :n].T.copy(), nx=s["nx"].numpy()[:n].copy(),
+                    hits=self._global_hits(s["hits"].numpy().view(np.uint16)[:, :n].T, half), nx=s["nx"].numpy()[:n].copy(),
                     nuv=s["nuv"].numpy()[:n].copy(), status=s["status"].numpy().view(np.uint32).copy(), off=off)
+
+    def _global_hits(self, local, half):
+        """Zone-local u16 hit indices [n][12] of the dense seeds -> global u32 indices (LHCB_NO_HIT kept)."""
+        zo = self.h["zone_off"].numpy().view(np.uint32).astype(np.int64)
+        base = zo[half[:, None] * 12 + np.arange(12)[None, :]]
+        return np.where(local == 0xFFFF, NO_HIT, base + local.astype(np.int64)).astype(np.uint32)
 
     def long_to_host(self):
         l, n = self.long, int(self._hl.n)

@@ -29,19 +29,20 @@ def _deps():
         [os.path.join(HERE, "..", "include", "lhcb.h")]
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    override = os.environ.get("LHCB_B200_LIB")       # a prebuilt variant (e.g. a -DLHCB_STAGE_CLOCKS diagnostic build)
-    if override:
-        return override
-    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in _deps()):
-        return LIB
-    cmd = [NVCC, *FLAGS, *sources(), "-o", LIB]
+def build(force: bool = False, verbose: bool = False, stage_clocks: bool = False) -> str:
+    """Compile the library (if the sources are newer).  stage_clocks=True builds the diagnostic variant
+    liblhcb_b200_clk.so (-DLHCB_STAGE_CLOCKS: per-stage cycle counters read by lhcb_debug_stage_clocks; used by
+    `bench.py --stage-clocks` only, never by the timed path)."""
+    lib = LIB.replace(".so", "_clk.so") if stage_clocks else LIB
+    if not force and os.path.exists(lib) and all(os.path.getmtime(lib) >= os.path.getmtime(d) for d in _deps()):
+        return lib
+    cmd = [NVCC, *FLAGS, *(["-DLHCB_STAGE_CLOCKS"] if stage_clocks else []), *sources(), "-o", lib]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or r.returncode != 0:
         sys.stderr.write(r.stdout + r.stderr)
     if r.returncode != 0:
         raise RuntimeError("nvcc failed: " + " ".join(cmd))
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":

@@ -379,6 +379,7 @@ struct lhcb_pipeline {
   uint32_t *zone_off, *velo_off, *ut_off;
   float *hit_x, *vx, *vy, *vtx, *vty, *ux;
   uint8_t* urow;
+  uint16_t* ustrip;
   int8_t* pol;
   // slot buffers of one slice (lhcb_seeds_t / lhcb_long_t layout)
   uint32_t *s_count, *s_hits, *s_status; float *s_state, *s_par; uint8_t *s_nx, *s_nuv;
@@ -386,12 +387,13 @@ struct lhcb_pipeline {
   void* order_ws;
   // dense outputs of the whole batch
   uint32_t *d_s_off, *d_l_off, *d_s_status, *d_l_status;
-  float *d_state, *d_par; uint32_t* d_hits; uint8_t *d_nx, *d_nuv;
+  float *d_state, *d_par; uint16_t* d_hits; uint8_t *d_nx, *d_nuv;
   uint32_t *d_seed, *d_velo, *d_ut; uint8_t* d_nut; float *d_qop, *d_chi2;
   uint32_t *totals, *slice_totals;    // device: [2], [n_slices][4]
   uint32_t* h_totals;                 // pinned host mirror of slice_totals
   // one graph per slice
-  struct Graph { cudaGraphExec_t exec; int ne; unsigned flags; } * graphs;
+  struct Graph { cudaGraphExec_t exec; int e0, ne; unsigned flags; } * graphs;
+  int* e0;                            // [n_slices + 1] first event of each slice of the current batch
   uint64_t h2d, d2h;
   int launches;
 };
@@ -401,9 +403,12 @@ template <class T>
 cudaError_t dalloc(T** p, size_t n) { return cudaMalloc((void**)p, (n ? n : 1) * sizeof(T)); }
 
 // the kernels of one slice on the compute stream (captured into the slice's graph)
-int enqueue_slice(lhcb_pipeline* p, int k, int e0, int ne, bool has_ut, bool has_pol, bool want_par) {
+int enqueue_slice(lhcb_pipeline* p, int k, int e0, int ne, bool has_ut, bool has_pol, bool want_par, bool strips) {
   lhcb_ctx* c = p->ctx;
   cudaStream_t s = p->st_k;
+  if (has_ut && strips)                                      // the slice's UT hits arrived as strip numbers
+    lhcb::ut_decode_kernel<<<296, 256, 0, s>>>(p->ut_off + (size_t)e0 * 4, p->ut_off + (size_t)(e0 + ne) * 4, p->ustrip, p->ux,
+                                               c->geom.ut_strip_x0, c->geom.ut_strip_pitch);
   const size_t z0 = (size_t)e0 * 24;
   lhcb_events_t dev_ev = {ne, (uint32_t)p->max_hits, p->zone_off + z0, p->hit_x, has_pol ? p->pol + e0 : nullptr};
   lhcb_velo_t dev_v = {ne, p->velo_off + e0, p->vx, p->vy, p->vtx, p->vty, has_pol ? p->pol + e0 : nullptr};
@@ -425,7 +430,7 @@ int enqueue_slice(lhcb_pipeline* p, int k, int e0, int ne, bool has_ut, bool has
   q.totals = p->totals; q.slice_totals = p->slice_totals + (size_t)k * 4;
   q.s_off = p->d_s_off + (size_t)e0 * 2; q.l_off = p->d_l_off + e0;
   q.cap_s = p->cap_s; q.cap_l = p->cap_l;
-  q.d_state = p->d_state; q.d_par = want_par ? p->d_par : nullptr; q.d_hits = p->d_hits; q.d_nx = p->d_nx; q.d_nuv = p->d_nuv;
+  q.d_state = p->d_state; q.d_par = want_par ? p->d_par : nullptr; q.d_hits = p->d_hits; q.zone_off = p->zone_off + z0; q.d_nx = p->d_nx; q.d_nuv = p->d_nuv;
   q.d_seed = p->d_seed; q.d_velo = p->d_velo; q.d_ut = p->d_ut; q.d_nut = p->d_nut; q.d_qop = p->d_qop; q.d_chi2 = p->d_chi2;
   lhcb::compact_scan_kernel<<<2, lhcb::kScanThreads, 0, s>>>(q);
   const int groups = 3 * ne, per = lhcb::kGatherThreads / 32;
@@ -451,9 +456,9 @@ void lhcb_pipeline_destroy(lhcb_pipeline* p) {
     if (p->ev_k && p->ev_k[k]) cudaEventDestroy(p->ev_k[k]);
     if (p->graphs && p->graphs[k].exec) cudaGraphExecDestroy(p->graphs[k].exec);
   }
-  delete[] p->ev_in; delete[] p->ev_k; delete[] p->graphs;
+  delete[] p->ev_in; delete[] p->ev_k; delete[] p->graphs; delete[] p->e0;
   for (void* q : {(void*)p->zone_off, (void*)p->velo_off, (void*)p->ut_off, (void*)p->hit_x, (void*)p->vx, (void*)p->vy,
-                  (void*)p->vtx, (void*)p->vty, (void*)p->ux, (void*)p->urow, (void*)p->pol, (void*)p->s_count,
+                  (void*)p->vtx, (void*)p->vty, (void*)p->ux, (void*)p->urow, (void*)p->ustrip, (void*)p->pol, (void*)p->s_count,
                   (void*)p->s_hits, (void*)p->s_status, (void*)p->s_state, (void*)p->s_par, (void*)p->s_nx, (void*)p->s_nuv,
                   (void*)p->l_count, (void*)p->l_seed, (void*)p->l_velo, (void*)p->l_ut, (void*)p->l_status, (void*)p->l_nut,
                   (void*)p->l_qop, (void*)p->l_chi2, p->order_ws, (void*)p->d_s_off, (void*)p->d_l_off, (void*)p->d_s_status,
@@ -476,7 +481,7 @@ int lhcb_pipeline_create(lhcb_ctx* c, int max_events, size_t max_hits, size_t ma
   if (!p) return LHCB_ERR_BAD_ARGUMENT;
   std::memset(p, 0, sizeof(*p));
   p->ctx = c; p->max_events = max_events; p->slice = slice_events < max_events ? slice_events : max_events;
-  p->n_slices = (max_events + p->slice - 1) / p->slice;
+  p->n_slices = (max_events + p->slice - 1) / p->slice + 3;   // the last slice is cut in up to four pieces (shorter tail)
   p->max_hits = max_hits; p->max_velo = max_velo; p->max_ut = max_ut;
   const size_t ms = c->geom.max_seeds_per_half, ml = c->geom.max_long_per_event, sl = p->slice;
   p->cap_s = (uint32_t)(max_seeds_total ? max_seeds_total : (size_t)max_events * 2 * ms);
@@ -488,7 +493,8 @@ int lhcb_pipeline_create(lhcb_ctx* c, int max_events, size_t max_hits, size_t ma
   p->ev_in = new (std::nothrow) cudaEvent_t[p->n_slices]();
   p->ev_k = new (std::nothrow) cudaEvent_t[p->n_slices]();
   p->graphs = new (std::nothrow) lhcb_pipeline::Graph[p->n_slices]();
-  if (!p->ev_in || !p->ev_k || !p->graphs) { lhcb_pipeline_destroy(p); return LHCB_ERR_BAD_ARGUMENT; }
+  p->e0 = new (std::nothrow) int[p->n_slices + 1]();
+  if (!p->ev_in || !p->ev_k || !p->graphs || !p->e0) { lhcb_pipeline_destroy(p); return LHCB_ERR_BAD_ARGUMENT; }
   for (int k = 0; k < p->n_slices; ++k) {
     ok(cudaEventCreateWithFlags(&p->ev_in[k], cudaEventDisableTiming));
     ok(cudaEventCreateWithFlags(&p->ev_k[k], cudaEventDisableTiming));
@@ -496,7 +502,7 @@ int lhcb_pipeline_create(lhcb_ctx* c, int max_events, size_t max_hits, size_t ma
   ok(dalloc(&p->zone_off, (size_t)max_events * 24 + 1)); ok(dalloc(&p->velo_off, (size_t)max_events + 1));
   ok(dalloc(&p->ut_off, (size_t)max_events * 4 + 1)); ok(dalloc(&p->hit_x, max_hits + 8));
   ok(dalloc(&p->vx, max_velo)); ok(dalloc(&p->vy, max_velo)); ok(dalloc(&p->vtx, max_velo)); ok(dalloc(&p->vty, max_velo));
-  ok(dalloc(&p->ux, max_ut + 8)); ok(dalloc(&p->urow, max_ut + 32)); ok(dalloc(&p->pol, (size_t)max_events));
+  ok(dalloc(&p->ux, max_ut + 8)); ok(dalloc(&p->urow, max_ut + 32)); ok(dalloc(&p->ustrip, max_ut + 8)); ok(dalloc(&p->pol, (size_t)max_events));
   ok(dalloc(&p->s_count, sl * 2)); ok(dalloc(&p->s_status, sl * 2)); ok(dalloc(&p->s_state, 5 * cs));
   ok(dalloc(&p->s_par, 7 * cs)); ok(dalloc(&p->s_hits, 12 * cs)); ok(dalloc(&p->s_nx, cs)); ok(dalloc(&p->s_nuv, cs));
   ok(dalloc(&p->l_count, sl)); ok(dalloc(&p->l_status, sl)); ok(dalloc(&p->l_seed, cl)); ok(dalloc(&p->l_velo, cl));
@@ -523,7 +529,7 @@ int lhcb_reconstruct_host(lhcb_pipeline* p, const lhcb_events_t* ev, const lhcb_
       !so->off || !so->state || !so->hits || !so->nx || !so->nuv || !so->status || !lo->off || !lo->seed_idx ||
       !lo->velo_idx || !lo->ut_idx || !lo->n_ut || !lo->qop || !lo->chi2 || !lo->status)
     return LHCB_ERR_BAD_ARGUMENT;
-  if (ut && (!ut->off || !ut->x0 || !ut->row)) return LHCB_ERR_BAD_ARGUMENT;   // the pipeline ships strip rows, not two floats per hit
+  if (ut && (!ut->off || (!ut->x0 && !ut->strip) || !ut->row)) return LHCB_ERR_BAD_ARGUMENT;   // strip rows, not two floats per hit
   const int n = ev->n_events;
   p->h2d = p->d2h = 0; p->launches = 0;
   so->n = 0; lo->n = 0;
@@ -551,11 +557,26 @@ int lhcb_reconstruct_host(lhcb_pipeline* p, const lhcb_events_t* ev, const lhcb_
     ce = cudaMemcpy2DAsync(h, hpitch, d, dpitch, width, rows, cudaMemcpyDeviceToHost, p->st_out);
   };
   const bool has_pol = ev->polarity != nullptr, has_ut = ut != nullptr, want_par = so->par != nullptr;
-  const unsigned flags = (has_pol ? 1u : 0u) | (has_ut ? 2u : 0u) | (want_par ? 4u : 0u) | (c->nn_on ? 8u : 0u) | (c->uv_hough ? 16u : 0u);
-  const int ns = (n + p->slice - 1) / p->slice;
+  const bool strips = has_ut && ut->strip != nullptr;
+  const unsigned flags = (has_pol ? 1u : 0u) | (has_ut ? 2u : 0u) | (want_par ? 4u : 0u) | (c->nn_on ? 8u : 0u) |
+                         (c->uv_hough ? 16u : 0u) | (strips ? 32u : 0u);
+  // slice table: full slices, the last one cut into halves (1/2, 1/4, 1/4) so that the part of the pipeline that
+  // nothing overlaps (kernels and output copies of the final slice) is short
+  int ns = 0;
+  {
+    int e = 0;
+    while (n - e > p->slice) { p->e0[ns++] = e; e += p->slice; }
+    int rem = n - e;
+    for (int piece = 0; piece < 2 && rem >= 512; ++piece) {
+      const int half = ((rem / 2) + 63) & ~63;
+      p->e0[ns++] = e; e += half; rem -= half;
+    }
+    p->e0[ns++] = e;
+    p->e0[ns] = n;
+  }
   // ---- all input copies, slice by slice, on the copy-in stream
   for (int k = 0; k < ns && ce == cudaSuccess; ++k) {
-    const int e0 = k * p->slice, ne = (n - e0) < p->slice ? (n - e0) : p->slice;
+    const int e0 = p->e0[k], ne = p->e0[k + 1] - e0;
     const size_t z0 = (size_t)e0 * 24, z1 = (size_t)(e0 + ne) * 24;
     const size_t h0 = ev->zone_off[z0], h1 = ev->zone_off[z1];
     const size_t v0 = velo->off[e0], v1 = velo->off[e0 + ne];
@@ -570,7 +591,8 @@ int lhcb_reconstruct_host(lhcb_pipeline* p, const lhcb_events_t* ev, const lhcb_
     if (has_ut) {
       const size_t u0 = ut->off[(size_t)e0 * 4], u1 = ut->off[(size_t)(e0 + ne) * 4];
       H2D(p->ut_off + (size_t)e0 * 4, ut->off + (size_t)e0 * 4, ((size_t)ne * 4 + 1) * 4);
-      H2D(p->ux + u0, ut->x0 + u0, (u1 - u0) * 4);
+      if (strips) H2D(p->ustrip + u0, ut->strip + u0, (u1 - u0) * 2);
+      else H2D(p->ux + u0, ut->x0 + u0, (u1 - u0) * 4);
       H2D(p->urow + u0, ut->row + u0, u1 - u0);
     }
     if (ce == cudaSuccess) ce = cudaEventRecord(p->ev_in[k], p->st_in);
@@ -578,33 +600,33 @@ int lhcb_reconstruct_host(lhcb_pipeline* p, const lhcb_events_t* ev, const lhcb_
   // ---- kernels: one graph per slice on the compute stream
   if (ce == cudaSuccess) ce = cudaMemsetAsync(p->totals, 0, 8, p->st_k);
   for (int k = 0; k < ns && ce == cudaSuccess && rc == LHCB_OK; ++k) {
-    const int e0 = k * p->slice, ne = (n - e0) < p->slice ? (n - e0) : p->slice;
+    const int e0 = p->e0[k], ne = p->e0[k + 1] - e0;
     lhcb_pipeline::Graph& G = p->graphs[k];
-    if (!G.exec || G.ne != ne || G.flags != flags) {
+    if (!G.exec || G.e0 != e0 || G.ne != ne || G.flags != flags) {
       if (G.exec) { cudaGraphExecDestroy(G.exec); G.exec = nullptr; }
       cudaGraph_t graph = nullptr;
       ce = cudaStreamBeginCapture(p->st_k, cudaStreamCaptureModeThreadLocal);
       if (ce != cudaSuccess) break;
-      rc = enqueue_slice(p, k, e0, ne, has_ut, has_pol, want_par);
+      rc = enqueue_slice(p, k, e0, ne, has_ut, has_pol, want_par, strips);
       const cudaError_t ec = cudaStreamEndCapture(p->st_k, &graph);
       if (rc != LHCB_OK) { if (graph) cudaGraphDestroy(graph); break; }
       ce = ec;
       if (ce == cudaSuccess) ce = cudaGraphInstantiate(&G.exec, graph, 0);
       if (graph) cudaGraphDestroy(graph);
       if (ce != cudaSuccess) { G.exec = nullptr; break; }
-      G.ne = ne; G.flags = flags;
+      G.e0 = e0; G.ne = ne; G.flags = flags;
     }
     ce = cudaStreamWaitEvent(p->st_k, p->ev_in[k], 0);
     if (ce == cudaSuccess) ce = cudaGraphLaunch(G.exec, p->st_k);
     if (ce == cudaSuccess) ce = cudaEventRecord(p->ev_k[k], p->st_k);
-    p->launches += 5;                                        // order, seeding, matching, scan, gather
+    p->launches += strips ? 6 : 5;                           // (strip decoding,) order, seeding, matching, scan, gather
   }
   // ---- outputs: as soon as a slice's totals are known, exactly its entries are copied
   uint32_t seeds_end = 0, long_end = 0;
   for (int k = 0; k < ns && ce == cudaSuccess && rc == LHCB_OK; ++k) {
-    const int e0 = k * p->slice, ne = (n - e0) < p->slice ? (n - e0) : p->slice;
+    const int e0 = p->e0[k], ne = p->e0[k + 1] - e0;
     ce = cudaEventSynchronize(p->ev_k[k]);
-    if (ce != cudaSuccess) break;
+      if (ce != cudaSuccess) break;
     const uint32_t sb = p->h_totals[k * 4], se = p->h_totals[k * 4 + 1], lb = p->h_totals[k * 4 + 2], le = p->h_totals[k * 4 + 3];
     if (se > p->cap_s || le > p->cap_l || se > so->cap || le > lo->cap) { rc = LHCB_ERR_CAPACITY; break; }
     seeds_end = se; long_end = le;
@@ -612,7 +634,7 @@ int lhcb_reconstruct_host(lhcb_pipeline* p, const lhcb_events_t* ev, const lhcb_
     D2H(so->off + (size_t)e0 * 2, p->d_s_off + (size_t)e0 * 2, ((size_t)ne * 2 + 1) * 4);
     D2H(so->status + (size_t)e0 * 2, p->d_s_status + (size_t)e0 * 2, (size_t)ne * 8);
     D2H2D(so->state + sb, hs * 4, p->d_state + sb, CS * 4, nsd * 4, 5);
-    D2H2D(so->hits + sb, hs * 4, p->d_hits + sb, CS * 4, nsd * 4, 12);
+    D2H2D(so->hits + sb, hs * 2, p->d_hits + sb, CS * 2, nsd * 2, 12);
     if (want_par) D2H2D(so->par + sb, hs * 4, p->d_par + sb, CS * 4, nsd * 4, 7);
     D2H(so->nx + sb, p->d_nx + sb, nsd);
     D2H(so->nuv + sb, p->d_nuv + sb, nsd);

@@ -71,6 +71,15 @@ order_kernel(int n_events, const uint32_t* __restrict__ zone_off, const uint32_t
     }
 }
 
+// UT strip numbers -> x0 for the hits [range[0], range[1]) (read on the device: the grid is fixed, so the
+// launch can sit in a CUDA graph).  x0 = x_origin + strip * pitch, two float32 operations (-fmad=false).
+__global__ void ut_decode_kernel(const uint32_t* __restrict__ range_begin, const uint32_t* __restrict__ range_end,
+                                 const uint16_t* __restrict__ strip, float* __restrict__ x0, float x_origin, float pitch) {
+  const uint32_t b = *range_begin, e = *range_end;
+  for (uint32_t i = b + blockIdx.x * blockDim.x + threadIdx.x; i < e; i += gridDim.x * blockDim.x)
+    x0[i] = x_origin + (float)strip[i] * pitch;
+}
+
 // ---------------------------------------------------------------------------------------------- compaction
 struct CompactParams {
   int n_events;                 // events of this slice
@@ -86,7 +95,8 @@ struct CompactParams {
   uint32_t* s_off;              // [2 n_events + 1] of this slice, absolute (batch) positions
   uint32_t* l_off;              // [n_events + 1]
   uint32_t cap_s, cap_l;
-  float* d_state; float* d_par; uint32_t* d_hits; uint8_t *d_nx, *d_nuv;
+  float* d_state; float* d_par; uint16_t* d_hits; uint8_t *d_nx, *d_nuv;
+  const uint32_t* zone_off;     // of this slice: dense hits are zone-local (hit index - first hit of its (half, layer) zone)
   uint32_t *d_seed, *d_velo, *d_ut; uint8_t* d_nut; float *d_qop, *d_chi2, *d_ghost;
   uint32_t long_velo_rebase, long_ut_rebase;   // (reserved: indices are already batch-global)
 };
@@ -152,7 +162,10 @@ compact_gather_kernel(const __grid_constant__ CompactParams p) {
 #pragma unroll
       for (int k = 0; k < 5; ++k) p.d_state[(size_t)k * p.cap_s + b + i] = p.s_state[(size_t)k * ct + s0 + i];
 #pragma unroll
-      for (int k = 0; k < 12; ++k) p.d_hits[(size_t)k * p.cap_s + b + i] = p.s_hits[(size_t)k * ct + s0 + i];
+      for (int k = 0; k < 12; ++k) {
+        const uint32_t hg = p.s_hits[(size_t)k * ct + s0 + i];
+        p.d_hits[(size_t)k * p.cap_s + b + i] = hg == LHCB_NO_HIT ? (uint16_t)0xFFFF : (uint16_t)(hg - p.zone_off[(size_t)g * 12 + k]);
+      }
       if (p.d_par)
 #pragma unroll
         for (int k = 0; k < 7; ++k) p.d_par[(size_t)k * p.cap_s + b + i] = p.s_par[(size_t)k * ct + s0 + i];

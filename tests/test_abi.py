@@ -26,7 +26,7 @@ def test_library_exports_every_declared_symbol():
 def test_struct_sizes_match_header():
     # sizes implied by the header's field lists (floats/ints are 4 bytes, no padding needed)
     assert C.sizeof(LhcbGeom) == 4 * (12 + 12 + 2 + 5 + 6 + 1 + 4 + 2 + 2 + 2 + 3 + 3 + 3 + 5 + 2 + 1 + 1 + 4 + 8 + 1
-                                      + 4 + 4 + 16 + 16 + 1 + 2 + 2 + 8)
+                                      + 4 + 4 + 16 + 16 + 1 + 2 + 2 + 2 + 8)
     assert C.sizeof(LhcbDerived) == 4 * (6 + 6 + 12 + 6 * 12 + 2 * 24 + 6 + 9 * 2 + 12 + 14 + 3 + 4 + 5 + 4 + 7 + 4
                                          + 16 + 1 + 32 + 7 * 18 + 64 * 12)
 

@@ -25,16 +25,16 @@ def test_pipeline_output_equals_oracle(nominal):
     assert not gs["status"].any() and not gl["status"].any()
     os_, om, _ = reconstruct_parallel(ev, workers=4)
     n_s, n_l = assert_batch_identical(os_, om, gs, gl, "pipeline")
-    assert n_s > 150 * 300 and n_l > 90 * 300 and launches == 15
+    assert n_s > 150 * 300 and n_l > 90 * 300 and launches in (18, 24, 30)
     # offsets: event-half h owns [off[h], off[h+1]) and the long tracks of event e refer to seeds of event e
     assert gs["off"][-1] == n_s and gl["off"][-1] == n_l
     ev_of_seed = np.repeat(np.arange(600), np.diff(gs["off"])) // 2
     assert np.array_equal(ev_of_seed[gl["seed"]], gl["event"])
-    # exactly the found entries are copied back: record sizes 98 B per seed (state, hits, par, nx, nuv), 33 B per long track
-    want = n_s * (5 * 4 + 12 * 4 + 7 * 4 + 2) + n_l * (4 + 4 + 16 + 1 + 4 + 4) + (600 + 300 + 2 * 3) * 4 + 900 * 4
+    # exactly the found entries are copied back: record sizes 74 B per seed (state, hits, par, nx, nuv), 33 B per long track
+    want = n_s * (5 * 4 + 12 * 2 + 7 * 4 + 2) + n_l * (4 + 4 + 16 + 1 + 4 + 4) + (600 + 300 + 2 * 3) * 4 + 900 * 4
     assert abs(d2h - want) <= 0.1 * want, (d2h, want)
     # inputs: hits, offsets, VELO states, UT x0 + one row byte per UT hit
-    assert h2d < 4 * ev.n_hits + 16 * len(ev.velo_x) + 5 * len(ev.ut_x0) + 300 * 140
+    assert h2d < 4 * ev.n_hits + 16 * len(ev.velo_x) + 3 * len(ev.ut_x0) + 300 * 140
     pipe.close()
     c.close()
 
