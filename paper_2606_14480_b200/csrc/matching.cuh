@@ -63,6 +63,7 @@ struct MatchParams {
   float* ghost;
   const uint32_t* shits;    // [12][seed_cap_total] hit indices of the seeds or NULL (tie-break of reading A21)
   const uint32_t* order;    // optional CTA -> event map (heaviest events first) or NULL
+  const uint32_t* done;     // optional per-half "seeds are in global memory" flags of the Seeding (see SeedParams)
 };
 
 struct __align__(8) MatchCand {
@@ -285,10 +286,6 @@ matching_kernel(const __grid_constant__ MatchParams p) {
   LHCB_CLK_INIT
   const uint32_t v0 = p.velo_off[e];
   const int nv = (int)(p.velo_off[e + 1] - v0);
-  int c0 = (int)p.seed_count[2 * e], c1 = (int)p.seed_count[2 * e + 1];
-  if (c0 > p.max_seeds) c0 = p.max_seeds;
-  if (c1 > p.max_seeds) c1 = p.max_seeds;
-  const int ns = c0 + c1;
   if (nv > p.max_velo) {
     if (tid == 0) { p.count[e] = 0; p.status[e] = LHCB_ST_VELO_OVERFLOW; }
     return;
@@ -344,7 +341,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
   // [bin(a), bin(b)] whatever the rounding; values outside +-0.4 land in the edge bins
   auto ty_bin = [](float t) { return (int)fminf(fmaxf((t + 0.4f) * ((float)kTyBins / 0.8f), 0.f), (float)(kTyBins - 1)); };
   for (int v = tid; v < nv; v += T) velo_best[v] = kNoKey;
-  for (int s = tid; s < ns; s += T) seed_best[s] = kNoKey;
+  for (int s = tid; s < 2 * p.max_seeds; s += T) seed_best[s] = kNoKey;
   for (int b = tid; b < kTyBins; b += T) vcur[b] = 0;
   __syncthreads();
   // ---- M0: counting sort of the VELO states into t_y bins (order inside a bin is irrelevant: the bins
@@ -373,6 +370,25 @@ matching_kernel(const __grid_constant__ MatchParams p) {
   __syncthreads();
   LHCB_CLK(9)
 
+  // ---- the seeds of this event: when the Seeding grid may still be running (programmatic dependent launch,
+  // lhcb_order's workspace), wait until both of its halves have raised their flag
+  if (p.done) {
+    if (tid == 0) {
+      const uint32_t* f = p.done + 2 * (size_t)e;
+      uint32_t a = 0, b = 0;
+      for (;;) {
+        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(a) : "l"(f) : "memory");
+        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(b) : "l"(f + 1) : "memory");
+        if (a != 0u && b != 0u) break;
+        __nanosleep(256);
+      }
+    }
+    __syncthreads();
+  }
+  int c0 = (int)p.seed_count[2 * e], c1 = (int)p.seed_count[2 * e + 1];
+  if (c0 > p.max_seeds) c0 = p.max_seeds;
+  if (c1 > p.max_seeds) c1 = p.max_seeds;
+  const int ns = c0 + c1;
   // ---- M1/M2: all seed x VELO pairs (L279), restricted to the |dty| range of each seed ----------
   const size_t sct = p.seed_cap_total;
   auto slot_of = [&](int s) { return s < c0 ? (size_t)(2 * e) * p.max_seeds + s : (size_t)(2 * e + 1) * p.max_seeds + (s - c0); };

@@ -27,23 +27,54 @@ __device__ __forceinline__ int order_bucket(uint32_t w, int shift) {
   return kOrderBuckets - 1 - (int)(b < (uint32_t)kOrderBuckets ? b : (uint32_t)kOrderBuckets - 1);
 }
 
-// one CTA.  seed_order[2 n_events], match_order[n_events] (either may be NULL)
+constexpr int kOrderPerThread = 32;   // weights a thread keeps in registers between the two passes
+constexpr int kOrderMaxSorted = 3072; // batches above this many events run without the workspace (host decision, lhcb_api.cu)
+
+// one CTA.  seed_order[2 n_events], match_order[n_events] (either may be NULL), done[2 n_events].
+// Up to 32 halves per thread (32,768 halves: the 16,384-event batch) are loaded once, all loads in flight
+// together, and kept in registers for the scatter pass; larger batches take a plain two-pass loop.
 __global__ void __launch_bounds__(kOrderThreads)
 order_kernel(int n_events, const uint32_t* __restrict__ zone_off, const uint32_t* __restrict__ ut_off,
-             const uint32_t* __restrict__ velo_off, uint32_t* __restrict__ seed_order, uint32_t* __restrict__ match_order) {
+             const uint32_t* __restrict__ velo_off, uint32_t* __restrict__ seed_order, uint32_t* __restrict__ match_order,
+             uint32_t* __restrict__ done) {
   __shared__ int cur[2][kOrderBuckets];
   const int tid = threadIdx.x;
   for (int i = tid; i < 2 * kOrderBuckets; i += kOrderThreads) (&cur[0][0])[i] = 0;
-  __syncthreads();
   const int nh = 2 * n_events;
-  if (seed_order)
-    for (int h = tid; h < nh; h += kOrderThreads)
-      atomicAdd(&cur[0][order_bucket(zone_off[(size_t)h * 12 + 12] - zone_off[(size_t)h * 12], 4)], 1);
-  if (match_order)
-    for (int e = tid; e < n_events; e += kOrderThreads) {
-      const uint32_t w = ut_off ? ut_off[(size_t)e * 4 + 4] - ut_off[(size_t)e * 4] : 32u * (velo_off[e + 1] - velo_off[e]);
-      atomicAdd(&cur[1][order_bucket(w, 5)], 1);
+  // "seeds are in global memory" flags: up unless a Seeding run lowers them (a Matching on given seeds passes)
+  for (int h = tid; h < nh; h += kOrderThreads) done[h] = 1u;
+  const bool fast = nh <= kOrderThreads * kOrderPerThread;
+  auto seed_w = [&](int h) { return zone_off[(size_t)h * 12 + 12] - zone_off[(size_t)h * 12]; };
+  auto match_w = [&](int e) {
+    return ut_off ? ut_off[(size_t)e * 4 + 4] - ut_off[(size_t)e * 4] : 32u * (velo_off[e + 1] - velo_off[e]);
+  };
+  uint8_t bs[kOrderPerThread], bm[kOrderPerThread / 2];
+  if (fast) {
+#pragma unroll
+    for (int k = 0; k < kOrderPerThread; ++k) {
+      const int h = tid + k * kOrderThreads;
+      bs[k] = (seed_order && h < nh) ? (uint8_t)order_bucket(seed_w(h), 4) : (uint8_t)0;
     }
+#pragma unroll
+    for (int k = 0; k < kOrderPerThread / 2; ++k) {
+      const int e = tid + k * kOrderThreads;
+      bm[k] = (match_order && e < n_events) ? (uint8_t)order_bucket(match_w(e), 5) : (uint8_t)0;
+    }
+  }
+  __syncthreads();
+  if (fast) {
+#pragma unroll
+    for (int k = 0; k < kOrderPerThread; ++k)
+      if (seed_order && tid + k * kOrderThreads < nh) atomicAdd(&cur[0][bs[k]], 1);
+#pragma unroll
+    for (int k = 0; k < kOrderPerThread / 2; ++k)
+      if (match_order && tid + k * kOrderThreads < n_events) atomicAdd(&cur[1][bm[k]], 1);
+  } else {
+    if (seed_order)
+      for (int h = tid; h < nh; h += kOrderThreads) atomicAdd(&cur[0][order_bucket(seed_w(h), 4)], 1);
+    if (match_order)
+      for (int e = tid; e < n_events; e += kOrderThreads) atomicAdd(&cur[1][order_bucket(match_w(e), 5)], 1);
+  }
   __syncthreads();
   if (tid < 64) {                                           // exclusive scan of the 256 buckets of each list, one warp each
     const int which = tid >> 5, lane = tid & 31;
@@ -61,14 +92,23 @@ order_kernel(int n_events, const uint32_t* __restrict__ zone_off, const uint32_t
     }
   }
   __syncthreads();
-  if (seed_order)
-    for (int h = tid; h < nh; h += kOrderThreads)
-      seed_order[atomicAdd(&cur[0][order_bucket(zone_off[(size_t)h * 12 + 12] - zone_off[(size_t)h * 12], 4)], 1)] = (uint32_t)h;
-  if (match_order)
-    for (int e = tid; e < n_events; e += kOrderThreads) {
-      const uint32_t w = ut_off ? ut_off[(size_t)e * 4 + 4] - ut_off[(size_t)e * 4] : 32u * (velo_off[e + 1] - velo_off[e]);
-      match_order[atomicAdd(&cur[1][order_bucket(w, 5)], 1)] = (uint32_t)e;
+  if (fast) {
+#pragma unroll
+    for (int k = 0; k < kOrderPerThread; ++k) {
+      const int h = tid + k * kOrderThreads;
+      if (seed_order && h < nh) seed_order[atomicAdd(&cur[0][bs[k]], 1)] = (uint32_t)h;
     }
+#pragma unroll
+    for (int k = 0; k < kOrderPerThread / 2; ++k) {
+      const int e = tid + k * kOrderThreads;
+      if (match_order && e < n_events) match_order[atomicAdd(&cur[1][bm[k]], 1)] = (uint32_t)e;
+    }
+  } else {
+    if (seed_order)
+      for (int h = tid; h < nh; h += kOrderThreads) seed_order[atomicAdd(&cur[0][order_bucket(seed_w(h), 4)], 1)] = (uint32_t)h;
+    if (match_order)
+      for (int e = tid; e < n_events; e += kOrderThreads) match_order[atomicAdd(&cur[1][order_bucket(match_w(e), 5)], 1)] = (uint32_t)e;
+  }
 }
 
 // UT strip numbers -> x0 for the hits [range[0], range[1]) (read on the device: the grid is fixed, so the

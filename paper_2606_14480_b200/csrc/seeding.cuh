@@ -92,6 +92,8 @@ struct SeedParams {
   const float* hit_x;
   const int8_t* pol;
   const uint32_t* order;   // optional CTA -> event-half map (heaviest halves first) or NULL
+  uint32_t* done;          // optional per-half flags (workspace of lhcb_order): 0 while the half is being seeded, 1 when its
+                           // seeds are in global memory; lets the Matching start before the whole Seeding grid has drained
   uint32_t* count;
   float* state;
   float* par;
@@ -412,7 +414,11 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     constexpr int nw = (12 * (kLutBins + 1) + 1) / 2;
     for (int i = tid; i < nw; i += T) L32[i] = 0xFFFFFFFFu;
   }
+  if (p.done && tid == 0) { p.done[half_id] = 0u; __threadfence(); }
   __syncthreads();                                         // the mbarrier is initialised; the tail hits are in place
+  // programmatic dependent launch: once every CTA of this grid has passed this point (its flag is down), the
+  // Matching grid may be scheduled into the SM resources the last wave leaves free; its CTAs wait on the flags
+  if (p.done) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   {
     uint32_t done = 0;
     while (!done) {
@@ -454,7 +460,10 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   unsigned long long* tbl = reinterpret_cast<unsigned long long*>(smem + off_w);   // aliases trip
   const int trip_cap = w_stat / 8;
   if (H.n_xhits > trip_cap) {                               // clone table would not fit
-    if (tid == 0) { p.count[half_id] = 0; p.status[half_id] = LHCB_ST_HITS_OVERFLOW; }
+    if (tid == 0) {
+      p.count[half_id] = 0; p.status[half_id] = LHCB_ST_HITS_OVERFLOW;
+      if (p.done) { __threadfence(); p.done[half_id] = 1u; }
+    }
     return;
   }
   // the first hit of every occupied bin marks its entry ...
@@ -969,6 +978,10 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     if (ns > p.max_seeds) { ns = p.max_seeds; st |= LHCB_ST_SEED_OVERFLOW; }
     p.count[half_id] = (uint32_t)ns;
     p.status[half_id] = st;
+    if (p.done) {                                            // every seed store of the CTA precedes the barrier above
+      __threadfence();
+      asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p.done + half_id), "r"(1u) : "memory");
+    }
   }
 }
 
