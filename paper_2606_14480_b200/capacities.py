@@ -11,7 +11,7 @@ Observed maxima over the 16,384 events of configs[2] (seed 2), per event-half: 2
 three-hit combinations per iteration (the queue holds both iterations), 432 x-z candidates, 138 clone-kill survivors, 135 seeds; per
 event: 163 VELO states, 3,639 UT hits, 150 chi2-accepted pairs, 166 UT hypotheses.
 """
-NOMINAL = dict(max_hits_per_half=3072, max_xz_cand_per_half=512, max_triplets_per_half=2304,
+NOMINAL = dict(max_hits_per_half=2944, max_xz_cand_per_half=512, max_triplets_per_half=2304,
                max_seeds_per_half=192, max_long_per_event=256, max_match_cand_per_event=192,
                max_velo_per_event=192, max_ut_per_event=3840)
 

@@ -35,7 +35,7 @@
 namespace lhcb {
 
 #ifndef LHCB_LUT_BINS
-#define LHCB_LUT_BINS 320
+#define LHCB_LUT_BINS 256
 #endif
 #ifndef LHCB_ITEM_PAIRS
 #define LHCB_ITEM_PAIRS 4   // T3 hits per item of the pair walk (2, 4 or 8; measured 3.10 ms with 4 against 3.16 ms with 8)
@@ -105,7 +105,10 @@ struct SeedParams {
 };
 
 // all hit references inside the kernel are TILE indices (position in the staged, sentinel-framed tile)
-struct __align__(8) Triplet { uint16_t i1, i2, i3, it; };
+// a queued three-hit combination: zone-local indices of its hits in 10 bits each (a zone holds at most 1,023
+// hits, else the half is reported as LHCB_ST_HITS_OVERFLOW) and the iteration: i1 | i2 << 10 | i3 << 20 | it << 30
+typedef uint32_t Triplet;
+constexpr int kZoneIndexBits = 10;
 struct __align__(16) Cand { float ax, bx, cx, chi2; uint16_t hit[6]; uint8_t nx, it, keep, pattern; };   // nx = 0: rejected by the fit
 
 struct __align__(16) Zone { int b, e; float x0, invw; };   // hits [b, e) of the tile; one 16-byte shared-memory load
@@ -132,16 +135,23 @@ static_assert(sizeof(SeedSmemHeader) <= kSeedHeaderBytes, "shared-memory header 
 // The tile holds, per zone, [..., -inf, hits ..., +inf, ...].  W holds the triplet queue, then the clone table, then the
 // u/v queues; it starts right after the tile and ends where the candidates begin, so a half with fewer hits or
 // candidates than the capacities leaves more room for the queues.  The capacities guarantee
-// W >= max_trip * 8 bytes.  During S1 the (still empty) candidate slots hold the items of the pair walk.
+// W >= max_trip * 4 bytes (seed_w_bytes).  During S1 the (still empty) candidate slots hold the items of the pair walk.
 __host__ __device__ inline size_t seed_align16(size_t b) { return (b + 15) & ~(size_t)15; }
 __host__ __device__ inline size_t seed_off_kept() { return kSeedHeaderBytes + seed_align16(12 * (kLutBins + 1) * 2); }
 __host__ __device__ inline size_t seed_off_hits(int max_cand) { return seed_off_kept() + seed_align16((size_t)max_cand * 2); }
 // tile: per zone [-inf, -inf, hits ..., +inf]
 __host__ __device__ inline size_t seed_tile_bytes(int n_hits) { return seed_align16(((size_t)n_hits + 36) * 4 + 16); }
+// W minimum: the triplet queue.  (The clone table, 8 bytes per x-hit, takes W plus the candidate slots that are
+// still free when the clone kill starts; a half whose table does not fit is reported, LHCB_ST_HITS_OVERFLOW.)
+// W and the candidate slots together also hold the staging buffer of S0 (the half's hits before they move into the tile).
+__host__ __device__ inline size_t seed_w_bytes(int max_hits, int max_cand, int max_trip) {
+  const size_t q = (size_t)max_trip * sizeof(Triplet), stg = ((size_t)max_hits + 8) * 4, c = (size_t)max_cand * 32;
+  return seed_align16(stg > q + c ? stg - c : q);
+}
 __host__ __device__ inline size_t seed_smem_bytes(int max_hits, int max_cand, int max_trip) {
   size_t b = seed_off_hits(max_cand);
-  b += seed_tile_bytes(max_hits);                           // hits tile with its 24 sentinels
-  b += seed_align16((size_t)max_trip * 8);                 // work region W (minimum)
+  b += seed_tile_bytes(max_hits);                           // hits tile with its sentinels
+  b += seed_w_bytes(max_hits, max_cand, max_trip);         // work region W (minimum)
   b += (size_t)max_cand * 32;                              // candidates
   return b;
 }
@@ -368,7 +378,10 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   for (int z = 0; z < 13; ++z) zoff[z] = __ldg(zo + z);
   const int n_half = (int)(zoff[12] - zoff[0]);
   const uint32_t slot0 = (uint32_t)half_id * (uint32_t)p.max_seeds;
-  if (n_half > p.max_hits) {                               // uniform: whole CTA leaves
+  bool zone_too_big = false;
+#pragma unroll
+  for (int z = 0; z < 12; ++z) zone_too_big |= zoff[z + 1] - zoff[z] >= (1u << kZoneIndexBits);
+  if (n_half > p.max_hits || zone_too_big) {               // uniform: whole CTA leaves
     if (tid == 0) { p.count[half_id] = 0; p.status[half_id] = LHCB_ST_HITS_OVERFLOW; }
     return;
   }
@@ -458,14 +471,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   const int w_stat = p.smem_total - p.max_cand * (int)sizeof(Cand) - off_w;   // bytes of W with every candidate slot used
   Triplet* trip = reinterpret_cast<Triplet*>(smem + off_w);
   unsigned long long* tbl = reinterpret_cast<unsigned long long*>(smem + off_w);   // aliases trip
-  const int trip_cap = w_stat / 8;
-  if (H.n_xhits > trip_cap) {                               // clone table would not fit
-    if (tid == 0) {
-      p.count[half_id] = 0; p.status[half_id] = LHCB_ST_HITS_OVERFLOW;
-      if (p.done) { __threadfence(); p.done[half_id] = 1u; }
-    }
-    return;
-  }
+  const int trip_cap = w_stat / (int)sizeof(Triplet);
   // the first hit of every occupied bin marks its entry ...
 #pragma unroll 1
   for (int z = 0; z < 12; ++z) {
@@ -507,7 +513,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     const Zone z1n = H.zi[l1], z2n = H.zi[l2], z3n = H.zi[l3];
     const uint16_t* lut2 = lut + l2 * (kLutBins + 1);
     const uint16_t* lut3 = lut + l3 * (kLutBins + 1);
-    const int b1 = z1n.b, n1 = z1n.e - z1n.b;
+    const int b1 = z1n.b, n1 = z1n.e - z1n.b, b2 = z2n.b, b3 = z3n.b;
     const float r13 = p.r13[it], dx3 = p.dx3max[it], idz = p.inv_dz13[it], z1 = p.z1[it], dz12 = p.dz12[it];
     const float K = p.K[it];
 
@@ -565,11 +571,9 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
           while (xjj <= hi2) {
             if (jj >= e2) break;                                                 // hi2 = +inf: stop at the sentinel
             const int slot = smem_inc(&H.n_trip);
-            if (slot < trip_cap) {
-              Triplet tr;
-              tr.i1 = (uint16_t)i1; tr.i2 = (uint16_t)jj; tr.i3 = (uint16_t)(i3f + k); tr.it = (uint16_t)it;
-              trip[slot] = tr;
-            }
+            if (slot < trip_cap)
+              trip[slot] = (uint32_t)(i1 - b1) | ((uint32_t)(jj - b2) << kZoneIndexBits) |
+                           ((uint32_t)(i3f + k - b3) << (2 * kZoneIndexBits)) | ((uint32_t)it << (3 * kZoneIndexBits));
             ++jj;
             xjj = hx[jj];
           }
@@ -589,9 +593,12 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
 
     for (int t = tid; t < nt; t += T) {
       const Triplet tr = trip[t];
-      const int it = tr.it;                                  // the queue holds iteration 0 first: warps are uniform in it
+      const int it = (int)(tr >> (3 * kZoneIndexBits));      // the queue holds iteration 0 first: warps are uniform in it
       const int l1 = p.l1[it];
-      const float x1 = hx[tr.i1], x2 = hx[tr.i2], x3 = hx[tr.i3];
+      constexpr uint32_t zmask = (1u << kZoneIndexBits) - 1;
+      const int i1 = H.zi[l1].b + (int)(tr & zmask), i2 = H.zi[p.l2[it]].b + (int)((tr >> kZoneIndexBits) & zmask),
+                i3 = H.zi[p.l3[it]].b + (int)((tr >> (2 * kZoneIndexBits)) & zmask);
+      const float x1 = hx[i1], x2 = hx[i2], x3 = hx[i3];
       const float t13 = (x3 - x1) * p.inv_dz13[it];
       const float x2c = x1 + p.dz12[it] * t13;
       const float cx = (x2 - x2c) * p.inv_K[it];
@@ -616,7 +623,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
       if (k < p.max_cand) {
         Cand& cd = cand_end[-1 - k];
         cd.ax = ax; cd.bx = bx; cd.cx = cx; cd.chi2 = 0.f;
-        cd.hit[p.ss[it][0]] = tr.i1; cd.hit[p.ss[it][1]] = tr.i2; cd.hit[p.ss[it][2]] = tr.i3;
+        cd.hit[p.ss[it][0]] = (uint16_t)i1; cd.hit[p.ss[it][1]] = (uint16_t)i2; cd.hit[p.ss[it][2]] = (uint16_t)i3;
 #pragma unroll
         for (int q = 0; q < 3; ++q) cd.hit[p.os[it][q]] = (uint16_t)ho[q];     // -1 -> 0xFFFF
         cd.nx = (uint8_t)(6 - miss); cd.it = (uint8_t)it; cd.keep = 0; cd.pattern = (uint8_t)pattern;
@@ -674,6 +681,13 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   __syncthreads();
   // ---- S3: clone kill (O7) ------------------------------------------------------------------
   const int n_xhits = H.n_xhits;
+  if (n_xhits > (w_stat + (p.max_cand - nc) * (int)sizeof(Cand)) / 8) {   // uniform: the clone table does not fit
+    if (tid == 0) {
+      p.count[half_id] = 0; p.status[half_id] = H.status | LHCB_ST_HITS_OVERFLOW;
+      if (p.done) { __threadfence(); p.done[half_id] = 1u; }
+    }
+    return;
+  }
   for (int i = tid; i < n_xhits; i += T) tbl[i] = kNoKey;
   __syncthreads();
   for (int c = tid; c < nc; c += T) {
