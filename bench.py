@@ -338,20 +338,22 @@ def main():
     # ---- seeding with the Hough-cluster UV version, timed on its own --------------------------
     hough = None
     if rank == 0:
-        ctx.lhcb_set_uv_hough(True)
-        s_h = ctx.alloc_seeds(n)
+        ctx_h = Context(capacities.with_capacities(ev.geom, capacities.NOMINAL_HOUGH), device=local_rank)
+        ctx_h.lhcb_set_uv_hough(True)
+        s_h = ctx_h.alloc_seeds(n)
         e = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
         th_ = []
         for i in range(13):
-            e[0].record(stream); ctx.lhcb_seeding(dev, s_h, workspace=ws); e[1].record(stream); torch.cuda.synchronize()
+            e[0].record(stream); ctx_h.lhcb_seeding(dev, s_h); e[1].record(stream); torch.cuda.synchronize()
             if i >= 3:
                 th_.append(e[0].elapsed_time(e[1]))
-        ctx.lhcb_set_uv_hough(False)
         if int(s_h["status"].max().item()) != 0:
             raise SystemExit("capacity overflow in the Hough-cluster seeding")
+        ctx_h.close()
         hough = {"seeding_ms": float(np.median(th_)), "seeding_events_per_s": n / float(np.median(th_)) * 1e3,
                  "seeds_per_event": int(s_h["count"].sum().item()) / n,
-                 "note": "lhcb_seeding with lhcb_set_uv_hough (reading A20); the timed step uses the iterative default"}
+                 "note": "lhcb_seeding with lhcb_set_uv_hough (reading A20), capacities.NOMINAL_HOUGH (four CTAs per SM); "
+                         "the timed step uses the iterative default"}
         del s_h
 
     # ---- end to end through the host-buffer C-ABI call ---------------------------------------------------

@@ -15,6 +15,10 @@ NOMINAL = dict(max_hits_per_half=2944, max_xz_cand_per_half=512, max_triplets_pe
                max_seeds_per_half=192, max_long_per_event=256, max_match_cand_per_event=192,
                max_velo_per_event=192, max_ut_per_event=3840)
 
+# The Hough-cluster UV version (lhcb_set_uv_hough) keeps 136 bytes of tables per clone-kill survivor and queues
+# up to 32 hypotheses per survivor: it needs a larger work region than the iterative default, at four CTAs per SM.
+NOMINAL_HOUGH = dict(NOMINAL, max_triplets_per_half=4608)
+
 
 def with_capacities(geom: dict, caps: dict = NOMINAL) -> dict:
     g = dict(geom)
