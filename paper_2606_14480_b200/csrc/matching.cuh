@@ -291,7 +291,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     return;
   }
   if (tid < 4) hdr[tid] = 0;
-  if (tid == 4) hdr[9] = 0;                                  // chi2 tie seen (reading A21)
+  if (tid == 4) { hdr[9] = 0; hdr[10] = 0; }                 // chi2 tie seen (reading A21); preselected pairs of the tile
   // ---- UT x0 (and strip rows) of this event: bulk copies, overlapped with the all-pairs loop ----------
   uint32_t u_begin = 0, u_end = 0, ua0 = 0;
   bool ut_in_smem = false, rows_in_smem = false;
@@ -341,7 +341,6 @@ matching_kernel(const __grid_constant__ MatchParams p) {
   // [bin(a), bin(b)] whatever the rounding; values outside +-0.4 land in the edge bins
   auto ty_bin = [](float t) { return (int)fminf(fmaxf((t + 0.4f) * ((float)kTyBins / 0.8f), 0.f), (float)(kTyBins - 1)); };
   for (int v = tid; v < nv; v += T) velo_best[v] = kNoKey;
-  for (int s = tid; s < 2 * p.max_seeds; s += T) seed_best[s] = kNoKey;
   for (int b = tid; b < kTyBins; b += T) vcur[b] = 0;
   __syncthreads();
   // ---- M0: counting sort of the VELO states into t_y bins (order inside a bin is irrelevant: the bins
@@ -391,6 +390,8 @@ matching_kernel(const __grid_constant__ MatchParams p) {
   const int ns = c0 + c1;
   // ---- M1/M2: all seed x VELO pairs (L279), restricted to the |dty| range of each seed ----------
   const size_t sct = p.seed_cap_total;
+  uint32_t* pq = reinterpret_cast<uint32_t*>(seed_best);   // preselected pairs of a tile: (owner << 16) | VELO rank
+  const int pq_cap = 4 * p.max_seeds;
   auto slot_of = [&](int s) { return s < c0 ? (size_t)(2 * e) * p.max_seeds + s : (size_t)(2 * e + 1) * p.max_seeds + (s - c0); };
   for (int tile0 = 0; tile0 < ns; tile0 += T) {
     const int nown = ns - tile0 < T ? ns - tile0 : T;
@@ -436,25 +437,48 @@ matching_kernel(const __grid_constant__ MatchParams p) {
         if (!(fabsf(dx) < p.presel[0] && fabsf(dy) < p.presel[1] && adtx < p.presel[2] &&
               fabsf(dty) < p.presel[3]))                                           // Eq. 21
           continue;
-        const float tolx = p.cx0 + p.cx1 * (dtx * dtx);                            // Eq. 23
-        const float toly = p.cy0 + p.cy1 * (txV * txV + tyV * tyV);
-        const float chi2 = (((dx * dx) / tolx + (dy * dy) / toly) + (dtx * dtx) * p.inv_tol_tx) +
-                           (dty * dty) * p.inv_tol_ty;                             // Eq. 22
-        if (!(chi2 < p.chi2m_max)) continue;                                       // L301
-        const int k = smem_inc(&hdr[0]);
-        if (k < p.max_mc) {
-          MatchCand m;
-          m.seed = (uint16_t)(tile0 + t); m.velo = (uint16_t)v; m.chi2 = chi2; m.q0 = dtx * p.inv_KB;   // A10
-          m.gamma = 0.f; m.key = kNoKey;
-#pragma unroll
-          for (int l = 0; l < 4; ++l) m.ut[l] = 0xFFFF;
-          mc[k] = m;
-        }
+        // about one pair in eight of the range passes: queued, so that chi2_match (two divisions) and the pair
+        // record are done by a dense pass instead of two or three lanes of every warp
+        const int k = smem_inc(&hdr[10]);
+        if (k < pq_cap) pq[k] = ((uint32_t)t << 16) | (uint32_t)v;
       }
     }
     __syncthreads();
+    int nq = hdr[10];
+    if (nq > pq_cap) { nq = pq_cap; if (tid == 0) hdr[2] |= LHCB_ST_MATCH_OVERFLOW; }
+    for (int i = tid; i < nq; i += T) {
+      const uint32_t e_ = pq[i];
+      const int t = (int)(e_ >> 16), v = (int)(e_ & 0xFFFFu);
+      const float4 o = sown[t];
+      const float xS = o.x, ys = o.y, txS = o.z, tyS = o.w;
+      const float xV = svx[v], yV = svy[v], txV = svtx[v], tyV = svty[v];
+      // the same operations on the same operands as in the walk above: the same values
+      const float dtx = txS - txV, dty = tyS - tyV, adtx = fabsf(dtx);
+      const float zm = (((p.mag[0] + p.mag[1] * adtx) + p.mag[2] * (dtx * dtx)) + p.mag[3] * fabsf(xS)) +
+                       p.mag[4] * (txV * txV);                                   // Eq. 18
+      const float xs = xS + (zm - p.zS) * txS, xv = xV + (zm - p.zV) * txV;      // Eq. 17
+      const float yv = yV + p.dzyV * tyV;
+      const float dx = xs - xv, dy = ys - yv;
+      const float tolx = p.cx0 + p.cx1 * (dtx * dtx);                            // Eq. 23
+      const float toly = p.cy0 + p.cy1 * (txV * txV + tyV * tyV);
+      const float chi2 = (((dx * dx) / tolx + (dy * dy) / toly) + (dtx * dtx) * p.inv_tol_tx) +
+                         (dty * dty) * p.inv_tol_ty;                             // Eq. 22
+      if (!(chi2 < p.chi2m_max)) continue;                                       // L301
+      const int k = smem_inc(&hdr[0]);
+      if (k < p.max_mc) {
+        MatchCand m;
+        m.seed = (uint16_t)(tile0 + t); m.velo = (uint16_t)v; m.chi2 = chi2; m.q0 = dtx * p.inv_KB;   // A10
+        m.gamma = 0.f; m.key = kNoKey;
+#pragma unroll
+        for (int l = 0; l < 4; ++l) m.ut[l] = 0xFFFF;
+        mc[k] = m;
+      }
+    }
+    __syncthreads();
+    if (tid == 0) hdr[10] = 0;
     LHCB_CLK(11)
   }
+  for (int s = tid; s < 2 * p.max_seeds; s += T) seed_best[s] = kNoKey;   // (the queue of preselected pairs is dead)
   int nm = hdr[0];
   LHCB_DBG_MAX(4, nm)
   if (nm > p.max_mc) { nm = p.max_mc; if (tid == 0) hdr[2] |= LHCB_ST_MATCH_OVERFLOW; }
