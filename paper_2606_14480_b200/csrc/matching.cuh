@@ -7,9 +7,9 @@
 //   M1/M2  "all seed x VELO pairs" (L279) without touching most of them: the |dty| cut of Eq. 21 selects
 //          a contiguous range of the t_y-binned VELO states (the bins of the window edges, with a safety
 //          margin; the literal cut is still applied to every pair in the range, so the accepted set
-//          is exactly that of the exhaustive loop).  Pairs in range are flattened over the CTA:
-//          kink extrapolation (Eq. 17-18), preselection (Eq. 21), chi2_match (Eq. 22-23) < 2; accepted
-//          pairs are queued in shared memory
+//          is exactly that of the exhaustive loop).  Thread per seed over its range: kink extrapolation
+//          (Eq. 17-18), preselection (Eq. 21); the pairs that pass are queued and a dense pass computes
+//          chi2_match (Eq. 22-23) < 2 and writes the pair records
 //   M3a    thread per queued pair: loose UT window, layer by layer until one has hits; every such hit
 //          becomes a queued hypothesis (Eq. 19-20, Table 2, reading A13)
 //   M3b    thread per hypothesis: tight windows in the remaining layers, gamma_x refits; the best
@@ -99,7 +99,7 @@ __host__ __device__ inline size_t match_smem_bytes(int T, int max_seeds, int max
   b += (size_t)max_velo * 16;                // VELO states, sorted by ty
   b += match_align16((size_t)max_velo * 2);  // original index of each sorted state
   b += match_align16((size_t)(kTyBins + 1) * 2);   // start of each t_y bin
-  b += match_align16((size_t)(T + 1) * 4 + (size_t)T * 2 + 144);   // work-list scan scratch (two warp_sums buffers)
+  b += 144;                                  // two warp_sums buffers of the block scan
   b += match_align16(match_x_bytes(T, max_mc));
   b += (size_t)max_mc * sizeof(MatchCand);
   b += (size_t)2 * max_seeds * 8;            // best key per seed
@@ -264,10 +264,8 @@ matching_kernel(const __grid_constant__ MatchParams p) {
   off += match_align16((size_t)p.max_velo * 2);
   uint16_t* vbin = reinterpret_cast<uint16_t*>(smem + off);               // [kTyBins + 1]
   off += match_align16((size_t)(kTyBins + 1) * 2);
-  int* offs = reinterpret_cast<int*>(smem + off);                         // [T + 1]
-  uint16_t* firsts = reinterpret_cast<uint16_t*>(offs + T + 1);
-  int* warp_sums = reinterpret_cast<int*>(smem + off + (T + 1) * 4 + T * 2);
-  off += match_align16((size_t)(T + 1) * 4 + (size_t)T * 2 + 144);
+  int* warp_sums = reinterpret_cast<int*>(smem + off);                    // two buffers of the block scan (M0)
+  off += 144;
   unsigned char* regx = smem + off;
   int* vcur = reinterpret_cast<int*>(regx);                                // M0: [kTyBins] scatter cursors
   float4* sown = reinterpret_cast<float4*>(regx);                          // M1/M2: (x, y at z_match_y, tx, ty) of the tile's seeds
@@ -406,27 +404,11 @@ matching_kernel(const __grid_constant__ MatchParams p) {
       const int lst = vbin[ty_bin(tyS + w) + 1];
       cnt = lst - fst;
     }
-    int total;
-    const int ex = block_exscan<T>(cnt, warp_sums, flip, total);
-    offs[tid] = ex; firsts[tid] = (uint16_t)fst;
-    if (tid == T - 1) offs[T] = total;
-    __syncthreads();
     LHCB_CLK(10)
-    const int chunk = (total + T - 1) / T;
-    const int p0 = tid * chunk, p1 = p0 + chunk < total ? p0 + chunk : total;
-    if (p0 < p1) {
-      int t = owner_of(offs, nown, p0) - 1;
-      int nxt = -1, f = 0;
-      float xS = 0.f, txS = 0.f, tyS = 0.f, axS = 0.f, ys = 0.f;
-      for (int q = p0; q < p1; ++q) {
-        if (q >= nxt) {
-          do { ++t; nxt = offs[t + 1]; } while (q >= nxt);
-          const float4 o = sown[t];
-          xS = o.x; ys = o.y; txS = o.z; tyS = o.w;
-          axS = fabsf(xS);
-          f = (int)firsts[t] - offs[t];
-        }
-        const int v = f + q;                                                       // rank in ty order
+    if (tid < nown) {                                        // thread per seed: its own range of VELO states
+      const float4 o = sown[tid];
+      const float xS = o.x, ys = o.y, txS = o.z, tyS = o.w, axS = fabsf(xS);
+      for (int v = fst; v < fst + cnt; ++v) {
         const float xV = svx[v], yV = svy[v], txV = svtx[v], tyV = svty[v];
         const float dtx = txS - txV, dty = tyS - tyV, adtx = fabsf(dtx);
         const float zm = (((p.mag[0] + p.mag[1] * adtx) + p.mag[2] * (dtx * dtx)) + p.mag[3] * axS) +
@@ -437,10 +419,8 @@ matching_kernel(const __grid_constant__ MatchParams p) {
         if (!(fabsf(dx) < p.presel[0] && fabsf(dy) < p.presel[1] && adtx < p.presel[2] &&
               fabsf(dty) < p.presel[3]))                                           // Eq. 21
           continue;
-        // about one pair in eight of the range passes: queued, so that chi2_match (two divisions) and the pair
-        // record are done by a dense pass instead of two or three lanes of every warp
         const int k = smem_inc(&hdr[10]);
-        if (k < pq_cap) pq[k] = ((uint32_t)t << 16) | (uint32_t)v;
+        if (k < pq_cap) pq[k] = ((uint32_t)tid << 16) | (uint32_t)v;
       }
     }
     __syncthreads();
