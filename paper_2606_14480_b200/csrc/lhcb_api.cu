@@ -26,6 +26,7 @@ struct lhcb_ctx {
   int nn_on;
   int uv_hough;       // Hough-cluster UV seeding instead of the iterative one
   size_t seed_smem, match_smem, prep_smem;
+  int prep_variant;   // instantiation of prepare_kernel (threads x hits per thread) that covers the event capacity
   int match_threads;  // 128 when six CTAs fit an SM, else 256
   int seed_threads;   // 256 when four CTAs fit the SM's shared memory, else 512
   int seed_ctas;      // CTAs per SM the seeding kernel is compiled for (register budget)
@@ -169,8 +170,13 @@ int lhcb_geom_init(const lhcb_geom_t* g, int device, lhcb_ctx** out) {
     e = c->match_threads == 128
             ? cudaFuncSetAttribute(lhcb::matching_kernel<128, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->match_smem)
             : cudaFuncSetAttribute(lhcb::matching_kernel<256, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->match_smem);
+  // the preparation keeps one register per raw hit: T threads x R hits per thread >= the event capacity
+  c->prep_variant = 2 * G.max_hits_per_half <= 512 * 12 ? 0 : 2 * G.max_hits_per_half <= 1024 * 12 ? 1 : 2;
   if (e == cudaSuccess)
-    e = cudaFuncSetAttribute(lhcb::prepare_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->prep_smem);
+    e = cudaFuncSetAttribute(c->prep_variant == 0   ? (const void*)lhcb::prepare_kernel<512, 12, 3>
+                             : c->prep_variant == 1 ? (const void*)lhcb::prepare_kernel<1024, 12, 1>
+                                                    : (const void*)lhcb::prepare_kernel<1024, 16, 1>,
+                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->prep_smem);
   if (e == cudaSuccess) e = cudaMalloc(&c->d_P, sizeof(c->der.P));
   if (e == cudaSuccess) e = cudaMalloc(&c->d_Q, sizeof(c->der.Q));
   if (e == cudaSuccess) e = cudaMalloc(&c->d_nn, LHCB_GHOST_NN_SIZE * sizeof(float));
@@ -262,7 +268,9 @@ int lhcb_prepare(lhcb_ctx* c, const lhcb_raw_t* raw, uint32_t* zone_off, float* 
   p.n_events = raw->n_events;
   p.raw_off = raw->off; p.raw_x = raw->x; p.raw_zone = raw->zone;
   p.zone_off = zone_off; p.hit_x = hit_x; p.perm = perm; p.status = status;
-  lhcb::prepare_kernel<<<raw->n_events, lhcb::kPrepThreads, c->prep_smem, (cudaStream_t)stream>>>(p);
+  if (c->prep_variant == 0) lhcb::prepare_kernel<512, 12, 3><<<raw->n_events, 512, c->prep_smem, (cudaStream_t)stream>>>(p);
+  else if (c->prep_variant == 1) lhcb::prepare_kernel<1024, 12, 1><<<raw->n_events, 1024, c->prep_smem, (cudaStream_t)stream>>>(p);
+  else lhcb::prepare_kernel<1024, 16, 1><<<raw->n_events, 1024, c->prep_smem, (cudaStream_t)stream>>>(p);
   LHCB_CUDA(c, cudaGetLastError());
   c->last_launches = 1;
   return LHCB_OK;

@@ -63,6 +63,24 @@ def test_prepare_edge_cases(ctx):
     assert ctx.last_launch_count() == 0
 
 
+def test_prepare_crowded_cell(ctx):
+    """More than 255 hits in one (zone, x-bin) cell (identical x, x within one bin, x outside the binned range):
+    the kernel ranks such an event by all pairs; the order must still be the stable sort's."""
+    rng = np.random.default_rng(12)
+    sizes = np.array([900, 50, 1300, 0, 600])
+    raw_off = np.concatenate([[0], np.cumsum(sizes)]).astype(np.uint32)
+    n = int(raw_off[-1])
+    x = rng.uniform(-3000, 3000, n).astype(np.float32)
+    zone = rng.integers(0, 24, n).astype(np.uint8)
+    x[100:500] = 77.25; zone[100:500] = 5                      # 400 identical hits: ties by raw index
+    b2 = int(raw_off[2])
+    x[b2:b2 + 300] = rng.uniform(100.0, 101.0, 300).astype(np.float32); zone[b2:b2 + 300] = 9     # 300 hits inside one bin
+    x[b2 + 300:b2 + 330] = 100.5
+    b4 = int(raw_off[4])
+    x[b4:b4 + 280] = rng.uniform(5000, 9000, 280).astype(np.float32); zone[b4:b4 + 280] = 23      # beyond the last bin
+    check(ctx, raw_off, x, zone)
+
+
 def test_prepare_reports_bad_input_and_overflow(geom):
     from lhcb_gen import default_geom
     from paper_2606_14480_b200 import Context
