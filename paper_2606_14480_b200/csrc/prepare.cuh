@@ -15,7 +15,6 @@
 //       < (x', raw index'); more than half of the hits are alone in their cell and are already in place
 //   P5  hit_x and perm leave shared memory with 16-byte stores (the shared arrays are shifted by the event's
 //       misalignment so that shared and global addresses are aligned together)
-// The 6,144 cell counters are 16-bit (an event has at most 65,535 hits), two per 32-bit word.
 // Bins only group; the order is decided by exact float comparisons, so the output is bit-identical to a
 // stable sort whatever the rounding of the bin function.  A cell that collects more than kPrepCellMax hits
 // (never at any sane occupancy: it takes that many hits within 25 mm in one zone, or outside the binned range)
@@ -33,6 +32,10 @@ namespace lhcb {
 #endif
 constexpr int kPrepBins = LHCB_PREP_BINS;         // x bins per zone
 constexpr int kPrepCells = 24 * kPrepBins;
+#ifndef LHCB_PREP_BATCH
+#define LHCB_PREP_BATCH 4
+#endif
+constexpr int kPrepBatch = LHCB_PREP_BATCH;       // raw hits a thread loads before it processes them
 constexpr int kPrepCellMax = 64;                  // members of a cell the one-thread insertion sort handles
 
 struct PrepParams {
@@ -52,20 +55,11 @@ struct PrepParams {
 //  shifted | queue of the cells with more than one member]
 __host__ __device__ inline int prep_queue_cap(int max_hits) { return max_hits / 2 < kPrepCells ? max_hits / 2 : kPrepCells; }
 __host__ __device__ inline size_t prep_smem_bytes(int max_hits) {
-  size_t b = (size_t)kPrepCells * 2 + 512;
+  size_t b = (size_t)kPrepCells * 4 + 512;
   b += (((size_t)max_hits + 8) * 4 + 15) & ~(size_t)15;
   b += (((size_t)max_hits + 8) * 2 + 15) & ~(size_t)15;
   b += ((size_t)prep_queue_cap(max_hits) * 2 + 15) & ~(size_t)15;
   return b;
-}
-
-// 16-bit cell c lives in half (c & 1) of word c >> 1
-__device__ __forceinline__ unsigned int cell_add(unsigned int* cw, int c) {
-  const int sh = (c & 1) << 4;
-  return (atomicAdd(&cw[c >> 1], 1u << sh) >> sh) & 0xFFFFu;
-}
-__device__ __forceinline__ int cell_get(const unsigned int* cw, int c) {
-  return (int)((cw[c >> 1] >> ((c & 1) << 4)) & 0xFFFFu);
 }
 
 __device__ __forceinline__ int prep_cell(const PrepParams& p, float x, int zone) {
@@ -103,15 +97,15 @@ template <int T, int R, int MIN_CTAS>
 __global__ void __launch_bounds__(T, MIN_CTAS)
 prepare_kernel(const __grid_constant__ PrepParams p) {
   extern __shared__ __align__(16) unsigned char smem[];
-  unsigned int* cw = reinterpret_cast<unsigned int*>(smem);                       // kPrepCells / 2 words
-  int* warp_sums = reinterpret_cast<int*>(smem + (size_t)kPrepCells * 2);         // [2][kSeedThreadsMax / 32 + 1] at most
+  unsigned int* cw = reinterpret_cast<unsigned int*>(smem);                       // kPrepCells counters, then cell starts
+  int* warp_sums = reinterpret_cast<int*>(smem + (size_t)kPrepCells * 4);         // [2][kSeedThreadsMax / 32 + 1] at most
   int* flag = warp_sums + 100;
-  float* sx = reinterpret_cast<float*>(smem + (size_t)kPrepCells * 2 + 512);
+  float* sx = reinterpret_cast<float*>(smem + (size_t)kPrepCells * 4 + 512);
   uint16_t* si = reinterpret_cast<uint16_t*>(reinterpret_cast<unsigned char*>(sx) +
                                              ((((size_t)p.max_hits + 8) * 4 + 15) & ~(size_t)15));
   uint16_t* qcell = si + (((size_t)p.max_hits + 8 + 7) & ~(size_t)7);
   constexpr int per = kPrepCells / T;
-  static_assert(per * T == kPrepCells && per % 2 == 0, "whole words of cells per thread");
+  static_assert(per * T == kPrepCells && per % 2 == 0, "whole 8-byte groups of cells per thread");
   static_assert(T <= kSeedThreadsMax * 2, "scan scratch");
   const int tid = threadIdx.x, e = blockIdx.x;
   const uint32_t b = p.raw_off[e];
@@ -119,7 +113,7 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
   uint32_t* zo = p.zone_off + (size_t)e * 24;
   if (e == p.n_events - 1 && tid == 0) p.zone_off[(size_t)p.n_events * 24] = b + (uint32_t)n;
   const bool too_many = n > p.max_hits || n > 65535 || n > T * R;
-  for (int c = tid; c < kPrepCells / 8; c += T) reinterpret_cast<uint4*>(cw)[c] = make_uint4(0u, 0u, 0u, 0u);
+  for (int c = tid; c < kPrepCells / 4; c += T) reinterpret_cast<uint4*>(cw)[c] = make_uint4(0u, 0u, 0u, 0u);
   if (tid == 0) *flag = 0;
   __syncthreads();
   const float* __restrict__ rx = p.raw_x + b;
@@ -128,22 +122,22 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
   uint32_t A[R];
   if (!too_many) {
 #pragma unroll
-    for (int r0 = 0; r0 < R; r0 += 4) {                      // four independent loads in flight per thread
+    for (int r0 = 0; r0 < R; r0 += kPrepBatch) {             // kPrepBatch independent loads in flight per thread
       if (r0 * T >= n) {                                     // (uniform) no hits in these rounds
 #pragma unroll
-        for (int q = 0; q < 4; ++q) if (r0 + q < R) A[r0 + q] = 0u;
+        for (int q = 0; q < kPrepBatch; ++q) if (r0 + q < R) A[r0 + q] = 0u;
         continue;
       }
-      float x[4];
-      int z[4];
+      float x[kPrepBatch];
+      int z[kPrepBatch];
 #pragma unroll
-      for (int q = 0; q < 4; ++q) {
+      for (int q = 0; q < kPrepBatch; ++q) {
         const int i = tid + (r0 + q) * T;
         x[q] = 0.f; z[q] = 0;
         if (r0 + q < R && i < n) { x[q] = __ldg(rx + i); z[q] = __ldg(rz + i); }
       }
 #pragma unroll
-      for (int q = 0; q < 4; ++q) {
+      for (int q = 0; q < kPrepBatch; ++q) {
         const int i = tid + (r0 + q) * T;
         if (r0 + q < R) {
           A[r0 + q] = 0u;
@@ -151,7 +145,7 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
             if (z[q] >= 24 || !(fabsf(x[q]) <= 3.0e38f)) *flag = 1;          // invalid zone, NaN or infinity
             else {
               const int c = prep_cell(p, x[q], z[q]);
-              const unsigned int arr = cell_add(cw, c);
+              const unsigned int arr = atomicAdd(&cw[c], 1u);
               if (arr >= (unsigned)kPrepCellMax) atomicOr(flag, 2);
               A[r0 + q] = (uint32_t)c | (arr << 16);
             }
@@ -182,33 +176,38 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
   {
     unsigned int v[per];
     int sum = 0;
+    unsigned int mmask = 0u;                                 // my cells with more than one member
 #pragma unroll
     for (int k = 0; k < per / 2; ++k) {
-      const unsigned int w = cw[tid * (per / 2) + k];
-      v[2 * k] = w & 0xFFFFu; v[2 * k + 1] = w >> 16;
-      sum += (int)(v[2 * k] + v[2 * k + 1]);
+      const uint2 w = reinterpret_cast<const uint2*>(cw)[tid * (per / 2) + k];
+      v[2 * k] = w.x; v[2 * k + 1] = w.y;
     }
-    int multi = 0;                                           // my cells with more than one member
 #pragma unroll
-    for (int k = 0; k < per; ++k) multi += v[k] >= 2u ? 1 : 0;
+    for (int k = 0; k < per; ++k) {
+      sum += (int)v[k];
+      mmask |= (v[k] >= 2u ? 1u : 0u) << k;
+    }
+    const int multi = __popc(mmask);
     // one scan for both prefix sums: hits in the low half (an event has at most 65,535), queued cells above
     int total;
     int flip = 0;                                            // a single scan: only the first warp_sums buffer is used
     const int ex = block_exscan<T>(sum | (multi << 16), warp_sums, flip, total);
     int run = ex & 0xFFFF, qpos = ex >> 16;
     nqueued = total >> 16;
-#pragma unroll
-    for (int k = 0; k < per; ++k)
-      if (v[k] >= 2u) qcell[qpos++] = (uint16_t)(tid * per + k);
+    while (mmask) {
+      qcell[qpos++] = (uint16_t)(tid * per + __ffs(mmask) - 1);
+      mmask &= mmask - 1u;
+    }
 #pragma unroll
     for (int k = 0; k < per / 2; ++k) {
-      const unsigned int lo = (unsigned int)run; run += (int)v[2 * k];
-      const unsigned int hi = (unsigned int)run; run += (int)v[2 * k + 1];
-      cw[tid * (per / 2) + k] = lo | (hi << 16);
+      uint2 w;
+      w.x = (unsigned int)run; run += (int)v[2 * k];
+      w.y = (unsigned int)run; run += (int)v[2 * k + 1];
+      reinterpret_cast<uint2*>(cw)[tid * (per / 2) + k] = w;
     }
   }
   __syncthreads();
-  if (tid < 24) zo[tid] = b + (uint32_t)cell_get(cw, tid * kPrepBins);
+  if (tid < 24) zo[tid] = b + (uint32_t)cw[tid * kPrepBins];
   if (tid == 0) p.status[e] = 0u;
   // ---- P3: every hit to (start of its cell + arrival rank).
   // Position q of the event lives at index q + sh of the shared arrays, sh = b mod 4: shared and global
@@ -229,7 +228,7 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
       const int i = tid + (r0 + q) * T;
       if (r0 + q < R && i < n) {
         const uint32_t a = A[r0 + q];
-        const int dst = sh + cell_get(cw, (int)(a & 0xFFFFu)) + (int)(a >> 16);
+        const int dst = sh + (int)cw[a & 0xFFFFu] + (int)(a >> 16);
         sx[dst] = x[q];
         si[dst] = (uint16_t)i;
       }
@@ -240,7 +239,7 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
   {
     for (int q = tid; q < nqueued; q += T) {
       const int c = qcell[q];
-      const int start = cell_get(cw, c), cnt = (c + 1 < kPrepCells ? cell_get(cw, c + 1) : n) - start;
+      const int start = (int)cw[c], cnt = (c + 1 < kPrepCells ? (int)cw[c + 1] : n) - start;
       float* cx = sx + sh + start;
       uint16_t* ci = si + sh + start;
       for (int a = 1; a < cnt; ++a) {
