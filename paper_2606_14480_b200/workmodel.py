@@ -13,8 +13,8 @@ import math
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the 16,384-event cfg3 batch, from the
 # `ncu --set full` capture summarised in profiles/ (the bench cannot measure DRAM traffic itself)
-NCU_DRAM_BYTES_PER_LAUNCH = {"seeding_kernel": 273.038080e6 + 247.844864e6, "matching_kernel": 770.602240e6 + 54.298880e6}
-NCU_DRAM_SOURCE = "profiles/r1g_ncu_full.md"
+NCU_DRAM_BYTES_PER_LAUNCH = {"seeding_kernel": 273.200128e6 + 251.460096e6, "matching_kernel": 372.667648e6 + 48.049664e6}
+NCU_DRAM_SOURCE = "profiles/r2a_ncu_full.md"
 
 N_SM = 148
 LANES_PER_SM = 128
