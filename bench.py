@@ -158,16 +158,29 @@ def stage_clocks(args, local_rank):
 
 
 def pcie_bandwidth(torch, dev, nbytes=256 << 20):
-    h = torch.empty(nbytes, dtype=torch.uint8).pin_memory()
-    d = torch.empty(nbytes, dtype=torch.uint8, device=dev)
+    """GB/s host->device, device->host (one direction at a time), and of both directions running together (the
+    pipeline's steady state: inputs of a slice go in while results of an earlier one come out)."""
+    h, h2 = torch.empty(nbytes, dtype=torch.uint8).pin_memory(), torch.empty(nbytes, dtype=torch.uint8).pin_memory()
+    d, d2 = torch.empty(nbytes, dtype=torch.uint8, device=dev), torch.empty(nbytes, dtype=torch.uint8, device=dev)
     e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
-    best = [0.0, 0.0]
+    best = [0.0, 0.0, 0.0, 0.0]
     for _ in range(3):
         e[0].record(); d.copy_(h, non_blocking=True); e[1].record(); h.copy_(d, non_blocking=True); e[2].record()
         torch.cuda.synchronize()
         best[0] = max(best[0], nbytes / e[0].elapsed_time(e[1]) / 1e6)
         best[1] = max(best[1], nbytes / e[1].elapsed_time(e[2]) / 1e6)
-    return best            # GB/s host->device, device->host
+    s_in, s_out = torch.cuda.Stream(), torch.cuda.Stream()
+    a = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    for _ in range(3):
+        torch.cuda.synchronize()
+        with torch.cuda.stream(s_in):
+            a[0].record(); d.copy_(h, non_blocking=True); a[1].record()
+        with torch.cuda.stream(s_out):
+            a[2].record(); h2.copy_(d2, non_blocking=True); a[3].record()
+        torch.cuda.synchronize()
+        best[2] = max(best[2], nbytes / a[0].elapsed_time(a[1]) / 1e6)
+        best[3] = max(best[3], nbytes / a[2].elapsed_time(a[3]) / 1e6)
+    return best
 
 
 def main():
@@ -377,12 +390,17 @@ def main():
         n_s_e2e, n_l_e2e = int(pipe._hs.n), int(pipe._hl.n)
         assert n_l_e2e == n_long and n_s_e2e == n_seeds, "end-to-end result differs from the device-resident run"
         bw = pcie_bandwidth(torch, f"cuda:{local_rank}")
-        pcie_ms = max(h2d / bw[0], d2h / bw[1]) / 1e6
+        pcie_ms = max(h2d / bw[0], d2h / bw[1]) / 1e6               # each direction alone at its best rate
+        # both directions busy: d2h bytes move at the duplex rates, the rest of the input at the one-way rate
+        t_dup = d2h / bw[3] / 1e6
+        pcie_duplex_ms = t_dup + max(0.0, h2d - bw[2] * 1e6 * t_dup) / bw[0] / 1e6
         e2e = {"value": world * n * ke / dt, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                "ms_per_step": 1e3 * dt / ke, "launches_per_step": int(launches),
                "result_bytes": {"seeds": n_s_e2e * 46, "long_tracks": n_l_e2e * 33,
                                 "note": "46 B per seed (state, 12 zone-local hit indices, nx, nuv), 33 B per long track, + offsets and status words"},
-               "pcie_gbs": {"h2d": bw[0], "d2h": bw[1]}, "pcie_bound_ms": pcie_ms, "fraction_of_pcie_bound": pcie_ms / (1e3 * dt / ke),
+               "pcie_gbs": {"h2d": bw[0], "d2h": bw[1], "h2d_while_d2h": bw[2], "d2h_while_h2d": bw[3]},
+               "pcie_bound_ms": pcie_ms, "fraction_of_pcie_bound": pcie_ms / (1e3 * dt / ke),
+               "pcie_duplex_bound_ms": pcie_duplex_ms, "fraction_of_pcie_duplex_bound": pcie_duplex_ms / (1e3 * dt / ke),
                "api": "lhcb_reconstruct_host (pinned host buffers in, dense seeds + long tracks out; 2048-event slices on three "
                       "streams, one CUDA graph per slice)"}
         pipe.close()

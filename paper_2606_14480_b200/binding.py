@@ -122,12 +122,12 @@ def fill_geom(geom: dict) -> LhcbGeom:
 _LIB = None
 
 
-def load_library(build: bool = True, stage_clocks: bool = False) -> C.CDLL:
-    """dlopen the in-tree library (building it first if the sources are newer).  stage_clocks=True selects the
-    diagnostic build with per-stage cycle counters; it must be the first load of the process."""
+def load_library(build: bool = True, stage_clocks: bool = False, checked: bool = False) -> C.CDLL:
+    """dlopen the in-tree library (building it first if the sources are newer).  stage_clocks=True / checked=True
+    select a diagnostic build (per-stage cycle counters / index checks); it must be the first load of the process."""
     global _LIB
     if _LIB is None:
-        path = _build.build(stage_clocks=stage_clocks) if build else _build.LIB
+        path = _build.build(stage_clocks=stage_clocks, checked=checked) if build else _build.LIB
         if not os.path.exists(path):
             raise RuntimeError(f"CUDA library {path} is missing: run python -m paper_2606_14480_b200.build")
         lib = C.CDLL(path)

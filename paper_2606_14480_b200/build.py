@@ -29,14 +29,20 @@ def _deps():
         [os.path.join(HERE, "..", "include", "lhcb.h")]
 
 
-def build(force: bool = False, verbose: bool = False, stage_clocks: bool = False) -> str:
-    """Compile the library (if the sources are newer).  stage_clocks=True builds the diagnostic variant
-    liblhcb_b200_clk.so (-DLHCB_STAGE_CLOCKS: per-stage cycle counters read by lhcb_debug_stage_clocks; used by
-    `bench.py --stage-clocks` only, never by the timed path)."""
-    lib = LIB.replace(".so", "_clk.so") if stage_clocks else LIB
+def build(force: bool = False, verbose: bool = False, stage_clocks: bool = False, checked: bool = False) -> str:
+    """Compile the library (if the sources are newer).  Two diagnostic variants, never used by the timed path:
+    stage_clocks=True builds liblhcb_b200_clk.so (-DLHCB_STAGE_CLOCKS: per-stage cycle counters read by
+    lhcb_debug_stage_clocks; `bench.py --stage-clocks`); checked=True builds liblhcb_b200_chk.so (-DLHCB_CHECKED:
+    index checks on the shared-memory queues, tables and searches, read by lhcb_debug_checks;
+    tests/test_gpu_checked.py)."""
+    lib, extra = LIB, []
+    if stage_clocks:
+        lib, extra = LIB.replace(".so", "_clk.so"), ["-DLHCB_STAGE_CLOCKS"]
+    elif checked:
+        lib, extra = LIB.replace(".so", "_chk.so"), ["-DLHCB_CHECKED"]
     if not force and os.path.exists(lib) and all(os.path.getmtime(lib) >= os.path.getmtime(d) for d in _deps()):
         return lib
-    cmd = [NVCC, *FLAGS, *(["-DLHCB_STAGE_CLOCKS"] if stage_clocks else []), *sources(), "-o", lib]
+    cmd = [NVCC, *FLAGS, *extra, *sources(), "-o", lib]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or r.returncode != 0:
         sys.stderr.write(r.stdout + r.stderr)

@@ -365,6 +365,33 @@ const char* lhcb_error_string(int s) {
   }
 }
 
+#ifdef LHCB_CHECKED
+namespace lhcb {
+__global__ void check_selftest_kernel(int i, int n) { LHCB_CHECK_IDX(i, n); }
+}  // namespace lhcb
+// one deliberate check of index i against bound n on the device: the test of the checker itself
+int lhcb_debug_check_selftest(int i, int n) {
+  lhcb::check_selftest_kernel<<<1, 1>>>(i, n);
+  return cudaDeviceSynchronize() == cudaSuccess ? LHCB_OK : LHCB_ERR_CUDA;
+}
+// diagnostic build only (-DLHCB_CHECKED): out = {failed index checks, source line of the first failure, its index,
+// its bound, checks made (low word), checks made (high word)}; reset != 0 zeroes the counters
+int lhcb_debug_checks(unsigned int* out, int reset) {
+  if (out) {
+    unsigned long long n = 0;
+    if (cudaMemcpyFromSymbol(out, lhcb::g_check, sizeof(lhcb::g_check)) != cudaSuccess) return LHCB_ERR_CUDA;
+    if (cudaMemcpyFromSymbol(&n, lhcb::g_check_count, sizeof(n)) != cudaSuccess) return LHCB_ERR_CUDA;
+    out[4] = (unsigned int)n; out[5] = (unsigned int)(n >> 32);
+  }
+  if (reset) {
+    const unsigned int z[4] = {0, 0, 0, 0};
+    const unsigned long long zn = 0;
+    if (cudaMemcpyToSymbol(lhcb::g_check, z, sizeof(z)) != cudaSuccess) return LHCB_ERR_CUDA;
+    if (cudaMemcpyToSymbol(lhcb::g_check_count, &zn, sizeof(zn)) != cudaSuccess) return LHCB_ERR_CUDA;
+  }
+  return LHCB_OK;
+}
+#endif
 #ifdef LHCB_STAGE_CLOCKS
 // diagnostic builds only: out[0..15] cycles summed over CTAs per stage, out[16..23] maxima over CTAs of the
 // queue fills (lhcb::g_dbg_max); reset != 0 zeroes both

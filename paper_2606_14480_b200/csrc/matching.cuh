@@ -361,6 +361,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
   for (int v = tid; v < nv; v += T) {
     const float t = p.vty[v0 + v];
     const int r = atomicAdd(&vcur[ty_bin(t)], 1);
+    LHCB_CHECK_IDX(r, nv);
     svx[r] = p.vx[v0 + v]; svy[r] = p.vy[v0 + v]; svtx[r] = p.vtx[v0 + v]; svty[r] = t;
     sorig[r] = (uint16_t)v;
   }
@@ -408,6 +409,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     if (tid < nown) {                                        // thread per seed: its own range of VELO states
       const float4 o = sown[tid];
       const float xS = o.x, ys = o.y, txS = o.z, tyS = o.w, axS = fabsf(xS);
+      LHCB_CHECK_IDX(fst + cnt, nv + 1);
       for (int v = fst; v < fst + cnt; ++v) {
         const float xV = svx[v], yV = svy[v], txV = svtx[v], tyV = svty[v];
         const float dtx = txS - txV, dty = tyS - tyV, adtx = fabsf(dtx);
@@ -506,6 +508,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
         const float lo = x0e - w, hi = x0e + w;
         const int b = uo[i0], ee = uo[i0 + 1];
         for (int j = lower_bound(ux, b, ee, lo); j < ee && ux[j] <= hi; ++j) {
+          if (ut_in_smem) LHCB_CHECK_IDX(j, p.max_ut + 8);
           if (!cover(j, yi)) continue;
           found = true;
           const int slot = smem_inc(&hdr[3]);
@@ -534,6 +537,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
         ut_tight_walk(p, svx[v], svy[v], svtx[v], svty[v], fabsf(m.q0) * 1000.f, i0, jrel - rel0, ux, cover, uo, hy);
         key = ((unsigned long long)(4 - hy.n) << 50) | ((unsigned long long)__float_as_uint(hy.ssq) << 18) |
               (hq & 0x3FFFFu);
+        LHCB_CHECK_IDX(k, nm);
         atomicMin(&mc[k].key, key);
       }
       __syncthreads();
@@ -591,6 +595,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
   } else {
   for (int k = tid; k < nm; k += T) {
     const MatchCand& m = mc[k];
+    LHCB_CHECK_IDX(m.seed, ns); LHCB_CHECK_IDX(sorig[m.velo], nv);
     if ((m.key >> 50) <= key_ok)
       atomicMin(&seed_best[m.seed], ((unsigned long long)__float_as_uint(m.chi2) << 32) | sorig[m.velo]);
   }

@@ -145,6 +145,7 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
             if (z[q] >= 24 || !(fabsf(x[q]) <= 3.0e38f)) *flag = 1;          // invalid zone, NaN or infinity
             else {
               const int c = prep_cell(p, x[q], z[q]);
+              LHCB_CHECK_IDX(c, kPrepCells);
               const unsigned int arr = atomicAdd(&cw[c], 1u);
               if (arr >= (unsigned)kPrepCellMax) atomicOr(flag, 2);
               A[r0 + q] = (uint32_t)c | (arr << 16);
@@ -195,6 +196,7 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
     int run = ex & 0xFFFF, qpos = ex >> 16;
     nqueued = total >> 16;
     while (mmask) {
+      LHCB_CHECK_IDX(qpos, prep_queue_cap(p.max_hits));
       qcell[qpos++] = (uint16_t)(tid * per + __ffs(mmask) - 1);
       mmask &= mmask - 1u;
     }
@@ -229,6 +231,7 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
       if (r0 + q < R && i < n) {
         const uint32_t a = A[r0 + q];
         const int dst = sh + (int)cw[a & 0xFFFFu] + (int)(a >> 16);
+        LHCB_CHECK_IDX(dst - sh, n);
         sx[dst] = x[q];
         si[dst] = (uint16_t)i;
       }
@@ -240,6 +243,7 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
     for (int q = tid; q < nqueued; q += T) {
       const int c = qcell[q];
       const int start = (int)cw[c], cnt = (c + 1 < kPrepCells ? (int)cw[c + 1] : n) - start;
+      LHCB_CHECK_IDX(start + cnt, n + 1); LHCB_CHECK_IDX(cnt - 2, kPrepCellMax);
       float* cx = sx + sh + start;
       uint16_t* ci = si + sh + start;
       for (int a = 1; a < cnt; ++a) {

@@ -68,6 +68,26 @@ __device__ unsigned int g_dbg_max[8];     // maxima over CTAs: triplets, candida
 #define LHCB_DBG_MAX(i, v)
 #endif
 
+// Optional index checks (diagnostic build only: -DLHCB_CHECKED, tests/test_gpu_checked.py; compute-sanitizer is
+// closed on the GPU pool).  LHCB_CHECK_IDX(i, n) records an index outside
+// [0, n) in g_check = {failures, line of the first one, its index, its bound} and counts the checks made in
+// g_check_count; lhcb_debug_checks() reads them.  The release build compiles the checks away.
+#ifdef LHCB_CHECKED
+__device__ unsigned int g_check[4];
+__device__ unsigned long long g_check_count;
+__device__ __noinline__ void check_fail(int line, long long i, long long n) {
+  if (atomicAdd(&g_check[0], 1u) == 0u) { g_check[1] = (unsigned)line; g_check[2] = (unsigned)i; g_check[3] = (unsigned)n; }
+}
+#define LHCB_CHECK_IDX(i, n)                                                                          \
+  do {                                                                                                \
+    atomicAdd(&lhcb::g_check_count, 1ull);                                                            \
+    if ((unsigned long long)(long long)(i) >= (unsigned long long)(long long)(n))                     \
+      lhcb::check_fail(__LINE__, (long long)(i), (long long)(n));                                     \
+  } while (0)
+#else
+#define LHCB_CHECK_IDX(i, n)
+#endif
+
 struct SeedParams {
   float zb[12], gz[12], tan_a[12], inv_tan[12], inv_z[12], zt[12];
   float ywin_a[2][12], ywin_b[2][12];
@@ -167,7 +187,9 @@ __host__ __device__ inline size_t seed_smem_bytes(int max_hits, int max_cand, in
 __device__ __forceinline__ int zone_bin(const Zone& z, float v) {
   float t = (v - z.x0) * z.invw;
   t = fminf(fmaxf(t, 0.f), (float)(kLutBins - 1));
-  return __float_as_int(t + 8388608.f) & 0x3FF;
+  const int k = __float_as_int(t + 8388608.f) & 0x3FF;
+  LHCB_CHECK_IDX(k, kLutBins);
+  return k;
 }
 static_assert(kLutBins <= 1024, "zone_bin keeps ten bits");
 
@@ -184,6 +206,7 @@ __device__ __forceinline__ int lower_bound_v(const float* __restrict__ x, const 
   int i = lut[zone_bin(z, v)];
   float xi = x[i];
   while (xi < v) { ++i; xi = x[i]; }
+  LHCB_CHECK_IDX(i - z.b, z.e - z.b + 1);
   xv = xi;
   return i;
 }
@@ -199,6 +222,7 @@ __device__ __forceinline__ int upper_bound(const float* __restrict__ x, const ui
   int i = lut[zone_bin(z, v)];
   float xi = x[i];
   while (xi <= v) { ++i; xi = x[i]; }
+  LHCB_CHECK_IDX(i - z.b, z.e - z.b + 1);
   return i;
 }
 // plain binary searches (global-memory arrays without a bin table)
@@ -235,6 +259,7 @@ __device__ __forceinline__ int closest_hit(const float* __restrict__ x, const ui
   int i = lut[zone_bin(z, xp)];
   float xr = x[i];
   while (xr < xp) { ++i; xr = x[i]; }
+  LHCB_CHECK_IDX(i - z.b, z.e - z.b + 1);
   const float xl = x[i - 1], xll = x[i - 2];                 // (i - 2 is at worst a sentinel or padding)
   const float dl = fabsf(xl - xp), dr = fabsf(xr - xp);
   const bool left = dl <= dr;
@@ -246,6 +271,7 @@ __device__ __forceinline__ int closest_hit(const float* __restrict__ x, const ui
     --i;
     while (fabsf(x[i - 1] - xp) == d) --i;
   }
+  LHCB_CHECK_IDX(i - z.b, z.e - z.b + 1);
   return ok ? i : -1;
 }
 
@@ -450,6 +476,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     for (int z = 0; z < 12; ++z) {
       const int n = (int)(zoff[z + 1] - zoff[z]);
       const float* src = stg + (zoff[z] - a0);
+      LHCB_CHECK_IDX(off_hits + (pos + n + 1) * 4, off_w + 1);
       for (int i = tid; i < n; i += T) hx[pos + i] = src[i];
       if (tid == 32 + z) {                                 // sentinels, bin function, index map of zone z
         hx[pos - 2] = -inf; hx[pos - 1] = -inf; hx[pos + n] = inf;
@@ -480,6 +507,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     for (int i = zz.b + tid; i < zz.e; i += T) {
       const int k1 = zone_bin(zz, hx[i]);
       const int k0 = zone_bin(zz, hx[i - 1]);              // -inf in front of the first hit: bin 0
+      LHCB_CHECK_IDX(k1, kLutBins);
       if (i == zz.b || k1 != k0) L[k1] = (uint16_t)i;
     }
   }
@@ -566,11 +594,13 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
           if (lo2 < lo2p) { j = lut2[zone_bin(z2n, lo2)]; xj = hx[j]; }
           lo2p = lo2;
           while (xj < lo2) { ++j; xj = hx[j]; }
+          LHCB_CHECK_IDX(j - b2, e2 - b2 + 1);
           int jj = j;
           float xjj = xj;
           while (xjj <= hi2) {
             if (jj >= e2) break;                                                 // hi2 = +inf: stop at the sentinel
             const int slot = smem_inc(&H.n_trip);
+            LHCB_CHECK_IDX(jj - b2, e2 - b2);
             if (slot < trip_cap)
               trip[slot] = (uint32_t)(i1 - b1) | ((uint32_t)(jj - b2) << kZoneIndexBits) |
                            ((uint32_t)(i3f + k - b3) << (2 * kZoneIndexBits)) | ((uint32_t)it << (3 * kZoneIndexBits));
@@ -598,6 +628,8 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
       constexpr uint32_t zmask = (1u << kZoneIndexBits) - 1;
       const int i1 = H.zi[l1].b + (int)(tr & zmask), i2 = H.zi[p.l2[it]].b + (int)((tr >> kZoneIndexBits) & zmask),
                 i3 = H.zi[p.l3[it]].b + (int)((tr >> (2 * kZoneIndexBits)) & zmask);
+      LHCB_CHECK_IDX(i1 - H.zi[l1].b, H.zi[l1].e - H.zi[l1].b); LHCB_CHECK_IDX(i2 - H.zi[p.l2[it]].b, H.zi[p.l2[it]].e - H.zi[p.l2[it]].b);
+      LHCB_CHECK_IDX(i3 - H.zi[p.l3[it]].b, H.zi[p.l3[it]].e - H.zi[p.l3[it]].b);
       const float x1 = hx[i1], x2 = hx[i2], x3 = hx[i3];
       const float t13 = (x3 - x1) * p.inv_dz13[it];
       const float x2c = x1 + p.dz12[it] * t13;
@@ -696,7 +728,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     const unsigned long long key = clone_key(cd.chi2, cd.cx, cd.nx, cd.it);
 #pragma unroll
     for (int s = 0; s < 6; ++s)
-      if (cd.hit[s] != 0xFFFF) atomicMin(&tbl[H.xoff[s] + cd.hit[s]], key);
+      if (cd.hit[s] != 0xFFFF) { LHCB_CHECK_IDX(H.xoff[s] + cd.hit[s], n_xhits); atomicMin(&tbl[H.xoff[s] + cd.hit[s]], key); }
   }
   __syncthreads();
   for (int c = tid; c < nc; c += T) {
@@ -709,7 +741,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
       if (cd.hit[s] != 0xFFFF && tbl[H.xoff[s] + cd.hit[s]] == key) ++own;
     const bool keep = own >= 3 || (own >= 2 && cd.nx == 6);
     cd.keep = keep;
-    if (keep) kept[smem_inc(&H.n_kept)] = (uint16_t)c;
+    if (keep) { const int kk = smem_inc(&H.n_kept); LHCB_CHECK_IDX(kk, p.max_cand); kept[kk] = (uint16_t)c; }
   }
   __syncthreads();
   int nk = H.n_kept;
@@ -726,7 +758,8 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
     if (nk > nk_max) { nk = nk_max > 0 ? nk_max : 0; if (tid == 0) H.status |= LHCB_ST_UV_QUEUE_OVERFLOW; }
   }
   Cand* surv = reinterpret_cast<Cand*>(smem + off_w);
-  for (int k = tid; k < nk; k += T) surv[k] = cand_end[-1 - (int)kept[k]];
+  LHCB_CHECK_IDX(nk * 72, wbytes + 1);
+  for (int k = tid; k < nk; k += T) { LHCB_CHECK_IDX((int)kept[k], nc); surv[k] = cand_end[-1 - (int)kept[k]]; }
   unsigned long long* best = reinterpret_cast<unsigned long long*>(surv + nk);
   float* xps = reinterpret_cast<float*>(best + ((nk + 1) & ~1));          // [nk][8], 16-byte aligned: x_pred per stereo layer
   const int rest = wbytes - nk * 32 - ((nk + 1) & ~1) * 8 - nk * 32;      // >= 4096 - 8
@@ -874,7 +907,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
       {
         int i = q0 - ex; if (i < 0) i = 0;
         int iend = q0 + C - ex; if (iend > cnt) iend = cnt;
-        for (; i < iend; ++i) uitems[ex + i - q0] = ((uint32_t)tid << 16) | (uint32_t)(fst + i);
+        for (; i < iend; ++i) { LHCB_CHECK_IDX(ex + i - q0, C); uitems[ex + i - q0] = ((uint32_t)tid << 16) | (uint32_t)(fst + i); }
       }
       __syncthreads();
       const int nitems = total - q0 < C ? total - q0 : C;
@@ -894,7 +927,9 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
         UvLive lv;
         lv.item = ((uint32_t)w << 16) | (uint32_t)ih; lv.ty = ty;
         lv.h[0] = (uint16_t)h0; lv.h[1] = (uint16_t)h1; lv.h[2] = (uint16_t)h2; lv.n = (uint16_t)n;
-        live[smem_inc(&H.n_live)] = lv;
+        const int ls = smem_inc(&H.n_live);
+        LHCB_CHECK_IDX(ls, C);
+        live[ls] = lv;
       }
       __syncthreads();
       const int nl = H.n_live;
@@ -957,6 +992,7 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
   };
   for (int i = tid; i < nsucc; i += T) {
     fit_success(i);
+    LHCB_CHECK_IDX(u.k, nk);
     if (key != kNoKey) atomicMin(&best[u.k], key);
   }
   __syncthreads();
