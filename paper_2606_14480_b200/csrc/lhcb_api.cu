@@ -173,7 +173,7 @@ int lhcb_geom_init(const lhcb_geom_t* g, int device, lhcb_ctx** out) {
   // the preparation keeps one register per raw hit: T threads x R hits per thread >= the event capacity
   c->prep_variant = 2 * G.max_hits_per_half <= 512 * 12 ? 0 : 2 * G.max_hits_per_half <= 1024 * 12 ? 1 : 2;
   if (e == cudaSuccess)
-    e = cudaFuncSetAttribute(c->prep_variant == 0   ? (const void*)lhcb::prepare_kernel<512, 12, 3>
+    e = cudaFuncSetAttribute(c->prep_variant == 0   ? (const void*)lhcb::prepare_kernel<512, 12, 4>
                              : c->prep_variant == 1 ? (const void*)lhcb::prepare_kernel<1024, 12, 1>
                                                     : (const void*)lhcb::prepare_kernel<1024, 16, 1>,
                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->prep_smem);
@@ -268,7 +268,7 @@ int lhcb_prepare(lhcb_ctx* c, const lhcb_raw_t* raw, uint32_t* zone_off, float* 
   p.n_events = raw->n_events;
   p.raw_off = raw->off; p.raw_x = raw->x; p.raw_zone = raw->zone;
   p.zone_off = zone_off; p.hit_x = hit_x; p.perm = perm; p.status = status;
-  if (c->prep_variant == 0) lhcb::prepare_kernel<512, 12, 3><<<raw->n_events, 512, c->prep_smem, (cudaStream_t)stream>>>(p);
+  if (c->prep_variant == 0) lhcb::prepare_kernel<512, 12, 4><<<raw->n_events, 512, c->prep_smem, (cudaStream_t)stream>>>(p);
   else if (c->prep_variant == 1) lhcb::prepare_kernel<1024, 12, 1><<<raw->n_events, 1024, c->prep_smem, (cudaStream_t)stream>>>(p);
   else lhcb::prepare_kernel<1024, 16, 1><<<raw->n_events, 1024, c->prep_smem, (cudaStream_t)stream>>>(p);
   LHCB_CUDA(c, cudaGetLastError());

@@ -15,6 +15,7 @@
 //       < (x', raw index'); more than half of the hits are alone in their cell and are already in place
 //   P5  hit_x and perm leave shared memory with 16-byte stores (the shared arrays are shifted by the event's
 //       misalignment so that shared and global addresses are aligned together)
+// The 6,144 cell counters are 16-bit (an event has at most 65,535 hits), two per 32-bit word.
 // Bins only group; the order is decided by exact float comparisons, so the output is bit-identical to a
 // stable sort whatever the rounding of the bin function.  A cell that collects more than kPrepCellMax hits
 // (never at any sane occupancy: it takes that many hits within 25 mm in one zone, or outside the binned range)
@@ -51,15 +52,26 @@ struct PrepParams {
   uint32_t* status;
 };
 
-// [packed cells | scan scratch, flag, queue length | x by position, shifted by up to 3 | raw index by position,
+typedef uint16_t prep_cell_t;                     // 16-bit cells, two per word (an event has at most 65,535 hits): the
+                                                  // counters take 12 KB and four 512-thread CTAs share an SM
+
+// [cells | scan scratch, flag, queue length | x by position, shifted by up to 3 | raw index by position,
 //  shifted | queue of the cells with more than one member]
 __host__ __device__ inline int prep_queue_cap(int max_hits) { return max_hits / 2 < kPrepCells ? max_hits / 2 : kPrepCells; }
 __host__ __device__ inline size_t prep_smem_bytes(int max_hits) {
-  size_t b = (size_t)kPrepCells * 4 + 512;
+  size_t b = (size_t)kPrepCells * sizeof(prep_cell_t) + 512;
   b += (((size_t)max_hits + 8) * 4 + 15) & ~(size_t)15;
   b += (((size_t)max_hits + 8) * 2 + 15) & ~(size_t)15;
   b += ((size_t)prep_queue_cap(max_hits) * 2 + 15) & ~(size_t)15;
   return b;
+}
+
+__device__ __forceinline__ unsigned int cell_inc(unsigned int* cw, int c) {      // returns the count before
+  const int sh = (c & 1) << 4;
+  return (atomicAdd(&cw[c >> 1], 1u << sh) >> sh) & 0xFFFFu;
+}
+__device__ __forceinline__ int cell_start(const unsigned int* cw, int c) {
+  return (int)((cw[c >> 1] >> ((c & 1) << 4)) & 0xFFFFu);
 }
 
 __device__ __forceinline__ int prep_cell(const PrepParams& p, float x, int zone) {
@@ -98,14 +110,14 @@ __global__ void __launch_bounds__(T, MIN_CTAS)
 prepare_kernel(const __grid_constant__ PrepParams p) {
   extern __shared__ __align__(16) unsigned char smem[];
   unsigned int* cw = reinterpret_cast<unsigned int*>(smem);                       // kPrepCells counters, then cell starts
-  int* warp_sums = reinterpret_cast<int*>(smem + (size_t)kPrepCells * 4);         // [2][kSeedThreadsMax / 32 + 1] at most
+  int* warp_sums = reinterpret_cast<int*>(smem + (size_t)kPrepCells * sizeof(prep_cell_t));         // [2][kSeedThreadsMax / 32 + 1] at most
   int* flag = warp_sums + 100;
-  float* sx = reinterpret_cast<float*>(smem + (size_t)kPrepCells * 4 + 512);
+  float* sx = reinterpret_cast<float*>(smem + (size_t)kPrepCells * sizeof(prep_cell_t) + 512);
   uint16_t* si = reinterpret_cast<uint16_t*>(reinterpret_cast<unsigned char*>(sx) +
                                              ((((size_t)p.max_hits + 8) * 4 + 15) & ~(size_t)15));
   uint16_t* qcell = si + (((size_t)p.max_hits + 8 + 7) & ~(size_t)7);
   constexpr int per = kPrepCells / T;
-  static_assert(per * T == kPrepCells && per % 2 == 0, "whole 8-byte groups of cells per thread");
+  static_assert(per * T == kPrepCells && per % 2 == 0, "whole words of cells per thread");
   static_assert(T <= kSeedThreadsMax * 2, "scan scratch");
   const int tid = threadIdx.x, e = blockIdx.x;
   const uint32_t b = p.raw_off[e];
@@ -113,7 +125,7 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
   uint32_t* zo = p.zone_off + (size_t)e * 24;
   if (e == p.n_events - 1 && tid == 0) p.zone_off[(size_t)p.n_events * 24] = b + (uint32_t)n;
   const bool too_many = n > p.max_hits || n > 65535 || n > T * R;
-  for (int c = tid; c < kPrepCells / 4; c += T) reinterpret_cast<uint4*>(cw)[c] = make_uint4(0u, 0u, 0u, 0u);
+  for (int c = tid; c < kPrepCells * (int)sizeof(prep_cell_t) / 16; c += T) reinterpret_cast<uint4*>(cw)[c] = make_uint4(0u, 0u, 0u, 0u);
   if (tid == 0) *flag = 0;
   __syncthreads();
   const float* __restrict__ rx = p.raw_x + b;
@@ -146,7 +158,7 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
             else {
               const int c = prep_cell(p, x[q], z[q]);
               LHCB_CHECK_IDX(c, kPrepCells);
-              const unsigned int arr = atomicAdd(&cw[c], 1u);
+              const unsigned int arr = cell_inc(cw, c);
               if (arr >= (unsigned)kPrepCellMax) atomicOr(flag, 2);
               A[r0 + q] = (uint32_t)c | (arr << 16);
             }
@@ -180,8 +192,8 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
     unsigned int mmask = 0u;                                 // my cells with more than one member
 #pragma unroll
     for (int k = 0; k < per / 2; ++k) {
-      const uint2 w = reinterpret_cast<const uint2*>(cw)[tid * (per / 2) + k];
-      v[2 * k] = w.x; v[2 * k + 1] = w.y;
+      const unsigned int w = cw[tid * (per / 2) + k];
+      v[2 * k] = w & 0xFFFFu; v[2 * k + 1] = w >> 16;
     }
 #pragma unroll
     for (int k = 0; k < per; ++k) {
@@ -202,14 +214,13 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
     }
 #pragma unroll
     for (int k = 0; k < per / 2; ++k) {
-      uint2 w;
-      w.x = (unsigned int)run; run += (int)v[2 * k];
-      w.y = (unsigned int)run; run += (int)v[2 * k + 1];
-      reinterpret_cast<uint2*>(cw)[tid * (per / 2) + k] = w;
+      const unsigned int lo = (unsigned int)run; run += (int)v[2 * k];
+      const unsigned int hi = (unsigned int)run; run += (int)v[2 * k + 1];
+      cw[tid * (per / 2) + k] = lo | (hi << 16);
     }
   }
   __syncthreads();
-  if (tid < 24) zo[tid] = b + (uint32_t)cw[tid * kPrepBins];
+  if (tid < 24) zo[tid] = b + (uint32_t)cell_start(cw, tid * kPrepBins);
   if (tid == 0) p.status[e] = 0u;
   // ---- P3: every hit to (start of its cell + arrival rank).
   // Position q of the event lives at index q + sh of the shared arrays, sh = b mod 4: shared and global
@@ -230,7 +241,7 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
       const int i = tid + (r0 + q) * T;
       if (r0 + q < R && i < n) {
         const uint32_t a = A[r0 + q];
-        const int dst = sh + (int)cw[a & 0xFFFFu] + (int)(a >> 16);
+        const int dst = sh + cell_start(cw, (int)(a & 0xFFFFu)) + (int)(a >> 16);
         LHCB_CHECK_IDX(dst - sh, n);
         sx[dst] = x[q];
         si[dst] = (uint16_t)i;
@@ -242,7 +253,7 @@ prepare_kernel(const __grid_constant__ PrepParams p) {
   {
     for (int q = tid; q < nqueued; q += T) {
       const int c = qcell[q];
-      const int start = (int)cw[c], cnt = (c + 1 < kPrepCells ? (int)cw[c + 1] : n) - start;
+      const int start = cell_start(cw, c), cnt = (c + 1 < kPrepCells ? cell_start(cw, c + 1) : n) - start;
       LHCB_CHECK_IDX(start + cnt, n + 1); LHCB_CHECK_IDX(cnt - 2, kPrepCellMax);
       float* cx = sx + sh + start;
       uint16_t* ci = si + sh + start;
