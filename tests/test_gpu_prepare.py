@@ -81,6 +81,32 @@ def test_prepare_crowded_cell(ctx):
     check(ctx, raw_off, x, zone)
 
 
+def test_prepare_other_instantiations_and_unaligned_outputs(ctx):
+    """The largest event capacity (1,024 threads x 16 hits per thread) and output arrays that are not 16-byte
+    aligned (scalar stores instead of the vector ones): same result as the oracle."""
+    from lhcb_gen import default_geom
+    from paper_2606_14480_b200 import Context
+    ev = generate(config(4, 24))
+    raw = shuffle_raw(ev, seed=21)
+    c = Context(default_geom(max_hits_per_half=8000))
+    check(c, raw["raw_off"], raw["raw_x"], raw["raw_zone"])
+    c.close()
+    t = ctx.torch
+    up = lambda a, dt: t.from_numpy(np.ascontiguousarray(a, dt).view(np.int32 if dt == np.uint32 else dt)).to(ctx.dev)
+    n_events, n = len(raw["raw_off"]) - 1, len(raw["raw_x"])
+    hx = t.empty(n + 1, dtype=t.float32, device=ctx.dev)[1:]           # 4 bytes off a 16-byte boundary
+    pm = t.empty(n + 3, dtype=t.int32, device=ctx.dev)[3:]
+    out = dict(zone_off=t.empty(n_events * 24 + 1, dtype=t.int32, device=ctx.dev), hit_x=hx, perm=pm,
+               status=t.empty(n_events, dtype=t.int32, device=ctx.dev))
+    ctx.lhcb_prepare(up(raw["raw_off"], np.uint32), up(raw["raw_x"], np.float32), up(raw["raw_zone"], np.uint8), out)
+    t.cuda.synchronize()
+    ozo, ohx, opm = oracle_prepare(raw["raw_off"], raw["raw_x"], raw["raw_zone"])
+    assert not out["status"].cpu().numpy().any()
+    assert np.array_equal(out["zone_off"].cpu().numpy().view(np.uint32), ozo)
+    assert np.array_equal(hx.cpu().numpy().view(np.uint32), ohx.view(np.uint32))
+    assert np.array_equal(pm.cpu().numpy().view(np.uint32), opm)
+
+
 def test_prepare_reports_bad_input_and_overflow(geom):
     from lhcb_gen import default_geom
     from paper_2606_14480_b200 import Context
