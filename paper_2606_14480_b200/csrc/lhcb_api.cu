@@ -631,23 +631,28 @@ int lhcb_reconstruct_host(lhcb_pipeline* p, const lhcb_events_t* ev, const lhcb_
     p->e0[ns++] = e;
     p->e0[ns] = n;
   }
-  // ---- all input copies, slice by slice, on the copy-in stream
+  // ---- all input copies on the copy-in stream.  The small arrays (offsets, polarities, VELO states: a few per
+  // cent of the bytes) go first, each as ONE copy for the whole batch: a copy costs a few microseconds whatever
+  // its size, and a dozen of them per slice add up to a millisecond per batch.  The hits then follow slice by
+  // slice.
+  {
+    const size_t n_velo_all = velo->off[n];
+    H2D(p->zone_off, ev->zone_off, ((size_t)n * 24 + 1) * 4);
+    if (has_pol) H2D(p->pol, ev->polarity, (size_t)n);
+    H2D(p->velo_off, velo->off, ((size_t)n + 1) * 4);
+    H2D(p->vx, velo->x, n_velo_all * 4);
+    H2D(p->vy, velo->y, n_velo_all * 4);
+    H2D(p->vtx, velo->tx, n_velo_all * 4);
+    H2D(p->vty, velo->ty, n_velo_all * 4);
+    if (has_ut) H2D(p->ut_off, ut->off, ((size_t)n * 4 + 1) * 4);
+  }
   for (int k = 0; k < ns && ce == cudaSuccess; ++k) {
     const int e0 = p->e0[k], ne = p->e0[k + 1] - e0;
     const size_t z0 = (size_t)e0 * 24, z1 = (size_t)(e0 + ne) * 24;
     const size_t h0 = ev->zone_off[z0], h1 = ev->zone_off[z1];
-    const size_t v0 = velo->off[e0], v1 = velo->off[e0 + ne];
-    H2D(p->zone_off + z0, ev->zone_off + z0, (z1 - z0 + 1) * 4);
     H2D(p->hit_x + h0, ev->hit_x + h0, (h1 - h0) * 4);
-    if (has_pol) H2D(p->pol + e0, ev->polarity + e0, (size_t)ne);
-    H2D(p->velo_off + e0, velo->off + e0, ((size_t)ne + 1) * 4);
-    H2D(p->vx + v0, velo->x + v0, (v1 - v0) * 4);
-    H2D(p->vy + v0, velo->y + v0, (v1 - v0) * 4);
-    H2D(p->vtx + v0, velo->tx + v0, (v1 - v0) * 4);
-    H2D(p->vty + v0, velo->ty + v0, (v1 - v0) * 4);
     if (has_ut) {
       const size_t u0 = ut->off[(size_t)e0 * 4], u1 = ut->off[(size_t)(e0 + ne) * 4];
-      H2D(p->ut_off + (size_t)e0 * 4, ut->off + (size_t)e0 * 4, ((size_t)ne * 4 + 1) * 4);
       if (strips) H2D(p->ustrip + u0, ut->strip + u0, (u1 - u0) * 2);
       else H2D(p->ux + u0, ut->x0 + u0, (u1 - u0) * 4);
       H2D(p->urow + u0, ut->row + u0, u1 - u0);
@@ -688,21 +693,24 @@ int lhcb_reconstruct_host(lhcb_pipeline* p, const lhcb_events_t* ev, const lhcb_
     if (se > p->cap_s || le > p->cap_l || se > so->cap || le > lo->cap) { rc = LHCB_ERR_CAPACITY; break; }
     seeds_end = se; long_end = le;
     const size_t CS = p->cap_s, CL = p->cap_l, hs = so->cap, hl = lo->cap, nsd = se - sb, nl = le - lb;
-    D2H(so->off + (size_t)e0 * 2, p->d_s_off + (size_t)e0 * 2, ((size_t)ne * 2 + 1) * 4);
-    D2H(so->status + (size_t)e0 * 2, p->d_s_status + (size_t)e0 * 2, (size_t)ne * 8);
     D2H2D(so->state + sb, hs * 4, p->d_state + sb, CS * 4, nsd * 4, 5);
     D2H2D(so->hits + sb, hs * 2, p->d_hits + sb, CS * 2, nsd * 2, 12);
     if (want_par) D2H2D(so->par + sb, hs * 4, p->d_par + sb, CS * 4, nsd * 4, 7);
     D2H(so->nx + sb, p->d_nx + sb, nsd);
     D2H(so->nuv + sb, p->d_nuv + sb, nsd);
-    D2H(lo->off + e0, p->d_l_off + e0, ((size_t)ne + 1) * 4);
-    D2H(lo->status + e0, p->d_l_status + e0, (size_t)ne * 4);
     D2H(lo->seed_idx + lb, p->d_seed + lb, nl * 4);
     D2H(lo->velo_idx + lb, p->d_velo + lb, nl * 4);
     D2H2D(lo->ut_idx + lb, hl * 4, p->d_ut + lb, CL * 4, nl * 4, 4);
     D2H(lo->n_ut + lb, p->d_nut + lb, nl);
     D2H(lo->qop + lb, p->d_qop + lb, nl * 4);
     D2H(lo->chi2 + lb, p->d_chi2 + lb, nl * 4);
+  }
+  // offsets and status words of the whole batch: one copy each (the last slice's kernels have finished)
+  if (ce == cudaSuccess && rc == LHCB_OK) {
+    D2H(so->off, p->d_s_off, ((size_t)n * 2 + 1) * 4);
+    D2H(so->status, p->d_s_status, (size_t)n * 8);
+    D2H(lo->off, p->d_l_off, ((size_t)n + 1) * 4);
+    D2H(lo->status, p->d_l_status, (size_t)n * 4);
   }
   // every stream is drained before returning, whatever happened: no copy is left in flight on the caller's buffers
   const cudaError_t e1 = cudaStreamSynchronize(p->st_in), e2 = cudaStreamSynchronize(p->st_k), e3 = cudaStreamSynchronize(p->st_out);
