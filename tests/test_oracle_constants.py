@@ -102,6 +102,33 @@ def test_zmatch_and_tolerances(mode, rel, geom):
         assert toly == pytest.approx(GOLD[name][0], rel=max(rel * 50, 1e-5))
 
 
+def test_chi2_match_is_eq22_with_all_four_terms(oracle64):
+    """Eq. 22-23 as printed, every term non-zero at once (t_y^VELO included in rho^VELO): the four terms are
+    computed here from the pair's own dx, dy, dtx, dty and the printed constants."""
+    for velo4, dtx, dty, dx_want, dy_want in (([3.0, -2.0, 0.045, -0.121], 0.036, 0.009, 7.0, -5.0),
+                                              ([-1.5, 4.0, -0.070, 0.149], -0.028, -0.012, -11.0, 8.0)):
+        xv, yv, txv, tyv = velo4
+        txs, tys = txv + dtx, tyv + dty
+        ys = (yv + (10000.0 - 770.0) * tyv) - (10000.0 - 7826.0) * tys + dy_want
+        xs = 0.0
+        for _ in range(6):                                   # z_match depends (weakly) on |x_S|: fixed point
+            zm = oracle64.match_pair([xs, ys, txs, tys], velo4)["zm"]
+            xs = (xv + (zm - 770.0) * txv) - (zm - 7826.0) * txs + dx_want
+        seed4 = [xs, ys, txs, tys]
+        r = oracle64.match_pair(seed4, velo4)
+        txv, tyv = velo4[2], velo4[3]
+        tolx = 0.8 * (10.12 ** 2 + 101.0 ** 2 * r["dtx"] ** 2)
+        toly = 0.2 * (1.59 ** 2 + 212.1 ** 2 * (txv * txv + tyv * tyv))
+        want = r["dx"] ** 2 / tolx + r["dy"] ** 2 / toly + r["dtx"] ** 2 / 0.5 + r["dty"] ** 2 * 937.5
+        assert r["chi2"] == pytest.approx(want, rel=1e-12)
+        # the slope terms and the t_y^VELO part of tol_y are visible at this size
+        assert r["presel"] == 1.0 and abs(r["dx"] - dx_want) < 0.1 and abs(r["dy"] - dy_want) < 1e-6
+        assert r["dty"] ** 2 * 937.5 > 0.05 * want and 212.1 ** 2 * tyv * tyv > 0.1 * 1.59 ** 2
+        assert r["dty"] == pytest.approx(seed4[3] - velo4[3], rel=1e-12) and r["dtx"] == pytest.approx(seed4[2] - velo4[2], rel=1e-12)
+        # dy is taken at z = 10 m: both lines extrapolated there (L231)
+        assert r["dy"] == pytest.approx((seed4[1] + (10000.0 - 7826.0) * seed4[3]) - (velo4[1] + (10000.0 - 770.0) * velo4[3]), rel=1e-12)
+
+
 def test_gamma_and_ut_windows(oracle64):
     check("gamma_qop_1over3000", oracle64.gamma(1.0 / 3000.0))
     check("deflection_UTaX_p3000", oracle64.gamma(1.0 / 3000.0) * (2327.0 - 770.0) ** 2)

@@ -86,6 +86,23 @@ def test_selection_equals_the_literal_rule_of_L348():
     assert got == expect and len(got) > 50 * 40
     assert (sel["ghost"] < cut).all()
     assert len(got) < allc["n"]                                 # the selection does remove something
+    # a flat network (outputs squeezed around 1/2, all below the cut) with a 0.004 margin: now the margin decides
+    # some twenty removals (few seeds have two candidates), so a misread margin or comparison set shows
+    flat = w.copy(); flat[304:336] *= 0.02; flat[336] = 0.0; flat[337] = 0.8; flat[338] = 0.004
+    open_f = flat.copy(); open_f[337] = np.inf; open_f[338] = np.inf
+    _, _, _, allf = run(o, ev, open_f)
+    _, _, _, self_ = run(o, ev, flat)
+    pf = allf["ghost"].astype(np.float32)
+    assert (pf < 0.8).all() and pf.std() > 0.002
+    expect_f, removed_by_margin = set(), 0
+    for i in range(allf["n"]):
+        share = (allf["seed"] == allf["seed"][i]) | (allf["velo"] == allf["velo"][i])
+        share[i] = False
+        if (pf[i] >= (pf[share] + np.float32(0.004)).astype(np.float32)).any():
+            removed_by_margin += 1
+        else:
+            expect_f.add((int(allf["seed"][i]), int(allf["velo"][i])))
+    assert set(zip(self_["seed"].tolist(), self_["velo"].tolist())) == expect_f and removed_by_margin >= 10
     # without the network the chi2 ranking (A14) is unchanged
     m0 = o.matching(ev.n_events, seed_off, s["state"], ev, use_ut=True)
     assert "ghost" not in m0 and m0["n"] > 0

@@ -109,7 +109,38 @@ def test_hough_equals_the_literal_reading_in_python():
         best = python_hough(s["par"][i, :3], int(s["half"][i]), ev, zbase)
         assert best is not None
         same += [int(h) for h in s["hits"][i][UV_LAYERS]] == [int(h) for h in best[2]] and best[0] == s["nuv"][i]
-    assert same >= 0.99 * len(idx), (same, len(idx))
+    assert same >= len(idx) - 1, (same, len(idx))            # (one seed of slack for a chi2 tie in float64)
+
+
+def test_hough_finds_what_the_literal_reading_finds_for_every_survivor():
+    """The other direction, and the iterative version too: for EVERY x-z candidate that survives the clone kill
+    in a half, the literal Python reading decides whether there is a seed and with which stereo hits; the
+    oracle's seeds of that half must be exactly those (no seed lost to a cluster threshold, a window or a
+    hypothesis that is off by a fraction of a bin)."""
+    from tests.test_oracle_readings import python_uv_iterative
+    from types import SimpleNamespace
+    ev = generate(config(2, 2))
+    for hough in (True, False):
+        o = Oracle(G, "f64"); o.set_uv_hough(hough)
+        s = o.seeding(ev)
+        n_checked = mism = 0
+        for e in range(ev.n_events):
+            for half in range(2):
+                zbase = (e * 2 + half) * 12
+                d = o.seeding_debug(ev, e, half)
+                want = set()
+                for c in np.flatnonzero(d["c_keep"]):
+                    if hough:
+                        best = python_hough(d["c_par"][c, :3], half, ev, zbase)
+                    else:
+                        sub = SimpleNamespace(zone_off=ev.zone_off[e * 24:e * 24 + 25], hit_x64=ev.hit_x64)
+                        best = python_uv_iterative(d["c_par"][c, :3], half, sub)
+                    if best is not None:
+                        want.add((tuple(int(h) for h in d["c_hits"][c]), tuple(int(h) for h in best[2])))
+                sel = (s["event"] == e) & (s["half"] == half)
+                got = {(tuple(int(h) for h in hh[X_LAYERS]), tuple(int(h) for h in hh[UV_LAYERS])) for hh in s["hits"][sel]}
+                n_checked += len(want | got); mism += len(want ^ got)
+        assert n_checked > 250 and mism <= 2, (hough, n_checked, mism)     # (slack for chi2 ties / cut edges in float64)
 
 
 def test_hough_seed_invariants():

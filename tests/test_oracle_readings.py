@@ -178,6 +178,53 @@ def test_half_overlap_keeps_a_track_at_the_edge_of_its_half():
     assert Oracle(G, "f64").seeding(ev)["n"] == 0
 
 
+def test_first_layer_window_spans_the_half_plus_the_overlap():
+    """Eq. 16 / reading A19 in numbers: the first-layer stereo window of an x-z candidate holds exactly the hits
+    with y = (x_pred - x) / tan(alpha) in [-y_half_tol, y_max] (upper half; mirrored [y_min, +y_half_tol] in the
+    lower one).  Decoys 1 mm inside and 1 mm outside of each edge, in both first layers: the oracle's own step
+    counter of first-layer hits (uv_first) must count the track's hit and the two inner decoys per pass."""
+    par = xz_track(p=15000.0, tx0=0.02)
+    ax, bx, cx = par
+    tol, ymax, ymin = G["y_half_tol"], G["y_max"], G["y_min"]
+    for half, sign, edges in ((0, +1.0, (-tol, ymax)), (1, -1.0, (ymin, tol))):
+        hits = track_hits(par, lambda z: sign * 40.0, half=half)
+        inside = outside = 0
+        for lf in G["uv_first_layer"]:
+            xp = ax + bx * (Z[lf] - ZREF) + cx * g_of(Z[lf])
+            for edge, inward in ((edges[0], +1.0), (edges[1], -1.0)):
+                hits.append((half, lf, xp - (edge + inward * 1.0) * TA[lf])); inside += 1
+                hits.append((half, lf, xp - (edge - inward * 1.0) * TA[lf])); outside += 1
+        ev, _ = make_event(hits)
+        s = Oracle(G, "f64").seeding(ev)
+        assert s["n"] == 1 and s["nuv"][0] == 6, half
+        assert s["counters"]["xz_kept"] == 1
+        assert s["counters"]["uv_first"] == 2 + inside, (half, s["counters"]["uv_first"])     # 2 = the track's own hits
+
+
+def test_more_stereo_hits_beat_an_earlier_combination():
+    """L215 / L219: among the combinations of one x-z candidate the one with more stereo hits wins, whatever the
+    order they are found in.  Two straight lines in y share the x-z track: line A (t_y = 0.05) has four stereo hits
+    (layers 1, 2, 5, 6), line B (t_y = 0.03) all six.  In the first pass A's hit comes first (lower x in the u
+    layer), so B has to replace it; the seed carries B's six hits."""
+    par = xz_track(p=11000.0, q=-1, tx0=0.03)
+    hits_b = track_hits(par, lambda z: 0.03 * z)
+    hits_a = [h for h in track_hits(par, lambda z: 0.05 * z) if h[1] in (1, 2, 5, 6)]
+    assert hits_a[0][2] < hits_b[1][2]                       # A's first-layer hit is met first
+    ev, idx = make_event(hits_b + hits_a)
+    for mode in ("f64", "f32"):
+        s = Oracle(G, mode).seeding(ev)
+        assert s["n"] == 1 and s["nuv"][0] == 6, (mode, s["n"], s["nuv"])
+        assert [int(v) for v in s["hits"][0]] == [idx[l] for l in range(12)]
+    # ... and with equal numbers of hits the better chi2 wins: B's hits smeared, A complete and exact
+    rng = np.random.default_rng(5)
+    hits_b2 = [(h, l, x + (0.25 * rng.standard_normal() if l in UV_LAYERS else 0.0)) for (h, l, x) in hits_b]
+    hits_a2 = [h for h in track_hits(par, lambda z: 0.05 * z) if h[1] in UV_LAYERS]
+    ev, idx = make_event(hits_b2 + hits_a2)
+    s = Oracle(G, "f64").seeding(ev)
+    assert s["n"] == 1 and s["nuv"][0] == 6
+    assert [int(s["hits"][0][l]) for l in UV_LAYERS] == [idx[12 + k] for k in range(6)]      # line A's hits
+
+
 # --------------------------------------------------------------------------------------- A15
 def test_closest_hit_ties_go_to_the_lower_index():
     """Two hits at exactly the same x inside the +-1 mm window of the x extension (layer 3, searched by

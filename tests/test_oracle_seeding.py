@@ -216,6 +216,14 @@ def test_clone_kill_worked_examples(oracle32):
     assert keep.tolist() == [True, False]
     keep = oracle32.clone_kill([k(0.1, 0, 6), k(0.2, 0, 6)], [A, hits6(0, 1, 2, 3, 6, 7)], [6, 6], 8)
     assert keep.tolist() == [True, True]
+    # a five-hit track that keeps exactly three of its hits is retained ("at least three", L198), with four too
+    keep = oracle32.clone_kill([k(0.1, 0, 6), k(0.2, 0, 5)], [A, hits6(0, 1, 6, 7, 8)], [6, 5], 9)
+    assert keep.tolist() == [True, True]
+    keep = oracle32.clone_kill([k(0.1, 0, 6), k(0.2, 0, 5)], [A, hits6(0, 6, 7, 8, 9)], [6, 5], 10)
+    assert keep.tolist() == [True, True]
+    # a six-hit track that keeps one hit only is dropped (two are needed, L198)
+    keep = oracle32.clone_kill([k(0.1, 0, 6), k(0.2, 0, 6)], [A, hits6(0, 1, 2, 3, 4, 6)], [6, 6], 7)
+    assert keep.tolist() == [True, False]
 
 
 def test_clone_kill_invariants(oracle32, cfg2_small):
