@@ -109,3 +109,55 @@ def test_equal_chi2_candidates_of_a_seed_go_to_the_lower_velo_index():
                          ut_off=np.zeros(5, np.uint32), ut_x0=np.zeros(0), ut_ylo=np.zeros(0), ut_yhi=np.zeros(0))
     m = o.matching(1, np.array([0, 1], np.uint32), np.array([seed]), ev, use_ut=False)
     assert m["n"] == 1 and int(m["seed"][0]) == 0 and int(m["velo"][0]) == 1
+
+
+def test_first_layer_stereo_window_is_closed():
+    """Eq. 16 / A19: track at x = 0, y = 0, so the first-layer window of stereo layer l is [-y_max tan, +y_half_tol tan]
+    (upper half) exactly; hits ON both edges are first-layer hits (the oracle's uv_first counter), the next float64
+    beyond them are not."""
+    o = Oracle(G, "f64")
+    xl = {l: [0.0] for l in (0, 3, 4, 7, 8, 11)}
+    n_first = 0
+    hits = dict(xl); hits.update({l: [0.0] for l in (1, 2, 5, 6, 9, 10)})
+    for lf in G["uv_first_layer"]:
+        ta = G["scifi_tan_alpha"][lf]
+        a, b = 0.0 - (-G["y_half_tol"] * ta), 0.0 - (G["y_max"] * ta)       # x_pred - y tan(alpha) at both ends of the half
+        hits[lf] = hits[lf] + [a, b, up(a), up(b)]
+        n_first += 3                                                      # the track's own hit and the two edge hits
+    s = o.seeding(event(hits))
+    assert s["n"] == 1 and s["counters"]["xz_kept"] == 1
+    assert s["counters"]["uv_first"] == n_first, s["counters"]["uv_first"]
+
+
+def test_preselection_cuts_are_strict_on_every_variable(oracle64=None):
+    """Eq. 21 as printed: |dx| < 20 mm, |dy| < 150 mm, |dtx| < 1.5 (|dty| < 0.02 is in test_oracle_constants).  With
+    zero slopes dx = x_S - x_V and dy = y_S - y_V exactly; with t_x^V = 0, dtx = t_x^S exactly."""
+    o = Oracle(G, "f64")
+    below = lambda v: float(np.nextafter(v, 0.0))
+    for seed, velo, ok in (([20.0, 0, 0, 0], [0, 0, 0, 0], 0.0), ([below(20.0), 0, 0, 0], [0, 0, 0, 0], 1.0),
+                           ([0, 150.0, 0, 0], [0, 0, 0, 0], 0.0), ([0, below(150.0), 0, 0], [0, 0, 0, 0], 1.0),
+                           ([-20.0, 0, 0, 0], [0, 0, 0, 0], 0.0), ([0, -150.0, 0, 0], [0, 0, 0, 0], 0.0)):
+        r = o.match_pair([float(v) for v in seed], [float(v) for v in velo])
+        assert r["presel"] == ok, (seed, r)
+    # dtx: choose x_S so that dx = 0 at the z_match of this pair (fixed point on |x_S|), then dtx alone decides
+    for dtx, ok in ((1.5, 0.0), (below(1.5), 1.0)):
+        xs = 0.0
+        for _ in range(40):
+            zm = o.match_pair([xs, 0.0, dtx, 0.0], [0.0, 0.0, 0.0, 0.0])["zm"]
+            xs = (7826.0 - zm) * dtx
+        r = o.match_pair([xs, 0.0, dtx, 0.0], [0.0, 0.0, 0.0, 0.0])
+        assert abs(r["dx"]) < 1.0 and r["dtx"] == dtx and r["presel"] == ok, (dtx, r)
+
+
+def test_ut_strip_coverage_is_closed_at_the_tolerance():
+    """Reading A18: a strip covers y if y_lo - 1 mm <= y <= y_hi + 1 mm, closed.  VELO state on the z axis (y = 0 at
+    every layer): a strip starting exactly 1 mm above 0, or ending exactly 1 mm below, still covers it."""
+    o = Oracle(G, "f64")
+    tol = G["ut_y_tol"]
+    dz = G["ut_z"][0] - G["z_velo"]
+    x0e = (0.0 + 0.0 * dz) + G["gamma_ab"][0] * (dz * dz)
+    off = np.array([0, 1, 1, 1, 1], np.uint32)
+    for ylo, yhi, inside in ((tol, tol + 100.0, True), (up(tol), tol + 100.0, False), (-100.0 - tol, -tol, True),
+                             (-100.0 - tol, up(-tol), False)):
+        r = o.ut_search([0.0, 0.0, 0.0, 0.0], 0.0, off, np.array([x0e]), np.array([ylo]), np.array([yhi]))
+        assert r["n"] == (1 if inside else 0), (ylo, yhi, r)

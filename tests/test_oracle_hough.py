@@ -143,6 +143,20 @@ def test_hough_finds_what_the_literal_reading_finds_for_every_survivor():
         assert n_checked > 250 and mism <= 2, (hough, n_checked, mism)     # (slack for chi2 ties / cut edges in float64)
 
 
+def test_hough_seeds_a_track_with_exactly_the_minimum_of_stereo_hits():
+    """A20 with L215: a cluster that exactly `min_uv_hits` (4) layers vote for is a cluster, and a combination of
+    exactly four stereo hits is a seed: a hand-built track with stereo hits in layers 1, 5, 6 and 10 only."""
+    from tests.test_oracle_readings import make_event, track_hits, xz_track
+    par = xz_track(p=14000.0, q=+1, tx0=-0.02)
+    hits = [h for h in track_hits(par, lambda z: 0.04 * z) if h[1] in X_LAYERS or h[1] in (1, 5, 6, 10)]
+    ev, idx = make_event(hits)
+    for hough in (True, False):
+        o = Oracle(G, "f64"); o.set_uv_hough(hough)
+        s = o.seeding(ev)
+        assert s["n"] == 1 and s["nuv"][0] == 4 and s["nx"][0] == 6, (hough, s["n"])
+        assert sorted(int(h) for h in s["hits"][0] if h != NO_HIT) == sorted(idx.values())
+
+
 def test_hough_seed_invariants():
     ev = generate(config(2, 6))
     o = Oracle(G, "f32"); o.set_uv_hough(True)
