@@ -161,3 +161,35 @@ def test_ut_strip_coverage_is_closed_at_the_tolerance():
                              (-100.0 - tol, up(-tol), False)):
         r = o.ut_search([0.0, 0.0, 0.0, 0.0], 0.0, off, np.array([x0e]), np.array([ylo]), np.array([yhi]))
         assert r["n"] == (1 if inside else 0), (ylo, yhi, r)
+
+
+def test_hit_with_global_index_zero_is_a_hit_like_any_other():
+    """Index 0 is a valid hit index (NO_HIT is 0xFFFFFFFF, "nothing found yet" is -1): (a) the first hit of the
+    event is the closest one in its layer although a decoy 0.5 mm further sits at index 1; (b) with no hit in layer 0
+    the first stereo hit has global index 0 and is attached like the others."""
+    from tests.test_oracle_readings import make_event, track_hits, xz_track
+    par = xz_track(p=13000.0, q=+1, tx0=0.01)
+    hits = track_hits(par, lambda z: 0.02 * z)
+    ev, idx = make_event(hits + [(0, 0, hits[0][2] + 0.5)])
+    assert idx[0] == 0
+    o = Oracle(G, "f64")
+    d = o.seeding_debug(ev, 0, 0)
+    it1 = d["c_it"] == 1                                      # iteration 1 reaches layer 0 by the +-1 mm extension
+    assert it1.sum() == 1 and d["c_hits"][it1][0][0] == 0
+    s = o.seeding(ev)
+    assert s["n"] >= 1 and all(int(h[0]) == 0 for h in s["hits"])
+    ev, idx = make_event([h for h in hits if h[1] != 0])
+    assert idx[0] == 0 and ev.zone_off[1] == 0                # (position 0 of the list is now the layer-1 stereo hit)
+    s = o.seeding(ev)
+    assert s["n"] == 1 and s["nx"][0] == 5 and s["nuv"][0] == 6 and int(s["hits"][0][1]) == 0
+
+
+def test_ut_strip_coverage_is_closed_in_the_tight_layers_too():
+    o = Oracle(G, "f64")
+    tol = G["ut_y_tol"]
+    x0 = np.array([G["gamma_ab"][0] * ((z - G["z_velo"]) ** 2) for z in G["ut_z"]])      # q/p = 0: gamma_x = A_gamma
+    off = np.array([0, 1, 2, 3, 4], np.uint32)
+    for ylo2, n in ((tol, 4), (up(tol), 3)):
+        ylo = np.array([-50.0, -50.0, ylo2, -50.0]); yhi = ylo + 100.0
+        r = o.ut_search([0.0, 0.0, 0.0, 0.0], 0.0, off, x0, ylo, yhi)
+        assert r["ok"] and r["n"] == n, (ylo2, r)
