@@ -3,7 +3,7 @@
 All intermediates of both kernels live in shared memory, so the capacities decide how many CTAs share
 an SM (include/lhcb.h: lhcb_launch_config).  The library defaults (all zero in the geometry) are sized
 for BASELINE.json configs[3] (mu = 7.6 plus displaced tracks); NOMINAL is sized for Run 3 nominal
-occupancy (mu ~ 5: configs[1] and configs[2]), where it lets four 256-thread seeding CTAs and six
+occupancy (mu ~ 5: configs[1] and configs[2]), where it lets five 256-thread seeding CTAs and six
 128-thread matching CTAs share an SM.  Exceeding a capacity is never silent: the per-half / per-event
 status words report it and the tests and bench.py fail on any set bit.
 

@@ -3,7 +3,7 @@
 // One CTA per event-half (L372): the half's twelve sorted hit zones are staged into shared memory and stay
 // there for every step (L370).  In the staged tile every zone is framed by a -inf and a +inf sentinel, so
 // that no search needs a bounds check.  Stages, separated by __syncthreads():
-//   S0  staging + bin tables           per zone, a 320-bin table "first hit with bin >= k" turns every lower
+//   S0  staging + bin tables           per zone, a 256-bin table "first hit with bin >= k" turns every lower
 //                                      bound into one lookup plus a short forward scan (about 0.5 hits per
 //                                      bin); the table is built by marking the first hit of every occupied
 //                                      bin and a ballot-based suffix fill, one warp per zone
@@ -40,7 +40,7 @@ namespace lhcb {
 #ifndef LHCB_ITEM_PAIRS
 #define LHCB_ITEM_PAIRS 4   // T3 hits per item of the pair walk (2, 4 or 8; measured 3.10 ms with 4 against 3.16 ms with 8)
 #endif
-constexpr int kSeedThreadsMax = 512;          // the kernel is instantiated for 256 x 4 CTAs/SM and 512 x 2 CTAs/SM
+constexpr int kSeedThreadsMax = 512;          // the kernel is instantiated for 256 x 5, 256 x 4 and 512 x 2 CTAs/SM
 constexpr int kLutBins = LHCB_LUT_BINS;       // bins of the per-zone search table
 constexpr int kItemPairs = LHCB_ITEM_PAIRS;
 constexpr int kTileIndexBits = 13;            // tile indices fit 13 bits: max_hits_per_half + 40 <= 8192
