@@ -39,7 +39,8 @@ typedef enum {
   LHCB_ERR_BAD_GEOMETRY = -2,   /* not 6 x-layers + 6 stereo layers, seed triple not on x-layers, ... */
   LHCB_ERR_CUDA = -3,           /* a CUDA runtime call failed (see lhcb_last_cuda_error) */
   LHCB_ERR_NOT_INITIALISED = -4,
-  LHCB_ERR_CAPACITY = -5        /* requested capacities do not fit shared memory of the device */
+  LHCB_ERR_CAPACITY = -5,       /* requested capacities do not fit shared memory of the device */
+  LHCB_ERR_STATIC_SCRATCH = -6  /* lhcb_seeding_static: more than LHCB_STATIC_MAX_EVENTS events in the batch */
 } lhcb_status;
 
 /* bits of the per-half / per-event `status` output words */
@@ -254,6 +255,43 @@ int lhcb_set_ghost_nn(lhcb_ctx* ctx, const float* nn);
  * workspace: NULL, or the workspace lhcb_order filled for this batch. */
 int lhcb_seeding(lhcb_ctx* ctx, const lhcb_events_t* events, lhcb_seeds_t* out, void* workspace,
                  void* cuda_stream);
+
+/* Seeding in heaviest-first CTA order without a workspace and without any allocation: lhcb_order + lhcb_seeding
+ * in one call, for the caller who has no device memory to give and may not ask the driver for any.
+ *
+ * Who that is.  The algorithms of the paper run inside a trigger application that reserves
+ * its device memory once at start-up and then loops over batches on several streams at a time.  Inside that
+ * loop cudaMalloc / cudaFree are off limits: either call waits until the whole device is idle, so one stream's
+ * allocation would stall every other stream's batch.  The same holds for a process whose device memory has
+ * already been handed in full to another allocator (a framework's caching pool): a cudaMalloc there simply
+ * fails.  Such a caller can still use plain lhcb_seeding (it needs no workspace), but then loses the
+ * heaviest-first CTA order that shortens the last wave of a batch of about 1,000 events: lhcb_order wants a
+ * workspace the caller cannot provide.  This call keeps that workspace inside the library instead.
+ *
+ * How.  The order tables and per-half flags (20 bytes per event) sit in one array of
+ * LHCB_STATIC_MAX_EVENTS * 20 = 61,440 bytes that is part of the library image: every GPU on which this
+ * library's kernels are loaded holds its own copy from module load until the process exits, whether or not
+ * this call is ever made.  The call makes no cudaMalloc, cudaFree or other allocating call; it enqueues
+ * two kernels (order, seeding) on cuda_stream and does not synchronise.  (lhcb_geom_init, at set-up, does allocate
+ * its three small constant tables, about 11 KB; it is this per-batch call that allocates nothing.)
+ *
+ * events / out: exactly as for lhcb_seeding -- device pointers owned by the caller, outputs fully overwritten,
+ * same seeds in the same slots as lhcb_seeding gives with or without a workspace.
+ *
+ * Limits and rules.
+ *   - events->n_events <= LHCB_STATIC_MAX_EVENTS (3,072), else LHCB_ERR_STATIC_SCRATCH is returned and nothing is
+ *     launched; split the batch or use lhcb_order + lhcb_seeding with your own workspace.  (Above that size
+ *     the heaviest-first order no longer pays and lhcb_seeding ignores a workspace anyway.)
+ *   - The first call on a device looks up the array's device address (once per device, cached) before it
+ *     launches anything; make that first call outside any stream capture, e.g. on a small warm-up batch.
+ *   - All calls on one device share the one array, also across contexts and threads.  Each call rewrites every
+ *     word its batch uses before reading it, so the previous call's contents never matter and calls that
+ *     follow each other in one stream are safe.  Two calls that can run on the GPU at the same time
+ *     (different streams, different contexts on the same device) race on the array and give undefined
+ *     results: serialise them, or give all but one of them lhcb_order + a workspace of their own.
+ *   - The array is private to this call: lhcb_matching afterwards takes workspace = NULL. */
+#define LHCB_STATIC_MAX_EVENTS 3072
+int lhcb_seeding_static(lhcb_ctx* ctx, const lhcb_events_t* events, lhcb_seeds_t* out, void* cuda_stream);
 
 /* Matching: kink extrapolation, preselection, chi2_match, UT hit search, one-to-one selection
  * (section 4).  `ut` may be NULL (no UT in the data taking, L307).  Of the seeds, count and state are

@@ -17,6 +17,7 @@ from . import build as _build
 
 F, I = C.c_float, C.c_int32
 NO_HIT = 0xFFFFFFFF
+STATIC_MAX_EVENTS = 3072        # LHCB_STATIC_MAX_EVENTS of include/lhcb.h
 
 ST_BITS = {1: "triplet_overflow", 2: "cand_overflow", 4: "seed_overflow", 8: "hits_overflow",
            16: "match_overflow", 32: "long_overflow", 64: "velo_overflow", 128: "ut_overflow", 256: "uv_queue_overflow", 512: "bad_raw_hit"}
@@ -25,7 +26,7 @@ EXPORTS = ["lhcb_geom_derive", "lhcb_geom_init", "lhcb_destroy", "lhcb_get_geom"
            "lhcb_seeding", "lhcb_matching", "lhcb_error_string", "lhcb_last_cuda_error",
            "lhcb_last_launch_count", "lhcb_pipeline_create", "lhcb_pipeline_destroy", "lhcb_reconstruct_host",
            "lhcb_pipeline_last_bytes", "lhcb_launch_config", "lhcb_prepare", "lhcb_set_ghost_nn", "lhcb_set_uv_hough",
-           "lhcb_order"]
+           "lhcb_order", "lhcb_seeding_static"]
 
 
 class LhcbGeom(C.Structure):
@@ -139,6 +140,7 @@ def load_library(build: bool = True, stage_clocks: bool = False, checked: bool =
         lib.lhcb_workspace_bytes.argtypes = [VP, C.c_int, C.c_size_t]
         lib.lhcb_workspace_bytes.restype = C.c_size_t
         lib.lhcb_seeding.argtypes = [VP, C.POINTER(LhcbEvents), C.POINTER(LhcbSeeds), VP, VP]
+        lib.lhcb_seeding_static.argtypes = [VP, C.POINTER(LhcbEvents), C.POINTER(LhcbSeeds), VP]
         lib.lhcb_matching.argtypes = [VP, C.POINTER(LhcbSeeds), C.POINTER(LhcbVelo), C.POINTER(LhcbUt),
                                       C.POINTER(LhcbLong), VP, VP]
         lib.lhcb_error_string.argtypes = [C.c_int]
@@ -333,6 +335,17 @@ class Context:
         s = self._seeds_struct(out)
         rc = self.lib.lhcb_seeding(self._ctx, C.byref(e), C.byref(s), _ptr(workspace), self._stream())
         _check(self.lib, self._ctx, rc, "lhcb_seeding")
+        return out
+
+    def lhcb_seeding_static(self, dev: DeviceEvents, out: dict) -> dict:
+        """Heaviest-first Seeding with the order tables in the library's built-in device array: for callers that
+        may not allocate device memory per batch (see include/lhcb.h).  `out` must come from alloc_seeds(), made
+        beforehand: this method allocates nothing either.  At most STATIC_MAX_EVENTS (3,072) events; calls that
+        overlap on the GPU race on the shared array."""
+        e = LhcbEvents(dev.n_events, dev.n_hits, _ptr(dev.zone_off), _ptr(dev.hit_x), _ptr(dev.polarity))
+        s = self._seeds_struct(out)
+        rc = self.lib.lhcb_seeding_static(self._ctx, C.byref(e), C.byref(s), self._stream())
+        _check(self.lib, self._ctx, rc, "lhcb_seeding_static")
         return out
 
     def lhcb_matching(self, seeds: dict, dev: DeviceEvents, out: Optional[dict] = None, use_ut: bool = True,

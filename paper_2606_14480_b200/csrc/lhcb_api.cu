@@ -6,6 +6,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "../../include/lhcb.h"
@@ -361,6 +362,9 @@ const char* lhcb_error_string(int s) {
     case LHCB_ERR_CUDA: return "CUDA runtime error";
     case LHCB_ERR_NOT_INITIALISED: return "context not initialised";
     case LHCB_ERR_CAPACITY: return "capacities exceed the shared memory of the device";
+    case LHCB_ERR_STATIC_SCRATCH:
+      return "batch has more events than the built-in scratch of lhcb_seeding_static holds (LHCB_STATIC_MAX_EVENTS = 3072): "
+             "split the batch, or use lhcb_order + lhcb_seeding with a workspace of your own";
     default: return "unknown status";
   }
 }
@@ -421,6 +425,54 @@ int lhcb_launch_config(const lhcb_ctx* c, int out[4]) {
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// lhcb_seeding_static (include/lhcb.h): the heaviest-first Seeding for callers that cannot bring a workspace.
+// The CTA order and the per-half flags that lhcb_order / lhcb_seeding keep in a caller-owned workspace live
+// here in an array that is part of the library image: the driver places it when the module is loaded on a
+// device and it stays there until the process exits, so no call ever allocates or frees for it.
+namespace {
+// same layout as lhcb_workspace_bytes: 5 words per event (Seeding order [2n], Matching order [n], flags [2n])
+static __device__ __align__(256) uint32_t g_static_ws[(size_t)LHCB_STATIC_MAX_EVENTS * 5];   // 61,440 bytes per device
+static_assert(LHCB_STATIC_MAX_EVENTS <= lhcb::kOrderMaxSorted, "lhcb_seeding ignores a workspace above kOrderMaxSorted events");
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mu;
+void* g_static_addr[kStaticMaxDevices];   // device address of g_static_ws on each device, once looked up
+
+// `g_static_ws` in host code names a host-side handle, not the memory the kernels see: its device address has to
+// be asked for, with the device current, once per device (each device holds its own copy of the array).
+cudaError_t static_ws_address(int device, void** out) {
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (device < kStaticMaxDevices && g_static_addr[device]) { *out = g_static_addr[device]; return cudaSuccess; }
+  void* a = nullptr;
+  const cudaError_t e = cudaGetSymbolAddress(&a, g_static_ws);
+  if (e != cudaSuccess) return e;
+  if (!a) return cudaErrorInvalidSymbol;
+  if (device < kStaticMaxDevices) g_static_addr[device] = a;
+  *out = a;
+  return cudaSuccess;
+}
+}  // namespace
+
+extern "C" int lhcb_seeding_static(lhcb_ctx* c, const lhcb_events_t* ev, lhcb_seeds_t* out, void* stream) {
+  if (!c) return LHCB_ERR_NOT_INITIALISED;
+  if (!ev || !out || ev->n_events < 0) return LHCB_ERR_BAD_ARGUMENT;
+  if (ev->n_events > LHCB_STATIC_MAX_EVENTS) return LHCB_ERR_STATIC_SCRATCH;   // nothing is launched
+  c->last_launches = 0;
+  if (ev->n_events == 0) return LHCB_OK;
+  LHCB_CUDA(c, cudaSetDevice(c->device));
+  void* ws = nullptr;
+  LHCB_CUDA(c, static_ws_address(c->device, &ws));
+  // order_kernel rewrites every word of the array that this batch's Seeding reads (order [0, 2n), flags [3n, 5n)),
+  // so what the previous call left behind is never seen; nothing has to start at zero
+  int rc = lhcb_order(c, ev, nullptr, nullptr, ws, stream);
+  if (rc != LHCB_OK) return rc;
+  rc = lhcb_seeding(c, ev, out, ws, stream);
+  if (rc != LHCB_OK) return rc;
+  c->last_launches = 2;
+  return LHCB_OK;
+}
 
 // ---------------------------------------------------------------------------------------------
 // Host-buffer pipeline: slices of events on three streams (H2D copies, kernels, D2H copies).  The kernels of
