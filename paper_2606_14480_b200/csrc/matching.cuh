@@ -289,7 +289,7 @@ matching_kernel(const __grid_constant__ MatchParams p) {
     return;
   }
   if (tid < 4) hdr[tid] = 0;
-  if (tid == 4) { hdr[9] = 0; hdr[10] = 0; }                 // chi2 tie seen (reading A21); preselected pairs of the tile
+  if (tid == 4) { hdr[9] = 0; hdr[10] = 0; hdr[11] = 0; }    // chi2 tie seen (reading A21); preselected pairs of the even / odd tiles
   // ---- UT x0 (and strip rows) of this event: bulk copies, overlapped with the all-pairs loop ----------
   uint32_t u_begin = 0, u_end = 0, ua0 = 0;
   bool ut_in_smem = false, rows_in_smem = false;
@@ -392,7 +392,12 @@ matching_kernel(const __grid_constant__ MatchParams p) {
   uint32_t* pq = reinterpret_cast<uint32_t*>(seed_best);   // preselected pairs of a tile: (owner << 16) | VELO rank
   const int pq_cap = 4 * p.max_seeds;
   auto slot_of = [&](int s) { return s < c0 ? (size_t)(2 * e) * p.max_seeds + s : (size_t)(2 * e + 1) * p.max_seeds + (s - c0); };
-  for (int tile0 = 0; tile0 < ns; tile0 += T) {
+  for (int tile0 = 0, par = 0; tile0 < ns; tile0 += T, par ^= 1) {
+    // two pair counters taken in turn.  Only a tile's closing barrier lies between its dense pass and the next
+    // tile's walk, so a counter cannot be cleared after that barrier without racing the first increments.  Thread 0
+    // clears the OTHER counter between the two barriers of each tile instead: its last reader finished before the
+    // previous tile's closing barrier, its next writer starts after this tile's
+    int* const pq_n = &hdr[10 + par];
     const int nown = ns - tile0 < T ? ns - tile0 : T;
     int cnt = 0, fst = 0;
     if (tid < nown) {
@@ -421,12 +426,13 @@ matching_kernel(const __grid_constant__ MatchParams p) {
         if (!(fabsf(dx) < p.presel[0] && fabsf(dy) < p.presel[1] && adtx < p.presel[2] &&
               fabsf(dty) < p.presel[3]))                                           // Eq. 21
           continue;
-        const int k = smem_inc(&hdr[10]);
+        const int k = smem_inc(pq_n);
         if (k < pq_cap) pq[k] = ((uint32_t)tid << 16) | (uint32_t)v;
       }
     }
     __syncthreads();
-    int nq = hdr[10];
+    int nq = *pq_n;
+    if (tid == 0) hdr[10 + (par ^ 1)] = 0;                   // the next tile's counter: idle since before the previous closing barrier
     if (nq > pq_cap) { nq = pq_cap; if (tid == 0) hdr[2] |= LHCB_ST_MATCH_OVERFLOW; }
     for (int i = tid; i < nq; i += T) {
       const uint32_t e_ = pq[i];
@@ -457,10 +463,11 @@ matching_kernel(const __grid_constant__ MatchParams p) {
       }
     }
     __syncthreads();
-    if (tid == 0) hdr[10] = 0;
     LHCB_CLK(11)
   }
   for (int s = tid; s < 2 * p.max_seeds; s += T) seed_best[s] = kNoKey;   // (the queue of preselected pairs is dead)
+  __syncthreads();                                         // without UT and without a network nothing else separates this reset
+                                                           // from the atomicMin of the selection below
   int nm = hdr[0];
   LHCB_DBG_MAX(4, nm)
   if (nm > p.max_mc) { nm = p.max_mc; if (tid == 0) hdr[2] |= LHCB_ST_MATCH_OVERFLOW; }

@@ -13,7 +13,7 @@ from tests.parity import assert_batch_identical, select_events
 pytestmark = pytest.mark.gpu
 
 
-def run_gpu(geom, ev, caps=None, order=False, hough=False):
+def run_gpu(geom, ev, caps=None, order=False, hough=False, use_ut=True):
     from paper_2606_14480_b200 import Context, DeviceEvents
     g = dict(geom)
     if caps:
@@ -24,7 +24,7 @@ def run_gpu(geom, ev, caps=None, order=False, hough=False):
     dev = DeviceEvents.from_host(ev)
     ws = c.lhcb_order(dev) if order else None
     s = c.lhcb_seeding(dev, workspace=ws)
-    l = c.lhcb_matching(s, dev, workspace=ws)
+    l = c.lhcb_matching(s, dev, workspace=ws, use_ut=use_ut)
     c.torch.cuda.synchronize()
     out = c.seeds_to_host(s), c.long_to_host(l), c.lhcb_launch_config()
     c.close()
@@ -66,6 +66,21 @@ def test_cfg2_1000_events_both_launch_configurations(cfg2_full):
         assert not gs["status"].any() and not gl["status"].any(), "capacity overflow"
         n_s, n_l = assert_batch_identical(os_, om, gs, gl, f"cfg2 {threads}")
         assert n_s > 150 * 1000 and n_l > 90 * 1000
+
+
+def test_cfg2_1000_events_without_ut_both_launch_configurations(cfg2_full):
+    """Data taking without the UT: every chi2-accepted pair goes straight to the one-to-one selection,
+    the path of the kernel in which only one barrier separates the reset of the per-seed minima from their use.
+    Three runs per configuration: a race there would not show every time."""
+    from paper_2606_14480_b200 import capacities
+    ev, (os_, _, _) = cfg2_full
+    os2, om2, _ = reconstruct_parallel(ev, use_ut=False)
+    assert (om2["n_ut"] == 0).all() and len(om2["seed"]) > 100 * 1000
+    for caps, order in ((None, False), (capacities.NOMINAL, True)):
+        for _ in range(3):
+            gs, gl, _ = run_gpu(ev.geom, ev, caps, order, use_ut=False)
+            assert not gs["status"].any() and not gl["status"].any(), "capacity overflow"
+            assert_batch_identical(os2, om2, gs, gl, f"cfg2 without UT, order={order}")
 
 
 def test_cfg4_2000_events_default_capacities_and_nominal_overflow_report():
