@@ -209,11 +209,14 @@ size_t lhcb_workspace_bytes(const lhcb_ctx* ctx, int n_events, size_t n_scifi_hi
  * ut == NULL), heaviest first, into `workspace` (device memory, lhcb_workspace_bytes(n_events) bytes).
  * lhcb_seeding / lhcb_matching called with THIS workspace for THE SAME batch start their CTAs in that order,
  * which shortens the last wave of a small batch (for batches above 3,072 events, a dozen waves or more, the call does
- * nothing and the workspace is ignored); the results are the same in the same slots.  With the workspace the Matching is
- * also launched as a programmatic dependent of the Seeding before it IN THE SAME STREAM: its CTAs may start while
- * the last Seeding wave drains and wait for per-half "seeds written" flags kept in the workspace.  `velo` may be
- * NULL (Seeding order only).  A workspace that lhcb_order has not filled for the batch must not be passed
- * to the two calls.  Enqueues one small kernel; does not synchronise. */
+ * nothing and the workspace is ignored); the results are the same in the same slots.  When lhcb_matching is the
+ * call that follows lhcb_seeding directly on this context, with the same workspace, stream and batch size, it
+ * is also launched as a programmatic dependent of that Seeding grid: its CTAs may start while the last Seeding
+ * wave drains and wait for per-half "seeds written" flags kept in the workspace (enqueue nothing of your own in
+ * that stream between the two calls).  In every other case (given seeds, another call in between) the Matching is
+ * an ordinary launch.  `velo` may be NULL: without `ut` as well the Matching order is then the identity, the
+ * workspace stays valid for lhcb_matching.  A workspace that lhcb_order has not filled for the batch must not be
+ * passed to the two calls.  Enqueues one small kernel; does not synchronise. */
 int lhcb_order(lhcb_ctx* ctx, const lhcb_events_t* events, const lhcb_velo_t* velo, const lhcb_ut_t* ut,
                void* workspace, void* cuda_stream);
 

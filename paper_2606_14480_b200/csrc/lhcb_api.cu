@@ -33,6 +33,12 @@ struct lhcb_ctx {
   int seed_ctas;      // CTAs per SM the seeding kernel is compiled for (register budget)
   int last_cuda_error;
   int last_launches;
+  // the last launch made through this context, when it was a Seeding with lhcb_order's workspace: only the
+  // lhcb_matching call that follows it directly, on the same stream, workspace and batch size, may be launched as
+  // its programmatic dependent (the per-half flags the Matching waits on are lowered and raised by THAT grid)
+  const void* pdl_ws;
+  const void* pdl_stream;
+  int pdl_events;
 };
 
 namespace {
@@ -220,6 +226,7 @@ int lhcb_order(lhcb_ctx* c, const lhcb_events_t* ev, const lhcb_velo_t* velo, co
   if (!c) return LHCB_ERR_NOT_INITIALISED;
   if (!ev || !workspace || ev->n_events < 0 || (velo && velo->n_events != ev->n_events)) return LHCB_ERR_BAD_ARGUMENT;
   c->last_launches = 0;
+  c->pdl_ws = nullptr;
   if (ev->n_events == 0) return LHCB_OK;
   if (!ev->zone_off || (velo && !velo->off) || (ut && !ut->off)) return LHCB_ERR_BAD_ARGUMENT;
   // a large batch is dozens of waves of CTAs: its tail is a small part of the run, and both the sorted order and
@@ -230,7 +237,7 @@ int lhcb_order(lhcb_ctx* c, const lhcb_events_t* ev, const lhcb_velo_t* velo, co
   uint32_t* so = static_cast<uint32_t*>(workspace);
   lhcb::order_kernel<<<1, lhcb::kOrderThreads, 0, (cudaStream_t)stream>>>(ev->n_events, ev->zone_off, ut ? ut->off : nullptr,
                                                                         velo ? velo->off : nullptr, so,
-                                                                        velo ? so + (size_t)ev->n_events * 2 : nullptr,
+                                                                        so + (size_t)ev->n_events * 2,   // identity without velo and ut
                                                                         so + (size_t)ev->n_events * 3);
   LHCB_CUDA(c, cudaGetLastError());
   c->last_launches = 1;
@@ -258,6 +265,7 @@ int lhcb_prepare(lhcb_ctx* c, const lhcb_raw_t* raw, uint32_t* zone_off, float* 
   if (!c) return LHCB_ERR_NOT_INITIALISED;
   if (!raw || raw->n_events < 0 || !zone_off) return LHCB_ERR_BAD_ARGUMENT;
   c->last_launches = 0;
+  c->pdl_ws = nullptr;
   if (raw->n_events == 0) return LHCB_OK;                    // zone_off[0] is then the caller's to set
   if (!raw->off || !status || (raw->n_hits && (!raw->x || !raw->zone || !hit_x))) return LHCB_ERR_BAD_ARGUMENT;
   LHCB_CUDA(c, cudaSetDevice(c->device));
@@ -281,6 +289,7 @@ int lhcb_seeding(lhcb_ctx* c, const lhcb_events_t* ev, lhcb_seeds_t* out, void* 
   if (!c) return LHCB_ERR_NOT_INITIALISED;
   if (!ev || !out || ev->n_events < 0) return LHCB_ERR_BAD_ARGUMENT;
   c->last_launches = 0;
+  c->pdl_ws = nullptr;
   if (ev->n_events == 0) return LHCB_OK;
   if (!ev->zone_off || (!ev->hit_x && ev->n_hits) || !out->count || !out->state || !out->par || !out->hits ||
       !out->nx || !out->nuv || !out->status)
@@ -305,6 +314,7 @@ int lhcb_seeding(lhcb_ctx* c, const lhcb_events_t* ev, lhcb_seeds_t* out, void* 
     lhcb::seeding_kernel<512, 2><<<ev->n_events * 2, 512, c->seed_smem, (cudaStream_t)stream>>>(p);
   LHCB_CUDA(c, cudaGetLastError());
   c->last_launches = 1;
+  if (workspace) { c->pdl_ws = workspace; c->pdl_stream = stream; c->pdl_events = ev->n_events; }
   return LHCB_OK;
 }
 
@@ -314,6 +324,9 @@ int lhcb_matching(lhcb_ctx* c, const lhcb_seeds_t* seeds, const lhcb_velo_t* vel
   if (!seeds || !velo || !out || velo->n_events < 0 || seeds->n_events != velo->n_events)
     return LHCB_ERR_BAD_ARGUMENT;
   c->last_launches = 0;
+  // programmatic dependent launch only straight after the Seeding launch whose flags this grid will wait on
+  const bool after_seeding = workspace && c->pdl_ws == workspace && c->pdl_stream == stream && c->pdl_events == velo->n_events;
+  c->pdl_ws = nullptr;
   if (velo->n_events == 0) return LHCB_OK;
   if (!seeds->count || !seeds->state || !velo->off || !out->count || !out->seed_idx || !out->velo_idx ||
       !out->ut_idx || !out->n_ut || !out->qop || !out->chi2 || !out->status)
@@ -337,15 +350,17 @@ int lhcb_matching(lhcb_ctx* c, const lhcb_seeds_t* seeds, const lhcb_velo_t* vel
   p.done = workspace ? static_cast<const uint32_t*>(workspace) + (size_t)velo->n_events * 3 : nullptr;
   p.long_cap_total = (size_t)velo->n_events * (size_t)c->geom.max_long_per_event;
   {
-    // with lhcb_order's workspace the launch is a programmatic dependent of the Seeding grid before it in the
-    // stream: its CTAs may start while the last Seeding wave drains and wait for their event's flags
+    // straight after a Seeding launch with the same workspace, the launch is a programmatic dependent of that grid:
+    // its CTAs may start while the last Seeding wave drains and wait for their event's flags.  After anything else
+    // (lhcb_order alone, given seeds, another call in between) it is an ordinary launch: the kernel has no
+    // griddepcontrol.wait, so nothing but those flags would order it against a still-running predecessor
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)velo->n_events); cfg.blockDim = dim3((unsigned)c->match_threads);
     cfg.dynamicSmemBytes = c->match_smem; cfg.stream = (cudaStream_t)stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr; cfg.numAttrs = workspace ? 1 : 0;
+    cfg.attrs = attr; cfg.numAttrs = (workspace && after_seeding) ? 1 : 0;
     if (c->match_threads == 128) LHCB_CUDA(c, cudaLaunchKernelEx(&cfg, lhcb::matching_kernel<128, 6>, p));
     else LHCB_CUDA(c, cudaLaunchKernelEx(&cfg, lhcb::matching_kernel<256, 3>, p));
   }
@@ -464,11 +479,12 @@ extern "C" int lhcb_seeding_static(lhcb_ctx* c, const lhcb_events_t* ev, lhcb_se
   LHCB_CUDA(c, cudaSetDevice(c->device));
   void* ws = nullptr;
   LHCB_CUDA(c, static_ws_address(c->device, &ws));
-  // order_kernel rewrites every word of the array that this batch's Seeding reads (order [0, 2n), flags [3n, 5n)),
+  // order_kernel rewrites every word of the array that belongs to this batch (orders [0, 3n), flags [3n, 5n)),
   // so what the previous call left behind is never seen; nothing has to start at zero
   int rc = lhcb_order(c, ev, nullptr, nullptr, ws, stream);
   if (rc != LHCB_OK) return rc;
   rc = lhcb_seeding(c, ev, out, ws, stream);
+  c->pdl_ws = nullptr;                                       // the array is private: no Matching is ever its dependent
   if (rc != LHCB_OK) return rc;
   c->last_launches = 2;
   return LHCB_OK;
@@ -501,7 +517,7 @@ struct lhcb_pipeline {
   uint32_t *totals, *slice_totals;    // device: [2], [n_slices][4]
   uint32_t* h_totals;                 // pinned host mirror of slice_totals
   // one graph per slice
-  struct Graph { cudaGraphExec_t exec; int e0, ne; unsigned flags; } * graphs;
+  struct Graph { cudaGraphExec_t exec; int e0, ne; unsigned flags; int launches; } * graphs;
   int* e0;                            // [n_slices + 1] first event of each slice of the current batch
   uint64_t h2d, d2h;
   int launches;
@@ -512,9 +528,11 @@ template <class T>
 cudaError_t dalloc(T** p, size_t n) { return cudaMalloc((void**)p, (n ? n : 1) * sizeof(T)); }
 
 // the kernels of one slice on the compute stream (captured into the slice's graph)
-int enqueue_slice(lhcb_pipeline* p, int k, int e0, int ne, bool has_ut, bool has_pol, bool want_par, bool strips) {
+int enqueue_slice(lhcb_pipeline* p, int k, int e0, int ne, bool has_ut, bool has_pol, bool want_par, bool strips,
+                  int* launches) {
   lhcb_ctx* c = p->ctx;
   cudaStream_t s = p->st_k;
+  *launches = (has_ut && strips) ? 1 : 0;
   if (has_ut && strips)                                      // the slice's UT hits arrived as strip numbers
     lhcb::ut_decode_kernel<<<296, 256, 0, s>>>(p->ut_off + (size_t)e0 * 4, p->ut_off + (size_t)(e0 + ne) * 4, p->ustrip, p->ux,
                                                c->geom.ut_strip_x0, c->geom.ut_strip_pitch);
@@ -526,10 +544,13 @@ int enqueue_slice(lhcb_pipeline* p, int k, int e0, int ne, bool has_ut, bool has
   lhcb_long_t dev_l = {p->l_count, p->l_seed, p->l_velo, p->l_ut, p->l_nut, p->l_qop, p->l_chi2, p->l_status, nullptr};
   int rc = lhcb_order(c, &dev_ev, &dev_v, has_ut ? &dev_u : nullptr, p->order_ws, s);
   if (rc != LHCB_OK) return rc;
+  *launches += c->last_launches;                             // 0 for a slice above kOrderMaxSorted events
   rc = lhcb_seeding(c, &dev_ev, &dev_s, p->order_ws, s);
   if (rc != LHCB_OK) return rc;
+  *launches += c->last_launches;
   rc = lhcb_matching(c, &dev_s, &dev_v, has_ut ? &dev_u : nullptr, &dev_l, p->order_ws, s);
   if (rc != LHCB_OK) return rc;
+  *launches += c->last_launches + 2;                         // + the two compaction kernels below
   lhcb::CompactParams q;
   std::memset(&q, 0, sizeof(q));
   q.n_events = ne; q.max_seeds = c->geom.max_seeds_per_half; q.max_long = c->geom.max_long_per_event;
@@ -721,7 +742,7 @@ int lhcb_reconstruct_host(lhcb_pipeline* p, const lhcb_events_t* ev, const lhcb_
       cudaGraph_t graph = nullptr;
       ce = cudaStreamBeginCapture(p->st_k, cudaStreamCaptureModeThreadLocal);
       if (ce != cudaSuccess) break;
-      rc = enqueue_slice(p, k, e0, ne, has_ut, has_pol, want_par, strips);
+      rc = enqueue_slice(p, k, e0, ne, has_ut, has_pol, want_par, strips, &G.launches);
       const cudaError_t ec = cudaStreamEndCapture(p->st_k, &graph);
       if (rc != LHCB_OK) { if (graph) cudaGraphDestroy(graph); break; }
       ce = ec;
@@ -733,7 +754,7 @@ int lhcb_reconstruct_host(lhcb_pipeline* p, const lhcb_events_t* ev, const lhcb_
     ce = cudaStreamWaitEvent(p->st_k, p->ev_in[k], 0);
     if (ce == cudaSuccess) ce = cudaGraphLaunch(G.exec, p->st_k);
     if (ce == cudaSuccess) ce = cudaEventRecord(p->ev_k[k], p->st_k);
-    p->launches += strips ? 6 : 5;                           // (strip decoding,) order, seeding, matching, scan, gather
+    p->launches += G.launches;                               // (strip decoding,) order, seeding, matching, scan, gather: counted at capture
   }
   // ---- outputs: as soon as a slice's totals are known, exactly its entries are copied
   uint32_t seeds_end = 0, long_end = 0;

@@ -30,7 +30,9 @@ __device__ __forceinline__ int order_bucket(uint32_t w, int shift) {
 constexpr int kOrderPerThread = 32;   // weights a thread keeps in registers between the two passes
 constexpr int kOrderMaxSorted = 3072; // batches above this many events run without the workspace (host decision, lhcb_api.cu)
 
-// one CTA.  seed_order[2 n_events], match_order[n_events] (either may be NULL), done[2 n_events].
+// one CTA.  seed_order[2 n_events], match_order[n_events] (either may be NULL), done[2 n_events].  Without UT
+// offsets and without VELO offsets there is nothing to weigh the events by: match_order is then the identity, so
+// that a workspace this kernel has filled is valid for lhcb_matching whatever lhcb_order was given.
 // Up to 32 halves per thread (32,768 halves: the 16,384-event batch) are loaded once, all loads in flight
 // together, and kept in registers for the scatter pass; larger batches take a plain two-pass loop.
 __global__ void __launch_bounds__(kOrderThreads)
@@ -44,6 +46,10 @@ order_kernel(int n_events, const uint32_t* __restrict__ zone_off, const uint32_t
   // "seeds are in global memory" flags: up unless a Seeding run lowers them (a Matching on given seeds passes)
   for (int h = tid; h < nh; h += kOrderThreads) done[h] = 1u;
   const bool fast = nh <= kOrderThreads * kOrderPerThread;
+  if (match_order && !ut_off && !velo_off) {
+    for (int e = tid; e < n_events; e += kOrderThreads) match_order[e] = (uint32_t)e;
+    match_order = nullptr;                                  // nothing to sort
+  }
   auto seed_w = [&](int h) { return zone_off[(size_t)h * 12 + 12] - zone_off[(size_t)h * 12]; };
   auto match_w = [&](int e) {
     return ut_off ? ut_off[(size_t)e * 4 + 4] - ut_off[(size_t)e * 4] : 32u * (velo_off[e + 1] - velo_off[e]);

@@ -408,7 +408,13 @@ seeding_kernel(const __grid_constant__ SeedParams p) {
 #pragma unroll
   for (int z = 0; z < 12; ++z) zone_too_big |= zoff[z + 1] - zoff[z] >= (1u << kZoneIndexBits);
   if (n_half > p.max_hits || zone_too_big) {               // uniform: whole CTA leaves
-    if (tid == 0) { p.count[half_id] = 0; p.status[half_id] = LHCB_ST_HITS_OVERFLOW; }
+    if (tid == 0) {
+      p.count[half_id] = 0; p.status[half_id] = LHCB_ST_HITS_OVERFLOW;
+      if (p.done) {                                          // published like every other exit: a dependent Matching CTA reads them
+        __threadfence();
+        asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p.done + half_id), "r"(1u) : "memory");
+      }
+    }
     return;
   }
   const int off_w = off_hits + (int)seed_tile_bytes(n_half);   // work region W: from the end of the tile to the first candidate slot

@@ -39,6 +39,26 @@ def test_pipeline_output_equals_oracle(nominal):
     c.close()
 
 
+def test_pipeline_2048_events_last_slice_cut_in_three():
+    """One slice of 2,048 events is the whole batch and therefore the last one: it is cut into pieces of 1,024, 512
+    and 512 events (the shape of the tail of the batch bench.py times), each with its own graph, order and
+    dependent Matching launch.  Seeds and long tracks of all 2,048 events against the oracle."""
+    from paper_2606_14480_b200 import Context, HostPipeline, capacities
+    ev = generate(config(2, 2048), workers=8)
+    c = Context(capacities.with_capacities(ev.geom))
+    pipe = HostPipeline(c, ev, slice_events=2048, want_par=True)
+    for rep in range(2):
+        _, _, launches = pipe.lhcb_reconstruct_host()
+    assert launches == 3 * 6                                             # strip decoding, order, seeding, matching, scan, gather
+    gs, gl = pipe.seeds_to_host(), pipe.long_to_host()
+    assert not gs["status"].any() and not gl["status"].any()
+    os_, om, _ = reconstruct_parallel(ev)
+    n_s, n_l = assert_batch_identical(os_, om, gs, gl, "pipeline, 2,048 events in 1,024 + 512 + 512")
+    assert n_s > 150 * 2048 and n_l > 90 * 2048
+    pipe.close()
+    c.close()
+
+
 def test_pipeline_reports_dense_capacity():
     from paper_2606_14480_b200 import Context, HostPipeline
     ev = generate(config(2, 8))
