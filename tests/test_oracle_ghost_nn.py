@@ -112,3 +112,72 @@ def test_selection_equals_the_literal_rule_of_L348():
     # without the network the chi2 ranking (A14) is unchanged
     m0 = o.matching(ev.n_events, seed_off, s["state"], ev, use_ut=True)
     assert "ghost" not in m0 and m0["n"] > 0
+
+
+def literal_selection(allc, cut, margin):
+    """PAPER.md L348 word for word, in float32: kept if "smaller than" the cut; removed if another kept track with
+    the same seed or the same VELO segment has a ghost probability "at least" `margin` lower."""
+    p = allc["ghost"].astype(np.float32)
+    kept = p < np.float32(cut)
+    out = set()
+    for i in np.flatnonzero(kept):
+        share = kept & ((allc["seed"] == allc["seed"][i]) | (allc["velo"] == allc["velo"][i]))
+        share[i] = False
+        if not (p[i] >= (p[share] + np.float32(margin)).astype(np.float32)).any():
+            out.add((int(allc["seed"][i]), int(allc["velo"][i])))
+    return out
+
+
+def exact_edge_cases(allc):
+    """From the unfiltered candidates: (i, cut) with cut = candidate i's own probability, and (i, j, margin) with
+    i and j sharing a segment, p_j < p_i <= 2 p_j (so that p_i - p_j and p_j + (p_i - p_j) are exact in float32:
+    the sum lands exactly on p_i), every other competitor of i being too high to matter."""
+    p = allc["ghost"].astype(np.float32)
+    i_cut = int(np.argsort(p)[len(p) // 2])
+    for i in range(allc["n"]):
+        share = (allc["seed"] == allc["seed"][i]) | (allc["velo"] == allc["velo"][i])
+        share[i] = False
+        js = np.flatnonzero(share)
+        if len(js) == 0:
+            continue
+        j = int(js[np.argmin(p[js])])
+        if not (p[j] < p[i] <= 2 * p[j]):
+            continue
+        m = np.float32(p[i] - p[j])
+        others = js[js != j]
+        if np.float32(p[j] + m) == p[i] and (np.float32(1) * (p[others] + m) > p[i]).all():
+            return i_cut, p[i_cut], i, j, m
+    raise AssertionError("no pair of candidates for the margin edge")
+
+
+def test_cut_is_strict_and_margin_is_inclusive_on_exact_float32_edges():
+    """ghost probability "smaller than 0.8" (a track AT the cut is dropped) and "at least 0.05
+    higher" (a track EXACTLY the margin above its competitor is removed).  Cut and margin are inputs, so both
+    edges can be hit exactly: the cut is set to a candidate's own probability, the margin to the float32
+    difference of two candidates that share a segment."""
+    ev = generate(config(2, 12))
+    o = Oracle(ev.geom, "f32")
+    # the flat network of the test above: probabilities squeezed around 1/2, so that tracks sharing a segment are
+    # within a factor two of each other
+    w = ghost_nn(); w[304:336] *= 0.02; w[336] = 0.0
+    open_w = w.copy(); open_w[337] = np.inf; open_w[338] = np.inf
+    _, _, _, allc = run(o, ev, open_w)
+    i_cut, p_cut, i, j, m = exact_edge_cases(allc)
+    key = lambda k: (int(allc["seed"][k]), int(allc["velo"][k]))
+    sel_of = lambda r: set(zip(r["seed"].tolist(), r["velo"].tolist()))
+    # the cut: at the candidate's own probability it is dropped, one float32 step above it is kept
+    for cut, kept in ((p_cut, False), (np.nextafter(p_cut, np.float32(2)), True)):
+        nn = w.copy(); nn[337] = cut; nn[338] = np.inf
+        got = sel_of(run(o, ev, nn)[3])
+        assert (key(i_cut) in got) == kept, (cut, kept)
+        assert got == literal_selection(allc, cut, np.inf)
+    # the margin: exactly p_i - p_j removes i, the next margin that lifts the sum past p_i keeps it (no other competitor of
+    # i is that low)
+    pi, pj = np.float32(allc["ghost"][i]), np.float32(allc["ghost"][j])
+    m_above = np.float32(np.nextafter(pi, np.float32(2)) - pj)        # the smallest margin whose float32 sum with p_j exceeds p_i
+    for margin, kept in ((m, False), (m_above, True)):
+        assert (np.float32(pj + np.float32(margin)) > pi) == kept
+        nn = w.copy(); nn[337] = np.inf; nn[338] = margin
+        got = sel_of(run(o, ev, nn)[3])
+        assert (key(i) in got) == kept and key(j) in got, (margin, kept)
+        assert got == literal_selection(allc, np.inf, margin)

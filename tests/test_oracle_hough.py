@@ -181,3 +181,47 @@ def test_hough_seed_invariants():
     assert e_h > 0.93 and abs(e_h - e_i) < 0.03
     # the x-z part is untouched by the choice of the UV version
     assert {tuple(h[X_LAYERS]) for h in s["hits"]} <= {tuple(c) for c in it["hits"][:, X_LAYERS]} | {tuple(h[X_LAYERS]) for h in s["hits"]}
+
+
+def hough_cap_event(n_decoys, decoy_layers=(1, 2, 5, 6, 9, 10)):
+    """One x-z track in the upper half whose true stereo hits sit in the middle of t_y bin 40, plus `n_decoys`
+    decoy clusters at lower t_y (bins 2+4i and 3+4i).  A decoy has one hit per layer of `decoy_layers`, alternately
+    0.3 bins above the lower edge of its first bin and 0.3 bins below the upper edge of its second bin: every one of
+    those layers votes for the cluster, but a straight line of fixed t_y (the four hypotheses of a cluster, L217) is
+    within 2 mm of at most half of the hits (a bin is 3.4-4.1 mm wide at the stereo layers), fewer than min_uv_hits:
+    a decoy takes one of the "up to eight" places and yields no seed.  The true hits vote in bin 40 only, so the
+    clusters (39, 40) and (40, 41) both have all six layers; (39, 40) comes first.  Returns (event, true hit indices)."""
+    from tests.test_oracle_readings import make_event, track_hits, xz_track
+    zmin = Z[UV_LAYERS].min(); tol = abs(G["y_half_tol"])
+    tlo = -tol / zmin; w = (G["y_max"] + tol) / zmin / 64.0
+    t_of = lambda b: tlo + b * w
+    par = xz_track(p=16000.0, q=-1, tx0=0.01)
+    hits = track_hits(par, lambda z: t_of(40.5) * z)
+    n_true = len(hits)
+    for i in range(n_decoys):
+        b = 2 + 4 * i
+        lo = track_hits(par, lambda z: t_of(b + 0.3) * z); hi = track_hits(par, lambda z: t_of(b + 1.7) * z)
+        for k, l in enumerate(UV_LAYERS):
+            if l in decoy_layers:
+                hits.append((lo if k % 2 == 0 else hi)[l])
+    ev, idx = make_event(hits)
+    return ev, sorted(idx[k] for k in range(n_true))
+
+
+def test_hough_takes_up_to_eight_clusters_most_populated_first_then_lower_ty():
+    """"Up to eight of the best bins" (reading A20: most voting layers first, then lower t_y).
+    With seven six-layer decoy clusters below it the true cluster is the eighth and is seeded; with eight it is the
+    ninth and is not; with eight five-layer decoys it ranks first again."""
+    for mode in ("f64", "f32"):
+        o = Oracle(G, mode); o.set_uv_hough(True)
+        ev, true_hits = hough_cap_event(7)
+        s = o.seeding(ev)
+        assert s["n"] == 1 and s["nuv"][0] == 6 and sorted(int(h) for h in s["hits"][0]) == true_hits, (mode, s["n"])
+        ev, _ = hough_cap_event(8)
+        assert o.seeding(ev)["n"] == 0, mode
+        ev, true_hits = hough_cap_event(8, decoy_layers=(1, 2, 5, 6, 9))
+        s = o.seeding(ev)
+        assert s["n"] == 1 and sorted(int(h) for h in s["hits"][0]) == true_hits, mode
+        # the iterative version has no such cap: it seeds the track whatever the decoys
+        it = Oracle(G, mode).seeding(hough_cap_event(8)[0])
+        assert it["n"] == 1

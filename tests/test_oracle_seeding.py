@@ -78,6 +78,29 @@ def test_triplets_equal_brute_force(cfgname, oracle32, cfg1_events, cfg2_small, 
     assert total > 500
 
 
+def test_triplets_equal_brute_force_with_an_asymmetric_band(cfg2_small):
+    """PAPER.md L175 ("one side exhibits a longer tail"; reading A4): the additive widths of the c_x band differ on
+    its two sides.  The default geometry has d_lo = d_hi, which hides a swap; here d_lo = 0.5e-6, d_hi = 2e-6."""
+    from lhcb_gen import default_geom
+    from oracle.binding import Oracle
+    g = default_geom(cx_band=[0.5, 1.8, 0.5e-6, 2.0e-6])
+    o = Oracle(g, "f32")
+    ev = cfg2_small
+    total = n_sym = 0
+    for event in range(2):
+        for half in (0, 1):
+            d = o.seeding_debug(ev, event, half)
+            got = {(int(i), *map(int, t)) for i, t in zip(d["t_it"], d["t_idx"][:, [0, 1, 2]])}
+            sure, edge = brute_triplets(ev, g, event, half)
+            assert sure <= got, "oracle misses triplets the cuts accept"
+            assert got <= (sure | edge), "oracle accepts triplets outside the cuts"
+            # the same cuts with the two widths swapped accept a different set: the asymmetry is exercised
+            swapped, _ = brute_triplets(ev, dict(g, cx_band=[0.5, 1.8, 2.0e-6, 0.5e-6]), event, half)
+            n_sym += len(sure ^ swapped)
+            total += len(got)
+    assert total > 500 and n_sym > 50
+
+
 # ----------------------------------------------------------------------------- O5 exact parabola
 def test_parabola3_is_lagrange_when_dratio_zero():
     g = default_geom(d_ratio=0.0)
