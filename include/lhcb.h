@@ -44,10 +44,11 @@ typedef enum {
 } lhcb_status;
 
 /* bits of the per-half / per-event `status` output words */
-#define LHCB_ST_TRIPLET_OVERFLOW 1u   /* more three-hit combinations than max_triplets_per_half */
+#define LHCB_ST_TRIPLET_OVERFLOW 1u   /* more three-hit combinations than max_triplets_per_half, or more two-hit work items in one
+                                         tile of T1 hits than 4*max_xz_cand_per_half */
 #define LHCB_ST_CAND_OVERFLOW 2u      /* more x-z candidates (>= min_x_hits) than max_xz_cand_per_half */
 #define LHCB_ST_SEED_OVERFLOW 4u      /* more seeds than max_seeds_per_half */
-#define LHCB_ST_HITS_OVERFLOW 8u      /* event-half has more hits than max_hits_per_half: half skipped */
+#define LHCB_ST_HITS_OVERFLOW 8u      /* event-half has more hits than max_hits_per_half, or one of its zones 1,024 or more: half skipped */
 #define LHCB_ST_MATCH_OVERFLOW 16u    /* more chi2-accepted pairs than max_match_cand_per_event */
 #define LHCB_ST_LONG_OVERFLOW 32u     /* more long tracks than max_long_per_event */
 #define LHCB_ST_VELO_OVERFLOW 64u     /* more VELO tracks than max_velo_per_event: event skipped */
@@ -89,9 +90,14 @@ typedef struct {
   int32_t min_ut_hits, ut_enabled;             /* 3 (L311); 0 disables the UT search (L307) */
   /* capacities; 0 selects the default in brackets */
   int32_t max_seeds_per_half;                  /* [256]  output slots per event-half */
-  int32_t max_xz_cand_per_half;                /* [1024] fitted x-z candidates per event-half */
+  int32_t max_xz_cand_per_half;                /* [1024] fitted x-z candidates per event-half.  The same region first holds the work
+                                                  items of the two-hit search: the T3 windows of one tile of T1 hits (one hit per
+                                                  thread of the CTA), cut into runs of four T3 hits, may not number more than
+                                                  4*max_xz_cand_per_half per iteration, else LHCB_ST_TRIPLET_OVERFLOW */
   int32_t max_long_per_event;                  /* [256]  output slots per event */
-  int32_t max_hits_per_half;                   /* [6144] SciFi hits staged per event-half (<= 8000) */
+  int32_t max_hits_per_half;                   /* [6144] SciFi hits staged per event-half (<= 8000).  Whatever this value, a single
+                                                  (half, layer) zone may hold at most 1,023 hits (zone-local indices are packed in
+                                                  10 bits): a half with a larger zone is skipped with LHCB_ST_HITS_OVERFLOW */
   int32_t max_triplets_per_half;               /* [4096] three-hit combinations per half, both iterations together (the queue also takes the
                                                   room a half leaves unused below max_hits_per_half) */
   int32_t max_match_cand_per_event;            /* [384]  chi2-accepted seed-VELO pairs per event */

@@ -20,6 +20,7 @@ def _run(args):
     from lhcb_gen import slice_events
     from oracle.binding import Oracle
     ev, mode, use_ut, hough, direct = _JOB["ev"], _JOB["mode"], _JOB["use_ut"], _JOB["hough"], _JOB["direct"]
+    nn = _JOB.get("nn")
     sub = slice_events(ev, a, b)
     o = Oracle(ev.geom, mode)
     if hough:
@@ -27,21 +28,28 @@ def _run(args):
     t = time.perf_counter()
     if direct:
         s = None
-        m = o.matching(sub.n_events, sub.seed_off, sub.seed_state.T, sub, use_ut=use_ut)
+        m = o.matching(sub.n_events, sub.seed_off, sub.seed_state.T, sub, use_ut=use_ut, nn=nn)
+    elif nn is not None:                                     # final selection by the ghost network (A14b), on the oracle's own seeds
+        s = o.seeding(sub)
+        seed_off = np.zeros(sub.n_events + 1, np.uint32)
+        np.cumsum(np.bincount(s["event"], minlength=sub.n_events), out=seed_off[1:])
+        m = o.matching(sub.n_events, seed_off, s["state"], sub, use_ut=use_ut, nn=nn,
+                       nhits=(s["nx"] + s["nuv"]).astype(np.uint8))
     else:
         s, m = o.reconstruct(sub, use_ut=use_ut)
     return a, b, s, m, time.perf_counter() - t
 
 
 def reconstruct_parallel(ev, workers: int | None = None, mode: str = "f32", use_ut: bool = True, hough: bool = False,
-                         direct_seeds: bool = False, shard_events: int | None = None):
+                         direct_seeds: bool = False, shard_events: int | None = None, nn=None):
     """(seeds, long tracks, info) of the whole batch; seeds is None for direct seeds (BASELINE.json configs[4]).
-    info: workers, wall seconds, summed CPU seconds, merged step counters."""
+    info: workers, wall seconds, summed CPU seconds, merged step counters.
+    nn: the 339 packed values of the ghost-killing network (reading A14b; long tracks then carry "ghost") or None."""
     workers = max(1, workers or os.cpu_count() or 1)
     n = ev.n_events
     shard = shard_events or max(1, -(-n // (workers * 4)))
     jobs = [(a, min(a + shard, n)) for a in range(0, n, shard)]
-    _JOB.update(ev=ev, mode=mode, use_ut=use_ut, hough=hough, direct=direct_seeds)
+    _JOB.update(ev=ev, mode=mode, use_ut=use_ut, hough=hough, direct=direct_seeds, nn=nn)
     t0 = time.perf_counter()
     if workers > 1 and len(jobs) > 1:
         with mp.get_context("fork").Pool(min(workers, len(jobs))) as pool:
@@ -81,6 +89,6 @@ def reconstruct_parallel(ev, workers: int | None = None, mode: str = "f32", use_
         out["n"] = int(sum(p["n"] for p in parts_))
         return out
     S = cat(seeds, ["event", "half", "state", "par", "hits", "nx", "nuv"]) if seeds else None
-    M = cat(longs, ["event", "seed", "velo", "ut", "n_ut", "qop", "chi2"])
+    M = cat(longs, ["event", "seed", "velo", "ut", "n_ut", "qop", "chi2"] + (["ghost"] if nn is not None else []))
     info = dict(workers=min(workers, len(jobs)), wall_s=wall, cpu_s=float(sum(p[4] for p in parts)), counters=counters)
     return S, M, info

@@ -92,7 +92,8 @@ def assert_batch_identical(orc_s, orc_m, gpu_s, gpu_m, what=""):
     po, pg = np.lexsort(lo.T[::-1]), np.lexsort(lg.T[::-1])
     assert lo.shape == lg.shape, (what, "long-track counts differ", lo.shape, lg.shape)
     assert np.array_equal(lo[po], lg[pg]), (what, "long tracks differ")
-    for name in ("qop", "chi2"):
+    names = ("qop", "chi2") + (("ghost",) if "ghost" in orc_m and gpu_m.get("ghost") is not None else ())
+    for name in names:
         a = np.ascontiguousarray(orc_m[name][po], np.float32).view(np.uint32)
         b = np.ascontiguousarray(gpu_m[name][pg], np.float32).view(np.uint32)
         assert np.array_equal(a, b), (what, name, "not bit-identical")

@@ -117,3 +117,112 @@ def test_hand_built_tracks_of_the_cpu_pins(geom, oracle32):
     os_, om = check(ctx, oracle32, ev, use_ut=False)
     assert os_["n"] >= n - 1
     ctx.close()
+
+
+def _grow_zone(ev, event, half, layer, n_target, rng):
+    """The batch with noise hits added to one (event, half, layer) zone until it holds n_target hits."""
+    z = (event * 2 + half) * 12 + layer
+    zo = ev.zone_off.astype(np.int64)
+    b, e = int(zo[z]), int(zo[z + 1])
+    add = n_target - (e - b)
+    assert add > 0
+    extra = rng.uniform(-2900.0, 2900.0, add).astype(np.float32)
+    x = np.concatenate([ev.hit_x[b:e], extra])
+    o = np.argsort(x, kind="stable")
+    ins = lambda a, new: np.concatenate([a[:b], np.concatenate([a[b:e], new])[o], a[e:]])
+    zo2 = zo.copy(); zo2[z + 1:] += add
+    return replace(ev, zone_off=zo2.astype(np.uint32), hit_x=ins(ev.hit_x, extra),
+                   hit_x64=ins(ev.hit_x64, extra.astype(np.float64)), hit_pid=ins(ev.hit_pid, np.full(add, -1, ev.hit_pid.dtype)))
+
+
+def test_zone_of_1023_hits_is_searched_and_1024_is_reported(geom, oracle32):
+    """include/lhcb.h, max_hits_per_half: zone-local hit indices are packed in 10 bits, so a single (half, layer) zone
+    may hold at most 1,023 hits even when the half as a whole fits.  At 1,023 the half is reconstructed like any
+    other; at 1,024 it is skipped with LHCB_ST_HITS_OVERFLOW (count 0), and every other half is untouched."""
+    from paper_2606_14480_b200 import Context, DeviceEvents
+    base = generate(config(2, 4))
+    E, H, L = 2, 1, 5                                        # a stereo layer of the lower half of event 2
+    ctx = Context(geom)
+    for n_zone in (1023, 1024):
+        ev = _grow_zone(base, E, H, L, n_zone, np.random.default_rng(5))
+        dev = DeviceEvents.from_host(ev)
+        s = ctx.lhcb_seeding(dev)
+        gs = ctx.seeds_to_host(s)
+        os_, _ = oracle32.reconstruct(ev, use_ut=False)
+        want_status = np.zeros(8, np.uint32)
+        if n_zone == 1024:
+            want_status[E * 2 + H] = 8
+            keep = ~((os_["event"] == E) & (os_["half"] == H))
+            assert (~keep).sum() > 50                        # the oracle has no such limit and does find seeds there
+            os_ = {k: (v[keep] if isinstance(v, np.ndarray) and len(v) == len(keep) else v) for k, v in os_.items()}
+            assert int(s["count"].cpu().numpy()[E * 2 + H]) == 0
+        assert np.array_equal(gs["status"], want_status), gs["status"]
+        r = compare_seeds(os_, gs)
+        assert r["n_orc"] == r["n_gpu"] == r["n_common"] and r["bit_equal"], r
+    ctx.close()
+
+
+def batch_of(singles, geom):
+    """Single-event objects of the CPU pins (tests.test_oracle_readings.make_event) as one batch without VELO / UT."""
+    from types import SimpleNamespace
+    zo, hx = [0], []
+    for e in singles:
+        zo += [int(v) + len(hx) for v in e.zone_off[1:]]
+        hx += [float(v) for v in e.hit_x64]
+    n = len(singles)
+    z = lambda: np.zeros(0, np.float32)
+    return SimpleNamespace(n_events=n, n_hits=len(hx), zone_off=np.array(zo, np.uint32), hit_x=np.array(hx, np.float32),
+                           hit_x64=np.array(hx, np.float64), polarity=np.full(n, -1, np.int8), geom=geom,
+                           velo_off=np.zeros(n + 1, np.uint32), velo_x=z(), velo_y=z(), velo_tx=z(), velo_ty=z(),
+                           ut_off=np.zeros(4 * n + 1, np.uint32), ut_x0=z(), ut_ylo=z(), ut_yhi=z(), ut_row=None)
+
+
+def test_hough_cluster_cap_events(geom):
+    """The three hand-built events of tests/test_oracle_hough.py that pin "up to eight of the best bins" (PAPER.md
+    L217): the true cluster eighth (seeded), ninth (not seeded), and first again behind eight five-layer decoys."""
+    from oracle.binding import Oracle
+    from paper_2606_14480_b200 import Context, capacities
+    from tests.test_oracle_hough import hough_cap_event
+    ev = batch_of([hough_cap_event(7)[0], hough_cap_event(8)[0], hough_cap_event(8, decoy_layers=(1, 2, 5, 6, 9))[0]], geom)
+    o = Oracle(geom, "f32"); o.set_uv_hough(True)
+    for g in (geom, capacities.with_capacities(geom, capacities.NOMINAL_HOUGH)):
+        ctx = Context(g)
+        ctx.lhcb_set_uv_hough(True)
+        os_, _ = check(ctx, o, ev, use_ut=False)
+        assert sorted(os_["event"].tolist()) == [0, 2]
+        ctx.close()
+
+
+def test_ghost_cut_and_margin_exact_edges(oracle32):
+    """PAPER.md L348 on exact float32 edges, as in tests/test_oracle_ghost_nn.py: cut = a candidate's own ghost
+    probability (dropped: "smaller than"), margin = the exact difference of two candidates sharing a segment (the
+    higher one removed: "at least"), and one step beyond each.  The kernel must take the same side as the oracle."""
+    from lhcb_gen import ghost_nn
+    from paper_2606_14480_b200 import Context, DeviceEvents
+    from tests.test_oracle_ghost_nn import exact_edge_cases, run
+    ev = generate(config(2, 12))
+    w = ghost_nn(); w[304:336] *= 0.02; w[336] = 0.0
+    open_w = w.copy(); open_w[337] = np.inf; open_w[338] = np.inf
+    os_, seed_off, nhits, allc = run(oracle32, ev, open_w)
+    i_cut, p_cut, i, j, m = exact_edge_cases(allc)
+    pi, pj = np.float32(allc["ghost"][i]), np.float32(allc["ghost"][j])
+    ctx = Context(ev.geom)
+    dev = DeviceEvents.from_host(ev)
+    s = ctx.lhcb_seeding(dev)
+    gs = ctx.seeds_to_host(s)
+    ok = dict(zip(range(os_["n"]), seed_keys(os_["event"], os_["half"], os_["hits"], os_["state"])))
+    gk = dict(zip((int(x) for x in gs["slot"]), seed_keys(gs["event"], gs["half"], gs["hits"], gs["state"])))
+    n_sel = []
+    for cut, margin in ((p_cut, np.inf), (np.nextafter(p_cut, np.float32(2)), np.inf), (np.inf, m),
+                        (np.inf, np.float32(np.nextafter(pi, np.float32(2)) - pj))):
+        nn = w.copy(); nn[337] = cut; nn[338] = margin
+        om = oracle32.matching(ev.n_events, seed_off, os_["state"], ev, use_ut=True, nn=nn, nhits=nhits)
+        ctx.lhcb_set_ghost_nn(nn)
+        gl = ctx.long_to_host(ctx.lhcb_matching(s, dev, use_ut=True))
+        assert (gl["status"] == 0).all()
+        rl = compare_long(om, gl, ok, gk)
+        assert rl["n_orc"] == rl["n_gpu"] == rl["n_common"] and rl["bit_equal"], (cut, margin, rl["only_orc"], rl["only_gpu"])
+        n_sel.append(rl["n_common"])
+    assert n_sel[1] == n_sel[0] + 1 or n_sel[1] > n_sel[0]     # the candidate at the cut comes back one step higher
+    assert n_sel[3] > n_sel[2]                                  # ... and the one exactly the margin above its competitor
+    ctx.close()

@@ -68,3 +68,23 @@ def test_pipeline_reports_dense_capacity():
         pipe.lhcb_reconstruct_host()
     pipe.close()
     c.close()
+
+
+def test_pipeline_cfg3_16384_events_in_the_shape_bench_times(cfg3_full):
+    """lhcb_reconstruct_host on the whole cfg3 batch exactly as bench.py's end-to-end leg runs it: NOMINAL
+    capacities, slices of 2,048 events (order + seeding + dependent matching + compaction in one graph per slice,
+    the last slice cut into 1,024 + 512 + 512), strips shipped as numbers.  Dense seeds and long tracks of all
+    16,384 events against the oracle."""
+    from paper_2606_14480_b200 import Context, HostPipeline, capacities
+    ev, (os_, om, _) = cfg3_full
+    c = Context(capacities.with_capacities(ev.geom))
+    pipe = HostPipeline(c, ev, slice_events=2048, want_par=True)
+    for rep in range(2):
+        _, _, launches = pipe.lhcb_reconstruct_host()
+    assert launches == 10 * 6                                            # seven full slices + three pieces
+    gs, gl = pipe.seeds_to_host(), pipe.long_to_host()
+    assert not gs["status"].any() and not gl["status"].any()
+    n_s, n_l = assert_batch_identical(os_, om, gs, gl, "pipeline, cfg3 in 2,048-event slices")
+    assert n_s > 170 * 16384 and n_l > 100 * 16384
+    pipe.close()
+    c.close()
