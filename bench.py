@@ -312,11 +312,11 @@ def main():
     value = world * n / (ms_per_step * 1e-3)
     clocks = clocks_summary(samples)
 
-    # ---- smaller batches (BASELINE.json configs[2]: 1,024 / 4,096 / 16,384 on one stream) -------------
+    # ---- smaller batches (BASELINE.json configs[2]: 1,024 / 4,096 / 16,384 on one stream; 2,048 = a slice of the host pipeline) -------------
     batches = {}
     if rank == 0:
         from lhcb_gen import slice_events
-        for nb in (1024, 4096):
+        for nb in (1024, 2048, 4096):
             if nb >= n:
                 continue
             sub = DeviceEvents.from_host(slice_events(ev, 0, nb), f"cuda:{local_rank}")
@@ -473,8 +473,21 @@ def main():
     except Exception:
         pass
     hbm_peak = peaks.get("hbm_gbs", 6650.0)
-    roofline = {"bound": "alu", "kernel": "seeding_kernel", "achieved": achieved / 1e12, "peak": peak / 1e12,
-                "unit": "Tlane-op/s", "frac": achieved / peak,
+    # ... and the shared-memory bandwidth its searches need (third row): whichever fraction is larger binds
+    smem_bytes = 4.0 * workmodel.smem_probe_loads(cnt, mean_zone)
+    smem_peak = workmodel.smem_peak(1965.0)
+    smem_ach = smem_bytes * n / seed_t
+    alu = {"achieved": achieved / 1e12, "peak": peak / 1e12, "unit": "Tlane-op/s", "frac": achieved / peak}
+    smem = {"algorithmic_bytes_per_event": smem_bytes, "achieved_tbs": smem_ach / 1e12, "peak_tbs": smem_peak / 1e12,
+            "frac": smem_ach / smem_peak, "unit": "TB/s",
+            "peak_source": "148 SM x 128 B/clk x 1965 MHz",
+            "model": "4-byte probe loads under the binary-search model of workmodel.smem_probe_loads, from the same oracle counters"}
+    binds_smem = smem["frac"] > alu["frac"]
+    roofline = {"bound": "smem" if binds_smem else "alu", "kernel": "seeding_kernel",
+                "achieved": smem["achieved_tbs"] if binds_smem else alu["achieved"],
+                "peak": smem["peak_tbs"] if binds_smem else alu["peak"],
+                "unit": smem["unit"] if binds_smem else alu["unit"],
+                "frac": max(smem["frac"], alu["frac"]), "alu": alu, "smem": smem,
                 "traffic": workmodel.NCU_DRAM_BYTES_PER_LAUNCH["seeding_kernel"] if n == 16384 else None,
                 "traffic_source": workmodel.NCU_DRAM_SOURCE,
                 "counters": "oracle step counters of this run's cpu_baseline leg (%d events)" % cpu["counters_events"],

@@ -28,7 +28,10 @@ __device__ __forceinline__ int order_bucket(uint32_t w, int shift) {
 }
 
 constexpr int kOrderPerThread = 32;   // weights a thread keeps in registers between the two passes
-constexpr int kOrderMaxSorted = 3072; // batches above this many events run without the workspace (host decision, lhcb_api.cu)
+#ifndef LHCB_ORDER_MAX_SORTED
+#define LHCB_ORDER_MAX_SORTED 3072
+#endif
+constexpr int kOrderMaxSorted = LHCB_ORDER_MAX_SORTED; // batches above this many events run without the workspace (host decision, lhcb_api.cu)
 
 // one CTA.  seed_order[2 n_events], match_order[n_events] (either may be NULL), done[2 n_events].  Without UT
 // offsets and without VELO offsets there is nothing to weigh the events by: match_order is then the identity, so

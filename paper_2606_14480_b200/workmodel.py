@@ -13,8 +13,8 @@ import math
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the 16,384-event cfg3 batch, from the
 # `ncu --set full` capture summarised in profiles/ (the bench cannot measure DRAM traffic itself)
-NCU_DRAM_BYTES_PER_LAUNCH = {"seeding_kernel": 273.200128e6 + 251.460096e6, "matching_kernel": 372.667648e6 + 48.049664e6}
-NCU_DRAM_SOURCE = "profiles/r2a_ncu_full.md"
+NCU_DRAM_BYTES_PER_LAUNCH = {"seeding_kernel": 273.247488e6 + 250.793472e6, "matching_kernel": 372.664320e6 + 47.819776e6}
+NCU_DRAM_SOURCE = "profiles/r3_ncu_full.md"
 
 N_SM = 148
 LANES_PER_SM = 128
@@ -38,6 +38,22 @@ def lane_ops(counters: dict, mean_zone: float = CFG3_MEAN_ZONE, mean_ut_zone: fl
                + counters["y_fits"] * 60)
     matching = counters["sv_pairs"] * 45 + counters["ut_steps"] * (15 + lgu)
     return seeding, matching
+
+
+def smem_probe_loads(counters: dict, mean_zone: float = CFG3_MEAN_ZONE):
+    """Algorithmic 4-byte shared-memory loads of the Seeding per event (third roofline row), under
+    the same binary-search model as lane_ops: a search costs ceil(log2 zone) probes, a window costs the hits it
+    holds.  Per T1 hit its x and two searches (Eq. 11); per pair the T3 hit and two searches (band of Eq. 12-14);
+    per triplet the T2 hit and three closest-hit searches (+-1 mm, one more load for the neighbour compared);
+    per first-layer stereo hit its x and five closest-hit searches (+-2 mm)."""
+    lg = math.ceil(math.log2(max(mean_zone, 2.0)))
+    return (counters["t1_hits"] * (1 + 2 * lg) + counters["pairs"] * (1 + 2 * lg)
+            + counters["triplets"] * (1 + 3 * (lg + 1)) + counters["uv_first"] * (1 + 5 * (lg + 1)))
+
+
+def smem_peak(sm_mhz: float) -> float:
+    """bytes per second: 148 SMs x 128 B per clock (32 banks x 4 B) x SM clock."""
+    return N_SM * 128 * sm_mhz * 1e6
 
 
 def alu_peak(sm_mhz: float) -> float:
